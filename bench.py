@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the PGD hot path on BASELINE.json's workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl reference]
+
+A bench "step" is ONE afs_pgd_run call: the whole hot path (S1..S10 of DESIGN.md) over one batch of B restarts for
+the configuration's PGD iteration count.  metric = PGD restart-steps per second = B * pgd_iterations / time.
+`value` is measured with X0 already resident in HBM (CUDA events on the launching stream, max over ranks);
+`e2e` is the same metric through afs_pgd_run_host: pinned HOST buffers, H2D and D2H copies inside the timed region.
+One JSON line is printed by rank 0.  N > 1 (torchrun): every rank runs the full configuration on its own draw of
+start points (weak scaling, restarts are independent: PAPER.md L164), no collective inside the loop, one all-gather
+of the best counts at the end.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as W  # noqa: E402
+
+
+# --------------------------------------------------------------------------------------------- algorithmic work
+def algorithmic_flops_per_restart_step(inst) -> float:
+    """SURVEY.md 8(d) / DESIGN.md section 7: minimal flops of objective + gradient + chain rule per constraint
+    (FMA = 2), 1 add per literal for the variable reduction, 5 per variable for step/clip/mask/sign."""
+    L = inst.lengths().astype(np.float64)
+    k = inst.k.astype(np.float64)
+    ty = inst.types
+    f = np.zeros_like(L)
+    f[ty == W.AFS_OR] = 5 * L[ty == W.AFS_OR] + 2
+    f[ty == W.AFS_XOR] = 3 * L[ty == W.AFS_XOR] + 1
+    f[ty == W.AFS_NAE] = 9 * L[ty == W.AFS_NAE]
+    two = (ty == W.AFS_EO) | (ty == W.AFS_AMO)
+    f[two] = 15 * L[two]
+    cnt = (ty == W.AFS_EK) | (ty == W.AFS_CARD)
+    K = np.minimum(k, L - k + 1) + 1
+    f[cnt] = 6 * L[cnt] * np.maximum(K[cnt], 1)
+    return float(f.sum() + inst.nnz + 5 * inst.n)
+
+
+def compulsory_hbm_bytes_per_step(inst, B) -> float:
+    """read X + write X (fp32) + literal CSR once"""
+    return float(2 * B * inst.n * 4 + inst.nnz * 4)
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+# --------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        mhz, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            parts = [x.strip() for x in r.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                mhz.append(float(parts[0])); mx = float(parts[1])
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[2:6]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return dict(sm_mhz=float(np.median(mhz)) if mhz else None, sm_max_mhz=mx, reasons=sorted(reasons),
+                    samples=len(mhz))
+
+
+# --------------------------------------------------------------------------------------------- oracle legs
+def oracle_sample(inst, cfg, B_o=None, steps_o=None, target_s=8.0):
+    """Time the oracle (as it stands) on a bounded sample: the first B_o restarts for steps_o PGD iterations.
+    Unless given, the sample is sized from a one-iteration probe so that it costs about `target_s` seconds."""
+    from oracle import ref
+    cores = ref.num_threads()
+    lr = float(np.float32(inst.lr))
+    if B_o is None or steps_o is None:
+        Bp = min(inst.B, cores)
+        t0 = time.perf_counter()
+        ref.pgd_run(inst, inst.X0[:Bp], 1, lr, mask=inst.mask)
+        rate = Bp / max(time.perf_counter() - t0, 1e-6)            # restart-steps per second, rough
+        B_o = min(inst.B, 32 * cores)
+        steps_o = int(min(max(round(target_s * rate / B_o), 1), max(inst.steps, 1)))
+        if steps_o == 1:
+            B_o = int(min(max(round(target_s * rate), cores), B_o))
+    t0 = time.perf_counter()
+    ref.pgd_run(inst, inst.X0[:B_o], steps_o, lr, mask=inst.mask)
+    dt = time.perf_counter() - t0
+    return dict(value=B_o * steps_o / dt, seconds=dt, cores=cores, B_o=B_o, steps_o=steps_o)
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg = args.config
+    inst = W.config(cfg)
+    from oracle import ref
+    for _ in range(args.warmup):
+        oracle_sample(inst, cfg, B_o=min(inst.B, 8), steps_o=1)
+    tot_units, tot_t, last = 0.0, 0.0, None
+    for _ in range(args.steps):
+        last = oracle_sample(inst, cfg)
+        tot_units += last["B_o"] * last["steps_o"]
+        tot_t += last["seconds"]
+    value = tot_units / tot_t
+    sample = "configs[%d] instance, first %d restarts x %d PGD iterations per bench step" % (cfg, last["B_o"], last["steps_o"])
+    line = dict(metric="pgd_restart_steps_per_sec", value=value, unit="restart-steps/s", n_gpus=args.gpus,
+                steps=args.steps, warmup=args.warmup, ms_per_step=1e3 * tot_t / args.steps, higher_is_better=True,
+                scaling="weak", vs_baseline=None, dtype="f64", data="synthetic", impl="reference",
+                config=dict(workload=inst.name, n=inst.n, m=inst.m, nnz=inst.nnz, B=last["B_o"],
+                            pgd_steps_per_call=last["steps_o"]),
+                literal_evals_per_sec=value * inst.nnz,
+                cpu_baseline=dict(value=value, unit="restart-steps/s", cores=ref.num_threads(), kind="oracle", sample=sample),
+                e2e=dict(value=value, unit="restart-steps/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------------------------------- CUDA arm
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2606_06656_b200 import build as afs_build
+    if rank == 0:
+        afs_build.build()
+    if world > 1:
+        dist.barrier()
+    import paper_2606_06656_b200 as afs
+
+    cfg = args.config
+    inst = W.config(cfg)
+    if world > 1:   # every rank its own start points (weak scaling), same instance
+        rng = np.random.Generator(np.random.PCG64(W.BASE_SEED + 1000 * (rank + 1) + cfg))
+        inst.X0 = rng.uniform(-1, 1, size=inst.X0.shape).astype(np.float32)
+    pgd_steps = inst.steps if args.pgd_steps is None else args.pgd_steps
+    lr = float(np.float32(inst.lr))
+    P = afs.Problem.from_instance(inst, device=local)
+    if args.mode is not None:
+        P.set_option(0, args.mode)
+    X0 = torch.from_numpy(inst.X0).cuda()
+    X = torch.empty_like(X0)
+    mask = None if inst.mask is None else torch.from_numpy(inst.mask).cuda()
+    out = dict(best_assign=torch.empty((inst.B, inst.n), dtype=torch.int8, device="cuda"),
+               best_sat=torch.empty(inst.B, dtype=torch.int32, device="cuda"),
+               best_step=torch.empty(inst.B, dtype=torch.int32, device="cuda"))
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def one_call(timed):
+        X.copy_(X0)
+        flush.fill_(1)                      # L2 flush between calls, outside the timed events
+        if timed:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+        P.pgd_run(X, pgd_steps, lr, mask=mask, out=out)
+        if timed:
+            e1.record(stream)
+            return e0, e1
+        return None
+
+    for _ in range(max(args.warmup, 0)):
+        one_call(False)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    torch.cuda.synchronize()
+    wall0 = time.perf_counter()
+    evs = [one_call(True) for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - wall0
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop() if sampler else None
+    dev_ms = sum(a.elapsed_time(b) for a, b in evs)
+    launches = P.info("launches") * args.steps
+    resident = P.info("resident")
+    t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        # the one exchange of the sharded job (DESIGN.md multi-GPU): best counts of every rank
+        gathered = [torch.empty_like(out["best_sat"]) for _ in range(world)]
+        dist.all_gather(gathered, out["best_sat"])
+    dev_ms = float(t.item())
+    units = float(inst.B) * pgd_steps * args.steps * world
+    value = units / (dev_ms * 1e-3)
+
+    # ---- e2e through the host entry point (pinned buffers; copies inside the timed region)
+    Xh0 = torch.from_numpy(inst.X0).pin_memory()
+    Xh = torch.empty_like(Xh0).pin_memory()
+    hout = dict(best_assign=torch.empty((inst.B, inst.n), dtype=torch.int8).pin_memory(),
+                best_sat=torch.empty(inst.B, dtype=torch.int32).pin_memory(),
+                best_step=torch.empty(inst.B, dtype=torch.int32).pin_memory())
+    mask_h = None if inst.mask is None else torch.from_numpy(inst.mask).pin_memory()
+    e2e_t = 0.0
+    n_e2e = max(1, min(args.steps, 3))
+    for i in range(1 + n_e2e):
+        Xh.copy_(Xh0)
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        P.pgd_run_host(Xh, pgd_steps, lr, mask=mask_h, out=hout)     # synchronises the stream before returning
+        dt = time.perf_counter() - t0
+        if i > 0:
+            e2e_t += dt
+    t2 = torch.tensor([e2e_t], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+    e2e_value = float(inst.B) * pgd_steps * n_e2e * world / float(t2.item())
+    h2d = inst.B * inst.n * 4 + (inst.n if inst.mask is not None else 0)
+    d2h = inst.B * inst.n * 4 + inst.B * inst.n + 8 * inst.B
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel
+    peaks = load_peaks()
+    flops_rs = algorithmic_flops_per_restart_step(inst)
+    bytes_step = compulsory_hbm_bytes_per_step(inst, inst.B)
+    fp32_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12          # TFLOP/s, DESIGN.md section 7
+    t_alu = flops_rs * inst.B / (fp32_peak * 1e12)
+    t_hbm = bytes_step / (peaks["hbm_gbs"] * 1e9)
+    per_iter_s = dev_ms * 1e-3 / (args.steps * pgd_steps)                   # whole PGD iteration, this rank
+    if t_alu >= t_hbm:
+        roof = dict(bound="alu", achieved=flops_rs * inst.B / per_iter_s / 1e12, peak=fp32_peak, unit="TFLOP/s")
+    else:
+        roof = dict(bound="hbm", achieved=bytes_step / per_iter_s / 1e9, peak=peaks["hbm_gbs"], unit="GB/s")
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = None
+    roof["peak_source"] = ("148 SMs x 128 FP32 lanes x 2 x sm_max_mhz (%s)" % peaks["source"]) if roof["bound"] == "alu" \
+        else "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"]
+    roof["kernel"] = "resident PGD kernel (whole call)" if resident else "all kernels of one PGD iteration (streaming path)"
+    roof["algorithmic_per_iteration"] = dict(flops=flops_rs * inst.B, hbm_bytes=bytes_step)
+
+    # ---- the oracle beside it (bounded sample, rank 0, N = 1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        o = oracle_sample(inst, cfg)
+        cpu = dict(value=o["value"], unit="restart-steps/s", cores=o["cores"], kind="oracle",
+                   sample="first %d restarts x %d PGD iterations of configs[%d] (%.1f s)" % (o["B_o"], o["steps_o"], cfg, o["seconds"]))
+
+    line = dict(metric="pgd_restart_steps_per_sec", value=value, unit="restart-steps/s", n_gpus=world,
+                steps=args.steps, warmup=args.warmup, ms_per_step=dev_ms / args.steps, higher_is_better=True,
+                scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+                config=dict(workload=inst.name, n=inst.n, m=inst.m, nnz=inst.nnz, B=inst.B, pgd_steps_per_call=pgd_steps,
+                            lr=inst.lr, masked_vars=int((inst.mask != 0).sum()) if inst.mask is not None else 0,
+                            l2="flushed between calls (256 MiB write), outside the timed events",
+                            path="resident" if resident else "streaming", parallelism="restarts x%d" % world),
+                literal_evals_per_sec=value * inst.nnz,
+                wall_ms_per_step=1e3 * wall / args.steps,
+                gpu_launches=int(launches),
+                e2e=dict(value=e2e_value, unit="restart-steps/s", h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h)),
+                roofline=roof, cpu_baseline=cpu, clocks=clocks)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1: the metric's workload)")
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--pgd-steps", type=int, default=None, help="override the configuration's PGD iteration count")
+    ap.add_argument("--mode", type=int, default=None, help="afs_set_option(0, mode): 1 streaming, 2 resident")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

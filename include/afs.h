@@ -1,0 +1,169 @@
+/*
+ * afs.h -- C ABI of afs-b200: batched projected gradient descent on the Walsh-Fourier objective of
+ * symmetric pseudo-Boolean constraints, hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * Citations: P:Lnn = PAPER.md line nn of arxiv/paper_2606_06656 (section / equation beside it);
+ * Gnn = the reading of that number in DESIGN.md section 2.
+ *
+ * Conventions
+ *   Polarity       True -> -1, False -> +1 (section 2.1).  An expansion FE_C is -1 when C is satisfied and
+ *                  +1 when violated; the objective is minimised and equals -m at a solution.
+ *   Literals       signed 1-based int32: +(v+1) is x_v, -(v+1) is NOT x_v (relaxed value -x_v, G7).
+ *   Layout         every batch array is row-major [B, n] (restart-major, variable fastest), as the caller sees it.
+ *                  The library keeps its own transposed working copies.
+ *   Ownership      the caller owns every array argument.  The library owns the handle and its internal workspace,
+ *                  which grows to the largest (B, steps) seen and is freed by afs_problem_destroy.
+ *   Memory space   stated per argument: "host" or "device".  Device pointers must belong to the device the
+ *                  problem was created on.
+ *   Asynchrony     afs_eval_grad*, afs_round_count*, afs_pgd_run* enqueue work on `cuda_stream` (a cudaStream_t
+ *                  passed as void*, NULL = the legacy default stream) and return without synchronising; they may
+ *                  (re)allocate workspace, which synchronises the device, the first time a larger B is seen.
+ *                  afs_problem_create / afs_problem_destroy / afs_pgd_run_host synchronise.
+ *                  One handle must not be used from two streams at once (the workspace is shared).
+ *   Errors         every entry point returns an afs_status; nothing is printed, nothing throws.  Invalid input is
+ *                  rejected at afs_problem_create.  There is no CPU fallback: without a CUDA device every device
+ *                  entry point returns AFS_ERR_CUDA.
+ *   Precision      the entry points compute in fp32.  The *_f64 twins are the fp64 verification build of the same
+ *                  kernels (BASELINE.json north_star: "first-20-step PGD trajectories ... in an fp64 verification
+ *                  build"); they take double arrays and are not tuned.
+ */
+#ifndef AFS_H
+#define AFS_H
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define AFS_API __attribute__((visibility("default")))
+#else
+#define AFS_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct afs_problem afs_problem; /* opaque; owns device copies of the bucketed CSR, tables, workspace */
+
+typedef enum {
+    AFS_OK = 0,
+    AFS_ERR_INVALID_ARG = 1,  /* NULL pointer, negative size, B < 1, steps < 0, non-finite lr ...           */
+    AFS_ERR_BAD_TYPE = 2,     /* constraint type outside afs_ctype                                            */
+    AFS_ERR_BAD_K = 3,        /* EK/CARD: k < 0 or k > L+1;  XOR: k not in {0,1};  NAE with L < 2 (G6)        */
+    AFS_ERR_BAD_LITERAL = 4,  /* literal 0 or |literal| > n_vars, empty constraint, row_ptr not monotone      */
+    AFS_ERR_DUP_VAR = 5,      /* the same variable twice in one constraint (G8; P:L41 assumes distinct)       */
+    AFS_ERR_ALLOC = 6,        /* host or device allocation failed                                             */
+    AFS_ERR_CUDA = 7,         /* CUDA runtime error, or no CUDA device                                        */
+    AFS_ERR_UNSUPPORTED = 8   /* valid request outside what this build supports (see each entry point)        */
+} afs_status;
+
+/* Symmetric constraint family of P:L60 (section 2.2) plus clauses (eq. 4). */
+typedef enum {
+    AFS_OR = 0,   /* at least one literal true                                   */
+    AFS_XOR = 1,  /* number of true literals has parity k (1 = odd, G2)          */
+    AFS_AMO = 2,  /* at most one                                                  */
+    AFS_EO = 3,   /* exactly one                                                  */
+    AFS_EK = 4,   /* exactly k                                                    */
+    AFS_NAE = 5,  /* not all equal (0 < #true < L), L >= 2                        */
+    AFS_CARD = 6  /* at least k (k = 0: always true, k = L+1: never true; G5)     */
+} afs_ctype;
+
+/*
+ * afs_problem_create -- S0 of the path: validate, bucket by (type, length class), build the forward and the
+ * transposed CSR, upload (P:L60 problem statement; "incurred once").  Synchronous.
+ *   n_vars, n_cons   n >= 1, m >= 0
+ *   row_ptr  host    int64[n_cons+1], row_ptr[0] = 0, non-decreasing; constraint c owns lits[row_ptr[c]..row_ptr[c+1])
+ *   lits     host    int32[nnz] signed 1-based literals, distinct variables within a constraint
+ *   types    host    int32[n_cons], afs_ctype values
+ *   k        host    int32[n_cons]; EK: exactly k; CARD: at least k; XOR: required parity (1 = odd); otherwise ignored
+ *   device           CUDA device ordinal
+ *   out              receives the handle (NULL on error)
+ * Limits of this build: count-type constraints (AMO/EO/EK/NAE/CARD and OR longer than 64) up to L = 1151
+ * literals, otherwise AFS_ERR_UNSUPPORTED.
+ */
+AFS_API afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const int64_t* row_ptr, const int32_t* lits,
+                              const int32_t* types, const int32_t* k, int32_t device, afs_problem** out);
+
+/* Frees the handle, its device tables and workspace.  NULL is a no-op.  Synchronises the device. */
+AFS_API void afs_problem_destroy(afs_problem* p);
+
+/*
+ * afs_coeffs -- the n+1 distinct Fourier coefficients a_0..a_L of one symmetric constraint (eq. 3, P:L49-L52;
+ * Appendix A closed forms P:L223-L255 with readings G2-G5).  Host only, exact big-integer numerators, result
+ * within 2 ulp of the exact rational.  a_out: host double[L+1].  1 <= L <= 4096.
+ * The kernels do not consume these numbers: they evaluate the same polynomial in the count basis (G10).
+ */
+AFS_API afs_status afs_coeffs(int32_t type, int32_t L, int32_t k, double* a_out);
+
+/*
+ * afs_eval_grad -- S1..S6: objective F[b] = sum_k FE_{C_k}(X_b) (eq. 5) and its gradient.
+ *   X  device float[B,n] (read only)      F  device float[B] or NULL      G  device float[B,n] or NULL
+ * G[b,v] = sum over the literals of v of sigma * dFE/dy, accumulated in a fixed order (deterministic, no float
+ * atomics).  Leave-one-out gradients use prefix/suffix products or stable-direction recurrences: no division by
+ * a factor that can vanish at x = +-1.
+ */
+AFS_API afs_status afs_eval_grad(afs_problem* p, const float* X, int32_t B, float* F, float* G, void* cuda_stream);
+AFS_API afs_status afs_eval_grad_f64(afs_problem* p, const double* X, int32_t B, double* F, double* G, void* cuda_stream);
+
+/*
+ * afs_round_count -- S9: round by sign and count satisfied constraints.  x < 0 -> True (-1); x >= 0,
+ * +-0.0 and NaN -> False (+1) (G13).  Integer arithmetic, bit-exact.
+ *   X  device float[B,n]     assign  device int8[B,n] or NULL (-1 True, +1 False)     sat  device int32[B]
+ */
+AFS_API afs_status afs_round_count(afs_problem* p, const float* X, int32_t B, int8_t* assign, int32_t* sat,
+                           void* cuda_stream);
+AFS_API afs_status afs_round_count_f64(afs_problem* p, const double* X, int32_t B, int8_t* assign, int32_t* sat,
+                               void* cuda_stream);
+
+/*
+ * afs_pgd_run -- S1..S10 looped `steps` times with no host round trip (P:L69 PGD; G11, G12, G14, G16):
+ *   entry:  fixed coordinates (mask[v] != 0) of X are overwritten with mask[v]
+ *   t = 0..steps:  round X_t, count satisfied constraints; a strictly larger count replaces the best
+ *                  t < steps:  X_{t+1} = clip(X_t - lr * grad F(X_t), -1, +1) on free coordinates
+ *   X            device float[B,n]   in: X_0, out: X_steps
+ *   steps >= 0, lr finite
+ *   mask         device int8[n] or NULL: 0 free, -1 fixed True, +1 fixed False
+ *   best_assign  device int8[B,n] or NULL   rounded iterate with the largest count (earliest on ties)
+ *   best_sat     device int32[B] or NULL    that count
+ *   best_step    device int32[B] or NULL    the iterate index in [0, steps] it was first reached at
+ */
+AFS_API afs_status afs_pgd_run(afs_problem* p, float* X, int32_t B, int32_t steps, float lr, const int8_t* mask,
+                       int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* cuda_stream);
+AFS_API afs_status afs_pgd_run_f64(afs_problem* p, double* X, int32_t B, int32_t steps, double lr, const int8_t* mask,
+                           int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* cuda_stream);
+
+/*
+ * afs_pgd_run_host -- the same call with HOST buffers (all pointers host; pinned memory recommended): copies X
+ * and mask to the device, runs afs_pgd_run, copies X, best_assign, best_sat, best_step back, synchronises.
+ * This is the end-to-end entry point bench.py times ("e2e").  Output pointers may be NULL.
+ */
+AFS_API afs_status afs_pgd_run_host(afs_problem* p, float* X, int32_t B, int32_t steps, float lr, const int8_t* mask,
+                            int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* cuda_stream);
+
+/*
+ * afs_problem_info -- integer facts about a handle, for tests and bench.py.  `what`:
+ *   0 n_vars  1 n_cons  2 nnz  3 constraints on the pull path  4 on the medium path  5 on the long path
+ *   6 scratch slots (literals whose gradient is materialised)  7 kernel launches enqueued by the last call
+ *   8 workspace bytes currently held  9 1 if the last afs_pgd_run used the tile-resident kernel, else 0
+ * Unknown `what` returns -1.
+ */
+AFS_API int64_t afs_problem_info(const afs_problem* p, int32_t what);
+
+/*
+ * afs_set_option -- tuning knobs (all have defaults; tests use them to force code paths).  `what`:
+ *   0 execution mode of afs_pgd_run: 0 auto, 1 force the streaming (one launch per phase per step) path,
+ *     2 force the tile-resident path (AFS_ERR_UNSUPPORTED at run time if the instance does not fit)
+ * Returns AFS_ERR_INVALID_ARG for unknown options or values.
+ */
+AFS_API afs_status afs_set_option(afs_problem* p, int32_t what, int64_t value);
+
+/* Static, never NULL. */
+AFS_API const char* afs_status_string(afs_status s);
+
+/* ABI version of this header: bumped when a signature changes. */
+AFS_API int32_t afs_abi_version(void);
+#define AFS_ABI_VERSION 1
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AFS_H */

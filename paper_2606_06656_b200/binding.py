@@ -1,0 +1,230 @@
+"""Thin ctypes binding over the C ABI of include/afs.h -- argument marshalling only.
+
+Every step of the path runs inside ``libafs_b200.so`` (hand-written CUDA); PyTorch is used for device memory and
+streams and nothing else.  There is no CPU fallback: if the shared library is missing, cannot be loaded, or no CUDA
+device is present, calls fail loudly.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libafs_b200.so")
+
+AFS_OR, AFS_XOR, AFS_AMO, AFS_EO, AFS_EK, AFS_NAE, AFS_CARD = range(7)
+
+EXPORTS = (
+    "afs_problem_create", "afs_problem_destroy", "afs_coeffs", "afs_eval_grad", "afs_eval_grad_f64",
+    "afs_round_count", "afs_round_count_f64", "afs_pgd_run", "afs_pgd_run_f64", "afs_pgd_run_host",
+    "afs_problem_info", "afs_set_option", "afs_status_string", "afs_abi_version",
+)
+
+_lib = None
+
+
+class AfsError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = int(status)
+        msg = lib().afs_status_string(status).decode()
+        super().__init__("%s: %s (status %d)" % (where, msg, status))
+
+
+def lib():
+    """Load libafs_b200.so (built in-tree by ``paper_2606_06656_b200.build``). Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(
+            "%s not found: build it with `python -m paper_2606_06656_b200.build` (nvcc, sm_100a). "
+            "There is no CPU fallback." % LIB_PATH)
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    L.afs_problem_create.argtypes = [i32, i32, vp, vp, vp, vp, i32, C.POINTER(vp)]
+    L.afs_problem_create.restype = C.c_int
+    L.afs_problem_destroy.argtypes = [vp]
+    L.afs_problem_destroy.restype = None
+    L.afs_coeffs.argtypes = [i32, i32, i32, vp]
+    L.afs_coeffs.restype = C.c_int
+    for name in ("afs_eval_grad", "afs_eval_grad_f64"):
+        f = getattr(L, name); f.argtypes = [vp, vp, i32, vp, vp, vp]; f.restype = C.c_int
+    for name in ("afs_round_count", "afs_round_count_f64"):
+        f = getattr(L, name); f.argtypes = [vp, vp, i32, vp, vp, vp]; f.restype = C.c_int
+    L.afs_pgd_run.argtypes = [vp, vp, i32, i32, C.c_float, vp, vp, vp, vp, vp]
+    L.afs_pgd_run.restype = C.c_int
+    L.afs_pgd_run_f64.argtypes = [vp, vp, i32, i32, C.c_double, vp, vp, vp, vp, vp]
+    L.afs_pgd_run_f64.restype = C.c_int
+    L.afs_pgd_run_host.argtypes = [vp, vp, i32, i32, C.c_float, vp, vp, vp, vp, vp]
+    L.afs_pgd_run_host.restype = C.c_int
+    L.afs_problem_info.argtypes = [vp, i32]
+    L.afs_problem_info.restype = i64
+    L.afs_set_option.argtypes = [vp, i32, i64]
+    L.afs_set_option.restype = C.c_int
+    L.afs_status_string.argtypes = [C.c_int]
+    L.afs_status_string.restype = C.c_char_p
+    L.afs_abi_version.restype = i32
+    _lib = L
+    return L
+
+
+def _chk(status: int, where: str):
+    if status != 0:
+        raise AfsError(status, where)
+
+
+def coeffs(ctype: int, L: int, k: int = 0) -> np.ndarray:
+    """afs_coeffs: a_0..a_L (fp64, host)."""
+    a = np.zeros(L + 1, dtype=np.float64)
+    _chk(lib().afs_coeffs(ctype, L, k, a.ctypes.data), "afs_coeffs")
+    return a
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _stream_ptr(device) -> int:
+    torch = _torch()
+    return int(torch.cuda.current_stream(device).cuda_stream)
+
+
+class Problem:
+    """afs_problem handle. Arrays in, torch CUDA tensors out; layouts are those of include/afs.h ([B, n] row-major)."""
+
+    INFO = {"n_vars": 0, "n_cons": 1, "nnz": 2, "n_pull": 3, "n_med": 4, "n_long": 5, "scratch_slots": 6,
+            "launches": 7, "workspace_bytes": 8, "resident": 9}
+
+    def __init__(self, n_vars: int, row_ptr, lits, types, k, device: int = 0):
+        self._h = C.c_void_p(None)
+        rp = np.ascontiguousarray(row_ptr, dtype=np.int64)
+        li = np.ascontiguousarray(lits, dtype=np.int32)
+        ty = np.ascontiguousarray(types, dtype=np.int32)
+        kk = np.ascontiguousarray(k, dtype=np.int32)
+        if rp.ndim != 1 or rp.shape[0] != ty.shape[0] + 1 or kk.shape != ty.shape:
+            raise ValueError("row_ptr / types / k shapes disagree")
+        if rp.shape[0] and li.shape[0] != int(rp[-1]):
+            raise ValueError("lits length != row_ptr[-1]")
+        self.n, self.m, self.nnz = int(n_vars), int(ty.shape[0]), int(li.shape[0])
+        self.device = int(device)
+        h = C.c_void_p(None)
+        _chk(lib().afs_problem_create(self.n, self.m, rp.ctypes.data, li.ctypes.data, ty.ctypes.data,
+                                      kk.ctypes.data, self.device, C.byref(h)), "afs_problem_create")
+        self._h = h
+
+    @classmethod
+    def from_instance(cls, inst, device: int = 0) -> "Problem":
+        return cls(inst.n, inst.row_ptr, inst.lits, inst.types, inst.k, device)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().afs_problem_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def info(self, what: str) -> int:
+        return int(lib().afs_problem_info(self._h, self.INFO[what]))
+
+    def set_option(self, what: int, value: int):
+        _chk(lib().afs_set_option(self._h, what, value), "afs_set_option")
+
+    # ------------------------------------------------------------------ helpers
+    def _dev(self):
+        return _torch().device("cuda", self.device)
+
+    def _check_X(self, X, dtype):
+        torch = _torch()
+        if not (isinstance(X, torch.Tensor) and X.is_cuda and X.dtype == dtype and X.dim() == 2
+                and X.shape[1] == self.n and X.is_contiguous() and X.device.index == self.device):
+            raise ValueError("X must be a contiguous CUDA %s tensor [B, %d] on device %d" % (dtype, self.n, self.device))
+
+    # ------------------------------------------------------------------ entry points
+    def eval_grad(self, X, want_F: bool = True, want_G: bool = True):
+        """afs_eval_grad / afs_eval_grad_f64 (chosen by X.dtype). Returns (F[B] or None, G[B,n] or None)."""
+        torch = _torch()
+        f64 = X.dtype == torch.float64
+        self._check_X(X, torch.float64 if f64 else torch.float32)
+        B = X.shape[0]
+        F = torch.empty(B, dtype=X.dtype, device=X.device) if want_F else None
+        G = torch.empty_like(X) if want_G else None
+        fn = lib().afs_eval_grad_f64 if f64 else lib().afs_eval_grad
+        _chk(fn(self._h, X.data_ptr(), B, F.data_ptr() if want_F else None, G.data_ptr() if want_G else None,
+                _stream_ptr(X.device)), "afs_eval_grad")
+        return F, G
+
+    def round_count(self, X, want_assign: bool = True):
+        """afs_round_count. Returns (assign int8[B,n] or None, sat int32[B])."""
+        torch = _torch()
+        f64 = X.dtype == torch.float64
+        self._check_X(X, torch.float64 if f64 else torch.float32)
+        B = X.shape[0]
+        sat = torch.empty(B, dtype=torch.int32, device=X.device)
+        assign = torch.empty((B, self.n), dtype=torch.int8, device=X.device) if want_assign else None
+        fn = lib().afs_round_count_f64 if f64 else lib().afs_round_count
+        _chk(fn(self._h, X.data_ptr(), B, assign.data_ptr() if want_assign else None, sat.data_ptr(),
+                _stream_ptr(X.device)), "afs_round_count")
+        return assign, sat
+
+    def pgd_run(self, X, steps: int, lr: float, mask=None, out=None):
+        """afs_pgd_run / _f64, in place on X (device). Returns dict(X, best_assign, best_sat, best_step).
+
+        ``out`` may carry preallocated ``best_assign`` / ``best_sat`` / ``best_step`` tensors (bench.py reuses them)."""
+        torch = _torch()
+        f64 = X.dtype == torch.float64
+        self._check_X(X, torch.float64 if f64 else torch.float32)
+        B = X.shape[0]
+        if mask is not None:
+            if not (mask.is_cuda and mask.dtype == torch.int8 and mask.numel() == self.n and mask.is_contiguous()):
+                raise ValueError("mask must be a contiguous CUDA int8 tensor [n]")
+        out = out or {}
+        ba = out.get("best_assign")
+        bs = out.get("best_sat")
+        bt = out.get("best_step")
+        if ba is None:
+            ba = torch.empty((B, self.n), dtype=torch.int8, device=X.device)
+        if bs is None:
+            bs = torch.empty(B, dtype=torch.int32, device=X.device)
+        if bt is None:
+            bt = torch.empty(B, dtype=torch.int32, device=X.device)
+        fn = lib().afs_pgd_run_f64 if f64 else lib().afs_pgd_run
+        _chk(fn(self._h, X.data_ptr(), B, int(steps), float(lr), mask.data_ptr() if mask is not None else None,
+                ba.data_ptr(), bs.data_ptr(), bt.data_ptr(), _stream_ptr(X.device)), "afs_pgd_run")
+        return dict(X=X, best_assign=ba, best_sat=bs, best_step=bt)
+
+    def pgd_run_host(self, X, steps: int, lr: float, mask=None, out=None):
+        """afs_pgd_run_host: X float32 [B,n] HOST tensor/array (pinned recommended), updated in place; H2D and D2H
+        copies happen inside the call. Returns dict of host tensors."""
+        torch = _torch()
+        if isinstance(X, np.ndarray):
+            X = torch.from_numpy(X)
+        if X.is_cuda or X.dtype != torch.float32 or X.dim() != 2 or X.shape[1] != self.n or not X.is_contiguous():
+            raise ValueError("X must be a contiguous host float32 tensor [B, n]")
+        B = X.shape[0]
+        if mask is not None:
+            if isinstance(mask, np.ndarray):
+                mask = torch.from_numpy(np.ascontiguousarray(mask, dtype=np.int8))
+            if mask.is_cuda or mask.dtype != torch.int8 or mask.numel() != self.n:
+                raise ValueError("mask must be a host int8 tensor [n]")
+        out = out or {}
+        ba = out.get("best_assign")
+        bs = out.get("best_sat")
+        bt = out.get("best_step")
+        if ba is None:
+            ba = torch.empty((B, self.n), dtype=torch.int8)
+        if bs is None:
+            bs = torch.empty(B, dtype=torch.int32)
+        if bt is None:
+            bt = torch.empty(B, dtype=torch.int32)
+        _chk(lib().afs_pgd_run_host(self._h, X.data_ptr(), B, int(steps), float(lr),
+                                    mask.data_ptr() if mask is not None else None, ba.data_ptr(), bs.data_ptr(),
+                                    bt.data_ptr(), _stream_ptr(self._dev())), "afs_pgd_run_host")
+        return dict(X=X, best_assign=ba, best_sat=bs, best_step=bt)

@@ -1,0 +1,127 @@
+// afs_internal.h -- host-side problem representation shared by the translation units of libafs_b200.
+// Not part of the ABI (include/afs.h is).  No code from oracle/ is used here or anywhere in csrc/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/afs.h"
+
+namespace afs {
+
+// ---- literal word: bit 31 = negated literal, bits 0..30 = variable index -------------------------------------
+constexpr uint32_t LIT_NEG = 0x80000000u;
+constexpr uint32_t LIT_VAR = 0x7fffffffu;
+
+// ---- execution classes (decided at create; S0 of the path) ---------------------------------------------------
+//  PULL : OR / XOR / NAE with L <= PULL_MAX_LEN.  No gradient is materialised: the variable pass recomputes each
+//         occurrence's leave-one-out product from the other literals (deterministic by construction).
+//  MED  : thread per (constraint, restart), prefix/suffix in registers: OR/XOR L<=64, NAE/EO/AMO L<=32;
+//         OR/XOR longer than 64 run a two-pass running-product kernel (scratch row = prefix storage).
+//  LONG : warp per (constraint, restart), count-basis DP + stable-direction leave-one-out recurrences:
+//         every EK/CARD, and whatever is too long for MED.
+constexpr int PULL_MAX_LEN = 5;
+constexpr int MED_MAX_PROD = 64;
+constexpr int MED_MAX_TWO = 32;
+constexpr int LONG_MAX_LEN = 1151;   // 9 rows x 128 cells hold q_0..q_L
+constexpr int MED_BUCKETS = 5;       // padded lengths 8, 16, 32, 64; bucket 4 = OR/XOR longer than 64 (two-pass kernel)
+constexpr int LONG_BUCKETS = 9;      // NR = 1..9 rows of 128 pmf cells
+
+// pull occurrence header (one uint32, followed by `nother` literal words)
+//   bits 0..1 kind (0 OR, 1 XOR, 2 NAE) | 2..4 nother | 5 own literal negated | 6 owner | 7 xor parity k
+constexpr uint32_t PH_KIND_OR = 0, PH_KIND_XOR = 1, PH_KIND_NAE = 2;
+
+struct MedCon {        // 16 bytes
+    int32_t off;       // first literal in med_lits / med_slots
+    int32_t L;
+    int32_t type;
+    int32_t k;
+};
+
+struct LongCon {       // 32 bytes
+    int32_t off;       // first literal in long_lits / long_slots
+    int32_t L;
+    int32_t type;
+    int32_t k;
+    int32_t tA, tB;    // leave-one-out pmf indices entering the gradient (true-count index, 0..L-1)
+    float wA, wB;      // their weights d_t in {-1, 0, +1}
+};
+
+struct CountCon {      // generic forward CSR entry for the count-only kernel: 16 bytes
+    int64_t off;
+    int32_t L;
+    int16_t type;
+    int16_t pad;
+    int32_t k;
+    int32_t pad2;
+};
+
+template <typename T>
+struct DevBuf {
+    T* p = nullptr;
+    size_t n = 0;
+};
+
+struct Workspace {
+    // all sized for (Bp, steps) below; grown on demand
+    int32_t Bp = 0;
+    int64_t sat_rows = 0;
+    void* XT[2] = {nullptr, nullptr};      // real [n][Bp]
+    void* scratch = nullptr;               // real [nslots][Bp]
+    int32_t* sat_hist = nullptr;           // [sat_rows][Bp]
+    int32_t* best_sat[2] = {nullptr, nullptr};
+    int32_t* best_step[2] = {nullptr, nullptr};
+    uint32_t* S[2] = {nullptr, nullptr};   // sign bits [n][Bp/32]
+    uint32_t* best_bits = nullptr;         // [n][Bp/32]
+    void* fe_med = nullptr;                // real [n_med][Bp]      (eval_grad only)
+    void* fe_long = nullptr;               // real [n_long][Bp]
+    void* f_part = nullptr;                // real [n_parts][Bp]
+    int32_t fe_Bp = 0;
+    int8_t* mask_dev = nullptr;            // staging for afs_pgd_run_host
+    void* host_stage_X = nullptr;          // device X[B,n] staging for afs_pgd_run_host
+    int8_t* host_stage_assign = nullptr;
+    int32_t* host_stage_sat = nullptr;
+    int32_t* host_stage_step = nullptr;
+    int64_t host_stage_B = 0;
+    size_t elem = 0;                       // sizeof(real) the buffers were sized for
+    size_t bytes = 0;
+};
+
+}  // namespace afs
+
+struct afs_problem {
+    int32_t n = 0, m = 0;
+    int64_t nnz = 0;
+    int device = 0;
+    int sm_count = 148;
+
+    // ---- device tables -------------------------------------------------------------------------------------
+    int32_t* d_pull_ptr = nullptr;      // [n+1] word offsets of each variable's occurrence stream
+    uint32_t* d_pull_words = nullptr;
+    int64_t pull_words = 0;
+    int32_t* d_slot_ptr = nullptr;      // [n+1] scratch rows of each variable (transposed-CSR order)
+    int64_t nslots = 0;
+
+    afs::MedCon* d_med = nullptr;       // sorted by bucket
+    uint32_t* d_med_lits = nullptr;
+    int32_t* d_med_slots = nullptr;
+    int32_t med_begin[afs::MED_BUCKETS + 1] = {0};
+
+    afs::LongCon* d_long = nullptr;     // sorted by bucket (NR), longest first inside a bucket
+    uint32_t* d_long_lits = nullptr;
+    int32_t* d_long_slots = nullptr;
+    int32_t long_begin[afs::LONG_BUCKETS + 1] = {0};
+    int32_t long_maxL[afs::LONG_BUCKETS] = {0};
+
+    afs::CountCon* d_count = nullptr;   // all m constraints, original order
+    uint32_t* d_count_lits = nullptr;
+
+    int64_t n_pull = 0, n_med = 0, n_long = 0;
+
+    // ---- run state -----------------------------------------------------------------------------------------
+    afs::Workspace ws;
+    int64_t last_launches = 0;
+    int32_t opt_mode = 0;
+    int32_t last_resident = 0;
+};

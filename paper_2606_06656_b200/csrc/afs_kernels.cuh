@@ -1,0 +1,737 @@
+// afs_kernels.cuh -- the streaming-path kernels (one launch per phase per step), templated on the arithmetic type
+// (float = product, double = fp64 verification build).  Working layout: XT[n][Bp], restart fastest, so that lane <->
+// restart gives one 128-byte line per (variable, 32 restarts) -- the "coalesced restart-major gathers" of
+// BASELINE.json.  P:Lnn = PAPER.md line nn.
+#pragma once
+#include "afs_internal.h"
+
+namespace afs {
+
+constexpr unsigned FULL = 0xffffffffu;
+constexpr int VAR_WARPS = 8;   // warps per CTA in the variable pass
+constexpr int VAR_VPW = 4;     // consecutive variables per warp
+
+// Is the constraint true when t of its L literals are true?  (Table 2; XOR parity k, G2)
+__device__ __forceinline__ bool pred(int type, int L, int k, int t)
+{
+    switch (type) {
+    case AFS_OR: return t >= 1;
+    case AFS_XOR: return ((t ^ k) & 1) == 0;
+    case AFS_AMO: return t <= 1;
+    case AFS_EO: return t == 1;
+    case AFS_EK: return t == k;
+    case AFS_NAE: return t > 0 && t < L;
+    case AFS_CARD: return t >= k;
+    default: return false;
+    }
+}
+
+template <typename real>
+__device__ __forceinline__ real ldx(const real* __restrict__ XT, uint32_t w, int Bp, int b)
+{
+    return XT[(size_t)(w & LIT_VAR) * Bp + b];
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// layout changes at the API boundary: X[B,n] <-> XT[n][Bp]
+// ------------------------------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void __launch_bounds__(256) k_transpose_in(const real* __restrict__ X, real* __restrict__ XT, int B, int n,
+                                                      int Bp, const int8_t* __restrict__ mask)
+{
+    __shared__ real tile[32][33];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int v0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
+    for (int r = ty; r < 32; r += 8) {
+        int b = b0 + r, v = v0 + tx;
+        real x = real(0);
+        if (b < B && v < n) x = X[(size_t)b * n + v] + real(0);   // + 0 turns -0.0 into +0.0 (G13)
+        tile[r][tx] = x;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        int v = v0 + r, b = b0 + tx;
+        if (v < n) {
+            real x = tile[tx][r];
+            if (mask) { int mk = mask[v]; if (mk != 0 && b < B) x = (real)mk; }   // fixed at entry
+            XT[(size_t)v * Bp + b] = x;
+        }
+    }
+}
+
+template <typename real>
+__global__ void __launch_bounds__(256) k_transpose_out(const real* __restrict__ XT, real* __restrict__ X, int B, int n,
+                                                       int Bp)
+{
+    __shared__ real tile[32][33];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int v0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
+    for (int r = ty; r < 32; r += 8) {
+        int v = v0 + r;
+        tile[r][tx] = v < n ? XT[(size_t)v * Bp + b0 + tx] : real(0);
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        int b = b0 + r, v = v0 + tx;
+        if (b < B && v < n) X[(size_t)b * n + v] = tile[tx][r];
+    }
+}
+
+// rounded assignment int8[B,n] from XT (S9): x < 0 -> -1 (True), else +1
+template <typename real>
+__global__ void __launch_bounds__(256) k_assign_out(const real* __restrict__ XT, int8_t* __restrict__ assign, int B,
+                                                    int n, int Bp)
+{
+    __shared__ int8_t tile[32][33];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int v0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
+    for (int r = ty; r < 32; r += 8) {
+        int v = v0 + r;
+        real x = v < n ? XT[(size_t)v * Bp + b0 + tx] : real(0);
+        tile[r][tx] = x < real(0) ? -1 : 1;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        int b = b0 + r, v = v0 + tx;
+        if (b < B && v < n) assign[(size_t)b * n + v] = tile[tx][r];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// S9 alone: satisfied-constraint count of one iterate, every constraint through the generic forward CSR.
+// Integer arithmetic only; thread = (constraint, restart), lanes over restarts.
+// ------------------------------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void __launch_bounds__(256) k_count(const CountCon* __restrict__ cons, const uint32_t* __restrict__ lits,
+                                               int m, const real* __restrict__ XT, int Bp, int32_t* __restrict__ sat)
+{
+    __shared__ int s_sat[8][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int b = blockIdx.y * 32 + lane;
+    int cnt = 0;
+    for (int c = blockIdx.x * 8 + warp; c < m; c += gridDim.x * 8) {
+        CountCon cc = cons[c];
+        int t = 0;
+        for (int j = 0; j < cc.L; ++j) {
+            uint32_t w = lits[cc.off + j];
+            real x = ldx(XT, w, Bp, b);
+            t += ((x < real(0)) != ((w >> 31) != 0)) ? 1 : 0;
+        }
+        cnt += pred(cc.type, cc.L, cc.k, t) ? 1 : 0;
+    }
+    s_sat[warp][lane] = cnt;
+    __syncthreads();
+    if (warp == 0) {
+        int tot = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) tot += s_sat[w][lane];
+        if (tot) atomicAdd(&sat[b], tot);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// MED class: thread = (constraint, restart); y gathered once into registers; division-free leave-one-out by
+// prefix / suffix products (OR, XOR, NAE) or a two-state prefix / suffix pmf (EO, AMO).  S1-S3, S5, S9.
+//   OR   FE = 2 prod u - 1                 dFE/dy_j = prod_{i!=j} u_i                      (u = (1+y)/2)
+//   XOR  FE = s prod y                     dFE/dy_j = s prod_{i!=j} y_i                    (s = +1 odd parity, -1 even)
+//   NAE  FE = 2 prod u + 2 prod p - 1      dFE/dy_j = prod_{i!=j} u_i - prod_{i!=j} p_i     (p = (1-y)/2)
+//   EO   FE = 1 - 2 q_1                    dFE/dy_j = q_0^(-j) - q_1^(-j)
+//   AMO  FE = 1 - 2 (q_0 + q_1)            dFE/dy_j = - q_1^(-j)
+// (count basis, G10; d_t of P:L52).  The gradient written to scratch already carries the literal sign (S5).
+// ------------------------------------------------------------------------------------------------------------------
+template <typename real, int LP>
+__global__ void __launch_bounds__(128) k_med(const MedCon* __restrict__ cons, int c_begin, int c_end,
+                                             const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
+                                             const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
+                                             int32_t* __restrict__ sat, real* __restrict__ fe_out)
+{
+    __shared__ int s_sat[4][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int b = blockIdx.y * 32 + lane;
+    int satcnt = 0;
+    const real half = real(0.5), one = real(1);
+    for (int c = c_begin + blockIdx.x * 4 + warp; c < c_end; c += gridDim.x * 4) {
+        const MedCon mc = cons[c];
+        const uint32_t* lc = lits + mc.off;
+        const int32_t* sc = slots + mc.off;
+        real y[LP];
+        unsigned long long negmask = 0ull;
+        int t = 0;
+#pragma unroll
+        for (int j = 0; j < LP; ++j) {
+            real v = one;   // padding literal: constant False (y = +1), neutral for every type below
+            if (j < mc.L) {
+                uint32_t w = lc[j];
+                real x = ldx(XT, w, Bp, b);
+                bool neg = (w >> 31) != 0;
+                t += ((x < real(0)) != neg) ? 1 : 0;
+                v = neg ? -x : x;
+                if (neg) negmask |= 1ull << j;
+            }
+            y[j] = v;
+        }
+        satcnt += pred(mc.type, mc.L, mc.k, t) ? 1 : 0;
+        real fe;
+        if (mc.type == AFS_OR || mc.type == AFS_XOR) {
+            const bool is_or = mc.type == AFS_OR;
+            const real s = is_or ? one : ((mc.k & 1) ? one : -one);
+            real g[LP];
+            real pre = one;
+#pragma unroll
+            for (int j = 0; j < LP; ++j) {
+                real f = is_or ? half + half * y[j] : y[j];
+                y[j] = f;
+                g[j] = pre;
+                pre *= f;
+            }
+            fe = is_or ? real(2) * pre - one : s * pre;
+            real suf = s;
+#pragma unroll
+            for (int j = LP - 1; j >= 0; --j) {
+                g[j] *= suf;
+                suf *= y[j];
+            }
+#pragma unroll
+            for (int j = 0; j < LP; ++j)
+                if (j < mc.L) scratch[(size_t)sc[j] * Bp + b] = ((negmask >> j) & 1ull) ? -g[j] : g[j];
+        } else {
+            if constexpr (LP <= 32) {
+                if (mc.type == AFS_NAE) {
+                    real gu[LP], gp[LP];
+                    real pu = one, pp = one;
+#pragma unroll
+                    for (int j = 0; j < LP; ++j) {
+                        // a padding literal must be neutral in BOTH chains: treat it as absent (factor 1)
+                        real u = j < mc.L ? half + half * y[j] : one;
+                        real p = j < mc.L ? half - half * y[j] : one;
+                        gu[j] = pu; gp[j] = pp;
+                        pu *= u; pp *= p;
+                    }
+                    fe = real(2) * pu + real(2) * pp - one;
+                    real su = one, sp = one;
+#pragma unroll
+                    for (int j = LP - 1; j >= 0; --j) {
+                        real u = j < mc.L ? half + half * y[j] : one;
+                        real p = j < mc.L ? half - half * y[j] : one;
+                        gu[j] = gu[j] * su - gp[j] * sp;
+                        su *= u; sp *= p;
+                    }
+#pragma unroll
+                    for (int j = 0; j < LP; ++j)
+                        if (j < mc.L) scratch[(size_t)sc[j] * Bp + b] = ((negmask >> j) & 1ull) ? -gu[j] : gu[j];
+                } else {   // EO, AMO: pmf of the true count truncated to {0, 1}
+                    real P0[LP], P1[LP];
+                    real a0 = one, a1 = real(0);
+#pragma unroll
+                    for (int j = 0; j < LP; ++j) {
+                        real u = half + half * y[j], p = half - half * y[j];
+                        P0[j] = a0; P1[j] = a1;
+                        a1 = a1 * u + a0 * p;
+                        a0 = a0 * u;
+                    }
+                    const bool is_eo = mc.type == AFS_EO;
+                    fe = is_eo ? one - real(2) * a1 : one - real(2) * (a0 + a1);
+                    real s0 = one, s1 = real(0);
+#pragma unroll
+                    for (int j = LP - 1; j >= 0; --j) {
+                        real u = half + half * y[j], p = half - half * y[j];
+                        real q0 = P0[j] * s0;
+                        real q1 = P1[j] * s0 + P0[j] * s1;
+                        P0[j] = is_eo ? q0 - q1 : -q1;
+                        s1 = s1 * u + s0 * p;
+                        s0 = s0 * u;
+                    }
+#pragma unroll
+                    for (int j = 0; j < LP; ++j)
+                        if (j < mc.L) scratch[(size_t)sc[j] * Bp + b] = ((negmask >> j) & 1ull) ? -P0[j] : P0[j];
+                }
+            } else {
+                fe = real(0);
+            }
+        }
+        if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
+    }
+    if (sat) {
+        s_sat[warp][lane] = satcnt;
+        __syncthreads();
+        if (warp == 0) {
+            int tot = s_sat[0][lane] + s_sat[1][lane] + s_sat[2][lane] + s_sat[3][lane];
+            if (tot) atomicAdd(&sat[b], tot);
+        }
+    }
+}
+
+// OR / XOR longer than 64 literals: two passes, the scratch row of each literal holds the running prefix product
+// between them (no extra memory, no division).
+template <typename real>
+__global__ void __launch_bounds__(128) k_prod_long(const MedCon* __restrict__ cons, int c_begin, int c_end,
+                                                   const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
+                                                   const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
+                                                   int32_t* __restrict__ sat, real* __restrict__ fe_out)
+{
+    __shared__ int s_sat[4][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int b = blockIdx.y * 32 + lane;
+    int satcnt = 0;
+    const real half = real(0.5), one = real(1);
+    for (int c = c_begin + blockIdx.x * 4 + warp; c < c_end; c += gridDim.x * 4) {
+        const MedCon mc = cons[c];
+        const uint32_t* lc = lits + mc.off;
+        const int32_t* sc = slots + mc.off;
+        const bool is_or = mc.type == AFS_OR;
+        const real s = is_or ? one : ((mc.k & 1) ? one : -one);
+        real pre = one;
+        int t = 0;
+        for (int j = 0; j < mc.L; ++j) {
+            uint32_t w = lc[j];
+            real x = ldx(XT, w, Bp, b);
+            bool neg = (w >> 31) != 0;
+            t += ((x < real(0)) != neg) ? 1 : 0;
+            real yj = neg ? -x : x;
+            scratch[(size_t)sc[j] * Bp + b] = pre;
+            pre *= is_or ? half + half * yj : yj;
+        }
+        satcnt += pred(mc.type, mc.L, mc.k, t) ? 1 : 0;
+        if (fe_out) fe_out[(size_t)c * Bp + b] = is_or ? real(2) * pre - one : s * pre;
+        real suf = s;
+        for (int j = mc.L - 1; j >= 0; --j) {
+            uint32_t w = lc[j];
+            real x = ldx(XT, w, Bp, b);
+            bool neg = (w >> 31) != 0;
+            real yj = neg ? -x : x;
+            size_t idx = (size_t)sc[j] * Bp + b;
+            real g = scratch[idx] * suf;
+            scratch[idx] = neg ? -g : g;
+            suf *= is_or ? half + half * yj : yj;
+        }
+    }
+    if (sat) {
+        s_sat[warp][lane] = satcnt;
+        __syncthreads();
+        if (warp == 0) {
+            int tot = s_sat[0][lane] + s_sat[1][lane] + s_sat[2][lane] + s_sat[3][lane];
+            if (tot) atomicAdd(&sat[b], tot);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// LONG class: warp = (constraint, restart), CTA = one constraint x 8 restarts.  Count basis (G10):
+//   forward   q = pmf of the number of true literals, q_t <- q_t u_j + q_{t-1} p_j.  The pmf lives in registers,
+//             cell t = (row*32 + lane)*4 + c; rows that are still identically zero are skipped (warp-uniform).
+//   gradient  dFE/dy_j = sum_t d_t q_t^(-j) with at most two non-zero d_t.  q^(-j) comes from q by removing
+//             literal j in the STABLE direction: with s_t = u_j r_t,  s_t = q_t - (p_j/u_j) s_{t-1}  when p_j <= 1/2,
+//             else from the top with the roles of u and p swapped (reversed copy of q).  The divisor is >= 1/2:
+//             nothing that vanishes at x = +-1 is ever divided by (BASELINE.json subsystem (2)).
+// ------------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void load4(const float* p, float (&v)[4])
+{
+    float4 t = *reinterpret_cast<const float4*>(p);
+    v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+}
+__device__ __forceinline__ void load4(const double* p, double (&v)[4])
+{
+    double2 a = *reinterpret_cast<const double2*>(p), b = *reinterpret_cast<const double2*>(p + 2);
+    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+}
+
+template <typename real, int NR, int PH>
+__device__ __forceinline__ void dp_run(real (&q)[NR][4], const real* __restrict__ ys, int jbeg, int jend, int lane)
+{
+    const int src = (lane + 31) & 31;
+    for (int j = jbeg; j < jend; ++j) {
+        const real y = ys[j];
+        const real u = real(0.5) + real(0.5) * y, p = real(0.5) - real(0.5) * y;
+        real rot[PH + 1];
+#pragma unroll
+        for (int r = 0; r <= PH; ++r) rot[r] = __shfl_sync(FULL, q[r][3], src);
+#pragma unroll
+        for (int r = PH; r >= 0; --r) {
+            real carry = rot[r];
+            if (lane == 0) carry = r > 0 ? rot[r > 0 ? r - 1 : 0] : real(0);
+            q[r][3] = q[r][3] * u + q[r][2] * p;
+            q[r][2] = q[r][2] * u + q[r][1] * p;
+            q[r][1] = q[r][1] * u + q[r][0] * p;
+            q[r][0] = q[r][0] * u + carry * p;
+        }
+    }
+}
+
+template <typename real, int NR, int PH>
+struct DpPhases {
+    static __device__ __forceinline__ void run(real (&q)[NR][4], const real* __restrict__ ys, int L, int lane, int j)
+    {
+        if constexpr (PH < NR) {
+            // after literal j the count can reach j+1: row (j+1)/128 must be live, i.e. j <= 128 (PH+1) - 2
+            int jend = PH == NR - 1 ? L : min(L, 128 * (PH + 1) - 1);
+            dp_run<real, NR, PH>(q, ys, j, jend, lane);
+            DpPhases<real, NR, PH + 1>::run(q, ys, L, lane, jend > j ? jend : j);
+        }
+    }
+};
+
+template <typename real, int NR>
+__global__ void __launch_bounds__(256) k_long(const LongCon* __restrict__ cons, int c_begin,
+                                              const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
+                                              const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
+                                              int32_t* __restrict__ sat, real* __restrict__ fe_out, int LS, int QS)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    real* Ys = reinterpret_cast<real*>(smem_raw);   // [8][LS]  literal values of this CTA's 8 restarts
+    real* A = Ys + 8 * LS;                          // [8][QS]  q_0..q_L
+    real* Ar = A + 8 * QS;                          // [8][QS]  reversed: Ar[i] = q_{L-i}
+    __shared__ int s_cnt[8];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int groups = Bp >> 3;
+    const int c = c_begin + (int)(blockIdx.x / groups);
+    const int bg = (int)(blockIdx.x % groups);
+    const LongCon lc = cons[c];
+    const int L = lc.L;
+    const uint32_t* lw = lits + lc.off;
+    const int32_t* sw = slots + lc.off;
+    if (tid < 8) s_cnt[tid] = 0;
+    __syncthreads();
+    // ---- S1: gather the literal values of 8 consecutive restarts (one 32-byte sector per literal in fp32)
+    {
+        const int r = tid & 7;
+        for (int idx = tid; idx < ((L * 8 + 255) & ~255); idx += 256) {
+            int j = idx >> 3;
+            bool tr = false;
+            if (j < L) {
+                uint32_t w = lw[j];
+                real x = ldx(XT, w, Bp, bg * 8 + r);
+                bool neg = (w >> 31) != 0;
+                tr = (x < real(0)) != neg;
+                Ys[r * LS + j] = neg ? -x : x;
+            }
+            unsigned bal = __ballot_sync(FULL, tr);
+            if (lane < 8) {
+                int add = __popc(bal & (0x01010101u << lane));
+                if (add) atomicAdd(&s_cnt[lane], add);
+            }
+        }
+    }
+    __syncthreads();
+    const int b = bg * 8 + warp;
+    const real* ys = Ys + warp * LS;
+    real* Aw = A + warp * QS;
+    real* Arw = Ar + warp * QS;
+    // ---- S2: forward pmf
+    real q[NR][4];
+#pragma unroll
+    for (int r = 0; r < NR; ++r)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) q[r][i] = real(0);
+    if (lane == 0) q[0][0] = real(1);
+    DpPhases<real, NR, 0>::run(q, ys, L, lane, 0);
+    real fe = real(0);
+#pragma unroll
+    for (int r = 0; r < NR; ++r)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            int t = (r * 32 + lane) * 4 + i;
+            if (t <= L) {
+                Aw[t] = q[r][i];
+                Arw[L - t] = q[r][i];
+                fe += pred(lc.type, L, lc.k, t) ? -q[r][i] : q[r][i];   // sp_t = -1 where satisfied
+            }
+        }
+    for (int t = L + 1 + lane; t < QS; t += 32) { Aw[t] = real(0); Arw[t] = real(0); }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) fe += __shfl_xor_sync(FULL, fe, o);
+    if (lane == 0) {
+        if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
+        if (sat && pred(lc.type, L, lc.k, s_cnt[warp])) atomicAdd(&sat[b], 1);
+    }
+    __syncwarp();
+    // ---- S3 + S5: leave-one-out by stable-direction deconvolution, lanes over literals
+    const bool useA = lc.wA != 0.f, useB = lc.wB != 0.f;
+    for (int j0 = 0; j0 < L; j0 += 32) {
+        const int j = j0 + lane;
+        const bool act = j < L;
+        const real y = act ? ys[j] : real(1);
+        const real u = real(0.5) + real(0.5) * y, p = real(0.5) - real(0.5) * y;
+        const bool fwd = !(y < real(0));             // p <= 1/2
+        const real D = fwd ? u : p;                  // >= 1/2
+        const real R = (fwd ? p : u) / D;            // <= 1
+        const real* base = fwd ? Aw : Arw;
+        const int iA = fwd ? lc.tA : L - 1 - lc.tA;
+        const int iB = fwd ? lc.tB : L - 1 - lc.tB;
+        int iend = -1;
+        if (act && useA) iend = iA;
+        if (act && useB && iB > iend) iend = iB;
+        int wend = iend;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) wend = max(wend, __shfl_xor_sync(FULL, wend, o));
+        real s = real(0), sA = real(0), sB = real(0);
+        for (int i = 0; i <= wend; i += 4) {
+            real v[4];
+            load4(base + i, v);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                s = v[e] - R * s;
+                if (i + e == iA) sA = s;
+                if (i + e == iB) sB = s;
+            }
+        }
+        if (act) {
+            real g = ((useA ? (real)lc.wA * sA : real(0)) + (useB ? (real)lc.wB * sB : real(0))) / D;
+            uint32_t w = lw[j];
+            scratch[(size_t)sw[j] * Bp + b] = (w >> 31) ? -g : g;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Variable pass: thread = (variable, restart).  Fuses
+//   S1-S3,S5 for the PULL class (leave-one-out products recomputed per occurrence: no scratch, no atomics),
+//   S6   deterministic segmented reduction of the materialised gradients over the transposed CSR (fixed order),
+//   S7-S8 step, clip, fixed-variable mask,
+//   S9   sign bits of X_t (ballot) and the satisfied count of the clauses this variable owns,
+//   S10  merge of the previous iterate into the best-so-far (its count is complete once the previous launch ended).
+// EVAL = true is afs_eval_grad: writes G^T and per-warp objective partial sums instead of stepping.
+// ------------------------------------------------------------------------------------------------------------------
+template <typename real>
+struct VarArgs {
+    int n, Bp, t;
+    const int32_t* pull_ptr;
+    const uint32_t* pull_words;
+    const int32_t* slot_ptr;
+    const real* scratch;
+    const real* Xin;
+    real* Xout;
+    real lr;
+    const int8_t* mask;
+    int32_t* sat_cur;
+    const int32_t* sat_prev;
+    const int32_t* best_sat_in;
+    int32_t* best_sat_out;
+    const int32_t* best_step_in;
+    int32_t* best_step_out;
+    const uint32_t* S_prev;
+    uint32_t* S_cur;
+    uint32_t* best_bits;
+    real* GT;
+    real* Fpart;
+};
+
+template <typename real, bool EVAL>
+__global__ void __launch_bounds__(VAR_WARPS * 32) k_var(const VarArgs<real> a)
+{
+    __shared__ int s_sat[VAR_WARPS][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int tile = blockIdx.y, ntile = a.Bp >> 5;
+    const int b = tile * 32 + lane;
+    const int Bp = a.Bp;
+    const real half = real(0.5), one = real(1);
+    int satcnt = 0;
+    real fpart = real(0);
+    const int vbeg = (blockIdx.x * VAR_WARPS + warp) * VAR_VPW;
+    const int vend = min(vbeg + VAR_VPW, a.n);
+    // ---- S10: did the previous iterate improve on the best so far?
+    bool imp = false;
+    unsigned impmask = 0;
+    int sprev = 0;
+    if (!EVAL && a.t > 0) {
+        sprev = a.sat_prev[b];
+        imp = sprev > a.best_sat_in[b];
+        impmask = __ballot_sync(FULL, imp);
+    }
+    for (int v = vbeg; v < vend; ++v) {
+        if (!EVAL) {
+            if (impmask && lane == 0) {
+                size_t wi = (size_t)v * ntile + tile;
+                a.best_bits[wi] = (a.best_bits[wi] & ~impmask) | (a.S_prev[wi] & impmask);
+            }
+            if (v == 0) {
+                int bs = a.best_sat_in[b], st = a.best_step_in[b];
+                a.best_sat_out[b] = imp ? sprev : bs;
+                a.best_step_out[b] = imp ? a.t - 1 : st;
+            }
+        }
+        const real x = a.Xin[(size_t)v * Bp + b];
+        const bool xtrue = x < real(0);
+        int mk = 0;
+        if (!EVAL) {
+            unsigned sb = __ballot_sync(FULL, xtrue);
+            if (lane == 0) a.S_cur[(size_t)v * ntile + tile] = sb;
+            mk = a.mask ? a.mask[v] : 0;
+        }
+        real g = real(0);
+        // ---- PULL occurrences of v
+        int pos = a.pull_ptr[v];
+        const int pend = a.pull_ptr[v + 1];
+        while (pos < pend) {
+            const uint32_t hdr = a.pull_words[pos++];
+            const int kind = hdr & 3, nother = (hdr >> 2) & 7;
+            const bool ownneg = (hdr & 32u) != 0, owner = (hdr & 64u) != 0;
+            if (mk != 0 && !owner) { pos += nother; continue; }   // fixed variable: its gradient is never used
+            int tcount = (xtrue != ownneg) ? 1 : 0;
+            const real yown = ownneg ? -x : x;
+            if (kind == (int)PH_KIND_OR) {
+                real prod = one;
+                for (int i = 0; i < nother; ++i) {
+                    uint32_t w = a.pull_words[pos++];
+                    real xo = ldx(a.Xin, w, Bp, b);
+                    bool neg = (w >> 31) != 0;
+                    tcount += ((xo < real(0)) != neg) ? 1 : 0;
+                    prod *= half + half * (neg ? -xo : xo);
+                }
+                g += ownneg ? -prod : prod;
+                if (owner) {
+                    satcnt += tcount >= 1 ? 1 : 0;
+                    if (EVAL) fpart += real(2) * prod * (half + half * yown) - one;
+                }
+            } else if (kind == (int)PH_KIND_XOR) {
+                real prod = (hdr & 128u) ? one : -one;
+                for (int i = 0; i < nother; ++i) {
+                    uint32_t w = a.pull_words[pos++];
+                    real xo = ldx(a.Xin, w, Bp, b);
+                    bool neg = (w >> 31) != 0;
+                    tcount += ((xo < real(0)) != neg) ? 1 : 0;
+                    prod *= neg ? -xo : xo;
+                }
+                g += ownneg ? -prod : prod;
+                if (owner) {
+                    satcnt += ((tcount & 1) == (int)((hdr >> 7) & 1)) ? 1 : 0;
+                    if (EVAL) fpart += prod * yown;
+                }
+            } else {   // NAE
+                real pu = one, pp = one;
+                for (int i = 0; i < nother; ++i) {
+                    uint32_t w = a.pull_words[pos++];
+                    real xo = ldx(a.Xin, w, Bp, b);
+                    bool neg = (w >> 31) != 0;
+                    tcount += ((xo < real(0)) != neg) ? 1 : 0;
+                    real yo = neg ? -xo : xo;
+                    pu *= half + half * yo;
+                    pp *= half - half * yo;
+                }
+                real d = pu - pp;
+                g += ownneg ? -d : d;
+                if (owner) {
+                    satcnt += (tcount > 0 && tcount < nother + 1) ? 1 : 0;
+                    if (EVAL) fpart += real(2) * pu * (half + half * yown) + real(2) * pp * (half - half * yown) - one;
+                }
+            }
+        }
+        // ---- S6: materialised gradients of v, fixed (transposed-CSR) order
+        if (mk == 0) {
+            const int s1 = a.slot_ptr[v + 1];
+            for (int s = a.slot_ptr[v]; s < s1; ++s) g += a.scratch[(size_t)s * Bp + b];
+        }
+        if (EVAL) {
+            a.GT[(size_t)v * Bp + b] = g;
+        } else {
+            // ---- S7-S8
+            real xn = x - a.lr * g;
+            xn = xn > one ? one : xn;
+            xn = xn < -one ? -one : xn;
+            if (mk != 0) xn = x;
+            a.Xout[(size_t)v * Bp + b] = xn;
+        }
+    }
+    if (EVAL) {
+        a.Fpart[(size_t)(blockIdx.x * VAR_WARPS + warp) * Bp + b] = fpart;
+    } else {
+        s_sat[warp][lane] = satcnt;
+        __syncthreads();
+        if (warp == 0) {
+            int tot = 0;
+#pragma unroll
+            for (int w = 0; w < VAR_WARPS; ++w) tot += s_sat[w][lane];
+            if (tot) atomicAdd(&a.sat_cur[b], tot);
+        }
+    }
+}
+
+// F[b] = sum of the variable-pass partials, then the medium, then the long expansions -- fixed order, fp64 accumulator
+template <typename real>
+__global__ void k_reduce_F(const real* __restrict__ Fpart, int nparts, const real* __restrict__ fe_med, int n_med,
+                           const real* __restrict__ fe_long, int n_long, int Bp, int B, real* __restrict__ F)
+{
+    int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    double acc = 0.0;
+    for (int i = 0; i < nparts; ++i) acc += (double)Fpart[(size_t)i * Bp + b];
+    for (int i = 0; i < n_med; ++i) acc += (double)fe_med[(size_t)i * Bp + b];
+    for (int i = 0; i < n_long; ++i) acc += (double)fe_long[(size_t)i * Bp + b];
+    F[b] = (real)acc;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// End of afs_pgd_run: fold the last two iterates into the best-so-far, then write everything in the caller's
+// layout: X[B,n], best_assign int8[B,n], best_sat[B], best_step[B].
+// ------------------------------------------------------------------------------------------------------------------
+template <typename real>
+struct FinArgs {
+    int n, B, Bp, steps;
+    const real* XT;               // X_steps
+    const int32_t* sat_prev;      // counts of X_{steps-1} (unused when steps == 0)
+    const int32_t* sat_fin;       // counts of X_steps
+    const int32_t* best_sat_in;   // best over iterates 0..steps-2
+    const int32_t* best_step_in;
+    const uint32_t* S_prev;       // sign bits of X_{steps-1}
+    const uint32_t* best_bits;
+    real* X;
+    int8_t* best_assign;
+    int32_t* best_sat;
+    int32_t* best_step;
+};
+
+template <typename real>
+__global__ void __launch_bounds__(256) k_finalize(const FinArgs<real> a)
+{
+    __shared__ real tile[32][33];
+    __shared__ unsigned s_bits[32];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int v0 = blockIdx.x * 32, tileb = blockIdx.y, b0 = tileb * 32, ntile = a.Bp >> 5;
+    const int b = b0 + tx;
+    int best = a.best_sat_in[b], bstep = a.best_step_in[b];
+    bool imp1 = false;
+    if (a.steps >= 1) {
+        int sp = a.sat_prev[b];
+        imp1 = sp > best;
+        if (imp1) { best = sp; bstep = a.steps - 1; }
+    }
+    const unsigned m1 = __ballot_sync(FULL, imp1);
+    const int sf = a.sat_fin[b];
+    const bool imp2 = sf > best;
+    if (imp2) { best = sf; bstep = a.steps; }
+    const unsigned m2 = __ballot_sync(FULL, imp2);
+    for (int r = ty; r < 32; r += 8) {
+        int v = v0 + r;
+        real x = real(0);
+        unsigned bits = 0;
+        if (v < a.n) {
+            x = a.XT[(size_t)v * a.Bp + b];
+            size_t wi = (size_t)v * ntile + tileb;
+            bits = a.best_bits[wi];
+            if (m1) bits = (bits & ~m1) | (a.S_prev[wi] & m1);
+        }
+        unsigned fb = __ballot_sync(FULL, x < real(0));
+        bits = (bits & ~m2) | (fb & m2);
+        tile[r][tx] = x;
+        if (tx == 0) s_bits[r] = bits;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        int bb = b0 + r, v = v0 + tx;
+        if (bb < a.B && v < a.n) {
+            if (a.X) a.X[(size_t)bb * a.n + v] = tile[tx][r];
+            if (a.best_assign) a.best_assign[(size_t)bb * a.n + v] = ((s_bits[tx] >> r) & 1u) ? -1 : 1;
+        }
+    }
+    if (blockIdx.x == 0 && ty == 0 && b < a.B) {
+        if (a.best_sat) a.best_sat[b] = best;
+        if (a.best_step) a.best_step[b] = bstep;
+    }
+}
+
+__global__ void k_fill_i32(int32_t* p, size_t n, int32_t v)
+{
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = v;
+}
+
+}  // namespace afs

@@ -1,0 +1,349 @@
+// afs_run.cu -- workspace management, launch orchestration and the device entry points of include/afs.h.
+// Streaming path: per PGD step one launch per non-empty push bucket (medium / long constraints) plus one fused
+// variable pass; no host round trip inside the loop (everything is enqueued on the caller's stream).
+#include <cmath>
+#include <cstdio>
+
+#include "afs_kernels.cuh"
+
+using namespace afs;
+
+#define CU(x)                                \
+    do {                                     \
+        cudaError_t e_ = (x);                \
+        if (e_ != cudaSuccess) {             \
+            (void)cudaGetLastError();        \
+            return AFS_ERR_CUDA;             \
+        }                                    \
+    } while (0)
+
+namespace afs {
+
+static void free_ptr(void*& p) { if (p) cudaFree(p); p = nullptr; }
+template <typename T> static void free_ptr(T*& p) { if (p) cudaFree(p); p = nullptr; }
+
+void free_workspace(afs_problem* P)
+{
+    Workspace& w = P->ws;
+    free_ptr(w.XT[0]); free_ptr(w.XT[1]); free_ptr(w.scratch);
+    free_ptr(w.sat_hist); free_ptr(w.best_sat[0]); free_ptr(w.best_sat[1]);
+    free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.best_bits);
+    free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.f_part);
+    free_ptr(w.mask_dev); free_ptr(w.host_stage_X); free_ptr(w.host_stage_assign);
+    free_ptr(w.host_stage_sat); free_ptr(w.host_stage_step);
+    w = Workspace();
+}
+
+}  // namespace afs
+
+static int var_grid_x(int n) { return (n + VAR_WARPS * VAR_VPW - 1) / (VAR_WARPS * VAR_VPW); }
+
+template <typename T>
+static afs_status dev_alloc(T** p, size_t count, size_t& total)
+{
+    size_t bytes = (count ? count : 1) * sizeof(T);
+    if (cudaMalloc((void**)p, bytes) != cudaSuccess) { (void)cudaGetLastError(); *p = nullptr; return AFS_ERR_ALLOC; }
+    total += bytes;
+    return AFS_OK;
+}
+
+// (re)allocate the core workspace for padded batch Bp, element size `elem`, and `sat_rows` count rows
+static afs_status ensure_workspace(afs_problem* P, int Bp, size_t elem, int64_t sat_rows)
+{
+    Workspace& w = P->ws;
+    if (w.Bp >= Bp && w.elem >= elem && w.sat_rows >= sat_rows) return AFS_OK;
+    int nBp = Bp > w.Bp ? Bp : w.Bp;
+    size_t nelem = elem > w.elem ? elem : w.elem;
+    int64_t nrows = sat_rows > w.sat_rows ? sat_rows : w.sat_rows;
+    CU(cudaDeviceSynchronize());
+    afs::free_workspace(P);
+    size_t tot = 0;
+    afs_status st = AFS_OK;
+    auto A = [&](auto** p, size_t cnt) { if (st == AFS_OK) st = dev_alloc(p, cnt, tot); };
+    const size_t n = (size_t)P->n, ntile = (size_t)nBp / 32;
+    A((unsigned char**)&w.XT[0], n * nBp * nelem);
+    A((unsigned char**)&w.XT[1], n * nBp * nelem);
+    A((unsigned char**)&w.scratch, (size_t)P->nslots * nBp * nelem);
+    A(&w.sat_hist, (size_t)nrows * nBp);
+    A(&w.best_sat[0], (size_t)nBp); A(&w.best_sat[1], (size_t)nBp);
+    A(&w.best_step[0], (size_t)nBp); A(&w.best_step[1], (size_t)nBp);
+    A(&w.S[0], n * ntile); A(&w.S[1], n * ntile); A(&w.best_bits, n * ntile);
+    if (st != AFS_OK) { afs::free_workspace(P); return st; }
+    w.Bp = nBp; w.elem = nelem; w.sat_rows = nrows; w.bytes = tot;
+    return AFS_OK;
+}
+
+static afs_status ensure_eval_buffers(afs_problem* P, int Bp, size_t elem)
+{
+    Workspace& w = P->ws;
+    if (w.fe_Bp >= Bp && w.fe_med) return AFS_OK;
+    CU(cudaDeviceSynchronize());
+    free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.f_part);
+    size_t tot = 0;
+    afs_status st = AFS_OK;
+    auto A = [&](auto** p, size_t cnt) { if (st == AFS_OK) st = dev_alloc(p, cnt, tot); };
+    size_t e = w.elem > elem ? w.elem : elem;
+    A((unsigned char**)&w.fe_med, (size_t)P->n_med * w.Bp * e);
+    A((unsigned char**)&w.fe_long, (size_t)P->n_long * w.Bp * e);
+    A((unsigned char**)&w.f_part, (size_t)var_grid_x(P->n) * VAR_WARPS * w.Bp * e);
+    if (st != AFS_OK) return st;
+    w.fe_Bp = w.Bp; w.bytes += tot;
+    return AFS_OK;
+}
+
+// ----------------------------------------------------------------------------------------------------------------
+// push phase: gradients of the medium and long constraints of iterate XT into scratch (+ counts, + FE)
+// ----------------------------------------------------------------------------------------------------------------
+template <typename real, int NR>
+static afs_status launch_long(afs_problem* P, int bucket, const real* XT, int Bp, real* scratch, int32_t* sat, real* fe,
+                              cudaStream_t st)
+{
+    int c0 = P->long_begin[bucket], c1 = P->long_begin[bucket + 1];
+    if (c1 <= c0) return AFS_OK;
+    int Lmax = P->long_maxL[bucket];
+    int LS = ((Lmax + 31) / 32) * 32 + 4;
+    int QS = ((Lmax + 1 + 3) / 4) * 4 + 4;
+    size_t smem = (size_t)(8 * LS + 16 * QS) * sizeof(real);
+    static bool attr_set[2][LONG_BUCKETS] = {};
+    const int ti = sizeof(real) == 8 ? 1 : 0;
+    if (smem > 48 * 1024 && !attr_set[ti][bucket]) {
+        CU(cudaFuncSetAttribute(k_long<real, NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        attr_set[ti][bucket] = true;
+    }
+    if (smem > 227 * 1024) return AFS_ERR_UNSUPPORTED;
+    long long blocks = (long long)(c1 - c0) * (Bp / 8);
+    if (blocks > 0x7fffffffLL) return AFS_ERR_UNSUPPORTED;
+    k_long<real, NR><<<(unsigned)blocks, 256, smem, st>>>(P->d_long, c0, P->d_long_lits, P->d_long_slots, XT, Bp,
+                                                          scratch, sat, fe, LS, QS);
+    P->last_launches++;
+    return AFS_OK;
+}
+
+template <typename real>
+static afs_status launch_push(afs_problem* P, const real* XT, int Bp, real* scratch, int32_t* sat, real* fe_med,
+                              real* fe_long, cudaStream_t st)
+{
+    const int tiles = Bp / 32;
+    for (int bk = 0; bk < MED_BUCKETS; ++bk) {
+        int c0 = P->med_begin[bk], c1 = P->med_begin[bk + 1];
+        if (c1 <= c0) continue;
+        int gx = (c1 - c0 + 3) / 4;
+        int cap = (P->sm_count * 16 + tiles - 1) / tiles;   // enough CTAs to fill the chip, grid-stride beyond
+        if (gx > cap) gx = cap < 1 ? 1 : cap;
+        dim3 grid(gx, tiles);
+        switch (bk) {
+        case 0: k_med<real, 8><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
+        case 1: k_med<real, 16><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
+        case 2: k_med<real, 32><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
+        case 3: k_med<real, 64><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
+        default: k_prod_long<real><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
+        }
+        P->last_launches++;
+    }
+    afs_status s = AFS_OK;
+#define LONG_CASE(NRV) if (s == AFS_OK) s = launch_long<real, NRV>(P, NRV - 1, XT, Bp, scratch, sat, fe_long, st);
+    LONG_CASE(1) LONG_CASE(2) LONG_CASE(3) LONG_CASE(4) LONG_CASE(5) LONG_CASE(6) LONG_CASE(7) LONG_CASE(8) LONG_CASE(9)
+#undef LONG_CASE
+    return s;
+}
+
+template <typename real>
+static afs_status launch_count(afs_problem* P, const real* XT, int Bp, int32_t* sat, cudaStream_t st)
+{
+    CU(cudaMemsetAsync(sat, 0, (size_t)Bp * sizeof(int32_t), st));
+    if (P->m > 0) {
+        const int tiles = Bp / 32;
+        int gx = (P->m + 7) / 8;
+        int cap = (P->sm_count * 8 + tiles - 1) / tiles;
+        if (gx > cap) gx = cap < 1 ? 1 : cap;
+        k_count<real><<<dim3(gx, tiles), 256, 0, st>>>(P->d_count, P->d_count_lits, P->m, XT, Bp, sat);
+        P->last_launches++;
+    }
+    return AFS_OK;
+}
+
+static afs_status enter(afs_problem* P, int32_t B)
+{
+    if (!P || B < 1) return AFS_ERR_INVALID_ARG;
+    if (cudaSetDevice(P->device) != cudaSuccess) { (void)cudaGetLastError(); return AFS_ERR_CUDA; }
+    P->last_launches = 0;
+    return AFS_OK;
+}
+
+// ----------------------------------------------------------------------------------------------------------------
+template <typename real>
+static afs_status eval_grad_impl(afs_problem* P, const real* X, int32_t B, real* F, real* G, void* stream)
+{
+    afs_status s = enter(P, B);
+    if (s != AFS_OK) return s;
+    if (!X) return AFS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int Bp = ((B + 31) / 32) * 32;
+    if ((s = ensure_workspace(P, Bp, sizeof(real), 2)) != AFS_OK) return s;
+    if ((s = ensure_eval_buffers(P, Bp, sizeof(real))) != AFS_OK) return s;
+    Workspace& w = P->ws;
+    const int wBp = Bp;   // kernels run on the first Bp columns with row stride Bp
+    real* XT = (real*)w.XT[0];
+    real* GT = (real*)w.XT[1];
+    real* scratch = (real*)w.scratch;
+    real* fe_med = (real*)w.fe_med; real* fe_long = (real*)w.fe_long; real* fpart = (real*)w.f_part;
+    dim3 tg((P->n + 31) / 32, Bp / 32);
+    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, wBp, nullptr);
+    P->last_launches++;
+    if ((s = launch_push<real>(P, XT, wBp, scratch, nullptr, fe_med, fe_long, st)) != AFS_OK) return s;
+    VarArgs<real> a{};
+    a.n = P->n; a.Bp = wBp; a.t = 0;
+    a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.slot_ptr = P->d_slot_ptr;
+    a.scratch = scratch; a.Xin = XT; a.Xout = nullptr; a.lr = real(0); a.mask = nullptr;
+    a.GT = GT; a.Fpart = fpart;
+    const int gx = var_grid_x(P->n);
+    k_var<real, true><<<dim3(gx, Bp / 32), VAR_WARPS * 32, 0, st>>>(a);
+    P->last_launches++;
+    if (F) {
+        k_reduce_F<real><<<(B + 127) / 128, 128, 0, st>>>(fpart, gx * VAR_WARPS, fe_med, (int)P->n_med, fe_long,
+                                                         (int)P->n_long, wBp, B, F);
+        P->last_launches++;
+    }
+    if (G) {
+        k_transpose_out<real><<<tg, 256, 0, st>>>(GT, G, B, P->n, wBp);
+        P->last_launches++;
+    }
+    CU(cudaGetLastError());
+    return AFS_OK;
+}
+
+template <typename real>
+static afs_status round_count_impl(afs_problem* P, const real* X, int32_t B, int8_t* assign, int32_t* sat, void* stream)
+{
+    afs_status s = enter(P, B);
+    if (s != AFS_OK) return s;
+    if (!X || !sat) return AFS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int Bp = ((B + 31) / 32) * 32;
+    if ((s = ensure_workspace(P, Bp, sizeof(real), 2)) != AFS_OK) return s;
+    Workspace& w = P->ws;
+    real* XT = (real*)w.XT[0];
+    dim3 tg((P->n + 31) / 32, Bp / 32);
+    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, Bp, nullptr);
+    P->last_launches++;
+    if ((s = launch_count<real>(P, XT, Bp, w.sat_hist, st)) != AFS_OK) return s;
+    CU(cudaMemcpyAsync(sat, w.sat_hist, (size_t)B * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    if (assign) {
+        k_assign_out<real><<<tg, 256, 0, st>>>(XT, assign, B, P->n, Bp);
+        P->last_launches++;
+    }
+    CU(cudaGetLastError());
+    return AFS_OK;
+}
+
+template <typename real>
+static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps, real lr, const int8_t* mask,
+                               int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
+{
+    afs_status s = enter(P, B);
+    if (s != AFS_OK) return s;
+    if (!X || steps < 0 || !std::isfinite((double)lr)) return AFS_ERR_INVALID_ARG;
+    if (P->opt_mode == 2) return AFS_ERR_UNSUPPORTED;   // tile-resident path not built yet
+    cudaStream_t st = (cudaStream_t)stream;
+    const int Bp = ((B + 31) / 32) * 32;
+    if ((s = ensure_workspace(P, Bp, sizeof(real), (int64_t)steps + 1)) != AFS_OK) return s;
+    Workspace& w = P->ws;
+    P->last_resident = 0;
+    real* XT[2] = {(real*)w.XT[0], (real*)w.XT[1]};
+    real* scratch = (real*)w.scratch;
+    const int tiles = Bp / 32;
+    dim3 tg((P->n + 31) / 32, tiles);
+    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT[0], B, P->n, Bp, mask);
+    P->last_launches++;
+    CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)(steps + 1) * Bp * sizeof(int32_t), st));
+    k_fill_i32<<<(Bp + 255) / 256, 256, 0, st>>>(w.best_sat[0], (size_t)Bp, -1);
+    CU(cudaMemsetAsync(w.best_step[0], 0, (size_t)Bp * sizeof(int32_t), st));
+    P->last_launches++;
+    const int gx = var_grid_x(P->n);
+    for (int t = 0; t < steps; ++t) {
+        const real* Xin = XT[t & 1];
+        int32_t* sat_cur = w.sat_hist + (size_t)t * Bp;
+        if ((s = launch_push<real>(P, Xin, Bp, scratch, sat_cur, nullptr, nullptr, st)) != AFS_OK) return s;
+        VarArgs<real> a{};
+        a.n = P->n; a.Bp = Bp; a.t = t;
+        a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.slot_ptr = P->d_slot_ptr;
+        a.scratch = scratch; a.Xin = Xin; a.Xout = XT[(t + 1) & 1]; a.lr = lr; a.mask = mask;
+        a.sat_cur = sat_cur; a.sat_prev = t > 0 ? w.sat_hist + (size_t)(t - 1) * Bp : nullptr;
+        a.best_sat_in = w.best_sat[t & 1]; a.best_sat_out = w.best_sat[(t + 1) & 1];
+        a.best_step_in = w.best_step[t & 1]; a.best_step_out = w.best_step[(t + 1) & 1];
+        a.S_prev = w.S[(t + 1) & 1]; a.S_cur = w.S[t & 1]; a.best_bits = w.best_bits;
+        k_var<real, false><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
+        P->last_launches++;
+    }
+    // the last iterate: count only, then fold and write out
+    const real* Xfin = XT[steps & 1];
+    int32_t* sat_fin = w.sat_hist + (size_t)steps * Bp;
+    if ((s = launch_count<real>(P, Xfin, Bp, sat_fin, st)) != AFS_OK) return s;
+    FinArgs<real> f{};
+    f.n = P->n; f.B = B; f.Bp = Bp; f.steps = steps; f.XT = Xfin;
+    f.sat_prev = steps >= 1 ? w.sat_hist + (size_t)(steps - 1) * Bp : nullptr;
+    f.sat_fin = sat_fin;
+    f.best_sat_in = w.best_sat[steps & 1]; f.best_step_in = w.best_step[steps & 1];
+    f.S_prev = w.S[(steps + 1) & 1]; f.best_bits = w.best_bits;
+    f.X = X; f.best_assign = best_assign; f.best_sat = best_sat; f.best_step = best_step;
+    k_finalize<real><<<tg, 256, 0, st>>>(f);
+    P->last_launches++;
+    CU(cudaGetLastError());
+    return AFS_OK;
+}
+
+// ----------------------------------------------------------------------------------------------------------------
+extern "C" afs_status afs_eval_grad(afs_problem* p, const float* X, int32_t B, float* F, float* G, void* stream)
+{ return eval_grad_impl<float>(p, X, B, F, G, stream); }
+extern "C" afs_status afs_eval_grad_f64(afs_problem* p, const double* X, int32_t B, double* F, double* G, void* stream)
+{ return eval_grad_impl<double>(p, X, B, F, G, stream); }
+extern "C" afs_status afs_round_count(afs_problem* p, const float* X, int32_t B, int8_t* assign, int32_t* sat, void* stream)
+{ return round_count_impl<float>(p, X, B, assign, sat, stream); }
+extern "C" afs_status afs_round_count_f64(afs_problem* p, const double* X, int32_t B, int8_t* assign, int32_t* sat, void* stream)
+{ return round_count_impl<double>(p, X, B, assign, sat, stream); }
+extern "C" afs_status afs_pgd_run(afs_problem* p, float* X, int32_t B, int32_t steps, float lr, const int8_t* mask,
+                                  int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
+{ return pgd_run_impl<float>(p, X, B, steps, lr, mask, best_assign, best_sat, best_step, stream); }
+extern "C" afs_status afs_pgd_run_f64(afs_problem* p, double* X, int32_t B, int32_t steps, double lr, const int8_t* mask,
+                                      int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
+{ return pgd_run_impl<double>(p, X, B, steps, lr, mask, best_assign, best_sat, best_step, stream); }
+
+extern "C" afs_status afs_pgd_run_host(afs_problem* P, float* X, int32_t B, int32_t steps, float lr, const int8_t* mask,
+                                       int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
+{
+    afs_status s = enter(P, B);
+    if (s != AFS_OK) return s;
+    if (!X) return AFS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    Workspace& w = P->ws;
+    const size_t n = (size_t)P->n;
+    // the core workspace first: growing it later would free these staging buffers
+    if ((s = ensure_workspace(P, ((B + 31) / 32) * 32, sizeof(float), (int64_t)steps + 1)) != AFS_OK) return s;
+    if (w.host_stage_B < B) {
+        CU(cudaDeviceSynchronize());
+        free_ptr(w.mask_dev); free_ptr(w.host_stage_X); free_ptr(w.host_stage_assign);
+        free_ptr(w.host_stage_sat); free_ptr(w.host_stage_step);
+        size_t tot = 0;
+        afs_status a = AFS_OK;
+        auto A = [&](auto** p, size_t cnt) { if (a == AFS_OK) a = dev_alloc(p, cnt, tot); };
+        A(&w.mask_dev, n);
+        A((float**)&w.host_stage_X, n * B);
+        A(&w.host_stage_assign, n * B);
+        A(&w.host_stage_sat, (size_t)B);
+        A(&w.host_stage_step, (size_t)B);
+        if (a != AFS_OK) return a;
+        w.host_stage_B = B; w.bytes += tot;
+    }
+    float* dX = (float*)w.host_stage_X;
+    CU(cudaMemcpyAsync(dX, X, n * B * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (mask) CU(cudaMemcpyAsync(w.mask_dev, mask, n, cudaMemcpyHostToDevice, st));
+    s = pgd_run_impl<float>(P, dX, B, steps, lr, mask ? w.mask_dev : nullptr, w.host_stage_assign, w.host_stage_sat,
+                            w.host_stage_step, stream);
+    if (s != AFS_OK) return s;
+    CU(cudaMemcpyAsync(X, dX, n * B * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (best_assign) CU(cudaMemcpyAsync(best_assign, w.host_stage_assign, n * B, cudaMemcpyDeviceToHost, st));
+    if (best_sat) CU(cudaMemcpyAsync(best_sat, w.host_stage_sat, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
+    if (best_step) CU(cudaMemcpyAsync(best_step, w.host_stage_step, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return AFS_OK;
+}

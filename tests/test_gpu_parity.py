@@ -1,0 +1,391 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json's: satisfied counts and rounded assignments bit-exact; fp32 objective
+within 1e-4 relative (+1e-6 m absolute, reading G17); gradients within 1e-4 max|grad| per restart (G18); fp64 build
+trajectories within 1e-3 over 20 steps (expected ~1e-12)."""
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import ref
+
+pytestmark = pytest.mark.gpu
+
+LR = float(np.float32(0.1))
+
+
+@pytest.fixture(scope="module")
+def afs():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (run with -m 'not gpu' on CPU boxes)")
+    from paper_2606_06656_b200 import build
+    build.build()
+    import paper_2606_06656_b200 as pkg
+    return pkg
+
+
+def dev(a, dtype=None):
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+# ------------------------------------------------------------------------------------------------ cases
+def case_cnf(B=70):      # configs[0]/[3] shape, several variable chunks, ragged restart tail
+    return W.planted_kcnf(101, n=300, m=1260).with_run(None, B, 20)
+
+
+def case_random_cnf(B=64):
+    return W.random_kcnf(102, n=50, m=213).with_run(None, B, 20)
+
+
+def case_mixed(B=45):    # configs[1] shape plus NAE and EK so that all seven types appear
+    return W.mixed_pb(103, n=200, n_or=600, n_xor=40, n_eo=20, n_amo=20, n_card=12, n_nae=25, n_ek=8,
+                      nae_len=(2, 9), ek_len=(3, 30)).with_run(None, B, 20)
+
+
+def case_xor(B=96):      # configs[2] shape
+    return W.xor_dup(104, n=200, m=180).with_run(None, B, 20)
+
+
+def case_long(B=13):     # configs[4] shape: clauses + long CARD/EK + mask; lengths straddle the 128-cell rows
+    return W.long_pb(105, n=700, n_clauses=900, n_card=7, n_ek=4, long_len=(100, 420)).with_run(None, B, 20)
+
+
+def case_all_lengths(B=33):
+    """every type at lengths that exercise every kernel bucket (pull, 8/16/32/64 padded, two-pass, long rows)"""
+    rng = np.random.default_rng(7)
+    n = 400
+    rows, types, ks = [], [], []
+    def add(ty, L, k=0):
+        v = rng.choice(n, size=L, replace=False)
+        s = 1 - 2 * rng.integers(0, 2, size=L)
+        rows.append((s * (v + 1)).astype(np.int32)); types.append(ty); ks.append(k)
+    for L in (1, 2, 3, 5, 6, 8, 9, 16, 17, 32, 33, 64, 65, 130, 300):
+        add(W.AFS_OR, L); add(W.AFS_XOR, L, int(rng.integers(0, 2)))
+    for L in (2, 3, 5, 6, 8, 9, 16, 31, 32, 33, 70, 127, 128, 129, 255, 256, 300):
+        add(W.AFS_NAE, L); add(W.AFS_EO, L); add(W.AFS_AMO, L)
+        for k in sorted({0, 1, L // 3, L // 2, L - 1, L, L + 1}):
+            add(W.AFS_CARD, L, k); add(W.AFS_EK, L, k)
+    add(W.AFS_EO, 1); add(W.AFS_AMO, 1); add(W.AFS_CARD, 1, 1); add(W.AFS_EK, 1, 0)
+    inst = W.generate._pack("all_lengths", n, rows, types, ks, None, 7)
+    inst.with_run(rng, B, 10)
+    return inst
+
+
+CASES = {"cnf": case_cnf, "random_cnf": case_random_cnf, "mixed": case_mixed, "xor": case_xor, "long": case_long,
+         "all_lengths": case_all_lengths}
+
+
+def check_eval(afs, inst, X32, f64=False, sample=None):
+    import torch
+    P = afs.Problem.from_instance(inst)
+    X = dev(X32, torch.float64 if f64 else torch.float32)
+    F, G = P.eval_grad(X)
+    torch.cuda.synchronize()
+    F, G = F.cpu().numpy().astype(np.float64), G.cpu().numpy().astype(np.float64)
+    idx = np.arange(X32.shape[0]) if sample is None else sample
+    Fo, Go = ref.eval_grad(inst, X32[idx].astype(np.float64), 2)
+    ftol = (1e-4 if not f64 else 1e-11) * np.abs(Fo) + (1e-6 if not f64 else 1e-12) * inst.m
+    assert np.all(np.abs(F[idx] - Fo) <= ftol), ("F", np.abs(F[idx] - Fo).max(), ftol.min())
+    gmax = np.abs(Go).max(axis=1, keepdims=True)
+    gtol = (1e-4 if not f64 else 1e-11) * np.maximum(gmax, 1e-30)
+    err = np.abs(G[idx] - Go)
+    assert np.all(err <= gtol), ("G", (err / gtol).max())
+    P.close()
+    return err.max(), gmax.max()
+
+
+# ------------------------------------------------------------------------------------------------ eval_grad
+@pytest.mark.parametrize("name", list(CASES))
+def test_eval_grad_fp32_parity(afs, name):
+    inst = CASES[name]()
+    check_eval(afs, inst, inst.X0)
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_eval_grad_fp64_build_parity(afs, name):
+    inst = CASES[name]()
+    check_eval(afs, inst, inst.X0, f64=True)
+
+
+@pytest.mark.parametrize("name", ["mixed", "long", "all_lengths"])
+def test_eval_grad_at_clipped_points(afs, name):
+    # PGD iterates sit exactly on the faces x = +-1: leave-one-out must not divide by a vanishing factor
+    inst = CASES[name]()
+    rng = np.random.default_rng(5)
+    X = inst.X0.copy()
+    face = rng.random(X.shape) < 0.6
+    X[face] = np.sign(X[face])
+    X[0] = 1.0; X[1] = -1.0; X[2, ::2] = 0.0
+    check_eval(afs, inst, X)
+
+
+def sub_instance(inst, keep):
+    rows = [inst.lits[inst.row_ptr[c]:inst.row_ptr[c + 1]] for c in np.nonzero(keep)[0]]
+    return W.generate._pack("sub", inst.n, rows, inst.types[keep], inst.k[keep], None, 0)
+
+
+@pytest.mark.parametrize("name", ["mixed", "long", "all_lengths"])
+def test_eval_grad_per_bucket_subproblems(afs, name):
+    # G18 / H7: small-magnitude buckets must not hide behind O(1) clause gradients
+    inst = CASES[name]()
+    L = inst.lengths()
+    groups = {
+        "long": L > 64,
+        "card_ek": (inst.types == W.AFS_CARD) | (inst.types == W.AFS_EK),
+        "eo_amo_nae": (inst.types == W.AFS_EO) | (inst.types == W.AFS_AMO) | (inst.types == W.AFS_NAE),
+        "xor": inst.types == W.AFS_XOR,
+    }
+    for gname, keep in groups.items():
+        if keep.sum() == 0:
+            continue
+        sub = sub_instance(inst, keep)
+        check_eval(afs, sub, inst.X0[:9])
+
+
+# ------------------------------------------------------------------------------------------------ rounding + counts
+@pytest.mark.parametrize("name", list(CASES))
+def test_round_count_bit_exact(afs, name):
+    import torch
+    inst = CASES[name]()
+    X = inst.X0.copy()
+    X[0, :6] = [0.0, -0.0, 1.0, -1.0, 1e-30, -1e-30]          # G13
+    P = afs.Problem.from_instance(inst)
+    assign, sat = P.round_count(dev(X))
+    ao, so = ref.round_count(inst, X.astype(np.float64))
+    assert np.array_equal(assign.cpu().numpy(), ao) and np.array_equal(sat.cpu().numpy(), so)
+    a64, s64 = P.round_count(dev(X, torch.float64))
+    assert np.array_equal(a64.cpu().numpy(), ao) and np.array_equal(s64.cpu().numpy(), so)
+    # at Boolean corners too (every literal exactly +-1)
+    Xc = np.sign(inst.X0).astype(np.float32)
+    _, sat_c = P.round_count(dev(Xc), want_assign=False)
+    assert np.array_equal(sat_c.cpu().numpy(), ref.round_count(inst, Xc.astype(np.float64))[1])
+    P.close()
+
+
+# ------------------------------------------------------------------------------------------------ PGD
+@pytest.mark.parametrize("name", list(CASES))
+def test_pgd_fp64_build_trajectory_20_steps(afs, name):
+    import torch
+    inst = CASES[name]()
+    P = afs.Problem.from_instance(inst)
+    mask = None if inst.mask is None else dev(inst.mask)
+    orc = ref.pgd_run(inst, inst.X0, 20, LR, mask=inst.mask, want_traj=True)
+    for steps in (1, 7, 20):
+        X = dev(inst.X0, torch.float64)
+        out = P.pgd_run(X, steps, LR, mask=mask)
+        torch.cuda.synchronize()
+        d = np.abs(X.cpu().numpy() - orc["traj"][steps]).max()
+        assert d <= 1e-3, (steps, d)
+        assert d <= 1e-9, (steps, d)               # what the arithmetic actually delivers
+        # with matching trajectories the integer outputs must match the oracle's run exactly
+        o = ref.pgd_run(inst, inst.X0, steps, LR, mask=inst.mask)
+        assert np.array_equal(out["best_sat"].cpu().numpy(), o["best_sat"])
+        assert np.array_equal(out["best_step"].cpu().numpy(), o["best_step"])
+        assert np.array_equal(out["best_assign"].cpu().numpy(), o["best_assign"])
+    P.close()
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_pgd_fp32_one_step_and_invariants(afs, name):
+    import torch
+    inst = CASES[name]()
+    P = afs.Problem.from_instance(inst)
+    mask = None if inst.mask is None else dev(inst.mask)
+    # one step against the oracle's step: |dX| <= lr * 1e-4 max|grad| + rounding of x
+    X = dev(inst.X0)
+    P.pgd_run(X, 1, LR, mask=mask)
+    orc1 = ref.pgd_run(inst, inst.X0, 1, LR, mask=inst.mask, want_traj=True)
+    X0m = orc1["traj"][0]
+    _, Go = ref.eval_grad(inst, X0m, 2)
+    tol = LR * 1e-4 * np.abs(Go).max(axis=1, keepdims=True) + 2.5e-7
+    assert np.all(np.abs(X.cpu().numpy() - orc1["traj"][1]) <= tol)
+    # a 20-step run: properties that hold whatever the fp32 drift (G15)
+    X = dev(inst.X0)
+    out = P.pgd_run(X, 20, LR, mask=mask)
+    torch.cuda.synchronize()
+    Xf = X.cpu().numpy()
+    assert np.all(np.abs(Xf) <= 1.0)
+    if inst.mask is not None:
+        fixed = inst.mask != 0
+        assert np.array_equal(Xf[:, fixed], np.tile(inst.mask[fixed].astype(np.float32), (inst.B, 1)))
+    ba, bs, bt = (out[k].cpu().numpy() for k in ("best_assign", "best_sat", "best_step"))
+    assert set(np.unique(ba)) <= {-1, 1}
+    _, recount = ref.round_count(inst, ba.astype(np.float64))
+    assert np.array_equal(recount, bs)                                   # (i) oracle recount
+    _, sat0 = ref.round_count(inst, X0m)
+    assert np.all(bs >= sat0) and np.all((bt >= 0) & (bt <= 20))         # (ii)
+    # fp32 trajectory stays close to the oracle's over 20 steps on these small cases
+    orc = ref.pgd_run(inst, inst.X0, 20, LR, mask=inst.mask)
+    assert np.abs(Xf - orc["X"]).max() < 5e-3
+    P.close()
+
+
+@pytest.mark.parametrize("name", ["cnf", "mixed", "long"])
+def test_pgd_run_to_run_bit_reproducible_and_resumable(afs, name):
+    import torch
+    inst = CASES[name]()
+    P = afs.Problem.from_instance(inst)
+    mask = None if inst.mask is None else dev(inst.mask)
+    runs = []
+    for _ in range(2):
+        X = dev(inst.X0)
+        out = P.pgd_run(X, 12, LR, mask=mask)
+        torch.cuda.synchronize()
+        runs.append((X.cpu().numpy().copy(), {k: v.cpu().numpy().copy() for k, v in out.items() if k != "X"}))
+    assert np.array_equal(runs[0][0], runs[1][0])
+    for k in runs[0][1]:
+        assert np.array_equal(runs[0][1][k], runs[1][1][k])
+    # 12 steps == 5 steps then 7 steps on the returned X (G14/G15: X is caller-owned, a second call is resume)
+    X = dev(inst.X0)
+    a = P.pgd_run(X, 5, LR, mask=mask)
+    a_sat = a["best_sat"].cpu().numpy().copy()
+    b = P.pgd_run(X, 7, LR, mask=mask)
+    assert np.array_equal(X.cpu().numpy(), runs[0][0])
+    assert np.array_equal(np.maximum(a_sat, b["best_sat"].cpu().numpy()), runs[0][1]["best_sat"])
+    P.close()
+
+
+def test_pgd_per_iterate_counts_match_history(afs):
+    # best_sat / best_step equal max / first argmax of the per-iterate counts, obtained by single-step calls
+    import torch
+    inst = case_mixed(40)
+    P = afs.Problem.from_instance(inst)
+    X = dev(inst.X0)
+    hist = []
+    for t in range(9):
+        _, sat = P.round_count(X, want_assign=False)
+        hist.append(sat.cpu().numpy().copy())
+        P.pgd_run(X, 1, LR)
+    _, sat = P.round_count(X, want_assign=False)
+    hist.append(sat.cpu().numpy().copy())
+    hist = np.stack(hist)
+    X2 = dev(inst.X0)
+    out = P.pgd_run(X2, 9, LR)
+    assert np.array_equal(X2.cpu().numpy(), X.cpu().numpy())
+    assert np.array_equal(out["best_sat"].cpu().numpy(), hist.max(axis=0))
+    assert np.array_equal(out["best_step"].cpu().numpy(), hist.argmax(axis=0))
+    P.close()
+
+
+def test_host_entry_point_equals_device_entry_point(afs):
+    import torch
+    inst = case_long(10)
+    P = afs.Problem.from_instance(inst)
+    Xd = dev(inst.X0)
+    d = P.pgd_run(Xd, 6, LR, mask=dev(inst.mask))
+    Xh = torch.from_numpy(inst.X0.copy()).pin_memory()
+    h = P.pgd_run_host(Xh, 6, LR, mask=inst.mask)
+    assert np.array_equal(Xh.numpy(), Xd.cpu().numpy())
+    for k in ("best_assign", "best_sat", "best_step"):
+        assert np.array_equal(h[k].numpy(), d[k].cpu().numpy())
+    assert P.info("launches") > 0
+    P.close()
+
+
+# ------------------------------------------------------------------------------------------------ edge cases
+def test_edge_cases(afs):
+    import torch
+    # no constraints at all
+    empty = W.Instance("empty", 5, np.zeros(1, np.int64), np.zeros(0, np.int32), np.zeros(0, np.int32),
+                       np.zeros(0, np.int32))
+    P = afs.Problem.from_instance(empty)
+    X = dev(np.random.default_rng(0).uniform(-1, 1, (3, 5)).astype(np.float32))
+    X0 = X.clone()
+    F, G = P.eval_grad(X)
+    assert torch.all(F == 0) and torch.all(G == 0)
+    out = P.pgd_run(X, 4, LR)
+    assert torch.equal(X, X0) and torch.all(out["best_sat"] == 0) and torch.all(out["best_step"] == 0)
+    P.close()
+    # one variable, one unit clause, one restart
+    one = W.Instance("one", 1, np.array([0, 1], np.int64), np.array([-1], np.int32), np.array([W.AFS_OR], np.int32),
+                     np.zeros(1, np.int32))
+    P = afs.Problem.from_instance(one)
+    X = dev(np.array([[-0.25]], np.float32))
+    F, G = P.eval_grad(X)
+    assert abs(F.item() - 0.25) < 1e-7 and abs(G.item() + 1.0) < 1e-7          # FE = y = -x
+    out = P.pgd_run(X, 20, LR)
+    assert X.item() == 1.0 and out["best_sat"].item() == 1 and out["best_assign"].item() == 1
+    P.close()
+    # steps = 0 is rounding of X_0; an all-fixed mask keeps the plant and satisfies everything
+    inst = case_mixed(5)
+    P = afs.Problem.from_instance(inst)
+    X = dev(inst.X0)
+    out = P.pgd_run(X, 0, LR)
+    ao, so = ref.round_count(inst, inst.X0.astype(np.float64))
+    assert np.array_equal(out["best_assign"].cpu().numpy(), ao) and np.array_equal(out["best_sat"].cpu().numpy(), so)
+    assert np.array_equal(X.cpu().numpy(), inst.X0)
+    out = P.pgd_run(X, 3, LR, mask=dev(inst.plant))
+    assert torch.all(out["best_sat"] == inst.m) and torch.all(out["best_step"] == 0)
+    assert np.array_equal(X.cpu().numpy(), np.tile(inst.plant.astype(np.float32), (5, 1)))
+    # argument errors come back as status codes
+    with pytest.raises(afs.AfsError):
+        P.pgd_run(X, -1, LR)
+    with pytest.raises(afs.AfsError):
+        P.pgd_run(X, 1, float("nan"))
+    P.close()
+
+
+def test_duplicate_constraints_equal_doubled_step_fp64_build(afs):
+    # P:L110 / T11 through the CUDA path
+    import torch
+    base = W.xor_dup(9, n=64, m=50)
+    half = W.Instance("half", base.n, base.row_ptr[:51].copy(), base.lits[:150].copy(), base.types[:50].copy(),
+                      base.k[:50].copy())
+    X0 = np.random.default_rng(2).uniform(-1, 1, (33, 64))
+    Pa, Pb = afs.Problem.from_instance(base), afs.Problem.from_instance(half)
+    Xa, Xb = dev(X0), dev(X0)
+    Pa.pgd_run(Xa, 25, 0.05)
+    Pb.pgd_run(Xb, 25, 0.10)
+    assert (Xa - Xb).abs().max().item() < 1e-11
+    Pa.close(); Pb.close()
+
+
+# ------------------------------------------------------------------------------------------------ full BASELINE.json sizes
+FULL = {0: dict(sample=64, steps=200), 1: dict(sample=48, steps=500), 2: dict(sample=48, steps=1000),
+        3: dict(sample=24, steps=300), 4: dict(sample=4, steps=20)}
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+def test_full_size_configs_sampled_parity_and_properties(afs, cfg):
+    """At BASELINE.json's sizes, in the launch configuration bench.py times: objective / gradient parity on sampled
+    restarts (the oracle computes them one by one), counts bit-exact on all restarts, and the properties of
+    afs_pgd_run's outputs that hold at any size."""
+    import torch
+    inst = W.config(cfg)
+    spec = FULL[cfg]
+    P = afs.Problem.from_instance(inst)
+    rng = np.random.default_rng(cfg)
+    sample = np.sort(rng.choice(inst.B, size=min(spec["sample"], inst.B), replace=False))
+    check_eval(afs, inst, inst.X0, sample=sample)
+    _, sat0 = P.round_count(dev(inst.X0), want_assign=False)
+    so = ref.round_count(inst, inst.X0.astype(np.float64), want_assign=False)[1]
+    assert np.array_equal(sat0.cpu().numpy(), so)
+    mask = None if inst.mask is None else dev(inst.mask)
+    X = dev(inst.X0)
+    out = P.pgd_run(X, spec["steps"], LR, mask=mask)
+    torch.cuda.synchronize()
+    Xf = X.cpu().numpy()
+    assert np.all(np.abs(Xf) <= 1.0) and np.all(np.isfinite(Xf))
+    if inst.mask is not None:
+        fixed = inst.mask != 0
+        assert np.all(Xf[:, fixed] == inst.mask[fixed].astype(np.float32))
+    ba, bs, bt = (out[k].cpu().numpy() for k in ("best_assign", "best_sat", "best_step"))
+    _, recount = ref.round_count(inst, ba.astype(np.float64), want_assign=False)
+    assert np.array_equal(recount, bs)
+    X0m = inst.X0.astype(np.float64)
+    if inst.mask is not None:
+        X0m[:, fixed] = inst.mask[fixed]
+    sat_start = ref.round_count(inst, X0m, want_assign=False)[1]
+    assert np.all(bs >= sat_start) and np.all((bt >= 0) & (bt <= spec["steps"]))
+    # the returned X is itself an iterate: its count cannot beat the best
+    _, sat_end = P.round_count(X, want_assign=False)
+    assert np.all(sat_end.cpu().numpy() <= bs)
+    # descent happened: mean objective decreased
+    Fs, _ = P.eval_grad(dev(X0m.astype(np.float32)), want_G=False)
+    Fe, _ = P.eval_grad(X, want_G=False)
+    assert Fe.mean().item() < Fs.mean().item()
+    P.close()
