@@ -159,6 +159,10 @@ AFS_API afs_status afs_set_option(afs_problem* p, int32_t what, int64_t value);
 /* Static, never NULL. */
 AFS_API const char* afs_status_string(afs_status s);
 
+/* Text of the most recent CUDA runtime failure seen by the calling thread ("" if none): the CUDA error string and
+ * the source location inside the library.  Diagnostic only; valid until the next failing call on this thread. */
+AFS_API const char* afs_last_error_message(void);
+
 /* ABI version of this header: bumped when a signature changes. */
 AFS_API int32_t afs_abi_version(void);
 #define AFS_ABI_VERSION 1

@@ -20,7 +20,7 @@ AFS_OR, AFS_XOR, AFS_AMO, AFS_EO, AFS_EK, AFS_NAE, AFS_CARD = range(7)
 EXPORTS = (
     "afs_problem_create", "afs_problem_destroy", "afs_coeffs", "afs_eval_grad", "afs_eval_grad_f64",
     "afs_round_count", "afs_round_count_f64", "afs_pgd_run", "afs_pgd_run_f64", "afs_pgd_run_host",
-    "afs_problem_info", "afs_set_option", "afs_status_string", "afs_abi_version",
+    "afs_problem_info", "afs_set_option", "afs_status_string", "afs_abi_version", "afs_last_error_message",
 )
 
 _lib = None
@@ -30,7 +30,8 @@ class AfsError(RuntimeError):
     def __init__(self, status: int, where: str):
         self.status = int(status)
         msg = lib().afs_status_string(status).decode()
-        super().__init__("%s: %s (status %d)" % (where, msg, status))
+        detail = lib().afs_last_error_message().decode() if status == 7 else ""
+        super().__init__("%s: %s (status %d)%s" % (where, msg, status, " -- " + detail if detail else ""))
 
 
 def lib():
@@ -67,6 +68,7 @@ def lib():
     L.afs_status_string.argtypes = [C.c_int]
     L.afs_status_string.restype = C.c_char_p
     L.afs_abi_version.restype = i32
+    L.afs_last_error_message.restype = C.c_char_p
     _lib = L
     return L
 

@@ -57,11 +57,8 @@ struct CountCon {      // generic forward CSR entry for the count-only kernel: 1
     int32_t pad2;
 };
 
-template <typename T>
-struct DevBuf {
-    T* p = nullptr;
-    size_t n = 0;
-};
+// records cudaGetErrorString(e) + location for afs_last_error_message()
+void note_cuda_error(cudaError_t e, const char* file, int line);
 
 struct Workspace {
     // all sized for (Bp, steps) below; grown on demand

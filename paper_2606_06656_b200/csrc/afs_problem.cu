@@ -3,6 +3,7 @@
 // L223-L255) with exact big-integer numerators.
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
 #include <cstring>
 #include <new>
 #include <numeric>
@@ -15,6 +16,7 @@ using namespace afs;
     do {                                     \
         cudaError_t e_ = (x);                \
         if (e_ != cudaSuccess) {             \
+            afs::note_cuda_error(e_, __FILE__, __LINE__); \
             (void)cudaGetLastError();        \
             return AFS_ERR_CUDA;             \
         }                                    \
@@ -318,6 +320,18 @@ extern "C" const char* afs_status_string(afs_status s)
 }
 
 extern "C" int32_t afs_abi_version(void) { return AFS_ABI_VERSION; }
+
+namespace afs {
+static thread_local char g_last_error[256] = "";
+void note_cuda_error(cudaError_t e, const char* file, int line)
+{
+    const char* base = file;
+    for (const char* c = file; *c; ++c) if (*c == '/') base = c + 1;
+    snprintf(g_last_error, sizeof(g_last_error), "%s (%s:%d)", cudaGetErrorString(e), base, line);
+}
+}  // namespace afs
+
+extern "C" const char* afs_last_error_message(void) { return afs::g_last_error; }
 
 // =====================================================================================================================
 // afs_coeffs: eq. (3) through the Appendix-A closed forms (L223-L255; G2-G5).

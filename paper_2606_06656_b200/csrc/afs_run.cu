@@ -12,6 +12,7 @@ using namespace afs;
     do {                                     \
         cudaError_t e_ = (x);                \
         if (e_ != cudaSuccess) {             \
+            afs::note_cuda_error(e_, __FILE__, __LINE__); \
             (void)cudaGetLastError();        \
             return AFS_ERR_CUDA;             \
         }                                    \
@@ -104,13 +105,13 @@ static afs_status launch_long(afs_problem* P, int bucket, const real* XT, int Bp
     int LS = ((Lmax + 31) / 32) * 32 + 4;
     int QS = ((Lmax + 1 + 3) / 4) * 4 + 4;
     size_t smem = (size_t)(8 * LS + 16 * QS) * sizeof(real);
-    static bool attr_set[2][LONG_BUCKETS] = {};
+    static size_t attr_set[2][LONG_BUCKETS] = {};   // largest opt-in made so far, per kernel instance
     const int ti = sizeof(real) == 8 ? 1 : 0;
-    if (smem > 48 * 1024 && !attr_set[ti][bucket]) {
-        CU(cudaFuncSetAttribute(k_long<real, NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        attr_set[ti][bucket] = true;
+    if (smem > 226 * 1024) return AFS_ERR_UNSUPPORTED;
+    if (smem > 48 * 1024 && attr_set[ti][bucket] < smem) {
+        CU(cudaFuncSetAttribute(k_long<real, NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set[ti][bucket] = smem;
     }
-    if (smem > 227 * 1024) return AFS_ERR_UNSUPPORTED;
     long long blocks = (long long)(c1 - c0) * (Bp / 8);
     if (blocks > 0x7fffffffLL) return AFS_ERR_UNSUPPORTED;
     k_long<real, NR><<<(unsigned)blocks, 256, smem, st>>>(P->d_long, c0, P->d_long_lits, P->d_long_slots, XT, Bp,
