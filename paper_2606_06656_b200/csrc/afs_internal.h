@@ -19,8 +19,9 @@ constexpr uint32_t LIT_VAR = 0x7fffffffu;
 //         occurrence's leave-one-out product from the other literals (deterministic by construction).
 //  MED  : thread per (constraint, restart), prefix/suffix in registers: OR/XOR L<=64, NAE/EO/AMO L<=32;
 //         OR/XOR longer than 64 run a two-pass running-product kernel (scratch row = prefix storage).
+//  CMED : EK / CARD with L <= 64: thread per (constraint, restart), the whole pmf in registers.
 //  LONG : warp per (constraint, restart), count-basis DP + stable-direction leave-one-out recurrences:
-//         every EK/CARD, and whatever is too long for MED.
+//         EK/CARD longer than 64, and NAE/EO/AMO too long for MED.
 constexpr int PULL_MAX_LEN = 5;
 constexpr int MED_MAX_PROD = 64;
 constexpr int MED_MAX_TWO = 32;
@@ -28,9 +29,18 @@ constexpr int LONG_MAX_LEN = 1151;   // 9 rows x 128 cells hold q_0..q_L
 constexpr int MED_BUCKETS = 5;       // padded lengths 8, 16, 32, 64; bucket 4 = OR/XOR longer than 64 (two-pass kernel)
 constexpr int LONG_BUCKETS = 9;      // NR = 1..9 rows of 128 pmf cells
 
-// pull occurrence header (one uint32, followed by `nother` literal words)
-//   bits 0..1 kind (0 OR, 1 XOR, 2 NAE) | 2..4 nother | 5 own literal negated | 6 owner | 7 xor parity k
+// pull streams (S0 output for the PULL class).  Per variable its occurrences are grouped into RUNS of equal
+// (kind, number of other literals); a run is `count` occurrences x `nother` entries, one uint32 per OTHER literal:
+//   entry       bits 0..23 variable | 30 occurrence sign (first entry of the occurrence only) | 31 literal negated
+//   occurrence sign = own literal negated XOR (XOR constraint with even parity): the leave-one-out product enters
+//               the variable's gradient with that sign
+//   run word    bits 30..31 kind | 27..29 nother (1..4) | 0..26 count
+// Unit clauses (no other literal) contribute a constant to the gradient: pull_gconst[v].
+constexpr uint32_t PE_VAR = 0x00ffffffu, PE_SIGN = 1u << 30, PE_NEG = 1u << 31;
 constexpr uint32_t PH_KIND_OR = 0, PH_KIND_XOR = 1, PH_KIND_NAE = 2;
+constexpr int MAX_VARS = 1 << 24;
+constexpr int CM_BUCKETS = 4;        // EK / CARD with L <= 64: padded lengths 16, 32, 48, 64, pmf in registers
+constexpr int CM_MAX_LEN = 64;
 
 struct MedCon {        // 16 bytes
     int32_t off;       // first literal in med_lits / med_slots
@@ -73,6 +83,7 @@ struct Workspace {
     uint32_t* best_bits = nullptr;         // [n][Bp/32]
     void* fe_med = nullptr;                // real [n_med][Bp]      (eval_grad only)
     void* fe_long = nullptr;               // real [n_long][Bp]
+    void* fe_cm = nullptr;                 // real [n_cm][Bp]
     void* f_part = nullptr;                // real [n_parts][Bp]
     int32_t fe_Bp = 0;
     int8_t* mask_dev = nullptr;            // staging for afs_pgd_run_host
@@ -94,9 +105,14 @@ struct afs_problem {
     int sm_count = 148;
 
     // ---- device tables -------------------------------------------------------------------------------------
-    int32_t* d_pull_ptr = nullptr;      // [n+1] word offsets of each variable's occurrence stream
-    uint32_t* d_pull_words = nullptr;
+    int32_t* d_pull_ptr = nullptr;      // [n+1] entry offsets of each variable's pull stream
+    uint32_t* d_pull_words = nullptr;   // entries
     int64_t pull_words = 0;
+    int32_t* d_run_ptr = nullptr;       // [n+1] offsets into d_runs
+    uint32_t* d_runs = nullptr;         // run descriptors
+    float* d_pull_gconst = nullptr;     // [n] constant gradient of unit clauses
+    afs::CountCon* d_pc = nullptr;      // the PULL constraints alone (forward CSR), for counts and objective
+    uint32_t* d_pc_lits = nullptr;
     int32_t* d_slot_ptr = nullptr;      // [n+1] scratch rows of each variable (transposed-CSR order)
     int64_t nslots = 0;
 
@@ -111,10 +127,15 @@ struct afs_problem {
     int32_t long_begin[afs::LONG_BUCKETS + 1] = {0};
     int32_t long_maxL[afs::LONG_BUCKETS] = {0};
 
+    afs::LongCon* d_cm = nullptr;       // EK / CARD with L <= 64, sorted by padded length
+    uint32_t* d_cm_lits = nullptr;
+    int32_t* d_cm_slots = nullptr;
+    int32_t cm_begin[afs::CM_BUCKETS + 1] = {0};
+
     afs::CountCon* d_count = nullptr;   // all m constraints, original order
     uint32_t* d_count_lits = nullptr;
 
-    int64_t n_pull = 0, n_med = 0, n_long = 0;
+    int64_t n_pull = 0, n_med = 0, n_long = 0, n_cm = 0;
 
     // ---- run state -----------------------------------------------------------------------------------------
     afs::Workspace ws;

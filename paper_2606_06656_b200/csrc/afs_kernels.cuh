@@ -130,6 +130,97 @@ __global__ void __launch_bounds__(256) k_count(const CountCon* __restrict__ cons
 }
 
 // ------------------------------------------------------------------------------------------------------------------
+// Accessors: the constraint bodies below are written once and read x / write gradients through these, so the
+// streaming kernels (global XT[n][Bp], global scratch) and the tile-resident kernel (shared memory) share them.
+// ------------------------------------------------------------------------------------------------------------------
+template <typename real>
+struct XGlobal {
+    const real* __restrict__ p;
+    int stride, col;
+    __device__ __forceinline__ real operator()(uint32_t var) const { return p[(size_t)var * stride + col]; }
+};
+template <typename real>
+struct SGlobal {
+    real* __restrict__ p;
+    int stride, col;
+    __device__ __forceinline__ void put(int slot, real v) const { p[(size_t)slot * stride + col] = v; }
+    __device__ __forceinline__ real get(int slot) const { return p[(size_t)slot * stride + col]; }
+};
+
+// ------------------------------------------------------------------------------------------------------------------
+// CMED class: EK / CARD with L <= 64, thread = (constraint, restart), the whole pmf q_0..q_LP in registers.
+// The constraint is padded to LP literals with constant-False ones (u = 1, p = 0: they change nothing), so that the
+// reversed pmf is indexed at compile time.  Leave-one-out (G10): dFE/dy_j = q^(-j)_{k-1} [- q^(-j)_k
+// for EK].  Both stable recurrences run for every literal -- s_t = q_t - (p/u) s_{t-1} from the bottom up to t = k-1
+// (k for EK), sigma_i = q_{LP-i} - (u/p) sigma_{i-1} from the top down to the same indices -- and the result of the
+// direction whose ratio is <= 1 is kept; the other one is discarded by a select (it may be inf/NaN, never used).
+// ------------------------------------------------------------------------------------------------------------------
+template <typename real, int LP, typename XL, typename SW>
+__device__ __forceinline__ void cmed_body(const LongCon& lc, const uint32_t* __restrict__ lw,
+                                          const int32_t* __restrict__ sw, const XL& xl, const SW& sc, int& satcnt,
+                                          real& fe)
+{
+    const real half = real(0.5), one = real(1), zero = real(0);
+    const int L = lc.L;
+    real q[LP + 1];
+#pragma unroll
+    for (int t = 0; t <= LP; ++t) q[t] = zero;
+    q[0] = one;
+    int tc = 0;
+#pragma unroll
+    for (int j = 0; j < LP; ++j) {
+        if (j < L) {
+            uint32_t w = lw[j];
+            real x = xl(w & LIT_VAR);
+            bool neg = (w >> 31) != 0;
+            tc += ((x < zero) != neg) ? 1 : 0;
+            real y = neg ? -x : x;
+            real u = half + half * y, p = half - half * y;
+#pragma unroll
+            for (int i = j + 1; i >= 1; --i) q[i] = q[i] * u + q[i - 1] * p;
+            q[0] = q[0] * u;
+        }
+    }
+    satcnt += pred(lc.type, L, lc.k, tc) ? 1 : 0;
+    real f = zero;
+#pragma unroll
+    for (int t = 0; t <= LP; ++t) f += (lc.type == AFS_CARD ? t >= lc.k : t == lc.k) ? -q[t] : q[t];
+    fe = f;
+    // targets: tA = k-1 with weight +1 (valid iff wA != 0), tB = k with weight -1 (EK only, valid iff wB != 0)
+    const bool useA = lc.wA != 0.f, useB = lc.wB != 0.f;
+    const int tA = lc.tA, tB = lc.tB;
+    const int fend = useB ? tB : (useA ? tA : -1);                 // last forward index needed
+    const int bend = useA ? LP - 1 - tA : (useB ? LP - 1 - tB : -1);  // last top-down index needed (tA < tB)
+    for (int j = 0; j < L; ++j) {
+        uint32_t w = lw[j];
+        real x = xl(w & LIT_VAR);
+        bool neg = (w >> 31) != 0;
+        real y = neg ? -x : x;
+        real u = half + half * y, p = half - half * y;
+        const bool fwd = !(y < zero);
+        const real Rf = p / u, Rb = u / p;
+        real s = zero, sprev = zero;
+#pragma unroll
+        for (int t = 0; t <= LP; ++t) {
+            if (t <= fend) { sprev = s; s = q[t] - Rf * s; }
+        }
+        // forward: s = s_fend.  useB: s_tB = s, s_tA = sprev (tA = tB - 1 when both are used; if only B, A unused)
+        real fA = useB ? sprev : s, fB = s;
+        real z = zero, zprev = zero;
+#pragma unroll
+        for (int i = 0; i <= LP; ++i) {
+            if (i <= bend) { zprev = z; z = q[LP - i] - Rb * z; }
+        }
+        // top-down: z = sigma_bend.  useA: sigma at tA is z, sigma at tB (one index earlier) is zprev
+        real bA = z, bB = useA ? zprev : z;
+        real gA = fwd ? fA / u : bA / p;
+        real gB = fwd ? fB / u : bB / p;
+        real g = (useA ? gA : zero) - (useB ? gB : zero);
+        sc.put(sw[j], neg ? -g : g);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
 // MED class: thread = (constraint, restart); y gathered once into registers; division-free leave-one-out by
 // prefix / suffix products (OR, XOR, NAE) or a two-state prefix / suffix pmf (EO, AMO).  S1-S3, S5, S9.
 //   OR   FE = 2 prod u - 1                 dFE/dy_j = prod_{i!=j} u_i                      (u = (1+y)/2)
@@ -249,6 +340,34 @@ __global__ void __launch_bounds__(128) k_med(const MedCon* __restrict__ cons, in
                 fe = real(0);
             }
         }
+        if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
+    }
+    if (sat) {
+        s_sat[warp][lane] = satcnt;
+        __syncthreads();
+        if (warp == 0) {
+            int tot = s_sat[0][lane] + s_sat[1][lane] + s_sat[2][lane] + s_sat[3][lane];
+            if (tot) atomicAdd(&sat[b], tot);
+        }
+    }
+}
+
+template <typename real, int LP>
+__global__ void __launch_bounds__(128) k_cmed(const LongCon* __restrict__ cons, int c_begin, int c_end,
+                                              const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
+                                              const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
+                                              int32_t* __restrict__ sat, real* __restrict__ fe_out)
+{
+    __shared__ int s_sat[4][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int b = blockIdx.y * 32 + lane;
+    int satcnt = 0;
+    const XGlobal<real> xl{XT, Bp, b};
+    const SGlobal<real> sc{scratch, Bp, b};
+    for (int c = c_begin + blockIdx.x * 4 + warp; c < c_end; c += gridDim.x * 4) {
+        const LongCon lc = cons[c];
+        real fe;
+        cmed_body<real, LP>(lc, lits + lc.off, slots + lc.off, xl, sc, satcnt, fe);
         if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
     }
     if (sat) {
@@ -483,26 +602,31 @@ __global__ void __launch_bounds__(256) k_long(const LongCon* __restrict__ cons, 
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// Variable pass: thread = (variable, restart).  Fuses
-//   S1-S3,S5 for the PULL class (leave-one-out products recomputed per occurrence: no scratch, no atomics),
+// Variable pass: thread = (variable, restart), lanes over 32 restarts of one variable.  Fuses
+//   S1-S3,S5 for the PULL class: the leave-one-out product of every occurrence is recomputed from the other
+//        literals (no scratch, no atomics); occurrences come in runs of equal shape so the inner loops are
+//        branch-free; the warp stages 32 entries with one coalesced load and gathers several occurrences at once,
 //   S6   deterministic segmented reduction of the materialised gradients over the transposed CSR (fixed order),
 //   S7-S8 step, clip, fixed-variable mask,
-//   S9   sign bits of X_t (ballot) and the satisfied count of the clauses this variable owns,
-//   S10  merge of the previous iterate into the best-so-far (its count is complete once the previous launch ended).
-// EVAL = true is afs_eval_grad: writes G^T and per-warp objective partial sums instead of stepping.
+//   S9   sign bits of X_t (one ballot word per variable and restart tile; the counts of the PULL clauses are taken
+//        from these words by k_sat_pull),
+//   S10  merge of the previous iterate into the best-so-far (its count is complete once the previous launches ended).
+// EVAL = true is afs_eval_grad: writes G^T instead of stepping.
 // ------------------------------------------------------------------------------------------------------------------
 template <typename real>
 struct VarArgs {
     int n, Bp, t;
     const int32_t* pull_ptr;
     const uint32_t* pull_words;
+    const int32_t* run_ptr;
+    const uint32_t* runs;
+    const float* gconst;
     const int32_t* slot_ptr;
     const real* scratch;
     const real* Xin;
     real* Xout;
     real lr;
     const int8_t* mask;
-    int32_t* sat_cur;
     const int32_t* sat_prev;
     const int32_t* best_sat_in;
     int32_t* best_sat_out;
@@ -512,20 +636,103 @@ struct VarArgs {
     uint32_t* S_cur;
     uint32_t* best_bits;
     real* GT;
-    real* Fpart;
 };
 
-template <typename real, bool EVAL>
-__global__ void __launch_bounds__(VAR_WARPS * 32) k_var(const VarArgs<real> a)
+__device__ __forceinline__ float flip(float x, uint32_t signbit) { return __int_as_float(__float_as_int(x) ^ (int)signbit); }
+__device__ __forceinline__ double flip(double x, uint32_t signbit) { return signbit ? -x : x; }
+// +-0.5 with the sign of a negated literal: u = h x + 0.5 is (1 + y)/2 for y = +-x
+__device__ __forceinline__ float halfsigned(float, uint32_t signbit) { return __int_as_float(0x3f000000 | (int)signbit); }
+__device__ __forceinline__ double halfsigned(double, uint32_t signbit) { return signbit ? -0.5 : 0.5; }
+
+// One run: `count` occurrences of NOTHER other literals each, entries at words[beg ...).  xcol points at column b of
+// the X matrix (global XT or a shared-memory tile), rowstride is its row pitch in elements.  Returns the run's
+// contribution to dF/dx_v (already carrying the sign of the own literal).
+template <typename real, int KIND, int NOTHER>
+__device__ __forceinline__ real pull_run(const uint32_t* __restrict__ words, int beg, int count,
+                                         const real* __restrict__ xcol, size_t rowstride, int lane)
 {
-    __shared__ int s_sat[VAR_WARPS][32];
+    constexpr int OPC = 32 / NOTHER;              // occurrences per staged chunk of <= 32 entries
+    constexpr int U = NOTHER <= 2 ? 4 : 2;        // occurrences gathered together
+    const real one = real(1), half = real(0.5);
+    real g = real(0);
+    for (int o0 = 0; o0 < count; o0 += OPC) {
+        const int nocc = min(OPC, count - o0);
+        const uint32_t mine = words[beg + o0 * NOTHER + lane];   // over-read past the chunk is harmless (padded array)
+        for (int o = 0; o < nocc; o += U) {
+            uint32_t w[U][NOTHER];
+            real x[U][NOTHER];
+#pragma unroll
+            for (int u = 0; u < U; ++u)
+#pragma unroll
+                for (int i = 0; i < NOTHER; ++i) w[u][i] = __shfl_sync(FULL, mine, ((o + u) * NOTHER + i) & 31);
+#pragma unroll
+            for (int u = 0; u < U; ++u)
+#pragma unroll
+                for (int i = 0; i < NOTHER; ++i) x[u][i] = xcol[(size_t)(w[u][i] & PE_VAR) * rowstride];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                real d;
+                if (KIND == (int)PH_KIND_XOR) {
+                    real prod = flip(x[u][0], w[u][0] & PE_NEG);
+#pragma unroll
+                    for (int i = 1; i < NOTHER; ++i) prod *= flip(x[u][i], w[u][i] & PE_NEG);
+                    d = prod;
+                } else {
+                    real pu = halfsigned(one, w[u][0] & PE_NEG) * x[u][0] + half;
+#pragma unroll
+                    for (int i = 1; i < NOTHER; ++i) pu *= halfsigned(one, w[u][i] & PE_NEG) * x[u][i] + half;
+                    d = pu;
+                    if (KIND == (int)PH_KIND_NAE) {
+                        real pp = half - halfsigned(one, w[u][0] & PE_NEG) * x[u][0];
+#pragma unroll
+                        for (int i = 1; i < NOTHER; ++i) pp *= half - halfsigned(one, w[u][i] & PE_NEG) * x[u][i];
+                        d = pu - pp;
+                    }
+                }
+                d = flip(d, (w[u][0] & PE_SIGN) << 1);
+                if (o + u < nocc) g += d;
+            }
+        }
+    }
+    return g;
+}
+
+// all runs of one variable
+template <typename real>
+__device__ __forceinline__ real pull_variable(const uint32_t* __restrict__ runs, int rbeg, int rend,
+                                              const uint32_t* __restrict__ words, int wbeg,
+                                              const real* __restrict__ xcol, size_t rowstride, int lane)
+{
+    real g = real(0);
+    int pos = wbeg;
+    for (int r = rbeg; r < rend; ++r) {
+        const uint32_t d = runs[r];
+        const int count = (int)(d & 0x07ffffffu), nother = (int)((d >> 27) & 7u), kind = (int)(d >> 30);
+        real gr;
+#define AFS_RUN(K, N) gr = pull_run<real, K, N>(words, pos, count, xcol, rowstride, lane)
+        if (kind == (int)PH_KIND_OR) {
+            switch (nother) { case 1: AFS_RUN(0, 1); break; case 2: AFS_RUN(0, 2); break; case 3: AFS_RUN(0, 3); break; default: AFS_RUN(0, 4); break; }
+        } else if (kind == (int)PH_KIND_XOR) {
+            switch (nother) { case 1: AFS_RUN(1, 1); break; case 2: AFS_RUN(1, 2); break; case 3: AFS_RUN(1, 3); break; default: AFS_RUN(1, 4); break; }
+        } else {
+            switch (nother) { case 1: AFS_RUN(2, 1); break; case 2: AFS_RUN(2, 2); break; case 3: AFS_RUN(2, 3); break; default: AFS_RUN(2, 4); break; }
+        }
+#undef AFS_RUN
+        g += gr;
+        pos += count * nother;
+    }
+    return g;
+}
+
+template <typename real, bool EVAL>
+__global__ void __launch_bounds__(VAR_WARPS * 32, 4) k_var(const VarArgs<real> a)
+{
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int tile = blockIdx.y, ntile = a.Bp >> 5;
     const int b = tile * 32 + lane;
     const int Bp = a.Bp;
-    const real half = real(0.5), one = real(1);
-    int satcnt = 0;
-    real fpart = real(0);
+    const real one = real(1);
+    const real* __restrict__ xcol = a.Xin + b;
     const int vbeg = (blockIdx.x * VAR_WARPS + warp) * VAR_VPW;
     const int vend = min(vbeg + VAR_VPW, a.n);
     // ---- S10: did the previous iterate improve on the best so far?
@@ -544,81 +751,33 @@ __global__ void __launch_bounds__(VAR_WARPS * 32) k_var(const VarArgs<real> a)
                 a.best_bits[wi] = (a.best_bits[wi] & ~impmask) | (a.S_prev[wi] & impmask);
             }
             if (v == 0) {
-                int bs = a.best_sat_in[b], st = a.best_step_in[b];
+                int bs = a.best_sat_in[b], stp = a.best_step_in[b];
                 a.best_sat_out[b] = imp ? sprev : bs;
-                a.best_step_out[b] = imp ? a.t - 1 : st;
+                a.best_step_out[b] = imp ? a.t - 1 : stp;
             }
         }
-        const real x = a.Xin[(size_t)v * Bp + b];
-        const bool xtrue = x < real(0);
+        const real x = xcol[(size_t)v * Bp];
         int mk = 0;
         if (!EVAL) {
-            unsigned sb = __ballot_sync(FULL, xtrue);
+            unsigned sb = __ballot_sync(FULL, x < real(0));
             if (lane == 0) a.S_cur[(size_t)v * ntile + tile] = sb;
             mk = a.mask ? a.mask[v] : 0;
         }
         real g = real(0);
-        // ---- PULL occurrences of v
-        int pos = a.pull_ptr[v];
-        const int pend = a.pull_ptr[v + 1];
-        while (pos < pend) {
-            const uint32_t hdr = a.pull_words[pos++];
-            const int kind = hdr & 3, nother = (hdr >> 2) & 7;
-            const bool ownneg = (hdr & 32u) != 0, owner = (hdr & 64u) != 0;
-            if (mk != 0 && !owner) { pos += nother; continue; }   // fixed variable: its gradient is never used
-            int tcount = (xtrue != ownneg) ? 1 : 0;
-            const real yown = ownneg ? -x : x;
-            if (kind == (int)PH_KIND_OR) {
-                real prod = one;
-                for (int i = 0; i < nother; ++i) {
-                    uint32_t w = a.pull_words[pos++];
-                    real xo = ldx(a.Xin, w, Bp, b);
-                    bool neg = (w >> 31) != 0;
-                    tcount += ((xo < real(0)) != neg) ? 1 : 0;
-                    prod *= half + half * (neg ? -xo : xo);
-                }
-                g += ownneg ? -prod : prod;
-                if (owner) {
-                    satcnt += tcount >= 1 ? 1 : 0;
-                    if (EVAL) fpart += real(2) * prod * (half + half * yown) - one;
-                }
-            } else if (kind == (int)PH_KIND_XOR) {
-                real prod = (hdr & 128u) ? one : -one;
-                for (int i = 0; i < nother; ++i) {
-                    uint32_t w = a.pull_words[pos++];
-                    real xo = ldx(a.Xin, w, Bp, b);
-                    bool neg = (w >> 31) != 0;
-                    tcount += ((xo < real(0)) != neg) ? 1 : 0;
-                    prod *= neg ? -xo : xo;
-                }
-                g += ownneg ? -prod : prod;
-                if (owner) {
-                    satcnt += ((tcount & 1) == (int)((hdr >> 7) & 1)) ? 1 : 0;
-                    if (EVAL) fpart += prod * yown;
-                }
-            } else {   // NAE
-                real pu = one, pp = one;
-                for (int i = 0; i < nother; ++i) {
-                    uint32_t w = a.pull_words[pos++];
-                    real xo = ldx(a.Xin, w, Bp, b);
-                    bool neg = (w >> 31) != 0;
-                    tcount += ((xo < real(0)) != neg) ? 1 : 0;
-                    real yo = neg ? -xo : xo;
-                    pu *= half + half * yo;
-                    pp *= half - half * yo;
-                }
-                real d = pu - pp;
-                g += ownneg ? -d : d;
-                if (owner) {
-                    satcnt += (tcount > 0 && tcount < nother + 1) ? 1 : 0;
-                    if (EVAL) fpart += real(2) * pu * (half + half * yown) + real(2) * pp * (half - half * yown) - one;
-                }
-            }
-        }
-        // ---- S6: materialised gradients of v, fixed (transposed-CSR) order
-        if (mk == 0) {
+        if (mk == 0) {   // a fixed variable never moves: its gradient is not needed
+            g = (real)a.gconst[v];
+            g += pull_variable<real>(a.runs, a.run_ptr[v], a.run_ptr[v + 1], a.pull_words, a.pull_ptr[v], xcol,
+                                     (size_t)Bp, lane);
+            // ---- S6: materialised gradients of v, fixed (transposed-CSR) order
             const int s1 = a.slot_ptr[v + 1];
-            for (int s = a.slot_ptr[v]; s < s1; ++s) g += a.scratch[(size_t)s * Bp + b];
+            int s = a.slot_ptr[v];
+            const real* __restrict__ sc = a.scratch + b;
+            for (; s + 4 <= s1; s += 4) {
+                real g0 = sc[(size_t)s * Bp], g1 = sc[(size_t)(s + 1) * Bp];
+                real g2 = sc[(size_t)(s + 2) * Bp], g3 = sc[(size_t)(s + 3) * Bp];
+                g += g0; g += g1; g += g2; g += g3;
+            }
+            for (; s < s1; ++s) g += sc[(size_t)s * Bp];
         }
         if (EVAL) {
             a.GT[(size_t)v * Bp + b] = g;
@@ -631,30 +790,111 @@ __global__ void __launch_bounds__(VAR_WARPS * 32) k_var(const VarArgs<real> a)
             a.Xout[(size_t)v * Bp + b] = xn;
         }
     }
-    if (EVAL) {
-        a.Fpart[(size_t)(blockIdx.x * VAR_WARPS + warp) * Bp + b] = fpart;
-    } else {
-        s_sat[warp][lane] = satcnt;
-        __syncthreads();
-        if (warp == 0) {
-            int tot = 0;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// S9 for the PULL class, bit-parallel over restarts: the sign words S[v][tile] (bit r = "x_v < 0" for restart
+// tile*32 + r) written by the variable pass give the truth of 32 restarts of a clause with a few logic ops; the
+// per-restart totals are kept as vertical (bit-sliced) counters and unpacked once per thread.  Integers only.
+// thread = (chunk of clauses, restart tile).
+// ------------------------------------------------------------------------------------------------------------------
+constexpr int SATP_TG = 8;                            // restart tiles per CTA
+constexpr int SATP_CPB = 256 / SATP_TG;               // clause chunks per CTA
+
+template <int PLANES>
+__global__ void __launch_bounds__(256) k_sat_pull(const CountCon* __restrict__ cons, const uint32_t* __restrict__ lits,
+                                                  int m, int chunk, const uint32_t* __restrict__ S, int ntile,
+                                                  int32_t* __restrict__ sat)
+{
+    __shared__ int s_cnt[SATP_TG][32];
+    const int tl = threadIdx.x % SATP_TG;
+    const int tile = blockIdx.y * SATP_TG + tl;
+    const int ch = blockIdx.x * SATP_CPB + threadIdx.x / SATP_TG;
+    s_cnt[threadIdx.x >> 5][threadIdx.x & 31] = 0;
+    __syncthreads();
+    if (tile < ntile) {
+        uint32_t plane[PLANES];
 #pragma unroll
-            for (int w = 0; w < VAR_WARPS; ++w) tot += s_sat[w][lane];
-            if (tot) atomicAdd(&a.sat_cur[b], tot);
+        for (int p = 0; p < PLANES; ++p) plane[p] = 0u;
+        const int c1 = min(m, (ch + 1) * chunk);
+        bool any = false;
+        for (int c = ch * chunk; c < c1; ++c) {
+            const CountCon cc = cons[c];
+            uint32_t w = lits[cc.off];
+            uint32_t t0 = S[(size_t)(w & LIT_VAR) * ntile + tile] ^ ((w >> 31) ? 0xffffffffu : 0u);
+            uint32_t vor = t0, vand = t0, vxor = t0;
+            for (int j = 1; j < cc.L; ++j) {
+                w = lits[cc.off + j];
+                uint32_t tj = S[(size_t)(w & LIT_VAR) * ntile + tile] ^ ((w >> 31) ? 0xffffffffu : 0u);
+                vor |= tj; vand &= tj; vxor ^= tj;
+            }
+            uint32_t carry = cc.type == AFS_OR ? vor : cc.type == AFS_XOR ? ~(vxor ^ ((cc.k & 1) ? 0xffffffffu : 0u))
+                                                                          : (vor & ~vand);
+#pragma unroll
+            for (int p = 0; p < PLANES; ++p) {
+                uint32_t t = plane[p] & carry;
+                plane[p] ^= carry;
+                carry = t;
+            }
+            any = true;
+        }
+        if (any) {
+            for (int r = 0; r < 32; ++r) {
+                int cnt = 0;
+#pragma unroll
+                for (int p = 0; p < PLANES; ++p) cnt |= (int)((plane[p] >> r) & 1u) << p;
+                if (cnt) atomicAdd(&s_cnt[tl][r], cnt);
+            }
         }
     }
+    __syncthreads();
+    {
+        const int t2 = threadIdx.x >> 5, r = threadIdx.x & 31;
+        const int tile2 = blockIdx.y * SATP_TG + t2;
+        int cnt = s_cnt[t2][r];
+        if (tile2 < ntile && cnt) atomicAdd(&sat[tile2 * 32 + r], cnt);
+    }
+}
+
+// objective of the PULL class for afs_eval_grad (S2, S4): thread = (clause, restart), per-warp partial sums in a
+// fixed clause order.  OR 2 prod u - 1;  XOR s prod y;  NAE 2 prod u + 2 prod p - 1.
+template <typename real>
+__global__ void __launch_bounds__(256) k_fe_pull(const CountCon* __restrict__ cons, const uint32_t* __restrict__ lits,
+                                                 int m, const real* __restrict__ XT, int Bp, real* __restrict__ Fpart)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int b = blockIdx.y * 32 + lane;
+    const int part = blockIdx.x * 8 + warp, nparts = gridDim.x * 8;
+    const real half = real(0.5), one = real(1);
+    real acc = real(0);
+    for (int c = part; c < m; c += nparts) {
+        const CountCon cc = cons[c];
+        real pu = one, pp = one, py = one;
+        for (int j = 0; j < cc.L; ++j) {
+            uint32_t w = lits[cc.off + j];
+            real x = ldx(XT, w, Bp, b);
+            real y = (w >> 31) ? -x : x;
+            pu *= half + half * y; pp *= half - half * y; py *= y;
+        }
+        acc += cc.type == AFS_OR ? real(2) * pu - one
+             : cc.type == AFS_XOR ? ((cc.k & 1) ? py : -py)
+                                  : real(2) * pu + real(2) * pp - one;
+    }
+    Fpart[(size_t)part * Bp + b] = acc;
 }
 
 // F[b] = sum of the variable-pass partials, then the medium, then the long expansions -- fixed order, fp64 accumulator
 template <typename real>
 __global__ void k_reduce_F(const real* __restrict__ Fpart, int nparts, const real* __restrict__ fe_med, int n_med,
-                           const real* __restrict__ fe_long, int n_long, int Bp, int B, real* __restrict__ F)
+                           const real* __restrict__ fe_cm, int n_cm, const real* __restrict__ fe_long, int n_long,
+                           int Bp, int B, real* __restrict__ F)
 {
     int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     double acc = 0.0;
     for (int i = 0; i < nparts; ++i) acc += (double)Fpart[(size_t)i * Bp + b];
     for (int i = 0; i < n_med; ++i) acc += (double)fe_med[(size_t)i * Bp + b];
+    for (int i = 0; i < n_cm; ++i) acc += (double)fe_cm[(size_t)i * Bp + b];
     for (int i = 0; i < n_long; ++i) acc += (double)fe_long[(size_t)i * Bp + b];
     F[b] = (real)acc;
 }

@@ -105,7 +105,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
 
     try {
         // ------------------------------------------------------------ classification
-        enum { C_PULL = 0, C_MED = 1, C_LONG = 2 };
+        enum { C_PULL = 0, C_MED = 1, C_LONG = 2, C_CMED = 3 };
         std::vector<uint8_t> cls(m);
         for (int c = 0; c < m; ++c) {
             int L = (int)(row_ptr[c + 1] - row_ptr[c]);
@@ -114,6 +114,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
             if ((prod || ty == AFS_NAE) && L <= PULL_MAX_LEN) cls[c] = C_PULL;
             else if (prod) cls[c] = C_MED;   // any length: beyond MED_MAX_PROD the two-pass product kernel takes it
             else if ((ty == AFS_NAE || ty == AFS_EO || ty == AFS_AMO) && L <= MED_MAX_TWO) cls[c] = C_MED;
+            else if ((ty == AFS_EK || ty == AFS_CARD) && L <= CM_MAX_LEN) cls[c] = C_CMED;
             else cls[c] = C_LONG;
         }
         // ------------------------------------------------------------ scratch slots, transposed-CSR order
@@ -132,39 +133,61 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
 
         auto lit_word = [](int32_t l) -> uint32_t { return (uint32_t)(std::abs(l) - 1) | (l < 0 ? LIT_NEG : 0u); };
 
-        // ------------------------------------------------------------ pull streams
-        std::vector<int32_t> pull_ptr(n + 1, 0);
-        for (int c = 0; c < m; ++c)
-            if (cls[c] == C_PULL) {
-                int L = (int)(row_ptr[c + 1] - row_ptr[c]);
-                for (int64_t e = row_ptr[c]; e < row_ptr[c + 1]; ++e) pull_ptr[std::abs(lits[e])] += L;  // header + L-1
-                P->n_pull++;
+        // ------------------------------------------------------------ pull streams: runs of equal (kind, nother)
+        if (n > MAX_VARS) { delete P; return AFS_ERR_UNSUPPORTED; }
+        struct Occ { int c; int j; int key; };     // key = kind * 8 + nother
+        std::vector<std::vector<Occ>> occs(n);
+        std::vector<float> gconst(n, 0.f);
+        std::vector<CountCon> pc;
+        std::vector<uint32_t> pc_lits;
+        for (int c = 0; c < m; ++c) {
+            if (cls[c] != C_PULL) continue;
+            P->n_pull++;
+            int L = (int)(row_ptr[c + 1] - row_ptr[c]);
+            const int32_t* lc = lits + row_ptr[c];
+            CountCon cc; cc.off = (int64_t)pc_lits.size(); cc.L = L; cc.type = (int16_t)types[c]; cc.pad = 0; cc.k = k[c]; cc.pad2 = 0;
+            pc.push_back(cc);
+            for (int j = 0; j < L; ++j) pc_lits.push_back(lit_word(lc[j]));
+            int kind = types[c] == AFS_OR ? (int)PH_KIND_OR : types[c] == AFS_XOR ? (int)PH_KIND_XOR : (int)PH_KIND_NAE;
+            for (int j = 0; j < L; ++j) {
+                int v = std::abs(lc[j]) - 1;
+                bool sign = (lc[j] < 0) != (types[c] == AFS_XOR && !(k[c] & 1));
+                if (L == 1) { gconst[v] += sign ? -1.f : 1.f; continue; }   // OR: dFE/dy = 1; XOR: +-1
+                occs[v].push_back({c, j, kind * 8 + (L - 1)});
             }
-        for (int v = 0; v < n; ++v) {
-            int64_t s = (int64_t)pull_ptr[v + 1] + pull_ptr[v];
-            if (s > 0x7fffffff) { delete P; return AFS_ERR_UNSUPPORTED; }
-            pull_ptr[v + 1] = (int32_t)s;
         }
-        P->pull_words = pull_ptr[n];
-        std::vector<uint32_t> pull_words((size_t)P->pull_words);
-        {
-            std::vector<int32_t> pf(pull_ptr.begin(), pull_ptr.end() - 1);
-            for (int c = 0; c < m; ++c) {
-                if (cls[c] != C_PULL) continue;
-                int L = (int)(row_ptr[c + 1] - row_ptr[c]);
-                const int32_t* lc = lits + row_ptr[c];
-                uint32_t kind = types[c] == AFS_OR ? PH_KIND_OR : types[c] == AFS_XOR ? PH_KIND_XOR : PH_KIND_NAE;
-                for (int j = 0; j < L; ++j) {
-                    int v = std::abs(lc[j]) - 1;
-                    int32_t& w = pf[v];
-                    uint32_t hdr = kind | ((uint32_t)(L - 1) << 2) | (lc[j] < 0 ? 32u : 0u) | (j == 0 ? 64u : 0u) |
-                                   ((types[c] == AFS_XOR && (k[c] & 1)) ? 128u : 0u);
-                    pull_words[w++] = hdr;
-                    for (int i = 0; i < L; ++i)
-                        if (i != j) pull_words[w++] = lit_word(lc[i]);
+        std::vector<int32_t> pull_ptr(n + 1, 0), run_ptr(n + 1, 0);
+        std::vector<uint32_t> pull_words, runs;
+        for (int v = 0; v < n; ++v) {
+            auto& ov = occs[v];
+            std::stable_sort(ov.begin(), ov.end(), [](const Occ& a, const Occ& b) { return a.key < b.key; });
+            size_t i = 0;
+            while (i < ov.size()) {
+                size_t e = i;
+                while (e < ov.size() && ov[e].key == ov[i].key) ++e;
+                int kind = ov[i].key / 8, nother = ov[i].key % 8;
+                runs.push_back(((uint32_t)kind << 30) | ((uint32_t)nother << 27) | (uint32_t)(e - i));
+                for (; i < e; ++i) {
+                    int c = ov[i].c, j = ov[i].j;
+                    int L = (int)(row_ptr[c + 1] - row_ptr[c]);
+                    const int32_t* lc = lits + row_ptr[c];
+                    bool sign = (lc[j] < 0) != (types[c] == AFS_XOR && !(k[c] & 1));
+                    bool first = true;
+                    for (int q = 0; q < L; ++q) {
+                        if (q == j) continue;
+                        pull_words.push_back((uint32_t)(std::abs(lc[q]) - 1) | (lc[q] < 0 ? PE_NEG : 0u) |
+                                             ((first && sign) ? PE_SIGN : 0u));
+                        first = false;
+                    }
                 }
             }
+            if (pull_words.size() > 0x7fffff00u) { delete P; return AFS_ERR_UNSUPPORTED; }
+            pull_ptr[v + 1] = (int32_t)pull_words.size();
+            run_ptr[v + 1] = (int32_t)runs.size();
         }
+        occs.clear(); occs.shrink_to_fit();
+        pull_words.resize(pull_words.size() + 32, 0u);   // staged chunk loads may read up to 31 entries past a stream
+        P->pull_words = pull_ptr[n];
         // ------------------------------------------------------------ medium constraints (sorted by padded length)
         std::vector<MedCon> med;
         std::vector<uint32_t> med_lits;
@@ -198,38 +221,42 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
             P->n_med = (int64_t)ids.size();
         }
         // ------------------------------------------------------------ long constraints (sorted by row count, longest first)
-        std::vector<LongCon> lng;
-        std::vector<uint32_t> long_lits;
-        std::vector<int32_t> long_slots;
-        {
+        std::vector<LongCon> lng, cmv;
+        std::vector<uint32_t> long_lits, cm_lits;
+        std::vector<int32_t> long_slots, cm_slots;
+        auto build_count_class = [&](int want_cls, auto bucket_fn, int nbuckets, int32_t* begin, int32_t* maxL,
+                                     std::vector<LongCon>& out, std::vector<uint32_t>& olits, std::vector<int32_t>& oslots) {
             std::vector<int> ids;
-            for (int c = 0; c < m; ++c) if (cls[c] == C_LONG) ids.push_back(c);
-            auto nr_of = [&](int c) { return (int)((row_ptr[c + 1] - row_ptr[c] + 1 + 127) / 128); };   // rows for q_0..q_L
+            for (int c = 0; c < m; ++c) if (cls[c] == want_cls) ids.push_back(c);
             std::stable_sort(ids.begin(), ids.end(), [&](int a, int b) {
-                int ra = nr_of(a), rb = nr_of(b);
+                int ra = bucket_fn(a), rb = bucket_fn(b);
                 if (ra != rb) return ra < rb;
                 return (row_ptr[a + 1] - row_ptr[a]) > (row_ptr[b + 1] - row_ptr[b]);
             });
             int cur = 0;
-            P->long_begin[0] = 0;
+            begin[0] = 0;
             for (size_t i = 0; i < ids.size(); ++i) {
                 int c = ids[i];
-                int bk = nr_of(c) - 1;
-                while (cur < bk) P->long_begin[++cur] = (int32_t)i;
+                int bk = bucket_fn(c);
+                while (cur < bk) begin[++cur] = (int32_t)i;
                 LongCon lc;
-                lc.off = (int32_t)long_lits.size(); lc.L = (int32_t)(row_ptr[c + 1] - row_ptr[c]);
+                lc.off = (int32_t)olits.size(); lc.L = (int32_t)(row_ptr[c + 1] - row_ptr[c]);
                 lc.type = types[c]; lc.k = k[c];
                 long_targets(lc.type, lc.L, lc.k, lc);
-                P->long_maxL[bk] = std::max(P->long_maxL[bk], lc.L);
+                if (maxL) maxL[bk] = std::max(maxL[bk], lc.L);
                 for (int64_t e = row_ptr[c]; e < row_ptr[c + 1]; ++e) {
-                    long_lits.push_back(lit_word(lits[e]));
-                    long_slots.push_back(slot_of[e]);
+                    olits.push_back(lit_word(lits[e]));
+                    oslots.push_back(slot_of[e]);
                 }
-                lng.push_back(lc);
+                out.push_back(lc);
             }
-            while (cur < LONG_BUCKETS) P->long_begin[++cur] = (int32_t)ids.size();
-            P->n_long = (int64_t)ids.size();
-        }
+            while (cur < nbuckets) begin[++cur] = (int32_t)ids.size();
+            return (int64_t)ids.size();
+        };
+        P->n_long = build_count_class(C_LONG, [&](int c) { return (int)((row_ptr[c + 1] - row_ptr[c] + 1 + 127) / 128) - 1; },
+                                      LONG_BUCKETS, P->long_begin, P->long_maxL, lng, long_lits, long_slots);
+        P->n_cm = build_count_class(C_CMED, [&](int c) { return (int)((row_ptr[c + 1] - row_ptr[c] + 15) / 16) - 1; },
+                                    CM_BUCKETS, P->cm_begin, nullptr, cmv, cm_lits, cm_slots);
         // ------------------------------------------------------------ generic forward CSR for the count-only kernel
         std::vector<CountCon> cnt(m);
         std::vector<uint32_t> cnt_lits((size_t)P->nnz);
@@ -243,6 +270,11 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
         auto up = [&](auto** dst, const auto& src) { if (st == AFS_OK) st = upload(dst, src); };
         up(&P->d_pull_ptr, pull_ptr);
         up(&P->d_pull_words, pull_words);
+        up(&P->d_run_ptr, run_ptr);
+        up(&P->d_runs, runs);
+        up(&P->d_pull_gconst, gconst);
+        up(&P->d_pc, pc);
+        up(&P->d_pc_lits, pc_lits);
         up(&P->d_slot_ptr, slot_ptr);
         up(&P->d_med, med);
         up(&P->d_med_lits, med_lits);
@@ -250,6 +282,9 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
         up(&P->d_long, lng);
         up(&P->d_long_lits, long_lits);
         up(&P->d_long_slots, long_slots);
+        up(&P->d_cm, cmv);
+        up(&P->d_cm_lits, cm_lits);
+        up(&P->d_cm_slots, cm_slots);
         up(&P->d_count, cnt);
         up(&P->d_count_lits, cnt_lits);
         if (st != AFS_OK) { afs_problem_destroy(P); return st; }
@@ -270,8 +305,10 @@ extern "C" void afs_problem_destroy(afs_problem* p)
     cudaSetDevice(p->device);
     cudaDeviceSynchronize();
     cudaFree(p->d_pull_ptr); cudaFree(p->d_pull_words); cudaFree(p->d_slot_ptr);
+    cudaFree(p->d_run_ptr); cudaFree(p->d_runs); cudaFree(p->d_pull_gconst); cudaFree(p->d_pc); cudaFree(p->d_pc_lits);
     cudaFree(p->d_med); cudaFree(p->d_med_lits); cudaFree(p->d_med_slots);
     cudaFree(p->d_long); cudaFree(p->d_long_lits); cudaFree(p->d_long_slots);
+    cudaFree(p->d_cm); cudaFree(p->d_cm_lits); cudaFree(p->d_cm_slots);
     cudaFree(p->d_count); cudaFree(p->d_count_lits);
     afs::free_workspace(p);
     (void)cudaGetLastError();
@@ -287,7 +324,7 @@ extern "C" int64_t afs_problem_info(const afs_problem* p, int32_t what)
     case 2: return p->nnz;
     case 3: return p->n_pull;
     case 4: return p->n_med;
-    case 5: return p->n_long;
+    case 5: return p->n_long + p->n_cm;
     case 6: return p->nslots;
     case 7: return p->last_launches;
     case 8: return (int64_t)p->ws.bytes;

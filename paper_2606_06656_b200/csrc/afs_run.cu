@@ -29,7 +29,7 @@ void free_workspace(afs_problem* P)
     free_ptr(w.XT[0]); free_ptr(w.XT[1]); free_ptr(w.scratch);
     free_ptr(w.sat_hist); free_ptr(w.best_sat[0]); free_ptr(w.best_sat[1]);
     free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.best_bits);
-    free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.f_part);
+    free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.fe_cm); free_ptr(w.f_part);
     free_ptr(w.mask_dev); free_ptr(w.host_stage_X); free_ptr(w.host_stage_assign);
     free_ptr(w.host_stage_sat); free_ptr(w.host_stage_step);
     w = Workspace();
@@ -38,6 +38,9 @@ void free_workspace(afs_problem* P)
 }  // namespace afs
 
 static int var_grid_x(int n) { return (n + VAR_WARPS * VAR_VPW - 1) / (VAR_WARPS * VAR_VPW); }
+// number of per-warp partial sums of k_fe_pull: fixed per problem, so the objective is reproducible
+static int fe_pull_grid_x(const afs_problem* P) { int g = (int)((P->n_pull + 63) / 64); return g < 1 ? 1 : (g > 2048 ? 2048 : g); }
+static int fe_pull_parts(const afs_problem* P) { return fe_pull_grid_x(P) * 8; }
 
 template <typename T>
 static afs_status dev_alloc(T** p, size_t count, size_t& total)
@@ -79,14 +82,15 @@ static afs_status ensure_eval_buffers(afs_problem* P, int Bp, size_t elem)
     Workspace& w = P->ws;
     if (w.fe_Bp >= Bp && w.fe_med) return AFS_OK;
     CU(cudaDeviceSynchronize());
-    free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.f_part);
+    free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.fe_cm); free_ptr(w.f_part);
     size_t tot = 0;
     afs_status st = AFS_OK;
     auto A = [&](auto** p, size_t cnt) { if (st == AFS_OK) st = dev_alloc(p, cnt, tot); };
     size_t e = w.elem > elem ? w.elem : elem;
     A((unsigned char**)&w.fe_med, (size_t)P->n_med * w.Bp * e);
     A((unsigned char**)&w.fe_long, (size_t)P->n_long * w.Bp * e);
-    A((unsigned char**)&w.f_part, (size_t)var_grid_x(P->n) * VAR_WARPS * w.Bp * e);
+    A((unsigned char**)&w.fe_cm, (size_t)P->n_cm * w.Bp * e);
+    A((unsigned char**)&w.f_part, (size_t)fe_pull_parts(P) * w.Bp * e);
     if (st != AFS_OK) return st;
     w.fe_Bp = w.Bp; w.bytes += tot;
     return AFS_OK;
@@ -122,9 +126,24 @@ static afs_status launch_long(afs_problem* P, int bucket, const real* XT, int Bp
 
 template <typename real>
 static afs_status launch_push(afs_problem* P, const real* XT, int Bp, real* scratch, int32_t* sat, real* fe_med,
-                              real* fe_long, cudaStream_t st)
+                              real* fe_cm, real* fe_long, cudaStream_t st)
 {
     const int tiles = Bp / 32;
+    for (int bk = 0; bk < CM_BUCKETS; ++bk) {
+        int c0 = P->cm_begin[bk], c1 = P->cm_begin[bk + 1];
+        if (c1 <= c0) continue;
+        int gx = (c1 - c0 + 3) / 4;
+        int cap = (P->sm_count * 16 + tiles - 1) / tiles;
+        if (gx > cap) gx = cap < 1 ? 1 : cap;
+        dim3 grid(gx, tiles);
+        switch (bk) {
+        case 0: k_cmed<real, 16><<<grid, 128, 0, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat, fe_cm); break;
+        case 1: k_cmed<real, 32><<<grid, 128, 0, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat, fe_cm); break;
+        case 2: k_cmed<real, 48><<<grid, 128, 0, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat, fe_cm); break;
+        default: k_cmed<real, 64><<<grid, 128, 0, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat, fe_cm); break;
+        }
+        P->last_launches++;
+    }
     for (int bk = 0; bk < MED_BUCKETS; ++bk) {
         int c0 = P->med_begin[bk], c1 = P->med_begin[bk + 1];
         if (c1 <= c0) continue;
@@ -163,6 +182,29 @@ static afs_status launch_count(afs_problem* P, const real* XT, int Bp, int32_t* 
     return AFS_OK;
 }
 
+// S9 of the PULL class from the sign words of the iterate (bit-parallel over restarts)
+static afs_status launch_sat_pull(afs_problem* P, const uint32_t* S, int Bp, int32_t* sat, cudaStream_t st)
+{
+    if (P->n_pull == 0) return AFS_OK;
+    const int ntile = Bp / 32;
+    const int gy = (ntile + SATP_TG - 1) / SATP_TG;
+    // enough chunks to fill the chip, at most 1023 clauses each
+    long long want = (long long)P->sm_count * 8 * SATP_CPB / gy;
+    if (want < 1) want = 1;
+    int chunk = (int)((P->n_pull + want - 1) / want);
+    if (chunk < 15) chunk = 15;
+    if (chunk > 1023) chunk = 1023;
+    const int nchunks = (int)((P->n_pull + chunk - 1) / chunk);
+    dim3 grid((nchunks + SATP_CPB - 1) / SATP_CPB, gy);
+    const int m = (int)P->n_pull;
+    if (chunk <= 15) k_sat_pull<4><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, chunk, S, ntile, sat);
+    else if (chunk <= 63) k_sat_pull<6><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, chunk, S, ntile, sat);
+    else if (chunk <= 255) k_sat_pull<8><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, chunk, S, ntile, sat);
+    else k_sat_pull<10><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, chunk, S, ntile, sat);
+    P->last_launches++;
+    return AFS_OK;
+}
+
 static afs_status enter(afs_problem* P, int32_t B)
 {
     if (!P || B < 1) return AFS_ERR_INVALID_ARG;
@@ -187,23 +229,29 @@ static afs_status eval_grad_impl(afs_problem* P, const real* X, int32_t B, real*
     real* XT = (real*)w.XT[0];
     real* GT = (real*)w.XT[1];
     real* scratch = (real*)w.scratch;
-    real* fe_med = (real*)w.fe_med; real* fe_long = (real*)w.fe_long; real* fpart = (real*)w.f_part;
+    real* fe_med = (real*)w.fe_med; real* fe_long = (real*)w.fe_long; real* fe_cm = (real*)w.fe_cm;
+    real* fpart = (real*)w.f_part;
     dim3 tg((P->n + 31) / 32, Bp / 32);
     k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, wBp, nullptr);
     P->last_launches++;
-    if ((s = launch_push<real>(P, XT, wBp, scratch, nullptr, fe_med, fe_long, st)) != AFS_OK) return s;
+    if ((s = launch_push<real>(P, XT, wBp, scratch, nullptr, fe_med, fe_cm, fe_long, st)) != AFS_OK) return s;
     VarArgs<real> a{};
     a.n = P->n; a.Bp = wBp; a.t = 0;
-    a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.slot_ptr = P->d_slot_ptr;
+    a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
+    a.gconst = P->d_pull_gconst; a.slot_ptr = P->d_slot_ptr;
     a.scratch = scratch; a.Xin = XT; a.Xout = nullptr; a.lr = real(0); a.mask = nullptr;
-    a.GT = GT; a.Fpart = fpart;
+    a.GT = GT;
     const int gx = var_grid_x(P->n);
-    k_var<real, true><<<dim3(gx, Bp / 32), VAR_WARPS * 32, 0, st>>>(a);
-    P->last_launches++;
-    if (F) {
-        k_reduce_F<real><<<(B + 127) / 128, 128, 0, st>>>(fpart, gx * VAR_WARPS, fe_med, (int)P->n_med, fe_long,
-                                                         (int)P->n_long, wBp, B, F);
+    if (G) {
+        k_var<real, true><<<dim3(gx, Bp / 32), VAR_WARPS * 32, 0, st>>>(a);
         P->last_launches++;
+    }
+    if (F) {
+        const int fgx = fe_pull_grid_x(P);
+        k_fe_pull<real><<<dim3(fgx, Bp / 32), 256, 0, st>>>(P->d_pc, P->d_pc_lits, (int)P->n_pull, XT, wBp, fpart);
+        k_reduce_F<real><<<(B + 127) / 128, 128, 0, st>>>(fpart, fgx * 8, fe_med, (int)P->n_med, fe_cm, (int)P->n_cm,
+                                                         fe_long, (int)P->n_long, wBp, B, F);
+        P->last_launches += 2;
     }
     if (G) {
         k_transpose_out<real><<<tg, 256, 0, st>>>(GT, G, B, P->n, wBp);
@@ -264,17 +312,19 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     for (int t = 0; t < steps; ++t) {
         const real* Xin = XT[t & 1];
         int32_t* sat_cur = w.sat_hist + (size_t)t * Bp;
-        if ((s = launch_push<real>(P, Xin, Bp, scratch, sat_cur, nullptr, nullptr, st)) != AFS_OK) return s;
+        if ((s = launch_push<real>(P, Xin, Bp, scratch, sat_cur, nullptr, nullptr, nullptr, st)) != AFS_OK) return s;
         VarArgs<real> a{};
         a.n = P->n; a.Bp = Bp; a.t = t;
-        a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.slot_ptr = P->d_slot_ptr;
+        a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
+        a.gconst = P->d_pull_gconst; a.slot_ptr = P->d_slot_ptr;
         a.scratch = scratch; a.Xin = Xin; a.Xout = XT[(t + 1) & 1]; a.lr = lr; a.mask = mask;
-        a.sat_cur = sat_cur; a.sat_prev = t > 0 ? w.sat_hist + (size_t)(t - 1) * Bp : nullptr;
+        a.sat_prev = t > 0 ? w.sat_hist + (size_t)(t - 1) * Bp : nullptr;
         a.best_sat_in = w.best_sat[t & 1]; a.best_sat_out = w.best_sat[(t + 1) & 1];
         a.best_step_in = w.best_step[t & 1]; a.best_step_out = w.best_step[(t + 1) & 1];
         a.S_prev = w.S[(t + 1) & 1]; a.S_cur = w.S[t & 1]; a.best_bits = w.best_bits;
         k_var<real, false><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
         P->last_launches++;
+        if ((s = launch_sat_pull(P, w.S[t & 1], Bp, sat_cur, st)) != AFS_OK) return s;
     }
     // the last iterate: count only, then fold and write out
     const real* Xfin = XT[steps & 1];
