@@ -640,59 +640,92 @@ struct VarArgs {
 
 __device__ __forceinline__ float flip(float x, uint32_t signbit) { return __int_as_float(__float_as_int(x) ^ (int)signbit); }
 __device__ __forceinline__ double flip(double x, uint32_t signbit) { return signbit ? -x : x; }
-// +-0.5 with the sign of a negated literal: u = h x + 0.5 is (1 + y)/2 for y = +-x
-__device__ __forceinline__ float halfsigned(float, uint32_t signbit) { return __int_as_float(0x3f000000 | (int)signbit); }
-__device__ __forceinline__ double halfsigned(double, uint32_t signbit) { return signbit ? -0.5 : 0.5; }
+
+// Per-entry auxiliary word, decoded once per staged chunk (one entry per lane):
+//   fp32 OR/NAE: the bits of h = +-0.5 (sign = literal negated), so that u = h x + 0.5;   fp32 XOR: the sign mask
+//   fp64 (verification build): just the negation flag
+template <typename real, int KIND>
+__device__ __forceinline__ uint32_t pull_aux(uint32_t w)
+{
+    if (sizeof(real) == 4 && KIND != (int)PH_KIND_XOR) return 0x3f000000u | (w & PE_NEG);
+    return w & PE_NEG;
+}
+__device__ __forceinline__ float pull_u(float x, uint32_t aux) { return fmaf(__int_as_float((int)aux), x, 0.5f); }
+__device__ __forceinline__ double pull_u(double x, uint32_t aux) { return (aux ? -0.5 : 0.5) * x + 0.5; }
+__device__ __forceinline__ float pull_p(float x, uint32_t aux) { return fmaf(-__int_as_float((int)aux), x, 0.5f); }
+__device__ __forceinline__ double pull_p(double x, uint32_t aux) { return 0.5 - (aux ? -0.5 : 0.5) * x; }
+
+constexpr int PULL_SBUF = 48;   // uint2 slots per warp: 32 staged entries + slack for the unrolled tail (kept valid)
 
 // One run: `count` occurrences of NOTHER other literals each, entries at words[beg ...).  xcol points at column b of
-// the X matrix (global XT or a shared-memory tile), rowstride is its row pitch in elements.  Returns the run's
-// contribution to dF/dx_v (already carrying the sign of the own literal).
+// the X matrix (global XT or a shared-memory tile), rowbytes is its row pitch in bytes (rows * rowbytes < 2^32).
+// The warp loads 32 entries with one coalesced load, every lane decodes its entry (byte offset of the row, sign
+// material) into the warp's shared staging buffer, and all lanes then walk the occurrences reading whole records
+// with one broadcast LDS each.  Returns the run's contribution to dF/dx_v (carrying the own literal's sign).
 template <typename real, int KIND, int NOTHER>
 __device__ __forceinline__ real pull_run(const uint32_t* __restrict__ words, int beg, int count,
-                                         const real* __restrict__ xcol, size_t rowstride, int lane)
+                                         const real* __restrict__ xcol, uint32_t rowbytes, int lane, uint2* sbuf)
 {
     constexpr int OPC = 32 / NOTHER;              // occurrences per staged chunk of <= 32 entries
     constexpr int U = NOTHER <= 2 ? 4 : 2;        // occurrences gathered together
-    const real one = real(1), half = real(0.5);
+    const char* __restrict__ xb = reinterpret_cast<const char*>(xcol);
     real g = real(0);
     for (int o0 = 0; o0 < count; o0 += OPC) {
         const int nocc = min(OPC, count - o0);
-        const uint32_t mine = words[beg + o0 * NOTHER + lane];   // over-read past the chunk is harmless (padded array)
+        const uint32_t wm = words[beg + o0 * NOTHER + lane];   // reading past the run is harmless (valid entries / padding)
+        // the sign flag rides in bit 0 of the first offset of an occurrence; entries past the chunk (staged only so
+        // that the unrolled tail reads valid rows) must not carry it, or the tail's loads would be misaligned
+        const uint32_t sgn = lane < nocc * NOTHER ? (wm >> 30) & 1u : 0u;
+        sbuf[lane] = make_uint2((wm & PE_VAR) * rowbytes | sgn, pull_aux<real, KIND>(wm));
+        __syncwarp();
         for (int o = 0; o < nocc; o += U) {
-            uint32_t w[U][NOTHER];
+            uint2 e[U][NOTHER];
             real x[U][NOTHER];
 #pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const uint2* rec = sbuf + (o + u) * NOTHER;
+                if (NOTHER == 2) {
+                    uint4 t = *reinterpret_cast<const uint4*>(rec);
+                    e[u][0] = make_uint2(t.x, t.y); e[u][NOTHER - 1] = make_uint2(t.z, t.w);
+                } else if (NOTHER == 4) {
+                    uint4 t0 = *reinterpret_cast<const uint4*>(rec), t1 = *reinterpret_cast<const uint4*>(rec + 2);
+                    e[u][0] = make_uint2(t0.x, t0.y); e[u][1 % NOTHER] = make_uint2(t0.z, t0.w);
+                    e[u][2 % NOTHER] = make_uint2(t1.x, t1.y); e[u][3 % NOTHER] = make_uint2(t1.z, t1.w);
+                } else {
+#pragma unroll
+                    for (int i = 0; i < NOTHER; ++i) e[u][i] = rec[i];
+                }
+            }
+#pragma unroll
             for (int u = 0; u < U; ++u)
 #pragma unroll
-                for (int i = 0; i < NOTHER; ++i) w[u][i] = __shfl_sync(FULL, mine, ((o + u) * NOTHER + i) & 31);
-#pragma unroll
-            for (int u = 0; u < U; ++u)
-#pragma unroll
-                for (int i = 0; i < NOTHER; ++i) x[u][i] = xcol[(size_t)(w[u][i] & PE_VAR) * rowstride];
+                for (int i = 0; i < NOTHER; ++i)
+                    x[u][i] = *reinterpret_cast<const real*>(xb + (i == 0 ? (e[u][0].x & ~1u) : e[u][i].x));
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 real d;
                 if (KIND == (int)PH_KIND_XOR) {
-                    real prod = flip(x[u][0], w[u][0] & PE_NEG);
+                    real prod = flip(x[u][0], e[u][0].y);
 #pragma unroll
-                    for (int i = 1; i < NOTHER; ++i) prod *= flip(x[u][i], w[u][i] & PE_NEG);
+                    for (int i = 1; i < NOTHER; ++i) prod *= flip(x[u][i], e[u][i].y);
                     d = prod;
                 } else {
-                    real pu = halfsigned(one, w[u][0] & PE_NEG) * x[u][0] + half;
+                    real pu = pull_u(x[u][0], e[u][0].y);
 #pragma unroll
-                    for (int i = 1; i < NOTHER; ++i) pu *= halfsigned(one, w[u][i] & PE_NEG) * x[u][i] + half;
+                    for (int i = 1; i < NOTHER; ++i) pu *= pull_u(x[u][i], e[u][i].y);
                     d = pu;
                     if (KIND == (int)PH_KIND_NAE) {
-                        real pp = half - halfsigned(one, w[u][0] & PE_NEG) * x[u][0];
+                        real pp = pull_p(x[u][0], e[u][0].y);
 #pragma unroll
-                        for (int i = 1; i < NOTHER; ++i) pp *= half - halfsigned(one, w[u][i] & PE_NEG) * x[u][i];
+                        for (int i = 1; i < NOTHER; ++i) pp *= pull_p(x[u][i], e[u][i].y);
                         d = pu - pp;
                     }
                 }
-                d = flip(d, (w[u][0] & PE_SIGN) << 1);
+                d = flip(d, e[u][0].x << 31);
                 if (o + u < nocc) g += d;
             }
         }
+        __syncwarp();
     }
     return g;
 }
@@ -701,7 +734,7 @@ __device__ __forceinline__ real pull_run(const uint32_t* __restrict__ words, int
 template <typename real>
 __device__ __forceinline__ real pull_variable(const uint32_t* __restrict__ runs, int rbeg, int rend,
                                               const uint32_t* __restrict__ words, int wbeg,
-                                              const real* __restrict__ xcol, size_t rowstride, int lane)
+                                              const real* __restrict__ xcol, uint32_t rowbytes, int lane, uint2* sbuf)
 {
     real g = real(0);
     int pos = wbeg;
@@ -709,7 +742,7 @@ __device__ __forceinline__ real pull_variable(const uint32_t* __restrict__ runs,
         const uint32_t d = runs[r];
         const int count = (int)(d & 0x07ffffffu), nother = (int)((d >> 27) & 7u), kind = (int)(d >> 30);
         real gr;
-#define AFS_RUN(K, N) gr = pull_run<real, K, N>(words, pos, count, xcol, rowstride, lane)
+#define AFS_RUN(K, N) gr = pull_run<real, K, N>(words, pos, count, xcol, rowbytes, lane, sbuf)
         if (kind == (int)PH_KIND_OR) {
             switch (nother) { case 1: AFS_RUN(0, 1); break; case 2: AFS_RUN(0, 2); break; case 3: AFS_RUN(0, 3); break; default: AFS_RUN(0, 4); break; }
         } else if (kind == (int)PH_KIND_XOR) {
@@ -727,12 +760,16 @@ __device__ __forceinline__ real pull_variable(const uint32_t* __restrict__ runs,
 template <typename real, bool EVAL>
 __global__ void __launch_bounds__(VAR_WARPS * 32, 4) k_var(const VarArgs<real> a)
 {
+    __shared__ __align__(16) uint2 s_stage[VAR_WARPS][PULL_SBUF];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int tile = blockIdx.y, ntile = a.Bp >> 5;
     const int b = tile * 32 + lane;
     const int Bp = a.Bp;
     const real one = real(1);
     const real* __restrict__ xcol = a.Xin + b;
+    uint2* sbuf = s_stage[warp];
+    for (int i = lane; i < PULL_SBUF; i += 32) sbuf[i] = make_uint2(0u, 0u);   // slack slots must stay valid offsets
+    __syncwarp();
     const int vbeg = (blockIdx.x * VAR_WARPS + warp) * VAR_VPW;
     const int vend = min(vbeg + VAR_VPW, a.n);
     // ---- S10: did the previous iterate improve on the best so far?
@@ -767,7 +804,7 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 4) k_var(const VarArgs<real> a
         if (mk == 0) {   // a fixed variable never moves: its gradient is not needed
             g = (real)a.gconst[v];
             g += pull_variable<real>(a.runs, a.run_ptr[v], a.run_ptr[v + 1], a.pull_words, a.pull_ptr[v], xcol,
-                                     (size_t)Bp, lane);
+                                     (uint32_t)Bp * (uint32_t)sizeof(real), lane, sbuf);
             // ---- S6: materialised gradients of v, fixed (transposed-CSR) order
             const int s1 = a.slot_ptr[v + 1];
             int s = a.slot_ptr[v];

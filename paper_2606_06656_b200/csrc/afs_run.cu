@@ -208,6 +208,8 @@ static afs_status launch_sat_pull(afs_problem* P, const uint32_t* S, int Bp, int
 static afs_status enter(afs_problem* P, int32_t B)
 {
     if (!P || B < 1) return AFS_ERR_INVALID_ARG;
+    // row offsets inside the kernels are 32-bit byte offsets: n * Bp * 8 must stay below 4 GiB
+    if ((unsigned long long)P->n * (unsigned long long)(((B + 31) / 32) * 32) * 8ull >= (1ull << 32)) return AFS_ERR_UNSUPPORTED;
     if (cudaSetDevice(P->device) != cudaSuccess) { (void)cudaGetLastError(); return AFS_ERR_CUDA; }
     P->last_launches = 0;
     return AFS_OK;
