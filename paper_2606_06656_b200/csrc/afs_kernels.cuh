@@ -4,6 +4,7 @@
 // BASELINE.json.  P:Lnn = PAPER.md line nn.
 #pragma once
 #include "afs_internal.h"
+#include "afs_long.cuh"
 
 namespace afs {
 
@@ -430,173 +431,6 @@ __global__ void __launch_bounds__(128) k_prod_long(const MedCon* __restrict__ co
         if (warp == 0) {
             int tot = s_sat[0][lane] + s_sat[1][lane] + s_sat[2][lane] + s_sat[3][lane];
             if (tot) atomicAdd(&sat[b], tot);
-        }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------------------------
-// LONG class: warp = (constraint, restart), CTA = one constraint x 8 restarts.  Count basis (G10):
-//   forward   q = pmf of the number of true literals, q_t <- q_t u_j + q_{t-1} p_j.  The pmf lives in registers,
-//             cell t = (row*32 + lane)*4 + c; rows that are still identically zero are skipped (warp-uniform).
-//   gradient  dFE/dy_j = sum_t d_t q_t^(-j) with at most two non-zero d_t.  q^(-j) comes from q by removing
-//             literal j in the STABLE direction: with s_t = u_j r_t,  s_t = q_t - (p_j/u_j) s_{t-1}  when p_j <= 1/2,
-//             else from the top with the roles of u and p swapped (reversed copy of q).  The divisor is >= 1/2:
-//             nothing that vanishes at x = +-1 is ever divided by (BASELINE.json subsystem (2)).
-// ------------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void load4(const float* p, float (&v)[4])
-{
-    float4 t = *reinterpret_cast<const float4*>(p);
-    v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
-}
-__device__ __forceinline__ void load4(const double* p, double (&v)[4])
-{
-    double2 a = *reinterpret_cast<const double2*>(p), b = *reinterpret_cast<const double2*>(p + 2);
-    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
-}
-
-template <typename real, int NR, int PH>
-__device__ __forceinline__ void dp_run(real (&q)[NR][4], const real* __restrict__ ys, int jbeg, int jend, int lane)
-{
-    const int src = (lane + 31) & 31;
-    for (int j = jbeg; j < jend; ++j) {
-        const real y = ys[j];
-        const real u = real(0.5) + real(0.5) * y, p = real(0.5) - real(0.5) * y;
-        real rot[PH + 1];
-#pragma unroll
-        for (int r = 0; r <= PH; ++r) rot[r] = __shfl_sync(FULL, q[r][3], src);
-#pragma unroll
-        for (int r = PH; r >= 0; --r) {
-            real carry = rot[r];
-            if (lane == 0) carry = r > 0 ? rot[r > 0 ? r - 1 : 0] : real(0);
-            q[r][3] = q[r][3] * u + q[r][2] * p;
-            q[r][2] = q[r][2] * u + q[r][1] * p;
-            q[r][1] = q[r][1] * u + q[r][0] * p;
-            q[r][0] = q[r][0] * u + carry * p;
-        }
-    }
-}
-
-template <typename real, int NR, int PH>
-struct DpPhases {
-    static __device__ __forceinline__ void run(real (&q)[NR][4], const real* __restrict__ ys, int L, int lane, int j)
-    {
-        if constexpr (PH < NR) {
-            // after literal j the count can reach j+1: row (j+1)/128 must be live, i.e. j <= 128 (PH+1) - 2
-            int jend = PH == NR - 1 ? L : min(L, 128 * (PH + 1) - 1);
-            dp_run<real, NR, PH>(q, ys, j, jend, lane);
-            DpPhases<real, NR, PH + 1>::run(q, ys, L, lane, jend > j ? jend : j);
-        }
-    }
-};
-
-template <typename real, int NR>
-__global__ void __launch_bounds__(256) k_long(const LongCon* __restrict__ cons, int c_begin,
-                                              const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
-                                              const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
-                                              int32_t* __restrict__ sat, real* __restrict__ fe_out, int LS, int QS)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    real* Ys = reinterpret_cast<real*>(smem_raw);   // [8][LS]  literal values of this CTA's 8 restarts
-    real* A = Ys + 8 * LS;                          // [8][QS]  q_0..q_L
-    real* Ar = A + 8 * QS;                          // [8][QS]  reversed: Ar[i] = q_{L-i}
-    __shared__ int s_cnt[8];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int groups = Bp >> 3;
-    const int c = c_begin + (int)(blockIdx.x / groups);
-    const int bg = (int)(blockIdx.x % groups);
-    const LongCon lc = cons[c];
-    const int L = lc.L;
-    const uint32_t* lw = lits + lc.off;
-    const int32_t* sw = slots + lc.off;
-    if (tid < 8) s_cnt[tid] = 0;
-    __syncthreads();
-    // ---- S1: gather the literal values of 8 consecutive restarts (one 32-byte sector per literal in fp32)
-    {
-        const int r = tid & 7;
-        for (int idx = tid; idx < ((L * 8 + 255) & ~255); idx += 256) {
-            int j = idx >> 3;
-            bool tr = false;
-            if (j < L) {
-                uint32_t w = lw[j];
-                real x = ldx(XT, w, Bp, bg * 8 + r);
-                bool neg = (w >> 31) != 0;
-                tr = (x < real(0)) != neg;
-                Ys[r * LS + j] = neg ? -x : x;
-            }
-            unsigned bal = __ballot_sync(FULL, tr);
-            if (lane < 8) {
-                int add = __popc(bal & (0x01010101u << lane));
-                if (add) atomicAdd(&s_cnt[lane], add);
-            }
-        }
-    }
-    __syncthreads();
-    const int b = bg * 8 + warp;
-    const real* ys = Ys + warp * LS;
-    real* Aw = A + warp * QS;
-    real* Arw = Ar + warp * QS;
-    // ---- S2: forward pmf
-    real q[NR][4];
-#pragma unroll
-    for (int r = 0; r < NR; ++r)
-#pragma unroll
-        for (int i = 0; i < 4; ++i) q[r][i] = real(0);
-    if (lane == 0) q[0][0] = real(1);
-    DpPhases<real, NR, 0>::run(q, ys, L, lane, 0);
-    real fe = real(0);
-#pragma unroll
-    for (int r = 0; r < NR; ++r)
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            int t = (r * 32 + lane) * 4 + i;
-            if (t <= L) {
-                Aw[t] = q[r][i];
-                Arw[L - t] = q[r][i];
-                fe += pred(lc.type, L, lc.k, t) ? -q[r][i] : q[r][i];   // sp_t = -1 where satisfied
-            }
-        }
-    for (int t = L + 1 + lane; t < QS; t += 32) { Aw[t] = real(0); Arw[t] = real(0); }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) fe += __shfl_xor_sync(FULL, fe, o);
-    if (lane == 0) {
-        if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
-        if (sat && pred(lc.type, L, lc.k, s_cnt[warp])) atomicAdd(&sat[b], 1);
-    }
-    __syncwarp();
-    // ---- S3 + S5: leave-one-out by stable-direction deconvolution, lanes over literals
-    const bool useA = lc.wA != 0.f, useB = lc.wB != 0.f;
-    for (int j0 = 0; j0 < L; j0 += 32) {
-        const int j = j0 + lane;
-        const bool act = j < L;
-        const real y = act ? ys[j] : real(1);
-        const real u = real(0.5) + real(0.5) * y, p = real(0.5) - real(0.5) * y;
-        const bool fwd = !(y < real(0));             // p <= 1/2
-        const real D = fwd ? u : p;                  // >= 1/2
-        const real R = (fwd ? p : u) / D;            // <= 1
-        const real* base = fwd ? Aw : Arw;
-        const int iA = fwd ? lc.tA : L - 1 - lc.tA;
-        const int iB = fwd ? lc.tB : L - 1 - lc.tB;
-        int iend = -1;
-        if (act && useA) iend = iA;
-        if (act && useB && iB > iend) iend = iB;
-        int wend = iend;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) wend = max(wend, __shfl_xor_sync(FULL, wend, o));
-        real s = real(0), sA = real(0), sB = real(0);
-        for (int i = 0; i <= wend; i += 4) {
-            real v[4];
-            load4(base + i, v);
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                s = v[e] - R * s;
-                if (i + e == iA) sA = s;
-                if (i + e == iB) sB = s;
-            }
-        }
-        if (act) {
-            real g = ((useA ? (real)lc.wA * sA : real(0)) + (useB ? (real)lc.wB * sB : real(0))) / D;
-            uint32_t w = lw[j];
-            scratch[(size_t)sw[j] * Bp + b] = (w >> 31) ? -g : g;
         }
     }
 }

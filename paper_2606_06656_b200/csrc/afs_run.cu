@@ -99,29 +99,41 @@ static afs_status ensure_eval_buffers(afs_problem* P, int Bp, size_t elem)
 // ----------------------------------------------------------------------------------------------------------------
 // push phase: gradients of the medium and long constraints of iterate XT into scratch (+ counts, + FE)
 // ----------------------------------------------------------------------------------------------------------------
+template <typename real, int NR, int RPC>
+static afs_status launch_long_rpc(afs_problem* P, int bucket, const real* XT, int Bp, real* scratch, int32_t* sat,
+                                  real* fe, cudaStream_t st, int LS, int QS, size_t smem)
+{
+    int c0 = P->long_begin[bucket], c1 = P->long_begin[bucket + 1];
+    static size_t attr_set[2][LONG_BUCKETS] = {};   // largest opt-in made so far, per kernel instance
+    const int ti = sizeof(real) == 8 ? 1 : 0;
+    if (smem > 48 * 1024 && attr_set[ti][bucket] < smem) {
+        CU(cudaFuncSetAttribute(k_long<real, NR, RPC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set[ti][bucket] = smem;
+    }
+    long long blocks = (long long)(c1 - c0) * (Bp / RPC);
+    if (blocks > 0x7fffffffLL) return AFS_ERR_UNSUPPORTED;
+    k_long<real, NR, RPC><<<(unsigned)blocks, RPC * 32, smem, st>>>(P->d_long, c0, P->d_long_lits, P->d_long_slots, XT,
+                                                                    Bp, scratch, sat, fe, LS, QS);
+    P->last_launches++;
+    return AFS_OK;
+}
+
 template <typename real, int NR>
 static afs_status launch_long(afs_problem* P, int bucket, const real* XT, int Bp, real* scratch, int32_t* sat, real* fe,
                               cudaStream_t st)
 {
-    int c0 = P->long_begin[bucket], c1 = P->long_begin[bucket + 1];
-    if (c1 <= c0) return AFS_OK;
+    if (P->long_begin[bucket + 1] <= P->long_begin[bucket]) return AFS_OK;
     int Lmax = P->long_maxL[bucket];
-    int LS = ((Lmax + 31) / 32) * 32 + 4;
-    int QS = ((Lmax + 1 + 3) / 4) * 4 + 4;
-    size_t smem = (size_t)(8 * LS + 16 * QS) * sizeof(real);
-    static size_t attr_set[2][LONG_BUCKETS] = {};   // largest opt-in made so far, per kernel instance
-    const int ti = sizeof(real) == 8 ? 1 : 0;
-    if (smem > 226 * 1024) return AFS_ERR_UNSUPPORTED;
-    if (smem > 48 * 1024 && attr_set[ti][bucket] < smem) {
-        CU(cudaFuncSetAttribute(k_long<real, NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set[ti][bucket] = smem;
-    }
-    long long blocks = (long long)(c1 - c0) * (Bp / 8);
-    if (blocks > 0x7fffffffLL) return AFS_ERR_UNSUPPORTED;
-    k_long<real, NR><<<(unsigned)blocks, 256, smem, st>>>(P->d_long, c0, P->d_long_lits, P->d_long_slots, XT, Bp,
-                                                          scratch, sat, fe, LS, QS);
-    P->last_launches++;
-    return AFS_OK;
+    int LS = ((Lmax + 3 + 31) / 32) * 32;            // list order: L entries + at most 3 neutral ones
+    int QS = ((Lmax + 1 + 3 + 3) / 4) * 4 + 4;       // pmf q_0..q_L behind an offset of at most 3
+    const size_t per_restart = (size_t)LS * (sizeof(real) + sizeof(uint16_t)) + (size_t)QS * sizeof(real);
+    // restarts per CTA: 8 keeps whole 32-byte sectors in the gather (fp32); 4 packs more warps per SM for the longest rows
+    const size_t budget = 227 * 1024;
+    const int w8 = (int)(budget / (8 * per_restart + 1024 + 64)) * 8, w4 = (int)(budget / (4 * per_restart + 1024 + 64)) * 4;
+    if (w4 == 0) return AFS_ERR_UNSUPPORTED;
+    if (w8 >= w4 || w8 >= 32)
+        return launch_long_rpc<real, NR, 8>(P, bucket, XT, Bp, scratch, sat, fe, st, LS, QS, 8 * per_restart);
+    return launch_long_rpc<real, NR, 4>(P, bucket, XT, Bp, scratch, sat, fe, st, LS, QS, 4 * per_restart);
 }
 
 template <typename real>
