@@ -1,20 +1,28 @@
 // afs_long.cuh -- the LONG class: EK / CARD longer than 64 literals (and NAE / EO / AMO too long for the register
 // kernels).  warp = (constraint, restart), CTA = one constraint x RPC restarts.  Count basis (G10):
+//
+//   Q(z) = prod_j (u_j + p_j z),  u = (1+y)/2, p = (1-y)/2,  q_t = [z^t] Q = Pr[t literals true]
+//
 //   gather    per literal the ratio R = min(u, p) / max(u, p) in [0, 1] and its direction (type A: p <= 1/2, type B:
-//             p > 1/2); max(u, p) = 1 / (1 + R) because u + p = 1.  The literals of a restart are then compacted by
-//             type (A first, padded with neutral R = 0 entries to a multiple of four, then B).
-//   forward   Q(z) = prod_j (u_j + p_j z) = prod_A (1 + R_j z) * prod_B (z + R_j) / prod_j (1 + R_j): the pmf q of the
-//             number of true literals is built with ONE FMA per cell and literal -- A: q_t += R q_{t-1};  B: q_t =
-//             q_{t-1} + R q_t -- and the scalar 1 / prod (1 + R_j) is applied every 32 literals (growth inside a block
-//             <= 2^32).  The pmf lives in registers, cell t = (row*32 + lane)*4 + c; rows that are still identically
-//             zero are skipped (warp-uniform).
+//             p > 1/2); max(u, p) = 1 / (1 + R) because u + p = 1.  A literal on the boundary of the cube has R = 0:
+//             y = +1 is the factor 1, y = -1 is the factor z -- an exact shift of the pmf, no arithmetic.  PGD iterates
+//             sit on that boundary in most coordinates (clipping; fixed variables), so the pmf is
+//             built from the INTERIOR literals only:  Q(z) = z^nB0 * Qred(z),  deg Qred = Leff.
+//   lists     the literals of a restart are compacted into  [ B interior | A interior | A boundary | B boundary ],
+//             the interior sections padded with neutral R = 0 entries to multiples of four.
+//   forward   Qred = rev(prod_B (1 + R_j w)) * prod_A (1 + R_j z) / prod (1 + R_j): every literal is the one-FMA
+//             update q_t += R q_{t-1}; after the B section the coefficient vector is reversed once (prod_B (z + R_j)
+//             is the reversal of prod_B (1 + R_j w)).  The scalar 1 / prod (1 + R_j) is applied every 32 literals
+//             (growth inside a block <= 2^32).  The pmf lives in registers, cell t = (row*32 + lane)*4 + c; rows that
+//             are still identically zero are skipped (warp-uniform).
 //   gradient  dFE/dy_j = sum_t d_t q_t^(-j) with at most two non-zero d_t.  q^(-j) comes from q by removing
 //             literal j in the STABLE direction: s_t = q_t - R_j s_{t-1} from the bottom for type A, the same
 //             recurrence from the top for type B; q^(-j) = (1 + R_j) s.  Nothing that vanishes at x = +-1 is ever
 //             divided by (BASELINE.json subsystem (2)).  A warp runs chains of one direction and one length; every
-//             lane carries up to four chains that share each broadcast load of q.
-// The pmf sits in shared memory at A[off + t] with off = (3 - L) mod 4, so that the top-down chains read aligned
-// 16-byte blocks from index 0 and the bottom-up chains after at most three scalar steps.
+//             lane carries up to four chains that share each broadcast load of q.  Boundary literals need no chain:
+//             q^(-j) = q (y = +1) or q shifted by one (y = -1).
+// The reduced pmf sits in shared memory at A[off + t] with off = (3 - Leff) mod 4, so that the top-down chains read
+// aligned 16-byte blocks from index 0 and the bottom-up chains after at most three scalar steps.
 #pragma once
 #include "afs_internal.h"
 
@@ -30,9 +38,11 @@ __device__ __forceinline__ void load4(const double* p, double (&v)[4])
     double2 a = *reinterpret_cast<const double2*>(p), b = *reinterpret_cast<const double2*>(p + 2);
     v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
 }
+__device__ __forceinline__ float recip(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ double recip(double x) { return 1.0 / x; }
 
-// one literal on the live rows 0..PH
-template <typename real, int NR, int PH, bool TYPEB>
+// one literal, q_t += R q_{t-1}, on the live rows 0..PH
+template <typename real, int NR, int PH>
 __device__ __forceinline__ void dp_step(real (&q)[NR][4], const real R, const int lane)
 {
     const int src = (lane + 31) & 31;
@@ -43,73 +53,52 @@ __device__ __forceinline__ void dp_step(real (&q)[NR][4], const real R, const in
     for (int r = PH; r >= 0; --r) {
         real carry = rot[r];
         if (lane == 0) carry = r > 0 ? rot[r > 0 ? r - 1 : 0] : real(0);
-        if (!TYPEB) {
-            q[r][3] = fma(R, q[r][2], q[r][3]);
-            q[r][2] = fma(R, q[r][1], q[r][2]);
-            q[r][1] = fma(R, q[r][0], q[r][1]);
-            q[r][0] = fma(R, carry, q[r][0]);
-        } else {
-            q[r][3] = fma(R, q[r][3], q[r][2]);
-            q[r][2] = fma(R, q[r][2], q[r][1]);
-            q[r][1] = fma(R, q[r][1], q[r][0]);
-            q[r][0] = fma(R, q[r][0], carry);
-        }
+        q[r][3] = fma(R, q[r][2], q[r][3]);
+        q[r][2] = fma(R, q[r][1], q[r][2]);
+        q[r][1] = fma(R, q[r][0], q[r][1]);
+        q[r][0] = fma(R, carry, q[r][0]);
     }
 }
 
+// steps [s0, s1) with rows 0..PH live; s0 and s1 are multiples of 4
 template <typename real, int NR, int PH>
-__device__ __forceinline__ void dp_rescale(real (&q)[NR][4], real& P)
-{
-    const real sc = real(1) / P;
-#pragma unroll
-    for (int r = 0; r <= PH; ++r)
-#pragma unroll
-        for (int i = 0; i < 4; ++i) q[r][i] *= sc;
-    P = real(1);
-}
-
-// steps [s0, s1) of one type with rows 0..PH live; s0 is a multiple of 4
-template <typename real, int NR, int PH, bool TYPEB>
 __device__ __forceinline__ void dp_segment(real (&q)[NR][4], const real* __restrict__ Rc, int s0, int s1, int lane,
                                            real& P)
 {
-    int s = s0;
-    for (; s + 4 <= s1; s += 4) {
+#pragma unroll 1
+    for (int s = s0; s < s1; s += 4) {
         real R[4];
         load4(Rc + s, R);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             P = fma(P, R[e], P);
-            dp_step<real, NR, PH, TYPEB>(q, R[e], lane);
+            dp_step<real, NR, PH>(q, R[e], lane);
         }
-        if (((s + 4) & 31) == 0) dp_rescale<real, NR, PH>(q, P);
-    }
-    for (; s < s1; ++s) {   // tail of the type-B section (at most three literals; no 32-boundary can fall inside)
-        const real R = Rc[s];
-        P = fma(P, R, P);
-        dp_step<real, NR, PH, TYPEB>(q, R, lane);
+        if (((s + 4) & 31) == 0) {
+            const real sc = recip(P);
+#pragma unroll
+            for (int r = 0; r <= PH; ++r)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) q[r][i] *= sc;
+            P = real(1);
+        }
     }
 }
 
 template <typename real, int NR, int PH>
 struct DpPhases {
-    // nA4: end of the (padded) type-A section, send: end of the type-B section
-    static __device__ __forceinline__ void run(real (&q)[NR][4], const real* __restrict__ Rc, int nA4, int send, int lane,
+    // steps [s0, s1) of the list
+    static __device__ __forceinline__ void run(real (&q)[NR][4], const real* __restrict__ Rc, int s0, int s1, int lane,
                                                real& P)
     {
         if constexpr (PH < NR) {
             // rows 0..PH hold cells 0 .. 128(PH+1)-1; a group of four steps starting at s raises the degree to at most
             // s+4, so it may run in this phase while s + 4 <= 128(PH+1) - 1, i.e. (s a multiple of 4) s < 128(PH+1) - 4.
             // The last phase holds every cell up to L and takes everything that is left.
-            const int lo = PH == 0 ? 0 : 128 * PH - 4;
-            const int hi = PH == NR - 1 ? send + 4 : 128 * (PH + 1) - 4;
-            if (lo < send) {
-                const int a1 = min(hi, nA4);
-                if (lo < a1) dp_segment<real, NR, PH, false>(q, Rc, lo, a1, lane, P);
-                const int b0 = max(lo, nA4), b1 = min(hi, send);
-                if (b0 < b1) dp_segment<real, NR, PH, true>(q, Rc, b0, b1, lane, P);
-            }
-            DpPhases<real, NR, PH + 1>::run(q, Rc, nA4, send, lane, P);
+            const int lo = max(s0, PH == 0 ? 0 : 128 * PH - 4);
+            const int hi = PH == NR - 1 ? s1 : min(s1, 128 * (PH + 1) - 4);
+            if (lo < hi) dp_segment<real, NR, PH>(q, Rc, lo, hi, lane, P);
+            DpPhases<real, NR, PH + 1>::run(q, Rc, s0, s1, lane, P);
         }
     }
 };
@@ -126,13 +115,33 @@ __device__ __forceinline__ void chain_advance(const real* __restrict__ A0, int& 
         for (int u = 0; u < U; ++u) s[u] = fma(-R[u], s[u], v);
         ++i;
     }
-    for (; i + 3 <= target; i += 4) {
-        real v[4];
-        if (REV) load4(A0 - i - 3, v); else load4(A0 + i, v);
+    int nblk = (target + 1 - i) >> 2;
+    if (nblk > 0) {
+        const real* p = REV ? A0 - i - 3 : A0 + i;
+        i += nblk * 4;
+#pragma unroll 1
+        for (; nblk >= 2; nblk -= 2) {
+            real v[4], w[4];
+            load4(p, v);
+            load4(REV ? p - 4 : p + 4, w);
+            p = REV ? p - 8 : p + 8;
 #pragma unroll
-        for (int e = 0; e < 4; ++e)
+            for (int e = 0; e < 4; ++e)
 #pragma unroll
-            for (int u = 0; u < U; ++u) s[u] = fma(-R[u], s[u], REV ? v[3 - e] : v[e]);
+                for (int u = 0; u < U; ++u) s[u] = fma(-R[u], s[u], REV ? v[3 - e] : v[e]);
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+#pragma unroll
+                for (int u = 0; u < U; ++u) s[u] = fma(-R[u], s[u], REV ? w[3 - e] : w[e]);
+        }
+        if (nblk) {
+            real v[4];
+            load4(p, v);
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+#pragma unroll
+                for (int u = 0; u < U; ++u) s[u] = fma(-R[u], s[u], REV ? v[3 - e] : v[e]);
+        }
     }
     for (; i <= target; ++i) {
         const real v = REV ? A0[-i] : A0[i];
@@ -141,12 +150,10 @@ __device__ __forceinline__ void chain_advance(const real* __restrict__ A0, int& 
     }
 }
 
-// one round of up to 32*U literals of one direction: list entries [0, cnt)
+// one round of up to 32*U interior literals of one direction: list entries [0, cnt)
 template <typename real, int U, bool REV>
-__device__ __forceinline__ void deconv_round(const real* __restrict__ A0, int mis, const uint16_t* __restrict__ lst,
-                                             const real* __restrict__ Rc, int cnt, int c1, int c2, real w1, real w2,
-                                             const uint32_t* __restrict__ lw, const int32_t* __restrict__ sw,
-                                             real* __restrict__ scratch, size_t Bp, int b, int lane)
+__device__ __forceinline__ void deconv_round(const real* __restrict__ A0, int mis, real* __restrict__ Rc, int cnt,
+                                             int c1, int c2, real w1, real w2, int lane)
 {
     real R[U], s[U], s1[U];
 #pragma unroll
@@ -163,23 +170,15 @@ __device__ __forceinline__ void deconv_round(const real* __restrict__ A0, int mi
 #pragma unroll
     for (int u = 0; u < U; ++u) {
         const int e = u * 32 + lane;
-        if (e < cnt) {
-            const int j = (int)lst[e];
-            const real g = (w1 * s1[u] + w2 * s[u]) * (real(1) + R[u]);
-            const uint32_t w = lw[j];
-            scratch[(size_t)sw[j] * Bp + b] = (w >> 31) ? -g : g;
-        }
+        if (e < cnt) Rc[e] = (w1 * s1[u] + w2 * s[u]) * (real(1) + R[u]);   // dFE/dy_j replaces the ratio
     }
 }
 
 template <typename real, bool REV>
-__device__ __forceinline__ void deconv_dir(const real* __restrict__ A0, int mis, const uint16_t* __restrict__ lst,
-                                           const real* __restrict__ Rc, int cnt, int c1, int c2, real w1, real w2,
-                                           const uint32_t* __restrict__ lw, const int32_t* __restrict__ sw,
-                                           real* __restrict__ scratch, size_t Bp, int b, int lane)
+__device__ __forceinline__ void deconv_dir(const real* __restrict__ A0, int mis, real* __restrict__ Rc, int cnt, int c1,
+                                           int c2, real w1, real w2, int lane)
 {
-#define AFS_ROUND(UU) \
-    deconv_round<real, UU, REV>(A0, mis, lst + e0, Rc + e0, rem, c1, c2, w1, w2, lw, sw, scratch, Bp, b, lane)
+#define AFS_ROUND(UU) deconv_round<real, UU, REV>(A0, mis, Rc + e0, rem, c1, c2, w1, w2, lane)
     for (int e0 = 0; e0 < cnt;) {
         const int rem = cnt - e0;
         if (rem > 96) { AFS_ROUND(4); e0 += 128; }
@@ -213,7 +212,7 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
     extern __shared__ __align__(16) unsigned char smem_raw[];
     real* RcAll = reinterpret_cast<real*>(smem_raw);              // [RPC][LS]  ratios in list order
     real* AAll = RcAll + RPC * LS;                                // [RPC][QS]  signed ratios (gather), then the pmf
-    uint16_t* LstAll = reinterpret_cast<uint16_t*>(AAll + RPC * QS);   // [RPC][LS]  literal index of each list entry
+    uint16_t* InvAll = reinterpret_cast<uint16_t*>(AAll + RPC * QS);   // [RPC][LS]  list position of each literal
     __shared__ int s_cnt[RPC];
     constexpr int NT = RPC * 32;
     constexpr unsigned FULLM = 0xffffffffu;
@@ -242,8 +241,8 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
                 const real y = neg ? -x : x;
                 const real u = real(0.5) + real(0.5) * y, p = real(0.5) - real(0.5) * y;
                 const bool fwd = !(y < real(0));             // p <= 1/2: type A
-                const real R = fwd ? p / u : u / p;          // in [0, 1]; the divisor is >= 1/2
-                AAll[r * QS + j] = fwd ? R : -R;             // -0.0 keeps the direction when R = 0
+                const real R = fwd ? p / u : u / p;          // in [0, 1]; the divisor is >= 1/2; 0 on the boundary
+                AAll[r * QS + j] = fwd ? R : -R;             // the sign bit is the direction (-0.0 for y = -1)
             }
             unsigned bal = __ballot_sync(FULLM, tr);
             if (lane < RPC) {
@@ -256,33 +255,46 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
     const int b = bg * RPC + warp;
     real* Rc = RcAll + warp * LS;
     real* Aw = AAll + warp * QS;
-    uint16_t* lst = LstAll + warp * LS;
-    // ---- compaction by direction: A entries [0, nA), zeros up to nA4, B entries [nA4, nA4 + nB)
-    int nA = 0;
+    uint16_t* inv = InvAll + warp * LS;
+    // ---- lists: [B interior, pad | A interior, pad | A boundary | B boundary]
+    int nBr = 0, nAr = 0, nA0 = 0;
     for (int j0 = 0; j0 < L; j0 += 32) {
         const int j = j0 + lane;
-        nA += __popc(__ballot_sync(FULLM, j < L && !signbit(Aw[j < L ? j : 0])));
+        const bool act = j < L;
+        const real rs = Aw[act ? j : 0];
+        const bool isB = signbit(rs), intr = rs != real(0);
+        nBr += __popc(__ballot_sync(FULLM, act && isB && intr));
+        nAr += __popc(__ballot_sync(FULLM, act && !isB && intr));
+        nA0 += __popc(__ballot_sync(FULLM, act && !isB && !intr));
     }
-    const int nA4 = (nA + 3) & ~3, nB = L - nA, send = nA4 + nB;
+    const int nB0 = L - nBr - nAr - nA0;
+    const int nBr4 = (nBr + 3) & ~3, nAr4 = (nAr + 3) & ~3, send = nBr4 + nAr4, Leff = nBr + nAr;
     {
         const unsigned lt = (1u << lane) - 1u;
-        int pa = 0, pb = nA4;
+        int pBr = 0, pAr = nBr4, pA0 = send, pB0 = send + nA0;
         for (int j0 = 0; j0 < L; j0 += 32) {
             const int j = j0 + lane;
             const bool act = j < L;
             const real rs = Aw[act ? j : 0];
-            const bool isB = act && signbit(rs);
-            const bool isA = act && !isB;
-            const unsigned bA = __ballot_sync(FULLM, isA), bB = __ballot_sync(FULLM, isB);
-            const int pos = isA ? pa + __popc(bA & lt) : pb + __popc(bB & lt);
-            if (act) { Rc[pos] = fabs(rs); lst[pos] = (uint16_t)j; }
-            pa += __popc(bA); pb += __popc(bB);
+            const bool isB = signbit(rs), intr = rs != real(0);
+            const bool cBr = act && isB && intr, cAr = act && !isB && intr, cA0 = act && !isB && !intr,
+                       cB0 = act && isB && !intr;
+            const unsigned mBr = __ballot_sync(FULLM, cBr), mAr = __ballot_sync(FULLM, cAr),
+                           mA0 = __ballot_sync(FULLM, cA0), mB0 = __ballot_sync(FULLM, cB0);
+            int pos = cBr ? pBr + __popc(mBr & lt) : cAr ? pAr + __popc(mAr & lt)
+                    : cA0 ? pA0 + __popc(mA0 & lt) : pB0 + __popc(mB0 & lt);
+            if (act) {
+                inv[j] = (uint16_t)pos;
+                if (intr) Rc[pos] = fabs(rs);
+            }
+            pBr += __popc(mBr); pAr += __popc(mAr); pA0 += __popc(mA0); pB0 += __popc(mB0);
         }
-        if (lane < nA4 - nA) Rc[nA + lane] = real(0);
+        if (lane < nBr4 - nBr) Rc[nBr + lane] = real(0);
+        if (lane < nAr4 - nAr) Rc[nBr4 + nAr + lane] = real(0);
     }
     __syncwarp();
-    // ---- S2: forward pmf
-    const int off = (3 - L) & 3;
+    // ---- S2: forward pmf of the interior literals
+    const int off = (3 - Leff) & 3;
     {
         real q[NR][4];
 #pragma unroll
@@ -291,20 +303,42 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
             for (int i = 0; i < 4; ++i) q[r][i] = real(0);
         if (lane == 0) q[0][0] = real(1);
         real P = real(1);
-        DpPhases<real, NR, 0>::run(q, Rc, nA4, send, lane, P);
-        const real sc = real(1) / P;
-        real fe = real(0);
         for (int t = lane; t < QS; t += 32) Aw[t] = real(0);   // the signed ratios are no longer needed
         __syncwarp();
+        if (nBr > 0) {
+            DpPhases<real, NR, 0>::run(q, Rc, 0, nBr4, lane, P);
+            // prod_B (z + R_j) is the reversal of prod_B (1 + R_j w): c_t -> c_{nBr - t}, through shared memory
+#pragma unroll
+            for (int r = 0; r < NR; ++r)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    int t = (r * 32 + lane) * 4 + i;
+                    if (t <= nBr) Aw[t] = q[r][i];
+                }
+            __syncwarp();
+#pragma unroll
+            for (int r = 0; r < NR; ++r)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    int t = (r * 32 + lane) * 4 + i;
+                    q[r][i] = t <= nBr ? Aw[nBr - t] : real(0);
+                }
+            __syncwarp();
+            for (int t = lane; t <= nBr; t += 32) Aw[t] = real(0);
+            __syncwarp();
+        }
+        DpPhases<real, NR, 0>::run(q, Rc, nBr4, send, lane, P);
+        const real sc = recip(P);
+        real fe = real(0);
 #pragma unroll
         for (int r = 0; r < NR; ++r)
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 int t = (r * 32 + lane) * 4 + i;
-                if (t <= L) {
+                if (t <= Leff) {
                     const real v = q[r][i] * sc;
                     Aw[off + t] = v;
-                    fe += long_pred(lc.type, L, lc.k, t) ? -v : v;   // sp_t = -1 where satisfied
+                    fe += long_pred(lc.type, L, lc.k, t + nB0) ? -v : v;   // sp = -1 where satisfied
                 }
             }
 #pragma unroll
@@ -315,23 +349,49 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
         }
     }
     __syncwarp();
-    // ---- S3 + S5: leave-one-out by stable-direction deconvolution
+    // ---- S3 + S5: leave-one-out
     const bool useA = lc.wA != 0.f, useB = lc.wB != 0.f;
-    if (!useA && !useB) {   // constant expansion (CARD with k = 0 or k = L+1): zero gradient
-        for (int j = lane; j < L; j += 32) scratch[(size_t)sw[j] * Bp + b] = real(0);
-        return;
-    }
     // capture points in true-count index space, t1 <= t2 (equal if only one is used)
     int t1 = lc.tA, t2 = lc.tB;
     real w1 = (real)lc.wA, w2 = (real)lc.wB;
     if (!useA) { t1 = t2; w1 = real(0); }
     if (!useB) { t2 = t1; w2 = w1; w1 = real(0); }
     if (t1 > t2) { int tt = t1; t1 = t2; t2 = tt; real ww = w1; w1 = w2; w2 = ww; }
-    // type A: bottom-up chain over q_0, q_1, ...; captures at t1 then t2
-    deconv_dir<real, false>(Aw + off, off, lst, Rc, nA, t1, t2, w1, w2, lw, sw, scratch, (size_t)Bp, b, lane);
-    // type B: top-down chain over q_L, q_{L-1}, ...; chain index i <-> t = L-1-i, so t2 is met first
-    deconv_dir<real, true>(Aw + off + L, 0, lst + nA4, Rc + nA4, nB, L - 1 - t2, L - 1 - t1, w2, w1, lw, sw, scratch,
-                           (size_t)Bp, b, lane);
+    const real* qr = Aw + off;   // qr[tau] = reduced pmf, tau in [0, Leff]; q_t = qr[t - nB0]
+    // boundary literals: y = +1 leaves q unchanged, y = -1 removes one shift (q^(-j)_t = q_{t+1}).  Every dFE/dy_j
+    // goes to Rc at the literal's list position; the CTA then writes whole 32-byte sectors of the scratch rows.
+    {
+        auto qat = [&](int tau) -> real { return (tau >= 0 && tau <= Leff) ? qr[tau] : real(0); };
+        const real gA0 = w1 * qat(t1 - nB0) + w2 * qat(t2 - nB0);
+        const real gB0 = w1 * qat(t1 + 1 - nB0) + w2 * qat(t2 + 1 - nB0);
+        for (int e = lane; e < nA0 + nB0; e += 32) Rc[send + e] = e < nA0 ? gA0 : gB0;
+    }
+    // interior literals: q^(-j)_t = qred^(-j)_{t - nB0}, qred^(-j) has degree Leff - 1
+    int c1 = t1 - nB0, c2 = t2 - nB0;
+    const bool v1 = c1 >= 0 && c1 <= Leff - 1 && w1 != real(0), v2 = c2 >= 0 && c2 <= Leff - 1 && w2 != real(0);
+    if (!v1 && !v2) {   // the expansion does not depend on the interior literals here (or is constant): zero gradient
+        for (int e = lane; e < send; e += 32) Rc[e] = real(0);
+    } else {
+        if (!v1) { c1 = c2; w1 = real(0); }
+        if (!v2) { c2 = c1; w2 = w1; w1 = real(0); }
+        // type A: bottom-up chain over qr_0, qr_1, ...; captures at c1 then c2
+        deconv_dir<real, false>(qr, off, Rc + nBr4, nAr, c1, c2, w1, w2, lane);
+        // type B: top-down chain over qr_Leff, qr_{Leff-1}, ...; chain index i <-> tau = Leff-1-i, so c2 is met first
+        deconv_dir<real, true>(qr + Leff, 0, Rc, nBr, Leff - 1 - c2, Leff - 1 - c1, w2, w1, lane);
+    }
+    __syncthreads();
+    // ---- S5 + write-out: thread = (literal, restart), restart fastest
+    {
+        const int r = tid % RPC;
+        const real* Rr = RcAll + r * LS;
+        const uint16_t* ir = InvAll + r * LS;
+        real* dst = scratch + (size_t)bg * RPC + r;
+        for (int idx = tid; idx < L * RPC; idx += NT) {
+            const int j = idx / RPC;
+            const real g = Rr[ir[j]];
+            dst[(size_t)sw[j] * Bp] = (lw[j] >> 31) ? -g : g;
+        }
+    }
 }
 
 }  // namespace afs
