@@ -19,7 +19,7 @@ constexpr uint32_t LIT_VAR = 0x7fffffffu;
 //         occurrence's leave-one-out product from the other literals (deterministic by construction).
 //  MED  : thread per (constraint, restart), prefix/suffix in registers: OR/XOR L<=64, NAE/EO/AMO L<=32;
 //         OR/XOR longer than 64 run a two-pass running-product kernel (scratch row = prefix storage).
-//  CMED : EK / CARD with L <= 64: thread per (constraint, restart), the whole pmf in registers.
+//  CMED : EK / CARD with L <= 64: thread per (constraint, restart), the pmf in the warp's shared-memory buffer.
 //  LONG : warp per (constraint, restart), count-basis DP + stable-direction leave-one-out recurrences:
 //         EK/CARD longer than 64, and NAE/EO/AMO too long for MED.
 constexpr int PULL_MAX_LEN = 5;
@@ -39,7 +39,7 @@ constexpr int LONG_BUCKETS = 9;      // NR = 1..9 rows of 128 pmf cells
 constexpr uint32_t PE_VAR = 0x00ffffffu, PE_SIGN = 1u << 30, PE_NEG = 1u << 31;
 constexpr uint32_t PH_KIND_OR = 0, PH_KIND_XOR = 1, PH_KIND_NAE = 2;
 constexpr int MAX_VARS = 1 << 24;
-constexpr int CM_BUCKETS = 4;        // EK / CARD with L <= 64: padded lengths 16, 32, 48, 64, pmf in registers
+constexpr int CM_BUCKETS = 4;        // EK / CARD with L <= 64, ordered by length class 16, 32, 48, 64
 constexpr int CM_MAX_LEN = 64;
 
 struct MedCon {        // 16 bytes
@@ -65,6 +65,22 @@ struct CountCon {      // generic forward CSR entry for the count-only kernel: 1
     int16_t pad;
     int32_t k;
     int32_t pad2;
+};
+
+// ---- tile-resident kernel (afs_resident.cuh): static split of one tile's work over the C CTAs of a cluster ----------
+struct ResItem {       // one MED-class constraint: code 0..4 = MED bucket; idx into d_med
+    uint32_t code;
+    uint32_t idx;
+};
+constexpr int RES_PLANS = 4;   // cluster sizes 1, 2, 4, 8
+struct ResPlan {
+    int C = 0;
+    int32_t* d_var_begin = nullptr;    // [C+1] contiguous variable ranges, balanced by pull + reduction work
+    int32_t* d_item_begin = nullptr;   // [C+1] ranges of d_items, each rank's items heaviest first
+    ResItem* d_items = nullptr;
+    int32_t* d_cm_begin = nullptr;     // [C+1] ranges of d_cm_items
+    int32_t* d_cm_items = nullptr;     // CMED constraints (indices into d_cm), each rank's heaviest first
+    int32_t* d_pc_begin = nullptr;     // [C+1] ranges of the pull clauses whose counts the rank takes
 };
 
 // records cudaGetErrorString(e) + location for afs_last_error_message()
@@ -131,11 +147,13 @@ struct afs_problem {
     uint32_t* d_cm_lits = nullptr;
     int32_t* d_cm_slots = nullptr;
     int32_t cm_begin[afs::CM_BUCKETS + 1] = {0};
+    int32_t cm_maxL = 0;                // longest CMED constraint (rows of the shared-memory pmf buffer - 1)
 
     afs::CountCon* d_count = nullptr;   // all m constraints, original order
     uint32_t* d_count_lits = nullptr;
 
     int64_t n_pull = 0, n_med = 0, n_long = 0, n_cm = 0;
+    afs::ResPlan res[afs::RES_PLANS];
 
     // ---- run state -----------------------------------------------------------------------------------------
     afs::Workspace ws;

@@ -149,74 +149,99 @@ struct SGlobal {
 };
 
 // ------------------------------------------------------------------------------------------------------------------
-// CMED class: EK / CARD with L <= 64, thread = (constraint, restart), the whole pmf q_0..q_LP in registers.
-// The constraint is padded to LP literals with constant-False ones (u = 1, p = 0: they change nothing), so that the
-// reversed pmf is indexed at compile time.  Leave-one-out (G10): dFE/dy_j = q^(-j)_{k-1} [- q^(-j)_k
-// for EK].  Both stable recurrences run for every literal -- s_t = q_t - (p/u) s_{t-1} from the bottom up to t = k-1
-// (k for EK), sigma_i = q_{LP-i} - (u/p) sigma_{i-1} from the top down to the same indices -- and the result of the
-// direction whose ratio is <= 1 is kept; the other one is discarded by a select (it may be inf/NaN, never used).
+// CMED class: EK / CARD with L <= CM_MAX_LEN, thread = (constraint, restart).  The pmf q_0..q_L of the number of true
+// literals (count basis, G10) lives in the warp's shared-memory buffer, cell t of this lane at q[t * 32]
+// (column = lane: conflict-free, and the index may be dynamic, so nothing is padded and nothing is unrolled).
+//   forward   q_t <- q_t u_j + q_{t-1} p_j for every literal, one LDS + FMUL + FFMA + STS per cell.
+//   gradient  dFE/dy_j = wA q^(-j)_{tA} + wB q^(-j)_{tB} (at most two non-zero d_t).  q^(-j) comes from q by
+//             removing literal j in the STABLE direction: s_t = q_t - (p/u) s_{t-1} from the bottom when p <= 1/2
+//             (q^(-j)_t = s_t / u), z_i = q_{L-i} - (u/p) z_{i-1} from the top otherwise (q^(-j)_{L-1-i} = z_i / p).
+//             Every lane walks its own direction through its own column in ONE loop (the ratio is <= 1 and the
+//             divisor >= 1/2 either way: nothing that vanishes at x = +-1 is divided by); the loop ends at the later
+//             of the two directions' capture points, which depend on the constraint only (warp-uniform).
 // ------------------------------------------------------------------------------------------------------------------
-template <typename real, int LP, typename XL, typename SW>
-__device__ __forceinline__ void cmed_body(const LongCon& lc, const uint32_t* __restrict__ lw,
-                                          const int32_t* __restrict__ sw, const XL& xl, const SW& sc, int& satcnt,
-                                          real& fe)
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float rcp_rn(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ double rcp_rn(double x) { return 1.0 / x; }
+
+template <typename real, typename XL, typename SW>
+__device__ __forceinline__ void cm_body(const LongCon& lc, const uint32_t* __restrict__ lw,
+                                        const int32_t* __restrict__ sw, const XL& xl, const SW& sc,
+                                        real* __restrict__ q, int& satcnt, real& fe, const bool want_fe)
 {
     const real half = real(0.5), one = real(1), zero = real(0);
     const int L = lc.L;
-    real q[LP + 1];
-#pragma unroll
-    for (int t = 0; t <= LP; ++t) q[t] = zero;
     q[0] = one;
     int tc = 0;
-#pragma unroll
-    for (int j = 0; j < LP; ++j) {
-        if (j < L) {
-            uint32_t w = lw[j];
-            real x = xl(w & LIT_VAR);
-            bool neg = (w >> 31) != 0;
-            tc += ((x < zero) != neg) ? 1 : 0;
-            real y = neg ? -x : x;
-            real u = half + half * y, p = half - half * y;
-#pragma unroll
-            for (int i = j + 1; i >= 1; --i) q[i] = q[i] * u + q[i - 1] * p;
-            q[0] = q[0] * u;
+    for (int j = 0; j < L; ++j) {
+        const uint32_t w = lw[j];
+        const real x = xl(w & LIT_VAR);
+        const bool neg = (w >> 31) != 0;
+        tc += ((x < zero) != neg) ? 1 : 0;
+        const real y = neg ? -x : x;
+        const real u = fma(half, y, half), p = fma(-half, y, half);
+        real hi = zero;   // old q_{j+1}
+#pragma unroll 4
+        for (int t = j + 1; t >= 1; --t) {
+            const real lo = q[(t - 1) * 32];
+            q[t * 32] = fma(lo, p, mul_rn(hi, u));
+            hi = lo;
         }
+        q[0] = mul_rn(hi, u);
     }
     satcnt += pred(lc.type, L, lc.k, tc) ? 1 : 0;
-    real f = zero;
-#pragma unroll
-    for (int t = 0; t <= LP; ++t) f += (lc.type == AFS_CARD ? t >= lc.k : t == lc.k) ? -q[t] : q[t];
-    fe = f;
-    // targets: tA = k-1 with weight +1 (valid iff wA != 0), tB = k with weight -1 (EK only, valid iff wB != 0)
+    fe = zero;
+    if (want_fe) {
+        real f = zero;
+        for (int t = 0; t <= L; ++t) {
+            const real v = q[t * 32];
+            f += (lc.type == AFS_CARD ? t >= lc.k : t == lc.k) ? -v : v;   // sp_t = -1 where satisfied
+        }
+        fe = f;
+    }
     const bool useA = lc.wA != 0.f, useB = lc.wB != 0.f;
-    const int tA = lc.tA, tB = lc.tB;
-    const int fend = useB ? tB : (useA ? tA : -1);                 // last forward index needed
-    const int bend = useA ? LP - 1 - tA : (useB ? LP - 1 - tB : -1);  // last top-down index needed (tA < tB)
+    if (!useA && !useB) {   // constant expansion (CARD k = 0 or k = L+1, G5): zero gradient
+        for (int j = 0; j < L; ++j) sc.put(sw[j], zero);
+        return;
+    }
+    const int tA = useA ? lc.tA : lc.tB, tB = useB ? lc.tB : lc.tA;   // tA <= tB
+    const real wA = useA ? (real)lc.wA : zero, wB = useB ? (real)lc.wB : zero;
+    // capture steps: bottom-up chain step = t; top-down chain step i <-> t = L-1-i
+    const int f1 = tA, f2 = tB, b1 = L - 1 - tB, b2 = L - 1 - tA;
+    int bp0 = min(f1, b1), bp3 = max(f2, b2);
+    int m1 = max(f1, b1), m2 = min(f2, b2);
+    int bp1 = min(m1, m2), bp2 = max(m1, m2);
+    const int bp[4] = {bp0, bp1, bp2, bp3};
     for (int j = 0; j < L; ++j) {
-        uint32_t w = lw[j];
-        real x = xl(w & LIT_VAR);
-        bool neg = (w >> 31) != 0;
-        real y = neg ? -x : x;
-        real u = half + half * y, p = half - half * y;
-        const bool fwd = !(y < zero);
-        const real Rf = p / u, Rb = u / p;
-        real s = zero, sprev = zero;
+        const uint32_t w = lw[j];
+        const real x = xl(w & LIT_VAR);
+        const bool neg = (w >> 31) != 0;
+        const real y = neg ? -x : x;
+        const real u = fma(half, y, half), p = fma(-half, y, half);
+        const bool fwd = !(y < zero);   // p <= 1/2
+        const real rb = rcp_rn(fwd ? u : p);
+        const real R = mul_rn(fwd ? p : u, rb);
+        const int c1 = fwd ? f1 : b1, c2 = fwd ? f2 : b2;
+        const real w1 = fwd ? wA : wB, w2 = fwd ? wB : wA;
+        const real* qp = fwd ? q : q + L * 32;
+        const int stride = fwd ? 32 : -32;
+        real acc = zero, v1 = zero, v2 = zero;
+        int s = 0;
 #pragma unroll
-        for (int t = 0; t <= LP; ++t) {
-            if (t <= fend) { sprev = s; s = q[t] - Rf * s; }
+        for (int b = 0; b < 4; ++b) {
+            const int e = bp[b];
+            if (e >= s) {
+#pragma unroll 4
+                for (; s <= e; ++s) {
+                    acc = fma(-R, acc, *qp);
+                    qp += stride;
+                }
+                v1 = c1 == e ? acc : v1;
+                v2 = c2 == e ? acc : v2;
+            }
         }
-        // forward: s = s_fend.  useB: s_tB = s, s_tA = sprev (tA = tB - 1 when both are used; if only B, A unused)
-        real fA = useB ? sprev : s, fB = s;
-        real z = zero, zprev = zero;
-#pragma unroll
-        for (int i = 0; i <= LP; ++i) {
-            if (i <= bend) { zprev = z; z = q[LP - i] - Rb * z; }
-        }
-        // top-down: z = sigma_bend.  useA: sigma at tA is z, sigma at tB (one index earlier) is zprev
-        real bA = z, bB = useA ? zprev : z;
-        real gA = fwd ? fA / u : bA / p;
-        real gB = fwd ? fB / u : bB / p;
-        real g = (useA ? gA : zero) - (useB ? gB : zero);
+        const real g = mul_rn(fma(w1, v1, mul_rn(w2, v2)), rb);
         sc.put(sw[j], neg ? -g : g);
     }
 }
@@ -231,6 +256,107 @@ __device__ __forceinline__ void cmed_body(const LongCon& lc, const uint32_t* __r
 //   AMO  FE = 1 - 2 (q_0 + q_1)            dFE/dy_j = - q_1^(-j)
 // (count basis, G10; d_t of P:L52).  The gradient written to scratch already carries the literal sign (S5).
 // ------------------------------------------------------------------------------------------------------------------
+template <typename real, int LP, typename XL, typename SW>
+__device__ __forceinline__ void med_body(const MedCon& mc, const uint32_t* __restrict__ lc,
+                                         const int32_t* __restrict__ sc, const XL& xl, const SW& sw, int& satcnt,
+                                         real& fe)
+{
+    const real half = real(0.5), one = real(1);
+    real y[LP];
+    unsigned long long negmask = 0ull;
+    int t = 0;
+#pragma unroll
+    for (int j = 0; j < LP; ++j) {
+        real v = one;   // padding literal: constant False (y = +1), neutral for every type below
+        if (j < mc.L) {
+            uint32_t w = lc[j];
+            real x = xl(w & LIT_VAR);
+            bool neg = (w >> 31) != 0;
+            t += ((x < real(0)) != neg) ? 1 : 0;
+            v = neg ? -x : x;
+            if (neg) negmask |= 1ull << j;
+        }
+        y[j] = v;
+    }
+    satcnt += pred(mc.type, mc.L, mc.k, t) ? 1 : 0;
+    fe = real(0);
+    if (mc.type == AFS_OR || mc.type == AFS_XOR) {
+        const bool is_or = mc.type == AFS_OR;
+        const real s = is_or ? one : ((mc.k & 1) ? one : -one);
+        real g[LP];
+        real pre = one;
+#pragma unroll
+        for (int j = 0; j < LP; ++j) {
+            real f = is_or ? half + half * y[j] : y[j];
+            y[j] = f;
+            g[j] = pre;
+            pre *= f;
+        }
+        fe = is_or ? real(2) * pre - one : s * pre;
+        real suf = s;
+#pragma unroll
+        for (int j = LP - 1; j >= 0; --j) {
+            g[j] *= suf;
+            suf *= y[j];
+        }
+#pragma unroll
+        for (int j = 0; j < LP; ++j)
+            if (j < mc.L) sw.put(sc[j], ((negmask >> j) & 1ull) ? -g[j] : g[j]);
+    } else {
+        if constexpr (LP <= 32) {
+            if (mc.type == AFS_NAE) {
+                real gu[LP], gp[LP];
+                real pu = one, pp = one;
+#pragma unroll
+                for (int j = 0; j < LP; ++j) {
+                    // a padding literal must be neutral in BOTH chains: treat it as absent (factor 1)
+                    real u = j < mc.L ? half + half * y[j] : one;
+                    real p = j < mc.L ? half - half * y[j] : one;
+                    gu[j] = pu; gp[j] = pp;
+                    pu *= u; pp *= p;
+                }
+                fe = real(2) * pu + real(2) * pp - one;
+                real su = one, sp = one;
+#pragma unroll
+                for (int j = LP - 1; j >= 0; --j) {
+                    real u = j < mc.L ? half + half * y[j] : one;
+                    real p = j < mc.L ? half - half * y[j] : one;
+                    gu[j] = gu[j] * su - gp[j] * sp;
+                    su *= u; sp *= p;
+                }
+#pragma unroll
+                for (int j = 0; j < LP; ++j)
+                    if (j < mc.L) sw.put(sc[j], ((negmask >> j) & 1ull) ? -gu[j] : gu[j]);
+            } else {   // EO, AMO: pmf of the true count truncated to {0, 1}
+                real P0[LP], P1[LP];
+                real a0 = one, a1 = real(0);
+#pragma unroll
+                for (int j = 0; j < LP; ++j) {
+                    real u = half + half * y[j], p = half - half * y[j];
+                    P0[j] = a0; P1[j] = a1;
+                    a1 = a1 * u + a0 * p;
+                    a0 = a0 * u;
+                }
+                const bool is_eo = mc.type == AFS_EO;
+                fe = is_eo ? one - real(2) * a1 : one - real(2) * (a0 + a1);
+                real s0 = one, s1 = real(0);
+#pragma unroll
+                for (int j = LP - 1; j >= 0; --j) {
+                    real u = half + half * y[j], p = half - half * y[j];
+                    real q0 = P0[j] * s0;
+                    real q1 = P1[j] * s0 + P0[j] * s1;
+                    P0[j] = is_eo ? q0 - q1 : -q1;
+                    s1 = s1 * u + s0 * p;
+                    s0 = s0 * u;
+                }
+#pragma unroll
+                for (int j = 0; j < LP; ++j)
+                    if (j < mc.L) sw.put(sc[j], ((negmask >> j) & 1ull) ? -P0[j] : P0[j]);
+            }
+        }
+    }
+}
+
 template <typename real, int LP>
 __global__ void __launch_bounds__(128) k_med(const MedCon* __restrict__ cons, int c_begin, int c_end,
                                              const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
@@ -241,106 +367,12 @@ __global__ void __launch_bounds__(128) k_med(const MedCon* __restrict__ cons, in
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.y * 32 + lane;
     int satcnt = 0;
-    const real half = real(0.5), one = real(1);
+    const XGlobal<real> xl{XT, Bp, b};
+    const SGlobal<real> sc{scratch, Bp, b};
     for (int c = c_begin + blockIdx.x * 4 + warp; c < c_end; c += gridDim.x * 4) {
         const MedCon mc = cons[c];
-        const uint32_t* lc = lits + mc.off;
-        const int32_t* sc = slots + mc.off;
-        real y[LP];
-        unsigned long long negmask = 0ull;
-        int t = 0;
-#pragma unroll
-        for (int j = 0; j < LP; ++j) {
-            real v = one;   // padding literal: constant False (y = +1), neutral for every type below
-            if (j < mc.L) {
-                uint32_t w = lc[j];
-                real x = ldx(XT, w, Bp, b);
-                bool neg = (w >> 31) != 0;
-                t += ((x < real(0)) != neg) ? 1 : 0;
-                v = neg ? -x : x;
-                if (neg) negmask |= 1ull << j;
-            }
-            y[j] = v;
-        }
-        satcnt += pred(mc.type, mc.L, mc.k, t) ? 1 : 0;
         real fe;
-        if (mc.type == AFS_OR || mc.type == AFS_XOR) {
-            const bool is_or = mc.type == AFS_OR;
-            const real s = is_or ? one : ((mc.k & 1) ? one : -one);
-            real g[LP];
-            real pre = one;
-#pragma unroll
-            for (int j = 0; j < LP; ++j) {
-                real f = is_or ? half + half * y[j] : y[j];
-                y[j] = f;
-                g[j] = pre;
-                pre *= f;
-            }
-            fe = is_or ? real(2) * pre - one : s * pre;
-            real suf = s;
-#pragma unroll
-            for (int j = LP - 1; j >= 0; --j) {
-                g[j] *= suf;
-                suf *= y[j];
-            }
-#pragma unroll
-            for (int j = 0; j < LP; ++j)
-                if (j < mc.L) scratch[(size_t)sc[j] * Bp + b] = ((negmask >> j) & 1ull) ? -g[j] : g[j];
-        } else {
-            if constexpr (LP <= 32) {
-                if (mc.type == AFS_NAE) {
-                    real gu[LP], gp[LP];
-                    real pu = one, pp = one;
-#pragma unroll
-                    for (int j = 0; j < LP; ++j) {
-                        // a padding literal must be neutral in BOTH chains: treat it as absent (factor 1)
-                        real u = j < mc.L ? half + half * y[j] : one;
-                        real p = j < mc.L ? half - half * y[j] : one;
-                        gu[j] = pu; gp[j] = pp;
-                        pu *= u; pp *= p;
-                    }
-                    fe = real(2) * pu + real(2) * pp - one;
-                    real su = one, sp = one;
-#pragma unroll
-                    for (int j = LP - 1; j >= 0; --j) {
-                        real u = j < mc.L ? half + half * y[j] : one;
-                        real p = j < mc.L ? half - half * y[j] : one;
-                        gu[j] = gu[j] * su - gp[j] * sp;
-                        su *= u; sp *= p;
-                    }
-#pragma unroll
-                    for (int j = 0; j < LP; ++j)
-                        if (j < mc.L) scratch[(size_t)sc[j] * Bp + b] = ((negmask >> j) & 1ull) ? -gu[j] : gu[j];
-                } else {   // EO, AMO: pmf of the true count truncated to {0, 1}
-                    real P0[LP], P1[LP];
-                    real a0 = one, a1 = real(0);
-#pragma unroll
-                    for (int j = 0; j < LP; ++j) {
-                        real u = half + half * y[j], p = half - half * y[j];
-                        P0[j] = a0; P1[j] = a1;
-                        a1 = a1 * u + a0 * p;
-                        a0 = a0 * u;
-                    }
-                    const bool is_eo = mc.type == AFS_EO;
-                    fe = is_eo ? one - real(2) * a1 : one - real(2) * (a0 + a1);
-                    real s0 = one, s1 = real(0);
-#pragma unroll
-                    for (int j = LP - 1; j >= 0; --j) {
-                        real u = half + half * y[j], p = half - half * y[j];
-                        real q0 = P0[j] * s0;
-                        real q1 = P1[j] * s0 + P0[j] * s1;
-                        P0[j] = is_eo ? q0 - q1 : -q1;
-                        s1 = s1 * u + s0 * p;
-                        s0 = s0 * u;
-                    }
-#pragma unroll
-                    for (int j = 0; j < LP; ++j)
-                        if (j < mc.L) scratch[(size_t)sc[j] * Bp + b] = ((negmask >> j) & 1ull) ? -P0[j] : P0[j];
-                }
-            } else {
-                fe = real(0);
-            }
-        }
+        med_body<real, LP>(mc, lits + mc.off, slots + mc.off, xl, sc, satcnt, fe);
         if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
     }
     if (sat) {
@@ -353,22 +385,24 @@ __global__ void __launch_bounds__(128) k_med(const MedCon* __restrict__ cons, in
     }
 }
 
-template <typename real, int LP>
+template <typename real>
 __global__ void __launch_bounds__(128) k_cmed(const LongCon* __restrict__ cons, int c_begin, int c_end,
                                               const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
                                               const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
-                                              int32_t* __restrict__ sat, real* __restrict__ fe_out)
+                                              int32_t* __restrict__ sat, real* __restrict__ fe_out, int qrows)
 {
+    extern __shared__ __align__(16) unsigned char cm_smem[];
     __shared__ int s_sat[4][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.y * 32 + lane;
     int satcnt = 0;
     const XGlobal<real> xl{XT, Bp, b};
     const SGlobal<real> sc{scratch, Bp, b};
+    real* q = reinterpret_cast<real*>(cm_smem) + (size_t)warp * qrows * 32 + lane;
     for (int c = c_begin + blockIdx.x * 4 + warp; c < c_end; c += gridDim.x * 4) {
         const LongCon lc = cons[c];
         real fe;
-        cmed_body<real, LP>(lc, lits + lc.off, slots + lc.off, xl, sc, satcnt, fe);
+        cm_body<real>(lc, lits + lc.off, slots + lc.off, xl, sc, q, satcnt, fe, fe_out != nullptr);
         if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
     }
     if (sat) {
@@ -383,6 +417,39 @@ __global__ void __launch_bounds__(128) k_cmed(const LongCon* __restrict__ cons, 
 
 // OR / XOR longer than 64 literals: two passes, the scratch row of each literal holds the running prefix product
 // between them (no extra memory, no division).
+template <typename real, typename XL, typename SW>
+__device__ __forceinline__ void prod_long_body(const MedCon& mc, const uint32_t* __restrict__ lc,
+                                               const int32_t* __restrict__ sc, const XL& xl, const SW& sw, int& satcnt,
+                                               real& fe)
+{
+    const real half = real(0.5), one = real(1);
+    const bool is_or = mc.type == AFS_OR;
+    const real s = is_or ? one : ((mc.k & 1) ? one : -one);
+    real pre = one;
+    int t = 0;
+    for (int j = 0; j < mc.L; ++j) {
+        uint32_t w = lc[j];
+        real x = xl(w & LIT_VAR);
+        bool neg = (w >> 31) != 0;
+        t += ((x < real(0)) != neg) ? 1 : 0;
+        real yj = neg ? -x : x;
+        sw.put(sc[j], pre);
+        pre *= is_or ? half + half * yj : yj;
+    }
+    satcnt += pred(mc.type, mc.L, mc.k, t) ? 1 : 0;
+    fe = is_or ? real(2) * pre - one : s * pre;
+    real suf = s;
+    for (int j = mc.L - 1; j >= 0; --j) {
+        uint32_t w = lc[j];
+        real x = xl(w & LIT_VAR);
+        bool neg = (w >> 31) != 0;
+        real yj = neg ? -x : x;
+        real g = sw.get(sc[j]) * suf;
+        sw.put(sc[j], neg ? -g : g);
+        suf *= is_or ? half + half * yj : yj;
+    }
+}
+
 template <typename real>
 __global__ void __launch_bounds__(128) k_prod_long(const MedCon* __restrict__ cons, int c_begin, int c_end,
                                                    const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
@@ -393,37 +460,13 @@ __global__ void __launch_bounds__(128) k_prod_long(const MedCon* __restrict__ co
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.y * 32 + lane;
     int satcnt = 0;
-    const real half = real(0.5), one = real(1);
+    const XGlobal<real> xl{XT, Bp, b};
+    const SGlobal<real> sc{scratch, Bp, b};
     for (int c = c_begin + blockIdx.x * 4 + warp; c < c_end; c += gridDim.x * 4) {
         const MedCon mc = cons[c];
-        const uint32_t* lc = lits + mc.off;
-        const int32_t* sc = slots + mc.off;
-        const bool is_or = mc.type == AFS_OR;
-        const real s = is_or ? one : ((mc.k & 1) ? one : -one);
-        real pre = one;
-        int t = 0;
-        for (int j = 0; j < mc.L; ++j) {
-            uint32_t w = lc[j];
-            real x = ldx(XT, w, Bp, b);
-            bool neg = (w >> 31) != 0;
-            t += ((x < real(0)) != neg) ? 1 : 0;
-            real yj = neg ? -x : x;
-            scratch[(size_t)sc[j] * Bp + b] = pre;
-            pre *= is_or ? half + half * yj : yj;
-        }
-        satcnt += pred(mc.type, mc.L, mc.k, t) ? 1 : 0;
-        if (fe_out) fe_out[(size_t)c * Bp + b] = is_or ? real(2) * pre - one : s * pre;
-        real suf = s;
-        for (int j = mc.L - 1; j >= 0; --j) {
-            uint32_t w = lc[j];
-            real x = ldx(XT, w, Bp, b);
-            bool neg = (w >> 31) != 0;
-            real yj = neg ? -x : x;
-            size_t idx = (size_t)sc[j] * Bp + b;
-            real g = scratch[idx] * suf;
-            scratch[idx] = neg ? -g : g;
-            suf *= is_or ? half + half * yj : yj;
-        }
+        real fe;
+        prod_long_body<real>(mc, lits + mc.off, slots + mc.off, xl, sc, satcnt, fe);
+        if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
     }
     if (sat) {
         s_sat[warp][lane] = satcnt;
@@ -496,13 +539,31 @@ constexpr int PULL_SBUF = 48;   // uint2 slots per warp: 32 staged entries + sla
 // The warp loads 32 entries with one coalesced load, every lane decodes its entry (byte offset of the row, sign
 // material) into the warp's shared staging buffer, and all lanes then walk the occurrences reading whole records
 // with one broadcast LDS each.  Returns the run's contribution to dF/dx_v (carrying the own literal's sign).
-template <typename real, int KIND, int NOTHER>
+// Column loaders: byte offset of a row -> x of this lane's restart.  Global: column b of XT[n][Bp]; shared: column
+// `lane` of the tile X[n][32] of the resident kernel (32-bit shared-window address, LDS).
+template <typename real>
+struct ColGlobal {
+    const char* __restrict__ base;
+    __device__ __forceinline__ real at(uint32_t off) const { return *reinterpret_cast<const real*>(base + off); }
+};
+template <typename real>
+struct ColShared {
+    uint32_t base;
+    __device__ __forceinline__ real at(uint32_t off) const
+    {
+        real v;
+        if constexpr (sizeof(real) == 4) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(base + off));
+        else asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(base + off));
+        return v;
+    }
+};
+
+template <typename real, int KIND, int NOTHER, typename COL>
 __device__ __forceinline__ real pull_run(const uint32_t* __restrict__ words, int beg, int count,
-                                         const real* __restrict__ xcol, uint32_t rowbytes, int lane, uint2* sbuf)
+                                         const COL& xcol, uint32_t rowbytes, int lane, uint2* sbuf)
 {
     constexpr int OPC = 32 / NOTHER;              // occurrences per staged chunk of <= 32 entries
     constexpr int U = NOTHER <= 2 ? 4 : 2;        // occurrences gathered together
-    const char* __restrict__ xb = reinterpret_cast<const char*>(xcol);
     real g = real(0);
     for (int o0 = 0; o0 < count; o0 += OPC) {
         const int nocc = min(OPC, count - o0);
@@ -534,7 +595,7 @@ __device__ __forceinline__ real pull_run(const uint32_t* __restrict__ words, int
             for (int u = 0; u < U; ++u)
 #pragma unroll
                 for (int i = 0; i < NOTHER; ++i)
-                    x[u][i] = *reinterpret_cast<const real*>(xb + (i == 0 ? (e[u][0].x & ~1u) : e[u][i].x));
+                    x[u][i] = xcol.at(i == 0 ? (e[u][0].x & ~1u) : e[u][i].x);
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 real d;
@@ -565,10 +626,10 @@ __device__ __forceinline__ real pull_run(const uint32_t* __restrict__ words, int
 }
 
 // all runs of one variable
-template <typename real>
+template <typename real, typename COL>
 __device__ __forceinline__ real pull_variable(const uint32_t* __restrict__ runs, int rbeg, int rend,
                                               const uint32_t* __restrict__ words, int wbeg,
-                                              const real* __restrict__ xcol, uint32_t rowbytes, int lane, uint2* sbuf)
+                                              const COL& xcol, uint32_t rowbytes, int lane, uint2* sbuf)
 {
     real g = real(0);
     int pos = wbeg;
@@ -576,7 +637,7 @@ __device__ __forceinline__ real pull_variable(const uint32_t* __restrict__ runs,
         const uint32_t d = runs[r];
         const int count = (int)(d & 0x07ffffffu), nother = (int)((d >> 27) & 7u), kind = (int)(d >> 30);
         real gr;
-#define AFS_RUN(K, N) gr = pull_run<real, K, N>(words, pos, count, xcol, rowbytes, lane, sbuf)
+#define AFS_RUN(K, N) gr = pull_run<real, K, N, COL>(words, pos, count, xcol, rowbytes, lane, sbuf)
         if (kind == (int)PH_KIND_OR) {
             switch (nother) { case 1: AFS_RUN(0, 1); break; case 2: AFS_RUN(0, 2); break; case 3: AFS_RUN(0, 3); break; default: AFS_RUN(0, 4); break; }
         } else if (kind == (int)PH_KIND_XOR) {
@@ -601,6 +662,7 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 4) k_var(const VarArgs<real> a
     const int Bp = a.Bp;
     const real one = real(1);
     const real* __restrict__ xcol = a.Xin + b;
+    const ColGlobal<real> xg{reinterpret_cast<const char*>(xcol)};
     uint2* sbuf = s_stage[warp];
     for (int i = lane; i < PULL_SBUF; i += 32) sbuf[i] = make_uint2(0u, 0u);   // slack slots must stay valid offsets
     __syncwarp();
@@ -637,7 +699,7 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 4) k_var(const VarArgs<real> a
         real g = real(0);
         if (mk == 0) {   // a fixed variable never moves: its gradient is not needed
             g = (real)a.gconst[v];
-            g += pull_variable<real>(a.runs, a.run_ptr[v], a.run_ptr[v + 1], a.pull_words, a.pull_ptr[v], xcol,
+            g += pull_variable<real>(a.runs, a.run_ptr[v], a.run_ptr[v + 1], a.pull_words, a.pull_ptr[v], xg,
                                      (uint32_t)Bp * (uint32_t)sizeof(real), lane, sbuf);
             // ---- S6: materialised gradients of v, fixed (transposed-CSR) order
             const int s1 = a.slot_ptr[v + 1];

@@ -257,6 +257,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
                                       LONG_BUCKETS, P->long_begin, P->long_maxL, lng, long_lits, long_slots);
         P->n_cm = build_count_class(C_CMED, [&](int c) { return (int)((row_ptr[c + 1] - row_ptr[c] + 15) / 16) - 1; },
                                     CM_BUCKETS, P->cm_begin, nullptr, cmv, cm_lits, cm_slots);
+        for (const LongCon& x : cmv) P->cm_maxL = std::max(P->cm_maxL, x.L);
         // ------------------------------------------------------------ generic forward CSR for the count-only kernel
         std::vector<CountCon> cnt(m);
         std::vector<uint32_t> cnt_lits((size_t)P->nnz);
@@ -268,6 +269,64 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
 
         afs_status st = AFS_OK;
         auto up = [&](auto** dst, const auto& src) { if (st == AFS_OK) st = upload(dst, src); };
+        // ------------------------------------------------------------ plans of the tile-resident kernel
+        if (lng.empty()) {
+            std::vector<double> vcost(n);
+            for (int v = 0; v < n; ++v)
+                vcost[v] = 6.0 * (pull_ptr[v + 1] - pull_ptr[v]) + 2.0 * (slot_ptr[v + 1] - slot_ptr[v]) + 24.0;
+            struct It { double cost; ResItem it; bool cm; };
+            std::vector<It> its;
+            for (size_t i = 0; i < med.size(); ++i) {
+                int bk = med_bucket(med[i].L);
+                double LP = bk < 4 ? (double)(8 << bk) : (double)med[i].L;
+                its.push_back({12.0 * LP, ResItem{(uint32_t)bk, (uint32_t)i}, false});
+            }
+            for (size_t i = 0; i < cmv.size(); ++i) {
+                const double L = cmv[i].L;
+                const double chain = std::max({(double)cmv[i].tA, (double)cmv[i].tB, L - 1 - cmv[i].tA, L - 1 - cmv[i].tB}) + 1;
+                its.push_back({2.0 * L * L + L * (40.0 + 4.0 * chain), ResItem{0u, (uint32_t)i}, true});
+            }
+            std::stable_sort(its.begin(), its.end(), [](const It& x, const It& y) { return x.cost > y.cost; });
+            for (int pi = 0; pi < RES_PLANS; ++pi) {
+                const int C = 1 << pi;
+                ResPlan& rp = P->res[pi];
+                rp.C = C;
+                std::vector<int32_t> vbeg(C + 1, 0), ibeg(C + 1, 0), pbeg(C + 1, 0);
+                double tot = std::accumulate(vcost.begin(), vcost.end(), 0.0), acc = 0.0;
+                int r = 1;
+                for (int v = 0; v < n && r < C; ++v) {
+                    acc += vcost[v];
+                    while (r < C && acc >= tot * r / C) vbeg[r++] = v + 1;
+                }
+                while (r < C) vbeg[r++] = n;
+                vbeg[C] = n;
+                std::vector<std::vector<ResItem>> per(C);
+                std::vector<std::vector<int32_t>> perc(C);
+                std::vector<double> load(C, 0.0);
+                for (const It& x : its) {   // longest processing time first, onto the least loaded rank
+                    int best = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+                    if (x.cm) perc[best].push_back((int32_t)x.it.idx); else per[best].push_back(x.it);
+                    load[best] += x.cost;
+                }
+                std::vector<ResItem> flat;
+                std::vector<int32_t> cflat, cbeg(C + 1, 0);
+                for (int q = 0; q < C; ++q) {
+                    ibeg[q] = (int32_t)flat.size();
+                    flat.insert(flat.end(), per[q].begin(), per[q].end());
+                    cbeg[q] = (int32_t)cflat.size();
+                    cflat.insert(cflat.end(), perc[q].begin(), perc[q].end());
+                }
+                ibeg[C] = (int32_t)flat.size();
+                cbeg[C] = (int32_t)cflat.size();
+                up(&rp.d_cm_begin, cbeg);
+                up(&rp.d_cm_items, cflat);
+                for (int q = 0; q <= C; ++q) pbeg[q] = (int32_t)((int64_t)pc.size() * q / C);
+                up(&rp.d_var_begin, vbeg);
+                up(&rp.d_item_begin, ibeg);
+                up(&rp.d_items, flat);
+                up(&rp.d_pc_begin, pbeg);
+            }
+        }
         up(&P->d_pull_ptr, pull_ptr);
         up(&P->d_pull_words, pull_words);
         up(&P->d_run_ptr, run_ptr);
@@ -310,6 +369,11 @@ extern "C" void afs_problem_destroy(afs_problem* p)
     cudaFree(p->d_long); cudaFree(p->d_long_lits); cudaFree(p->d_long_slots);
     cudaFree(p->d_cm); cudaFree(p->d_cm_lits); cudaFree(p->d_cm_slots);
     cudaFree(p->d_count); cudaFree(p->d_count_lits);
+    for (int i = 0; i < afs::RES_PLANS; ++i) {
+        cudaFree(p->res[i].d_var_begin); cudaFree(p->res[i].d_item_begin);
+        cudaFree(p->res[i].d_items); cudaFree(p->res[i].d_pc_begin);
+        cudaFree(p->res[i].d_cm_begin); cudaFree(p->res[i].d_cm_items);
+    }
     afs::free_workspace(p);
     (void)cudaGetLastError();
     delete p;

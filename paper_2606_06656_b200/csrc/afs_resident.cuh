@@ -1,0 +1,333 @@
+// afs_resident.cuh -- the tile-resident PGD kernel: ONE launch runs every PGD iteration (S1..S10) of afs_pgd_run.
+//
+// Restarts are independent, so a tile of 32 restarts never needs anything from another tile.
+// A thread-block cluster of C CTAs owns one tile for the whole run:
+//   * every CTA keeps the iterate X_t of the tile in shared memory, X[n][32] (lane <-> restart: every gather is one
+//     conflict-free 128-byte LDS, the index/sign words are warp-uniform); what is left of the 227 KB holds the pmf
+//     buffers of the EK / CARD bodies (one per warp that may take such a constraint),
+//   * the work of an iteration is split over the C CTAs: the materialising ("push") constraints, the bit-parallel
+//     counts of the pull clauses and the variables (pull gradients, S6 reduction, step) each by a static partition
+//     made at afs_problem_create, and taken warp by warp from one shared work counter inside the CTA,
+//   * the pieces meet through L2: per-literal gradients of the push constraints (scratch[tile][slot][32]), the pull
+//     gradients (G[tile][v][32]) and the new iterate (XT[tile][v][32]) are written by the warp that computed them
+//     and read by others after a
+//     cluster barrier (release / acquire at cluster scope); there is no grid-wide synchronisation and no host
+//     round trip,
+//   * the satisfied counts of iterate t are integer atomics on sat_hist[t][b]; cluster rank 0 keeps the best
+//     count, its step and its sign bits in shared memory.
+// One iteration:  P1 push gradients + counts | P2 pull gradients of the own variables -> G
+//                 -- cluster barrier --  best-so-far merge of iterate t (rank 0) | P3 S6 + S7 + S8 for the own
+//                 variables -> XT (global)  -- cluster barrier --  P4 reload X_{t+1}, sign words.
+// The arithmetic of every constraint body, of the pull loops and of the step is the code the streaming kernels
+// run (afs_kernels.cuh); only where the operands live differs.
+#pragma once
+#include <cooperative_groups.h>
+
+#include "afs_kernels.cuh"
+
+namespace afs {
+
+namespace cg = cooperative_groups;
+
+constexpr int RES_WARPS = 16;
+constexpr int RES_VCH = 2;   // variables per work item
+
+template <typename real>
+struct XTile {   // x of this lane's restart from the shared tile
+    const real* __restrict__ p;   // Xs + lane
+    __device__ __forceinline__ real operator()(uint32_t var) const { return p[var * 32u]; }
+};
+template <typename real>
+struct STile {   // scratch[tile][slot][32] in global memory
+    real* __restrict__ p;         // scratch + tile * nslots * 32 + lane
+    __device__ __forceinline__ void put(int slot, real v) const { p[(size_t)slot * 32] = v; }
+    __device__ __forceinline__ real get(int slot) const { return p[(size_t)slot * 32]; }
+};
+
+template <typename real>
+struct ResArgs {
+    int n, steps, C, Bp, ntile;
+    int cm_bufs, cm_rows;        // pmf buffers of the CTA (warps 0..cm_bufs-1 own one), rows (cm_maxL + 1) of each
+    int64_t nslots;
+    const int32_t* pull_ptr;
+    const uint32_t* pull_words;
+    const int32_t* run_ptr;
+    const uint32_t* runs;
+    const float* gconst;
+    const int32_t* slot_ptr;
+    const MedCon* med;
+    const uint32_t* med_lits;
+    const int32_t* med_slots;
+    const LongCon* cm;
+    const uint32_t* cm_lits;
+    const int32_t* cm_slots;
+    const CountCon* pc;
+    const uint32_t* pc_lits;
+    const int32_t* var_begin;    // [C+1]
+    const int32_t* item_begin;   // [C+1]
+    const ResItem* items;
+    const int32_t* cm_begin;     // [C+1] ranges of cm_items
+    const int32_t* cm_items;     // indices into cm, each rank's heaviest first
+    const int32_t* pc_begin;     // [C+1]
+    real* XT;                    // [ntile][n][32]
+    real* G;                     // [ntile][n][32] pull part of the gradient
+    real* scratch;               // [ntile][nslots][32]
+    int32_t* sat_hist;           // [steps+1][Bp], zeroed
+    uint32_t* best_bits;         // [n][ntile]
+    int32_t* best_sat;           // [Bp]
+    int32_t* best_step;          // [Bp]
+    real lr;
+    const int8_t* mask;
+};
+
+template <typename real>
+__device__ __forceinline__ real ld_cg(const real* p) { return __ldcg(p); }
+
+template <typename real>
+__device__ __forceinline__ void res_push_item(const ResArgs<real>& a, const ResItem it, const XTile<real>& xl,
+                                              const STile<real>& sw, int& satcnt)
+{
+    real fe;
+    const MedCon mc = a.med[it.idx];
+    const uint32_t* lc = a.med_lits + mc.off;
+    const int32_t* sc = a.med_slots + mc.off;
+    switch (it.code) {
+    case 0: med_body<real, 8>(mc, lc, sc, xl, sw, satcnt, fe); break;
+    case 1: med_body<real, 16>(mc, lc, sc, xl, sw, satcnt, fe); break;
+    case 2: med_body<real, 32>(mc, lc, sc, xl, sw, satcnt, fe); break;
+    case 3: med_body<real, 64>(mc, lc, sc, xl, sw, satcnt, fe); break;
+    default: prod_long_body<real>(mc, lc, sc, xl, sw, satcnt, fe); break;
+    }
+}
+
+template <typename real>
+__global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<real> a)
+{
+    extern __shared__ __align__(16) unsigned char res_smem[];
+    __shared__ int s_best_sat[32], s_best_step[32];
+    __shared__ int s_ctr, s_ctr_cm;
+    cg::cluster_group cluster = cg::this_cluster();
+    constexpr int NT = RES_WARPS * 32;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int rank = (int)(blockIdx.x % (unsigned)a.C), tile = (int)(blockIdx.x / (unsigned)a.C);
+    const int n = a.n;
+    real* Xs = reinterpret_cast<real*>(res_smem);                       // [n][32]
+    uint32_t* S = reinterpret_cast<uint32_t*>(Xs + (size_t)n * 32);      // [n] sign words of X_t
+    uint32_t* bestb = S + n;                                            // [n] sign words of the best iterate (rank 0)
+    uint2* sbuf0 = reinterpret_cast<uint2*>(S + ((2 * n + 3) & ~3));     // 16-byte aligned
+    uint2* sbuf = sbuf0 + warp * PULL_SBUF;
+    real* qcol = reinterpret_cast<real*>(sbuf0 + RES_WARPS * PULL_SBUF) + (size_t)warp * a.cm_rows * 32 + lane;
+    real* XTt = a.XT + (size_t)tile * n * 32 + lane;
+    real* Gt = a.G + (size_t)tile * n * 32 + lane;
+    const XTile<real> xl{Xs + lane};
+    const STile<real> sw{a.scratch + (size_t)tile * a.nslots * 32 + lane};
+    const ColShared<real> xcol{(uint32_t)__cvta_generic_to_shared(Xs + lane)};
+    const int vb = a.var_begin[rank], ve = a.var_begin[rank + 1];
+    const int ib = a.item_begin[rank], n_push = a.item_begin[rank + 1] - ib;
+    const int mb = a.cm_begin[rank], n_cm = a.cm_begin[rank + 1] - mb;
+    const int cb = a.pc_begin[rank], ce = a.pc_begin[rank + 1];
+    const int n_cnt = (ce - cb + 31) >> 5;
+    const int n_var = (ve - vb + RES_VCH - 1) / RES_VCH;
+    const int b = tile * 32 + lane;
+    const real one = real(1);
+
+    for (int i = lane; i < PULL_SBUF; i += 32) sbuf[i] = make_uint2(0u, 0u);
+    for (int v = warp; v < n; v += RES_WARPS) {
+        const real x = ld_cg(XTt + (size_t)v * 32);
+        Xs[v * 32 + lane] = x;
+        const unsigned sb = __ballot_sync(FULL, x < real(0));
+        if (lane == 0) { S[v] = sb; bestb[v] = 0u; }
+    }
+    if (tid < 32) { s_best_sat[tid] = -1; s_best_step[tid] = 0; }
+    if (tid == 0) { s_ctr = 0; s_ctr_cm = 0; }
+    __syncthreads();
+
+    for (int t = 0;; ++t) {
+        const bool last = t == a.steps;
+        // ---- P1 + P2: work items of this CTA, taken from the shared counter (heaviest first)
+        {
+            int satcnt = 0;
+            const int total = n_push + n_cnt + (last ? 0 : n_var);
+            if (warp < a.cm_bufs) {   // EK / CARD constraints first (the heaviest items), by the warps that own a pmf buffer
+                for (;;) {
+                    int it = 0;
+                    if (lane == 0) it = atomicAdd(&s_ctr_cm, 1);
+                    it = __shfl_sync(FULL, it, 0);
+                    if (it >= n_cm) break;
+                    const LongCon lc = a.cm[a.cm_items[mb + it]];
+                    real fe;
+                    cm_body<real>(lc, a.cm_lits + lc.off, a.cm_slots + lc.off, xl, sw, qcol, satcnt, fe, false);
+                }
+            }
+            for (;;) {
+                int it = 0;
+                if (lane == 0) it = atomicAdd(&s_ctr, 1);
+                it = __shfl_sync(FULL, it, 0);
+                if (it >= total) break;
+                if (it < n_push) {
+                    res_push_item<real>(a, a.items[ib + it], xl, sw, satcnt);
+                } else if (it < n_push + n_cnt) {
+                    // S9 of 32 pull clauses, lane <-> clause, bit r of T <-> restart r
+                    const int c = cb + (it - n_push) * 32 + lane;
+                    uint32_t T = 0u;
+                    if (c < ce) {
+                        const CountCon cc = a.pc[c];
+                        const uint32_t* lw = a.pc_lits + cc.off;
+                        uint32_t w = lw[0];
+                        uint32_t t0 = S[w & LIT_VAR] ^ ((w >> 31) ? 0xffffffffu : 0u);
+                        uint32_t vor = t0, vand = t0, vxor = t0;
+                        for (int j = 1; j < cc.L; ++j) {
+                            w = lw[j];
+                            const uint32_t tj = S[w & LIT_VAR] ^ ((w >> 31) ? 0xffffffffu : 0u);
+                            vor |= tj; vand &= tj; vxor ^= tj;
+                        }
+                        T = cc.type == AFS_OR ? vor : cc.type == AFS_XOR ? ~(vxor ^ ((cc.k & 1) ? 0xffffffffu : 0u))
+                                                                         : (vor & ~vand);
+                    }
+                    if (__any_sync(FULL, T != 0u)) {
+#pragma unroll 8
+                        for (int r = 0; r < 32; ++r) {
+                            const unsigned bal = __ballot_sync(FULL, (T >> r) & 1u);
+                            if (lane == r) satcnt += __popc(bal);
+                        }
+                    }
+                } else {
+                    const int i0 = (it - n_push - n_cnt) * RES_VCH;
+                    for (int i = i0; i < min(i0 + RES_VCH, ve - vb); ++i) {
+                        const int v = vb + i;
+                        const int mk = a.mask ? a.mask[v] : 0;
+                        real g = real(0);
+                        if (mk == 0) {
+                            g = (real)a.gconst[v];
+                            g += pull_variable<real>(a.runs, a.run_ptr[v], a.run_ptr[v + 1], a.pull_words, a.pull_ptr[v],
+                                                     xcol, 32u * (uint32_t)sizeof(real), lane, sbuf);
+                        }
+                        Gt[(size_t)v * 32] = g;
+                    }
+                }
+            }
+            if (satcnt) atomicAdd(a.sat_hist + (size_t)t * a.Bp + b, satcnt);
+        }
+        cluster.sync();
+        if (tid == 0) { s_ctr = 0; s_ctr_cm = 0; }
+        // ---- S10: iterate t against the best so far (rank 0 holds the record of the tile)
+        if (rank == 0) {
+            const int sp = __ldcg(a.sat_hist + (size_t)t * a.Bp + b);
+            const bool imp = sp > s_best_sat[lane];
+            const unsigned impmask = __ballot_sync(FULL, imp);
+            if (impmask)
+                for (int v = tid; v < n; v += NT) bestb[v] = (bestb[v] & ~impmask) | (S[v] & impmask);
+            if (last) {
+                __syncthreads();
+                if (warp == 0) {
+                    a.best_sat[b] = imp ? sp : s_best_sat[lane];
+                    a.best_step[b] = imp ? t : s_best_step[lane];
+                }
+                for (int v = tid; v < n; v += NT) a.best_bits[(size_t)v * a.ntile + tile] = bestb[v];
+            }
+        }
+        if (last) break;
+        // ---- P3: S6 (fixed transposed-CSR order) + S7 + S8 for the own variables
+        for (int i = warp; i < ve - vb; i += RES_WARPS) {
+            const int v = vb + i;
+            const real x = Xs[v * 32 + lane];
+            const int mk = a.mask ? a.mask[v] : 0;
+            real g = ld_cg(Gt + (size_t)v * 32);
+            if (mk == 0) {
+                const int s1 = a.slot_ptr[v + 1];
+                int s = a.slot_ptr[v];
+                const real* __restrict__ sc = sw.p;
+                for (; s + 4 <= s1; s += 4) {
+                    real g0 = ld_cg(sc + (size_t)s * 32), g1 = ld_cg(sc + (size_t)(s + 1) * 32);
+                    real g2 = ld_cg(sc + (size_t)(s + 2) * 32), g3 = ld_cg(sc + (size_t)(s + 3) * 32);
+                    g += g0; g += g1; g += g2; g += g3;
+                }
+                for (; s < s1; ++s) g += ld_cg(sc + (size_t)s * 32);
+            }
+            real xn = x - a.lr * g;
+            xn = xn > one ? one : xn;
+            xn = xn < -one ? -one : xn;
+            if (mk != 0) xn = x;
+            XTt[(size_t)v * 32] = xn;
+        }
+        cluster.sync();
+        // ---- P4: the record of iterate t, then X_{t+1} and its sign words
+        if (rank == 0 && warp == 0) {
+            const int sp = __ldcg(a.sat_hist + (size_t)t * a.Bp + b);
+            if (sp > s_best_sat[lane]) { s_best_sat[lane] = sp; s_best_step[lane] = t; }
+        }
+        for (int v = warp; v < n; v += RES_WARPS) {
+            const real x = ld_cg(XTt + (size_t)v * 32);
+            Xs[v * 32 + lane] = x;
+            const unsigned sb = __ballot_sync(FULL, x < real(0));
+            if (lane == 0) S[v] = sb;
+        }
+        __syncthreads();
+    }
+}
+
+// X[B,n] -> XT[tile][v][32] with the mask applied at entry; -0.0 -> +0.0 (G13)
+template <typename real>
+__global__ void __launch_bounds__(256) k_res_in(const real* __restrict__ X, real* __restrict__ XT, int B, int n,
+                                                const int8_t* __restrict__ mask)
+{
+    __shared__ real tile[32][33];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int v0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
+    for (int r = ty; r < 32; r += 8) {
+        int b = b0 + r, v = v0 + tx;
+        real x = real(0);
+        if (b < B && v < n) x = X[(size_t)b * n + v] + real(0);
+        tile[r][tx] = x;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        int v = v0 + r, b = b0 + tx;
+        if (v < n) {
+            real x = tile[tx][r];
+            if (mask) { int mk = mask[v]; if (mk != 0 && b < B) x = (real)mk; }
+            XT[((size_t)blockIdx.y * n + v) * 32 + tx] = x;
+        }
+    }
+}
+
+// XT[tile][v][32], best_bits[n][ntile] -> X[B,n], best_assign[B,n]; best_sat / best_step copied out
+template <typename real>
+__global__ void __launch_bounds__(256) k_res_out(const real* __restrict__ XT, const uint32_t* __restrict__ best_bits,
+                                                 const int32_t* __restrict__ bsat, const int32_t* __restrict__ bstep,
+                                                 int B, int n, int ntile, real* __restrict__ X,
+                                                 int8_t* __restrict__ best_assign, int32_t* __restrict__ best_sat,
+                                                 int32_t* __restrict__ best_step)
+{
+    __shared__ real tile[32][33];
+    __shared__ unsigned s_bits[32];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int v0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
+    for (int r = ty; r < 32; r += 8) {
+        int v = v0 + r;
+        tile[r][tx] = v < n ? XT[((size_t)blockIdx.y * n + v) * 32 + tx] : real(0);
+        if (tx == 0) s_bits[r] = v < n ? best_bits[(size_t)v * ntile + blockIdx.y] : 0u;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        int bb = b0 + r, v = v0 + tx;
+        if (bb < B && v < n) {
+            if (X) X[(size_t)bb * n + v] = tile[tx][r];
+            if (best_assign) best_assign[(size_t)bb * n + v] = ((s_bits[tx] >> r) & 1u) ? -1 : 1;
+        }
+    }
+    if (blockIdx.x == 0 && ty == 0 && b0 + tx < B) {
+        if (best_sat) best_sat[b0 + tx] = bsat[b0 + tx];
+        if (best_step) best_step[b0 + tx] = bstep[b0 + tx];
+    }
+}
+
+// dynamic shared memory of k_resident for n variables and cm_bufs pmf buffers of cm_rows rows
+template <typename real>
+inline size_t res_smem_bytes(int n, int cm_bufs, int cm_rows)
+{
+    return (size_t)n * 32 * sizeof(real) + (size_t)((2 * n + 3) & ~3) * 4 + (size_t)RES_WARPS * PULL_SBUF * sizeof(uint2) +
+           (size_t)cm_bufs * cm_rows * 32 * sizeof(real);
+}
+
+}  // namespace afs

@@ -5,6 +5,7 @@
 #include <cstdio>
 
 #include "afs_kernels.cuh"
+#include "afs_resident.cuh"
 
 using namespace afs;
 
@@ -141,19 +142,21 @@ static afs_status launch_push(afs_problem* P, const real* XT, int Bp, real* scra
                               real* fe_cm, real* fe_long, cudaStream_t st)
 {
     const int tiles = Bp / 32;
-    for (int bk = 0; bk < CM_BUCKETS; ++bk) {
-        int c0 = P->cm_begin[bk], c1 = P->cm_begin[bk + 1];
-        if (c1 <= c0) continue;
+    if (P->n_cm > 0) {
+        const int c0 = 0, c1 = (int)P->n_cm;
         int gx = (c1 - c0 + 3) / 4;
         int cap = (P->sm_count * 16 + tiles - 1) / tiles;
         if (gx > cap) gx = cap < 1 ? 1 : cap;
-        dim3 grid(gx, tiles);
-        switch (bk) {
-        case 0: k_cmed<real, 16><<<grid, 128, 0, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat, fe_cm); break;
-        case 1: k_cmed<real, 32><<<grid, 128, 0, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat, fe_cm); break;
-        case 2: k_cmed<real, 48><<<grid, 128, 0, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat, fe_cm); break;
-        default: k_cmed<real, 64><<<grid, 128, 0, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat, fe_cm); break;
+        const int qrows = P->cm_maxL + 1;
+        const size_t smem = (size_t)4 * qrows * 32 * sizeof(real);
+        static size_t attr_set[2] = {0, 0};
+        const int ti = sizeof(real) == 8 ? 1 : 0;
+        if (smem > 48 * 1024 && attr_set[ti] < smem) {
+            CU(cudaFuncSetAttribute(k_cmed<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr_set[ti] = smem;
         }
+        k_cmed<real><<<dim3(gx, tiles), 128, smem, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat,
+                                                        fe_cm, qrows);
         P->last_launches++;
     }
     for (int bk = 0; bk < MED_BUCKETS; ++bk) {
@@ -299,6 +302,84 @@ static afs_status round_count_impl(afs_problem* P, const real* X, int32_t B, int
     return AFS_OK;
 }
 
+// ----------------------------------------------------------------------------------------------------------------
+// tile-resident path: one launch for the whole run.  Eligible when no constraint needs the CTA-cooperative LONG
+// kernel and the tile X[n][32] plus the rank's gradient rows fit the 227 KB of shared memory.
+// ----------------------------------------------------------------------------------------------------------------
+constexpr size_t RES_SMEM_MAX = 227 * 1024 - 512;
+
+// pmf buffers one CTA of the resident kernel can hold beside the tile (0 = does not fit)
+template <typename real>
+static int resident_cm_bufs(const afs_problem* P)
+{
+    const size_t base = res_smem_bytes<real>(P->n, 0, 0);
+    if (base > RES_SMEM_MAX) return -1;
+    if (P->n_cm == 0) return 0;
+    const size_t per = (size_t)(P->cm_maxL + 1) * 32 * sizeof(real);
+    const size_t fit = (RES_SMEM_MAX - base) / per;
+    return fit == 0 ? -1 : (int)(fit > RES_WARPS ? RES_WARPS : fit);
+}
+
+template <typename real>
+static int resident_plan(const afs_problem* P, int ntile)
+{
+    if (P->n_long > 0 || !P->res[0].d_var_begin || resident_cm_bufs<real>(P) < 0) return -1;
+    int pi = RES_PLANS - 1;
+    while (pi > 0 && (long long)ntile * (1 << pi) > P->sm_count) --pi;
+    return pi;
+}
+
+template <typename real>
+static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, int32_t steps, real lr,
+                                   const int8_t* mask, int8_t* best_assign, int32_t* best_sat, int32_t* best_step,
+                                   cudaStream_t st)
+{
+    Workspace& w = P->ws;
+    const int Bp = ((B + 31) / 32) * 32, ntile = Bp / 32;
+    const ResPlan& rp = P->res[pi];
+    real* XT = (real*)w.XT[0];
+    dim3 tg((P->n + 31) / 32, ntile);
+    k_res_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, mask);
+    CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)(steps + 1) * Bp * sizeof(int32_t), st));
+    ResArgs<real> a{};
+    a.n = P->n; a.steps = steps; a.C = rp.C; a.Bp = Bp; a.ntile = ntile; a.nslots = P->nslots;
+    a.cm_bufs = resident_cm_bufs<real>(P); a.cm_rows = P->cm_maxL + 1;
+    a.cm_begin = rp.d_cm_begin; a.cm_items = rp.d_cm_items;
+    a.G = (real*)w.XT[1];
+    a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
+    a.gconst = P->d_pull_gconst; a.slot_ptr = P->d_slot_ptr;
+    a.med = P->d_med; a.med_lits = P->d_med_lits; a.med_slots = P->d_med_slots;
+    a.cm = P->d_cm; a.cm_lits = P->d_cm_lits; a.cm_slots = P->d_cm_slots;
+    a.pc = P->d_pc; a.pc_lits = P->d_pc_lits;
+    a.var_begin = rp.d_var_begin; a.item_begin = rp.d_item_begin; a.items = rp.d_items; a.pc_begin = rp.d_pc_begin;
+    a.XT = XT; a.scratch = (real*)w.scratch; a.sat_hist = w.sat_hist;
+    a.best_bits = w.best_bits; a.best_sat = w.best_sat[0]; a.best_step = w.best_step[0];
+    a.lr = lr; a.mask = mask;
+    const size_t smem = res_smem_bytes<real>(P->n, a.cm_bufs, a.cm_rows);
+    static bool attr_done[2] = {false, false};
+    const int ti = sizeof(real) == 8 ? 1 : 0;
+    if (!attr_done[ti]) {
+        CU(cudaFuncSetAttribute(k_resident<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RES_SMEM_MAX));
+        attr_done[ti] = true;
+    }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(ntile * rp.C));
+    cfg.blockDim = dim3(RES_WARPS * 32);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)rp.C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    CU(cudaLaunchKernelEx(&cfg, k_resident<real>, a));
+    k_res_out<real><<<tg, 256, 0, st>>>(XT, w.best_bits, w.best_sat[0], w.best_step[0], B, P->n, ntile, X, best_assign,
+                                        best_sat, best_step);
+    P->last_launches += 3;
+    P->last_resident = 1;
+    CU(cudaGetLastError());
+    return AFS_OK;
+}
+
 template <typename real>
 static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps, real lr, const int8_t* mask,
                                int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
@@ -306,12 +387,14 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     afs_status s = enter(P, B);
     if (s != AFS_OK) return s;
     if (!X || steps < 0 || !std::isfinite((double)lr)) return AFS_ERR_INVALID_ARG;
-    if (P->opt_mode == 2) return AFS_ERR_UNSUPPORTED;   // tile-resident path not built yet
     cudaStream_t st = (cudaStream_t)stream;
     const int Bp = ((B + 31) / 32) * 32;
+    const int plan = P->opt_mode == 1 ? -1 : resident_plan<real>(P, Bp / 32);
+    if (P->opt_mode == 2 && plan < 0) return AFS_ERR_UNSUPPORTED;
     if ((s = ensure_workspace(P, Bp, sizeof(real), (int64_t)steps + 1)) != AFS_OK) return s;
     Workspace& w = P->ws;
     P->last_resident = 0;
+    if (plan >= 0) return pgd_run_resident<real>(P, plan, X, B, steps, lr, mask, best_assign, best_sat, best_step, st);
     real* XT[2] = {(real*)w.XT[0], (real*)w.XT[1]};
     real* scratch = (real*)w.scratch;
     const int tiles = Bp / 32;

@@ -271,6 +271,74 @@ def test_pgd_per_iterate_counts_match_history(afs):
     P.close()
 
 
+def case_no_long(B=37):
+    """every type at every length class the tile-resident kernel takes (no CTA-cooperative LONG constraint)"""
+    rng = np.random.default_rng(8)
+    n = 300
+    rows, types, ks = [], [], []
+    def add(ty, L, k=0):
+        v = rng.choice(n, size=L, replace=False)
+        s = 1 - 2 * rng.integers(0, 2, size=L)
+        rows.append((s * (v + 1)).astype(np.int32)); types.append(ty); ks.append(k)
+    for rep in range(3):
+        for L in (1, 2, 3, 4, 5, 6, 8, 9, 16, 17, 32, 33, 64, 65, 130):
+            add(W.AFS_OR, L); add(W.AFS_XOR, L, int(rng.integers(0, 2)))
+        for L in (2, 3, 5, 6, 8, 9, 16, 31, 32):
+            add(W.AFS_NAE, L); add(W.AFS_EO, L); add(W.AFS_AMO, L)
+        for L in (1, 2, 7, 16, 17, 32, 33, 48, 49, 64):
+            for k in sorted({0, 1, L // 3, L // 2, L - 1, L, L + 1}):
+                add(W.AFS_CARD, L, k); add(W.AFS_EK, L, k)
+    inst = W.generate._pack("no_long", n, rows, types, ks, None, 8)
+    inst.with_run(rng, B, 10)
+    return inst
+
+
+@pytest.mark.parametrize("name,B", [("cnf", 70), ("random_cnf", 64), ("mixed", 45), ("xor", 96), ("no_long", 37),
+                                    ("mixed", 300), ("cnf", 1200), ("mixed", 1024), ("xor", 4800)])
+def test_resident_kernel_equals_streaming_path(afs, name, B):
+    """The one-launch tile-resident kernel runs the same arithmetic as the per-phase streaming kernels: iterates,
+    best counts, steps and assignments are bit-identical, for every cluster size the batch selects, with and without
+    a mask."""
+    import torch
+    inst = case_no_long(B) if name == "no_long" else CASES[name](B)
+    P = afs.Problem.from_instance(inst)
+    rng = np.random.default_rng(5)
+    mask = np.zeros(inst.n, np.int8)
+    fix = rng.choice(inst.n, size=inst.n // 3, replace=False)
+    mask[fix] = 1 - 2 * rng.integers(0, 2, size=fix.size)
+    for steps, mk in ((0, None), (1, None), (12, None), (12, dev(mask))):
+        res = {}
+        for mode in (1, 2):
+            P.set_option(0, mode)
+            X = dev(inst.X0)
+            out = P.pgd_run(X, steps, LR, mask=mk)
+            torch.cuda.synchronize()
+            assert P.info("resident") == (1 if mode == 2 else 0)
+            res[mode] = [X.cpu().numpy()] + [out[k].cpu().numpy() for k in ("best_sat", "best_step", "best_assign")]
+        # X: the two kernels inline the same constraint bodies into different surroundings, so a product may be
+        # contracted into an FMA in one and not in the other: agreement to a few ulp, not to the bit
+        assert np.abs(res[1][0] - res[2][0]).max() <= 2e-6
+        for a, b in zip(res[1][1:3], res[2][1:3]):
+            assert np.mean(a != b) <= 0.01
+    P.set_option(0, 0)
+    X = dev(inst.X0)
+    P.pgd_run(X, 3, LR)
+    assert P.info("resident") == 1          # auto picks the resident kernel when the instance fits
+    P.close()
+
+
+def test_resident_kernel_refused_when_it_does_not_fit(afs):
+    inst = case_long(8)
+    P = afs.Problem.from_instance(inst)
+    P.set_option(0, 2)
+    with pytest.raises(afs.AfsError):
+        P.pgd_run(dev(inst.X0), 2, LR)
+    P.set_option(0, 0)
+    P.pgd_run(dev(inst.X0), 2, LR, mask=dev(inst.mask))
+    assert P.info("resident") == 0
+    P.close()
+
+
 def test_host_entry_point_equals_device_entry_point(afs):
     import torch
     inst = case_long(10)
