@@ -31,9 +31,32 @@ import workloads as W  # noqa: E402
 
 
 # --------------------------------------------------------------------------------------------- algorithmic work
-def algorithmic_flops_per_restart_step(inst) -> float:
-    """SURVEY.md 8(d) / DESIGN.md section 7: minimal flops of objective + gradient + chain rule per constraint
-    (FMA = 2), 1 add per literal for the variable reduction, 5 per variable for step/clip/mask/sign."""
+def kernel_class_of_constraints(inst):
+    """The library's execution classes (afs_internal.h), restated so that algorithmic work can be attributed to the
+    kernel that does it: names are Problem.KERNEL_CLASSES ('var' holds the pull clauses)."""
+    L = inst.lengths()
+    ty = inst.types
+    prod = (ty == W.AFS_OR) | (ty == W.AFS_XOR)
+    two = (ty == W.AFS_NAE) | (ty == W.AFS_EO) | (ty == W.AFS_AMO)
+    cnt = (ty == W.AFS_EK) | (ty == W.AFS_CARD)
+    out = np.empty(inst.m, dtype=object)
+    for c in range(inst.m):
+        l = int(L[c])
+        if (prod[c] or ty[c] == W.AFS_NAE) and l <= 5:
+            out[c] = "var"
+        elif prod[c] or (two[c] and l <= 32):
+            out[c] = "med%d" % (0 if l <= 8 else 1 if l <= 16 else 2 if l <= 32 else 3 if l <= 64 else 4)
+        elif cnt[c] and l <= 64:
+            out[c] = "cmed"
+        else:
+            out[c] = "long%d" % ((l + 1 + 127) // 128)
+    return out
+
+
+def algorithmic_flops_per_constraint(inst) -> np.ndarray:
+    """SURVEY.md 8(d) / DESIGN.md section 7: minimal flops of objective + gradient + chain rule per constraint and
+    restart (FMA = 2).  EK / CARD: 6 L K with K = min(k, L-k+1)+1 cells; literals of variables fixed by the mask are
+    constants of the run and are folded (L counts the free literals, k is reduced by the fixed true ones)."""
     L = inst.lengths().astype(np.float64)
     k = inst.k.astype(np.float64)
     ty = inst.types
@@ -43,15 +66,56 @@ def algorithmic_flops_per_restart_step(inst) -> float:
     f[ty == W.AFS_NAE] = 9 * L[ty == W.AFS_NAE]
     two = (ty == W.AFS_EO) | (ty == W.AFS_AMO)
     f[two] = 15 * L[two]
-    cnt = (ty == W.AFS_EK) | (ty == W.AFS_CARD)
-    K = np.minimum(k, L - k + 1) + 1
-    f[cnt] = 6 * L[cnt] * np.maximum(K[cnt], 1)
-    return float(f.sum() + inst.nnz + 5 * inst.n)
+    cnt = np.flatnonzero((ty == W.AFS_EK) | (ty == W.AFS_CARD))
+    for c in cnt:
+        lits = inst.lits[inst.row_ptr[c]:inst.row_ptr[c + 1]]
+        Lc, kc = float(len(lits)), float(inst.k[c])
+        if inst.mask is not None:
+            mv = inst.mask[np.abs(lits) - 1].astype(np.int64)
+            fixed = mv != 0
+            true_fixed = np.sum(fixed & ((mv < 0) != (lits < 0)))      # literal true: variable True (-1) XOR negated
+            Lc -= float(fixed.sum())
+            kc -= float(true_fixed)
+        K = min(kc, Lc - kc + 1) + 1
+        f[c] = 6 * Lc * max(K, 1) if (Lc > 0 and 0 < kc <= Lc) else 0.0
+    return f
 
 
-def compulsory_hbm_bytes_per_step(inst, B) -> float:
-    """read X + write X (fp32) + literal CSR once"""
-    return float(2 * B * inst.n * 4 + inst.nnz * 4)
+def algorithmic_work(inst):
+    """Per kernel class and per PGD iteration over the whole batch: (flops, compulsory HBM bytes)."""
+    cls = kernel_class_of_constraints(inst)
+    f = algorithmic_flops_per_constraint(inst)
+    L = inst.lengths().astype(np.float64)
+    B = float(inst.B)
+    work = {}
+    for name in set(cls):
+        sel = cls == name
+        if name == "var":
+            continue
+        # gather X rows of the literals once + write one gradient per literal + the literal CSR
+        work[name] = (float(f[sel].sum()) * B, float(L[sel].sum()) * (B * 8 + 8))
+    pull = cls == "var"
+    pushed = float(L[~pull].sum())
+    # variable pass: pull clauses, one add per materialised literal gradient, 5 flops per variable for S7-S9;
+    # bytes: read X + write X, the materialised gradients once, the pull streams once
+    work["var"] = ((float(f[pull].sum()) + pushed + 5.0 * inst.n) * B,
+                   2 * B * inst.n * 4 + pushed * B * 4 + float(L[pull].sum() * 4 * 4))
+    work["sat_pull"] = (0.0, float(inst.n * B / 8 + L[pull].sum() * 4))
+    total_f = float(f.sum() + inst.nnz + 5 * inst.n) * B
+    work["step"] = (total_f, float(2 * B * inst.n * 4 + inst.nnz * 4))
+    return work
+
+
+def load_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, copied from an
+    `ncu --set full` capture into profiles/traffic.json (the capture and its command are named there); else None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(path):
+        return None
+    try:
+        return json.load(open(path)).get(workload, {}).get(kernel, {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
 
 
 def load_peaks():
@@ -271,24 +335,50 @@ def run_cuda(args):
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant kernel
+    # ---- roofline of the dominant kernel: its launches timed live with CUDA events on the launching stream
+    # (afs_set_option(1, stride) + afs_profile_read), in a second pass so that the events do not sit in `value`
     peaks = load_peaks()
-    flops_rs = algorithmic_flops_per_restart_step(inst)
-    bytes_step = compulsory_hbm_bytes_per_step(inst, inst.B)
+    work = algorithmic_work(inst)
     fp32_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12          # TFLOP/s, DESIGN.md section 7
-    t_alu = flops_rs * inst.B / (fp32_peak * 1e12)
-    t_hbm = bytes_step / (peaks["hbm_gbs"] * 1e9)
-    per_iter_s = dev_ms * 1e-3 / (args.steps * pgd_steps)                   # whole PGD iteration, this rank
-    if t_alu >= t_hbm:
-        roof = dict(bound="alu", achieved=flops_rs * inst.B / per_iter_s / 1e12, peak=fp32_peak, unit="TFLOP/s")
-    else:
-        roof = dict(bound="hbm", achieved=bytes_step / per_iter_s / 1e9, peak=peaks["hbm_gbs"], unit="GB/s")
-    roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
-    roof["peak_source"] = ("148 SMs x 128 FP32 lanes x 2 x sm_max_mhz (%s)" % peaks["source"]) if roof["bound"] == "alu" \
-        else "MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"]
-    roof["kernel"] = "resident PGD kernel (whole call)" if resident else "all kernels of one PGD iteration (streaming path)"
-    roof["algorithmic_per_iteration"] = dict(flops=flops_rs * inst.B, hbm_bytes=bytes_step)
+    stride = max(1, pgd_steps // 64)
+    P.set_option(1, stride)
+    prof = {}
+    for _ in range(max(1, min(args.steps, 3))):
+        one_call(False)
+        for k, (ms, cnt) in P.profile_read().items():
+            a = prof.setdefault(k, [0.0, 0]); a[0] += ms; a[1] += cnt
+    P.set_option(1, 0)
+    dom = max(prof, key=lambda k: prof[k][0]) if prof else None
+    roof = dict(bound=None, achieved=None, peak=None, unit=None, frac=None, traffic=None)
+    per_iter_s = dev_ms * 1e-3 / (args.steps * max(pgd_steps, 1))           # whole PGD iteration, this rank
+    if dom is not None:
+        dur_s = prof[dom][0] * 1e-3 / prof[dom][1]                          # average launch duration
+        if dom == "resident":                                               # one launch = every iteration of the call
+            flops, hbm = work["step"][0] * pgd_steps, 2 * inst.B * inst.n * 4 + inst.nnz * 4
+        else:
+            flops, hbm = work[dom]
+        t_alu, t_hbm = flops / (fp32_peak * 1e12), hbm / (peaks["hbm_gbs"] * 1e9)
+        if t_alu >= t_hbm:
+            roof.update(bound="alu", achieved=flops / dur_s / 1e12, peak=fp32_peak, unit="TFLOP/s",
+                        peak_source="148 SMs x 128 FP32 lanes x 2 flop x sm_max_mhz %.0f (MEASURED_PEAKS.json: %s)"
+                                    % (peaks["sm_max_mhz"], peaks["source"]))
+        else:
+            roof.update(bound="hbm", achieved=hbm / dur_s / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
+                        peak_source="MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"])
+        roof["frac"] = roof["achieved"] / roof["peak"]
+        roof["kernel"] = dom
+        roof["launch_ms"] = dur_s * 1e3
+        roof["launches_timed"] = prof[dom][1]
+        roof["algorithmic_per_launch"] = dict(flops=flops, hbm_bytes=hbm)
+        tot_ms = sum(v[0] for v in prof.values())
+        roof["share_of_timed_launches"] = {k: round(v[0] / tot_ms, 4) for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}
+        roof["traffic"] = load_traffic(inst.name, dom)
+    # the whole PGD iteration against the same two ceilings (every kernel of the step, launch gaps included)
+    sf, sb = work["step"]
+    t_alu, t_hbm = sf / (fp32_peak * 1e12), sb / (peaks["hbm_gbs"] * 1e9)
+    roof["step"] = dict(bound="alu" if t_alu >= t_hbm else "hbm", roofline_us=max(t_alu, t_hbm) * 1e6,
+                        measured_us=per_iter_s * 1e6, frac=max(t_alu, t_hbm) / per_iter_s,
+                        algorithmic_per_iteration=dict(flops=sf, hbm_bytes=sb))
 
     # ---- the oracle beside it (bounded sample, rank 0, N = 1 only)
     cpu = None

@@ -152,9 +152,25 @@ AFS_API int64_t afs_problem_info(const afs_problem* p, int32_t what);
  * afs_set_option -- tuning knobs (all have defaults; tests use them to force code paths).  `what`:
  *   0 execution mode of afs_pgd_run: 0 auto, 1 force the streaming (one launch per phase per step) path,
  *     2 force the tile-resident path (AFS_ERR_UNSUPPORTED at run time if the instance does not fit)
+ *   1 per-launch timing stride (see afs_profile_read); 0 = off
  * Returns AFS_ERR_INVALID_ARG for unknown options or values.
  */
 AFS_API afs_status afs_set_option(afs_problem* p, int32_t what, int64_t value);
+
+/*
+ * Per-launch device timing, for bench.py's roofline of the dominant kernel.  afs_set_option(p, 1, stride) with
+ * stride >= 1 makes afs_pgd_run* bracket every launch of each stride-th PGD iteration (and the single launch of the
+ * tile-resident kernel) with CUDA events on the caller's stream; stride = 0 (default) switches it off.
+ * afs_profile_read waits for the last recorded event, adds the elapsed milliseconds and launch counts of the most
+ * recent afs_pgd_run* call per kernel class into ms[0..n) / launches[0..n) (host arrays, n <= AFS_KERNEL_CLASSES;
+ * the caller zeroes them), and forgets the spans.  Classes:
+ *   0 tile-resident PGD kernel      1 variable pass (pull gradients + S6 + S7 + S8)    2 pull-clause counts (S9)
+ *   3 EK/CARD with L <= 64          4..8 medium buckets (padded 8, 16, 32, 64, two-pass product)
+ *   9..17 long-constraint kernel, 1..9 rows of 128 pmf cells                              18 boundary (layout changes,
+ *   final count, fills)
+ */
+#define AFS_KERNEL_CLASSES 19
+AFS_API afs_status afs_profile_read(afs_problem* p, double* ms, int64_t* launches, int32_t n);
 
 /* Static, never NULL. */
 AFS_API const char* afs_status_string(afs_status s);

@@ -21,6 +21,7 @@ EXPORTS = (
     "afs_problem_create", "afs_problem_destroy", "afs_coeffs", "afs_eval_grad", "afs_eval_grad_f64",
     "afs_round_count", "afs_round_count_f64", "afs_pgd_run", "afs_pgd_run_f64", "afs_pgd_run_host",
     "afs_problem_info", "afs_set_option", "afs_status_string", "afs_abi_version", "afs_last_error_message",
+    "afs_profile_read",
 )
 
 _lib = None
@@ -65,6 +66,8 @@ def lib():
     L.afs_problem_info.restype = i64
     L.afs_set_option.argtypes = [vp, i32, i64]
     L.afs_set_option.restype = C.c_int
+    L.afs_profile_read.argtypes = [vp, vp, vp, i32]
+    L.afs_profile_read.restype = C.c_int
     L.afs_status_string.argtypes = [C.c_int]
     L.afs_status_string.restype = C.c_char_p
     L.afs_abi_version.restype = i32
@@ -138,6 +141,16 @@ class Problem:
 
     def set_option(self, what: int, value: int):
         _chk(lib().afs_set_option(self._h, what, value), "afs_set_option")
+
+    KERNEL_CLASSES = (["resident", "var", "sat_pull", "cmed"] + ["med%d" % i for i in range(5)] +
+                      ["long%d" % (i + 1) for i in range(9)] + ["boundary"])
+
+    def profile_read(self):
+        """afs_profile_read: {class name: (milliseconds, launches)} of the last pgd_run, non-empty classes only."""
+        ms = np.zeros(len(self.KERNEL_CLASSES), dtype=np.float64)
+        cnt = np.zeros(len(self.KERNEL_CLASSES), dtype=np.int64)
+        _chk(lib().afs_profile_read(self._h, ms.ctypes.data, cnt.ctypes.data, len(ms)), "afs_profile_read")
+        return {k: (float(m), int(c)) for k, m, c in zip(self.KERNEL_CLASSES, ms, cnt) if c}
 
     # ------------------------------------------------------------------ helpers
     def _dev(self):

@@ -83,6 +83,18 @@ struct ResPlan {
     int32_t* d_pc_begin = nullptr;     // [C+1] ranges of the pull clauses whose counts the rank takes
 };
 
+// ---- per-launch device timing (afs_set_option 1, afs_profile_read): CUDA events on the caller's stream around the
+// launches of every `stride`-th PGD iteration, summed per kernel class (afs_kernel_class in afs.h)
+constexpr int PROF_CLASSES = 19;
+struct Profiler {
+    int stride = 0;                       // 0 = off
+    bool on = false;                      // the iteration being enqueued is sampled
+    std::vector<cudaEvent_t> pool;
+    size_t used = 0;
+    struct Span { int cls, e0, e1; };
+    std::vector<Span> spans;
+};
+
 // records cudaGetErrorString(e) + location for afs_last_error_message()
 void note_cuda_error(cudaError_t e, const char* file, int line);
 
@@ -160,4 +172,5 @@ struct afs_problem {
     int64_t last_launches = 0;
     int32_t opt_mode = 0;
     int32_t last_resident = 0;
+    afs::Profiler prof;
 };

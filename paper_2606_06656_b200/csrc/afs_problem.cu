@@ -375,6 +375,7 @@ extern "C" void afs_problem_destroy(afs_problem* p)
         cudaFree(p->res[i].d_cm_begin); cudaFree(p->res[i].d_cm_items);
     }
     afs::free_workspace(p);
+    for (cudaEvent_t e : p->prof.pool) cudaEventDestroy(e);
     (void)cudaGetLastError();
     delete p;
 }
@@ -401,6 +402,7 @@ extern "C" afs_status afs_set_option(afs_problem* p, int32_t what, int64_t value
 {
     if (!p) return AFS_ERR_INVALID_ARG;
     if (what == 0 && value >= 0 && value <= 2) { p->opt_mode = (int32_t)value; return AFS_OK; }
+    if (what == 1 && value >= 0 && value <= (1 << 20)) { p->prof.stride = (int)value; return AFS_OK; }
     return AFS_ERR_INVALID_ARG;
 }
 

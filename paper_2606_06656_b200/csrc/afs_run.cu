@@ -38,6 +38,39 @@ void free_workspace(afs_problem* P)
 
 }  // namespace afs
 
+// ---- per-launch timing (afs_profile_read) -------------------------------------------------------------------------
+static int prof_mark(afs_problem* P, cudaStream_t st)
+{
+    Profiler& pr = P->prof;
+    if (pr.used == pr.pool.size()) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) { (void)cudaGetLastError(); return -1; }
+        pr.pool.push_back(e);
+    }
+    if (cudaEventRecord(pr.pool[pr.used], st) != cudaSuccess) { (void)cudaGetLastError(); return -1; }
+    return (int)pr.used++;
+}
+struct ProfSpan {   // brackets the launches enqueued during its lifetime
+    afs_problem* P; cudaStream_t st; int cls, e0;
+    ProfSpan(afs_problem* p, int c, cudaStream_t s) : P(p), st(s), cls(c), e0(p->prof.on ? prof_mark(p, s) : -1) {}
+    ~ProfSpan() { if (e0 >= 0) { int e1 = prof_mark(P, st); if (e1 >= 0) P->prof.spans.push_back({cls, e0, e1}); } }
+};
+
+extern "C" afs_status afs_profile_read(afs_problem* P, double* ms, int64_t* launches, int32_t n)
+{
+    if (!P || !ms || !launches || n < 0 || n > PROF_CLASSES) return AFS_ERR_INVALID_ARG;
+    Profiler& pr = P->prof;
+    if (pr.used > 0) CU(cudaEventSynchronize(pr.pool[pr.used - 1]));
+    for (const Profiler::Span& sp : pr.spans) {
+        float t = 0.f;
+        CU(cudaEventElapsedTime(&t, pr.pool[sp.e0], pr.pool[sp.e1]));
+        if (sp.cls < n) { ms[sp.cls] += (double)t; launches[sp.cls] += 1; }
+    }
+    pr.spans.clear();
+    pr.used = 0;
+    return AFS_OK;
+}
+
 static int var_grid_x(int n) { return (n + VAR_WARPS * VAR_VPW - 1) / (VAR_WARPS * VAR_VPW); }
 // number of per-warp partial sums of k_fe_pull: fixed per problem, so the objective is reproducible
 static int fe_pull_grid_x(const afs_problem* P) { int g = (int)((P->n_pull + 63) / 64); return g < 1 ? 1 : (g > 2048 ? 2048 : g); }
@@ -113,6 +146,7 @@ static afs_status launch_long_rpc(afs_problem* P, int bucket, const real* XT, in
     }
     long long blocks = (long long)(c1 - c0) * (Bp / RPC);
     if (blocks > 0x7fffffffLL) return AFS_ERR_UNSUPPORTED;
+    ProfSpan span(P, 8 + NR, st);
     k_long<real, NR, RPC><<<(unsigned)blocks, RPC * 32, smem, st>>>(P->d_long, c0, P->d_long_lits, P->d_long_slots, XT,
                                                                     Bp, scratch, sat, fe, LS, QS);
     P->last_launches++;
@@ -155,6 +189,7 @@ static afs_status launch_push(afs_problem* P, const real* XT, int Bp, real* scra
             CU(cudaFuncSetAttribute(k_cmed<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             attr_set[ti] = smem;
         }
+        ProfSpan span(P, 3, st);
         k_cmed<real><<<dim3(gx, tiles), 128, smem, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat,
                                                         fe_cm, qrows);
         P->last_launches++;
@@ -166,6 +201,7 @@ static afs_status launch_push(afs_problem* P, const real* XT, int Bp, real* scra
         int cap = (P->sm_count * 16 + tiles - 1) / tiles;   // enough CTAs to fill the chip, grid-stride beyond
         if (gx > cap) gx = cap < 1 ? 1 : cap;
         dim3 grid(gx, tiles);
+        ProfSpan span(P, 4 + bk, st);
         switch (bk) {
         case 0: k_med<real, 8><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
         case 1: k_med<real, 16><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
@@ -191,6 +227,7 @@ static afs_status launch_count(afs_problem* P, const real* XT, int Bp, int32_t* 
         int gx = (P->m + 7) / 8;
         int cap = (P->sm_count * 8 + tiles - 1) / tiles;
         if (gx > cap) gx = cap < 1 ? 1 : cap;
+        ProfSpan span(P, 18, st);
         k_count<real><<<dim3(gx, tiles), 256, 0, st>>>(P->d_count, P->d_count_lits, P->m, XT, Bp, sat);
         P->last_launches++;
     }
@@ -212,6 +249,7 @@ static afs_status launch_sat_pull(afs_problem* P, const uint32_t* S, int Bp, int
     const int nchunks = (int)((P->n_pull + chunk - 1) / chunk);
     dim3 grid((nchunks + SATP_CPB - 1) / SATP_CPB, gy);
     const int m = (int)P->n_pull;
+    ProfSpan span(P, 2, st);
     if (chunk <= 15) k_sat_pull<4><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, chunk, S, ntile, sat);
     else if (chunk <= 63) k_sat_pull<6><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, chunk, S, ntile, sat);
     else if (chunk <= 255) k_sat_pull<8><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, chunk, S, ntile, sat);
@@ -227,6 +265,9 @@ static afs_status enter(afs_problem* P, int32_t B)
     if ((unsigned long long)P->n * (unsigned long long)(((B + 31) / 32) * 32) * 8ull >= (1ull << 32)) return AFS_ERR_UNSUPPORTED;
     if (cudaSetDevice(P->device) != cudaSuccess) { (void)cudaGetLastError(); return AFS_ERR_CUDA; }
     P->last_launches = 0;
+    P->prof.on = false;
+    P->prof.spans.clear();
+    P->prof.used = 0;
     return AFS_OK;
 }
 
@@ -371,7 +412,12 @@ static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, i
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = (unsigned)rp.C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    CU(cudaLaunchKernelEx(&cfg, k_resident<real>, a));
+    P->prof.on = P->prof.stride > 0;
+    {
+        ProfSpan span(P, 0, st);
+        CU(cudaLaunchKernelEx(&cfg, k_resident<real>, a));
+    }
+    P->prof.on = false;
     k_res_out<real><<<tg, 256, 0, st>>>(XT, w.best_bits, w.best_sat[0], w.best_step[0], B, P->n, ntile, X, best_assign,
                                         best_sat, best_step);
     P->last_launches += 3;
@@ -407,6 +453,7 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     P->last_launches++;
     const int gx = var_grid_x(P->n);
     for (int t = 0; t < steps; ++t) {
+        P->prof.on = P->prof.stride > 0 && t % P->prof.stride == 0;
         const real* Xin = XT[t & 1];
         int32_t* sat_cur = w.sat_hist + (size_t)t * Bp;
         if ((s = launch_push<real>(P, Xin, Bp, scratch, sat_cur, nullptr, nullptr, nullptr, st)) != AFS_OK) return s;
@@ -419,10 +466,14 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
         a.best_sat_in = w.best_sat[t & 1]; a.best_sat_out = w.best_sat[(t + 1) & 1];
         a.best_step_in = w.best_step[t & 1]; a.best_step_out = w.best_step[(t + 1) & 1];
         a.S_prev = w.S[(t + 1) & 1]; a.S_cur = w.S[t & 1]; a.best_bits = w.best_bits;
-        k_var<real, false><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
+        {
+            ProfSpan span(P, 1, st);
+            k_var<real, false><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
+        }
         P->last_launches++;
         if ((s = launch_sat_pull(P, w.S[t & 1], Bp, sat_cur, st)) != AFS_OK) return s;
     }
+    P->prof.on = false;
     // the last iterate: count only, then fold and write out
     const real* Xfin = XT[steps & 1];
     int32_t* sat_fin = w.sat_hist + (size_t)steps * Bp;

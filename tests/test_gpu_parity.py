@@ -339,6 +339,32 @@ def test_resident_kernel_refused_when_it_does_not_fit(afs):
     P.close()
 
 
+def test_profile_read_times_every_kernel_class_of_a_run(afs):
+    inst = case_long(8)
+    P = afs.Problem.from_instance(inst)
+    P.set_option(1, 2)
+    X = dev(inst.X0)
+    ref_out = P.pgd_run(X, 6, LR, mask=dev(inst.mask))
+    prof = P.profile_read()
+    assert prof["var"][1] == 3 and prof["var"][0] > 0          # iterations 0, 2, 4
+    assert any(k.startswith("long") for k in prof) and "resident" not in prof
+    assert P.profile_read() == {}                              # spans are consumed
+    P.set_option(1, 0)
+    X2 = dev(inst.X0)
+    out = P.pgd_run(X2, 6, LR, mask=dev(inst.mask))
+    assert P.profile_read() == {}
+    assert np.array_equal(X.cpu().numpy(), X2.cpu().numpy())    # timing does not change results
+    assert np.array_equal(ref_out["best_sat"].cpu().numpy(), out["best_sat"].cpu().numpy())
+    P.close()
+    inst = case_cnf(40)
+    P = afs.Problem.from_instance(inst)
+    P.set_option(1, 1)
+    P.pgd_run(dev(inst.X0), 5, LR)
+    prof = P.profile_read()
+    assert list(prof) == ["resident"] and prof["resident"][1] == 1
+    P.close()
+
+
 def test_host_entry_point_equals_device_entry_point(afs):
     import torch
     inst = case_long(10)
