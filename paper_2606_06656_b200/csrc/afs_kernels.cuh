@@ -544,12 +544,16 @@ constexpr int PULL_SBUF = 48;   // uint2 slots per warp: 32 staged entries + sla
 template <typename real>
 struct ColGlobal {
     const char* __restrict__ base;
-    __device__ __forceinline__ real at(uint32_t off) const { return *reinterpret_cast<const real*>(base + off); }
+    // c = sub-tile of 32 restarts handled by the same lane (RPL > 1): 32 elements further along the row
+    __device__ __forceinline__ real at(uint32_t off, int c = 0) const
+    {
+        return *reinterpret_cast<const real*>(base + off + c * 32 * (int)sizeof(real));
+    }
 };
 template <typename real>
 struct ColShared {
     uint32_t base;
-    __device__ __forceinline__ real at(uint32_t off) const
+    __device__ __forceinline__ real at(uint32_t off, int = 0) const
     {
         real v;
         if constexpr (sizeof(real) == 4) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(base + off));
@@ -558,13 +562,18 @@ struct ColShared {
     }
 };
 
-template <typename real, int KIND, int NOTHER, typename COL>
-__device__ __forceinline__ real pull_run(const uint32_t* __restrict__ words, int beg, int count,
-                                         const COL& xcol, uint32_t rowbytes, int lane, uint2* sbuf)
+// RPL = restart sub-tiles per lane: the lane works on restarts lane, lane + 32, ... of a tile of 32 * RPL restarts,
+// so every staged entry, every offset and every branch is paid once for RPL gathers.  g[c] += the run's contribution.
+template <typename real, int KIND, int NOTHER, int RPL, typename COL>
+__device__ __forceinline__ void pull_run(const uint32_t* __restrict__ words, int beg, int count, const COL& xcol,
+                                         uint32_t rowbytes, int lane, uint2* sbuf, real (&gout)[RPL])
 {
     constexpr int OPC = 32 / NOTHER;              // occurrences per staged chunk of <= 32 entries
-    constexpr int U = NOTHER <= 2 ? 4 : 2;        // occurrences gathered together
-    real g = real(0);
+    constexpr int U0 = NOTHER <= 2 ? 4 : 2;       // occurrences gathered together
+    constexpr int U = U0 / RPL >= 1 ? U0 / RPL : 1;
+    real g[RPL];
+#pragma unroll
+    for (int c = 0; c < RPL; ++c) g[c] = real(0);
     for (int o0 = 0; o0 < count; o0 += OPC) {
         const int nocc = min(OPC, count - o0);
         const uint32_t wm = words[beg + o0 * NOTHER + lane];   // reading past the run is harmless (valid entries / padding)
@@ -575,7 +584,7 @@ __device__ __forceinline__ real pull_run(const uint32_t* __restrict__ words, int
         __syncwarp();
         for (int o = 0; o < nocc; o += U) {
             uint2 e[U][NOTHER];
-            real x[U][NOTHER];
+            real x[U][NOTHER][RPL];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const uint2* rec = sbuf + (o + u) * NOTHER;
@@ -594,50 +603,59 @@ __device__ __forceinline__ real pull_run(const uint32_t* __restrict__ words, int
 #pragma unroll
             for (int u = 0; u < U; ++u)
 #pragma unroll
-                for (int i = 0; i < NOTHER; ++i)
-                    x[u][i] = xcol.at(i == 0 ? (e[u][0].x & ~1u) : e[u][i].x);
+                for (int i = 0; i < NOTHER; ++i) {
+                    const uint32_t off = i == 0 ? (e[u][0].x & ~1u) : e[u][i].x;
+#pragma unroll
+                    for (int c = 0; c < RPL; ++c) x[u][i][c] = xcol.at(off, c);
+                }
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                real d;
-                if (KIND == (int)PH_KIND_XOR) {
-                    real prod = flip(x[u][0], e[u][0].y);
+                const bool live = o + u < nocc;
 #pragma unroll
-                    for (int i = 1; i < NOTHER; ++i) prod *= flip(x[u][i], e[u][i].y);
-                    d = prod;
-                } else {
-                    real pu = pull_u(x[u][0], e[u][0].y);
+                for (int c = 0; c < RPL; ++c) {
+                    real d;
+                    if (KIND == (int)PH_KIND_XOR) {
+                        real prod = flip(x[u][0][c], e[u][0].y);
 #pragma unroll
-                    for (int i = 1; i < NOTHER; ++i) pu *= pull_u(x[u][i], e[u][i].y);
-                    d = pu;
-                    if (KIND == (int)PH_KIND_NAE) {
-                        real pp = pull_p(x[u][0], e[u][0].y);
+                        for (int i = 1; i < NOTHER; ++i) prod *= flip(x[u][i][c], e[u][i].y);
+                        d = prod;
+                    } else {
+                        real pu = pull_u(x[u][0][c], e[u][0].y);
 #pragma unroll
-                        for (int i = 1; i < NOTHER; ++i) pp *= pull_p(x[u][i], e[u][i].y);
-                        d = pu - pp;
+                        for (int i = 1; i < NOTHER; ++i) pu *= pull_u(x[u][i][c], e[u][i].y);
+                        d = pu;
+                        if (KIND == (int)PH_KIND_NAE) {
+                            real pp = pull_p(x[u][0][c], e[u][0].y);
+#pragma unroll
+                            for (int i = 1; i < NOTHER; ++i) pp *= pull_p(x[u][i][c], e[u][i].y);
+                            d = pu - pp;
+                        }
                     }
+                    d = flip(d, e[u][0].x << 31);
+                    if (live) g[c] += d;
                 }
-                d = flip(d, e[u][0].x << 31);
-                if (o + u < nocc) g += d;
             }
         }
         __syncwarp();
     }
-    return g;
+#pragma unroll
+    for (int c = 0; c < RPL; ++c) gout[c] += g[c];
 }
 
-// all runs of one variable
-template <typename real, typename COL>
-__device__ __forceinline__ real pull_variable(const uint32_t* __restrict__ runs, int rbeg, int rend,
-                                              const uint32_t* __restrict__ words, int wbeg,
-                                              const COL& xcol, uint32_t rowbytes, int lane, uint2* sbuf)
+// all runs of one variable: g[c] += sum over the runs (each run summed on its own first, in stream order)
+template <typename real, int RPL, typename COL>
+__device__ __forceinline__ void pull_variable(const uint32_t* __restrict__ runs, int rbeg, int rend,
+                                              const uint32_t* __restrict__ words, int wbeg, const COL& xcol,
+                                              uint32_t rowbytes, int lane, uint2* sbuf, real (&g)[RPL])
 {
-    real g = real(0);
+    real acc[RPL];
+#pragma unroll
+    for (int c = 0; c < RPL; ++c) acc[c] = real(0);
     int pos = wbeg;
     for (int r = rbeg; r < rend; ++r) {
         const uint32_t d = runs[r];
         const int count = (int)(d & 0x07ffffffu), nother = (int)((d >> 27) & 7u), kind = (int)(d >> 30);
-        real gr;
-#define AFS_RUN(K, N) gr = pull_run<real, K, N, COL>(words, pos, count, xcol, rowbytes, lane, sbuf)
+#define AFS_RUN(K, N) pull_run<real, K, N, RPL, COL>(words, pos, count, xcol, rowbytes, lane, sbuf, acc)
         if (kind == (int)PH_KIND_OR) {
             switch (nother) { case 1: AFS_RUN(0, 1); break; case 2: AFS_RUN(0, 2); break; case 3: AFS_RUN(0, 3); break; default: AFS_RUN(0, 4); break; }
         } else if (kind == (int)PH_KIND_XOR) {
@@ -646,19 +664,19 @@ __device__ __forceinline__ real pull_variable(const uint32_t* __restrict__ runs,
             switch (nother) { case 1: AFS_RUN(2, 1); break; case 2: AFS_RUN(2, 2); break; case 3: AFS_RUN(2, 3); break; default: AFS_RUN(2, 4); break; }
         }
 #undef AFS_RUN
-        g += gr;
         pos += count * nother;
     }
-    return g;
+#pragma unroll
+    for (int c = 0; c < RPL; ++c) g[c] += acc[c];
 }
 
-template <typename real, bool EVAL>
-__global__ void __launch_bounds__(VAR_WARPS * 32, 4) k_var(const VarArgs<real> a)
+template <typename real, bool EVAL, int RPL>
+__global__ void __launch_bounds__(VAR_WARPS * 32, RPL == 1 ? 4 : 2) k_var(const VarArgs<real> a)
 {
     __shared__ __align__(16) uint2 s_stage[VAR_WARPS][PULL_SBUF];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int tile = blockIdx.y, ntile = a.Bp >> 5;
-    const int b = tile * 32 + lane;
+    const int tile0 = blockIdx.y * RPL, ntile = a.Bp >> 5;     // this lane's restarts: (tile0 + c) * 32 + lane
+    const int b = tile0 * 32 + lane;
     const int Bp = a.Bp;
     const real one = real(1);
     const real* __restrict__ xcol = a.Xin + b;
@@ -669,58 +687,87 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 4) k_var(const VarArgs<real> a
     const int vbeg = (blockIdx.x * VAR_WARPS + warp) * VAR_VPW;
     const int vend = min(vbeg + VAR_VPW, a.n);
     // ---- S10: did the previous iterate improve on the best so far?
-    bool imp = false;
-    unsigned impmask = 0;
-    int sprev = 0;
-    if (!EVAL && a.t > 0) {
-        sprev = a.sat_prev[b];
-        imp = sprev > a.best_sat_in[b];
-        impmask = __ballot_sync(FULL, imp);
+    bool imp[RPL];
+    unsigned impmask[RPL];
+    int sprev[RPL];
+    bool anyimp = false;
+#pragma unroll
+    for (int c = 0; c < RPL; ++c) {
+        imp[c] = false; impmask[c] = 0u; sprev[c] = 0;
+        if (!EVAL && a.t > 0) {
+            sprev[c] = a.sat_prev[b + 32 * c];
+            imp[c] = sprev[c] > a.best_sat_in[b + 32 * c];
+            impmask[c] = __ballot_sync(FULL, imp[c]);
+            anyimp |= impmask[c] != 0u;
+        }
     }
     for (int v = vbeg; v < vend; ++v) {
         if (!EVAL) {
-            if (impmask && lane == 0) {
-                size_t wi = (size_t)v * ntile + tile;
-                a.best_bits[wi] = (a.best_bits[wi] & ~impmask) | (a.S_prev[wi] & impmask);
+            if (anyimp && lane == 0) {
+#pragma unroll
+                for (int c = 0; c < RPL; ++c)
+                    if (impmask[c]) {
+                        size_t wi = (size_t)v * ntile + tile0 + c;
+                        a.best_bits[wi] = (a.best_bits[wi] & ~impmask[c]) | (a.S_prev[wi] & impmask[c]);
+                    }
             }
             if (v == 0) {
-                int bs = a.best_sat_in[b], stp = a.best_step_in[b];
-                a.best_sat_out[b] = imp ? sprev : bs;
-                a.best_step_out[b] = imp ? a.t - 1 : stp;
+#pragma unroll
+                for (int c = 0; c < RPL; ++c) {
+                    int bs = a.best_sat_in[b + 32 * c], stp = a.best_step_in[b + 32 * c];
+                    a.best_sat_out[b + 32 * c] = imp[c] ? sprev[c] : bs;
+                    a.best_step_out[b + 32 * c] = imp[c] ? a.t - 1 : stp;
+                }
             }
         }
-        const real x = xcol[(size_t)v * Bp];
+        real x[RPL], g[RPL];
         int mk = 0;
+#pragma unroll
+        for (int c = 0; c < RPL; ++c) x[c] = xcol[(size_t)v * Bp + 32 * c];
         if (!EVAL) {
-            unsigned sb = __ballot_sync(FULL, x < real(0));
-            if (lane == 0) a.S_cur[(size_t)v * ntile + tile] = sb;
+#pragma unroll
+            for (int c = 0; c < RPL; ++c) {
+                unsigned sb = __ballot_sync(FULL, x[c] < real(0));
+                if (lane == 0) a.S_cur[(size_t)v * ntile + tile0 + c] = sb;
+            }
             mk = a.mask ? a.mask[v] : 0;
         }
-        real g = real(0);
+#pragma unroll
+        for (int c = 0; c < RPL; ++c) g[c] = real(0);
         if (mk == 0) {   // a fixed variable never moves: its gradient is not needed
-            g = (real)a.gconst[v];
-            g += pull_variable<real>(a.runs, a.run_ptr[v], a.run_ptr[v + 1], a.pull_words, a.pull_ptr[v], xg,
-                                     (uint32_t)Bp * (uint32_t)sizeof(real), lane, sbuf);
+            const real gc = (real)a.gconst[v];
+#pragma unroll
+            for (int c = 0; c < RPL; ++c) g[c] = gc;
+            pull_variable<real, RPL>(a.runs, a.run_ptr[v], a.run_ptr[v + 1], a.pull_words, a.pull_ptr[v], xg,
+                                     (uint32_t)Bp * (uint32_t)sizeof(real), lane, sbuf, g);
             // ---- S6: materialised gradients of v, fixed (transposed-CSR) order
             const int s1 = a.slot_ptr[v + 1];
             int s = a.slot_ptr[v];
             const real* __restrict__ sc = a.scratch + b;
             for (; s + 4 <= s1; s += 4) {
-                real g0 = sc[(size_t)s * Bp], g1 = sc[(size_t)(s + 1) * Bp];
-                real g2 = sc[(size_t)(s + 2) * Bp], g3 = sc[(size_t)(s + 3) * Bp];
-                g += g0; g += g1; g += g2; g += g3;
+#pragma unroll
+                for (int c = 0; c < RPL; ++c) {
+                    real g0 = sc[(size_t)s * Bp + 32 * c], g1 = sc[(size_t)(s + 1) * Bp + 32 * c];
+                    real g2 = sc[(size_t)(s + 2) * Bp + 32 * c], g3 = sc[(size_t)(s + 3) * Bp + 32 * c];
+                    g[c] += g0; g[c] += g1; g[c] += g2; g[c] += g3;
+                }
             }
-            for (; s < s1; ++s) g += sc[(size_t)s * Bp];
+            for (; s < s1; ++s)
+#pragma unroll
+                for (int c = 0; c < RPL; ++c) g[c] += sc[(size_t)s * Bp + 32 * c];
         }
-        if (EVAL) {
-            a.GT[(size_t)v * Bp + b] = g;
-        } else {
-            // ---- S7-S8
-            real xn = x - a.lr * g;
-            xn = xn > one ? one : xn;
-            xn = xn < -one ? -one : xn;
-            if (mk != 0) xn = x;
-            a.Xout[(size_t)v * Bp + b] = xn;
+#pragma unroll
+        for (int c = 0; c < RPL; ++c) {
+            if (EVAL) {
+                a.GT[(size_t)v * Bp + b + 32 * c] = g[c];
+            } else {
+                // ---- S7-S8
+                real xn = x[c] - a.lr * g[c];
+                xn = xn > one ? one : xn;
+                xn = xn < -one ? -one : xn;
+                if (mk != 0) xn = x[c];
+                a.Xout[(size_t)v * Bp + b + 32 * c] = xn;
+            }
         }
     }
 }

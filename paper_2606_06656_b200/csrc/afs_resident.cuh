@@ -196,13 +196,13 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
                     for (int i = i0; i < min(i0 + RES_VCH, ve - vb); ++i) {
                         const int v = vb + i;
                         const int mk = a.mask ? a.mask[v] : 0;
-                        real g = real(0);
+                        real g[1] = {real(0)};
                         if (mk == 0) {
-                            g = (real)a.gconst[v];
-                            g += pull_variable<real>(a.runs, a.run_ptr[v], a.run_ptr[v + 1], a.pull_words, a.pull_ptr[v],
-                                                     xcol, 32u * (uint32_t)sizeof(real), lane, sbuf);
+                            g[0] = (real)a.gconst[v];
+                            pull_variable<real, 1>(a.runs, a.run_ptr[v], a.run_ptr[v + 1], a.pull_words, a.pull_ptr[v],
+                                                   xcol, 32u * (uint32_t)sizeof(real), lane, sbuf, g);
                         }
-                        Gt[(size_t)v * 32] = g;
+                        Gt[(size_t)v * 32] = g[0];
                     }
                 }
             }

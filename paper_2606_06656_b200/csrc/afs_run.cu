@@ -130,6 +130,15 @@ static afs_status ensure_eval_buffers(afs_problem* P, int Bp, size_t elem)
     return AFS_OK;
 }
 
+// variable pass: as many 32-restart sub-tiles per lane as the batch allows (4, 2 or 1)
+template <typename real, bool EVAL>
+static void launch_var(const VarArgs<real>& a, int gx, int tiles, cudaStream_t st)
+{
+    if (sizeof(real) == 4 && tiles % 4 == 0) k_var<real, EVAL, 4><<<dim3(gx, tiles / 4), VAR_WARPS * 32, 0, st>>>(a);
+    else if (tiles % 2 == 0) k_var<real, EVAL, 2><<<dim3(gx, tiles / 2), VAR_WARPS * 32, 0, st>>>(a);
+    else k_var<real, EVAL, 1><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
+}
+
 // ----------------------------------------------------------------------------------------------------------------
 // push phase: gradients of the medium and long constraints of iterate XT into scratch (+ counts, + FE)
 // ----------------------------------------------------------------------------------------------------------------
@@ -301,7 +310,7 @@ static afs_status eval_grad_impl(afs_problem* P, const real* X, int32_t B, real*
     a.GT = GT;
     const int gx = var_grid_x(P->n);
     if (G) {
-        k_var<real, true><<<dim3(gx, Bp / 32), VAR_WARPS * 32, 0, st>>>(a);
+        launch_var<real, true>(a, gx, Bp / 32, st);
         P->last_launches++;
     }
     if (F) {
@@ -468,7 +477,7 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
         a.S_prev = w.S[(t + 1) & 1]; a.S_cur = w.S[t & 1]; a.best_bits = w.best_bits;
         {
             ProfSpan span(P, 1, st);
-            k_var<real, false><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
+            launch_var<real, false>(a, gx, tiles, st);
         }
         P->last_launches++;
         if ((s = launch_sat_pull(P, w.S[t & 1], Bp, sat_cur, st)) != AFS_OK) return s;
