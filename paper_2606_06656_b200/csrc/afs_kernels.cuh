@@ -569,7 +569,9 @@ __device__ __forceinline__ void pull_run(const uint32_t* __restrict__ words, int
                                          uint32_t rowbytes, int lane, uint2* sbuf, real (&gout)[RPL])
 {
     constexpr int OPC = 32 / NOTHER;              // occurrences per staged chunk of <= 32 entries
-    constexpr int U0 = NOTHER <= 2 ? 4 : 2;       // occurrences gathered together
+    // occurrences gathered together: 8 (NOTHER <= 2) or up to 16 loads in flight per lane.  More does not pay: on the
+    // large instances the pass moves ~7 TB/s out of L2 as it is, and the tail of a wider batch gathers rows it discards
+    constexpr int U0 = NOTHER <= 2 ? 4 : 2;
     constexpr int U = U0 / RPL >= 1 ? U0 / RPL : 1;
     real g[RPL];
 #pragma unroll
@@ -774,65 +776,93 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, RPL == 1 ? 4 : 2) k_var(const 
 
 // ------------------------------------------------------------------------------------------------------------------
 // S9 for the PULL class, bit-parallel over restarts: the sign words S[v][tile] (bit r = "x_v < 0" for restart
-// tile*32 + r) written by the variable pass give the truth of 32 restarts of a clause with a few logic ops; the
-// per-restart totals are kept as vertical (bit-sliced) counters and unpacked once per thread.  Integers only.
-// thread = (chunk of clauses, restart tile).
+// tile*32 + r) written by the variable pass give the truth of 32 restarts of a clause with a few logic ops.
+// thread = (clause, group of TPT restart tiles), lane <-> clause: the literal words are read once, the TPT sign words
+// of a literal are one 4*TPT-byte load, and every load of a clause is independent of the others.  The per-restart
+// totals come from a butterfly transposition (bit_column_sums: lane r collects restart r).  Integers only.
 // ------------------------------------------------------------------------------------------------------------------
-constexpr int SATP_TG = 8;                            // restart tiles per CTA
-constexpr int SATP_CPB = 256 / SATP_TG;               // clause chunks per CTA
+// Column sums of a 32 x 32 bit matrix held one row per lane: returns, in lane r, the number of lanes whose word has
+// bit r set.  Five butterfly steps; after step s a lane keeps the 32 >> s columns whose low s bits match its own lane
+// index, as packed (s+1)-bit counters.
+__device__ __forceinline__ int bit_column_sums(uint32_t w, int lane)
+{
+    uint32_t o;
+    o = __shfl_xor_sync(FULL, w, 1);
+    w = (lane & 1) ? ((w >> 1) & 0x55555555u) + ((o >> 1) & 0x55555555u) : (w & 0x55555555u) + (o & 0x55555555u);
+    o = __shfl_xor_sync(FULL, w, 2);
+    w = (lane & 2) ? ((w >> 2) & 0x33333333u) + ((o >> 2) & 0x33333333u) : (w & 0x33333333u) + (o & 0x33333333u);
+    o = __shfl_xor_sync(FULL, w, 4);
+    w = (lane & 4) ? ((w >> 4) & 0x0f0f0f0fu) + ((o >> 4) & 0x0f0f0f0fu) : (w & 0x0f0f0f0fu) + (o & 0x0f0f0f0fu);
+    o = __shfl_xor_sync(FULL, w, 8);
+    w = (lane & 8) ? ((w >> 8) & 0x00ff00ffu) + ((o >> 8) & 0x00ff00ffu) : (w & 0x00ff00ffu) + (o & 0x00ff00ffu);
+    o = __shfl_xor_sync(FULL, w, 16);
+    w = (lane & 16) ? (w >> 16) + (o >> 16) : (w & 0xffffu) + (o & 0xffffu);
+    return (int)w;
+}
 
-template <int PLANES>
+template <int TPT>
+struct SWords { uint32_t w[TPT]; };
+template <int TPT>
+__device__ __forceinline__ SWords<TPT> ld_swords(const uint32_t* __restrict__ p)
+{
+    SWords<TPT> r;
+    if constexpr (TPT == 4) { uint4 t = *reinterpret_cast<const uint4*>(p); r.w[0] = t.x; r.w[1] = t.y; r.w[2] = t.z; r.w[3] = t.w; }
+    else if constexpr (TPT == 2) { uint2 t = *reinterpret_cast<const uint2*>(p); r.w[0] = t.x; r.w[1] = t.y; }
+    else r.w[0] = *p;
+    return r;
+}
+
+template <int TPT>
 __global__ void __launch_bounds__(256) k_sat_pull(const CountCon* __restrict__ cons, const uint32_t* __restrict__ lits,
-                                                  int m, int chunk, const uint32_t* __restrict__ S, int ntile,
+                                                  int m, const uint32_t* __restrict__ S, int ntile,
                                                   int32_t* __restrict__ sat)
 {
-    __shared__ int s_cnt[SATP_TG][32];
-    const int tl = threadIdx.x % SATP_TG;
-    const int tile = blockIdx.y * SATP_TG + tl;
-    const int ch = blockIdx.x * SATP_CPB + threadIdx.x / SATP_TG;
-    s_cnt[threadIdx.x >> 5][threadIdx.x & 31] = 0;
+    __shared__ int s_cnt[TPT][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int tile0 = blockIdx.y * TPT;
+    if (threadIdx.x < TPT * 32) s_cnt[threadIdx.x >> 5][threadIdx.x & 31] = 0;
     __syncthreads();
-    if (tile < ntile) {
-        uint32_t plane[PLANES];
+    int cnt[TPT];
 #pragma unroll
-        for (int p = 0; p < PLANES; ++p) plane[p] = 0u;
-        const int c1 = min(m, (ch + 1) * chunk);
-        bool any = false;
-        for (int c = ch * chunk; c < c1; ++c) {
+    for (int k = 0; k < TPT; ++k) cnt[k] = 0;
+    const int stride = gridDim.x * 256;
+    for (int c0 = (blockIdx.x * 8 + warp) * 32; c0 < m; c0 += stride) {
+        const int c = c0 + lane;
+        uint32_t T[TPT];
+#pragma unroll
+        for (int k = 0; k < TPT; ++k) T[k] = 0u;
+        if (c < m) {
             const CountCon cc = cons[c];
-            uint32_t w = lits[cc.off];
-            uint32_t t0 = S[(size_t)(w & LIT_VAR) * ntile + tile] ^ ((w >> 31) ? 0xffffffffu : 0u);
-            uint32_t vor = t0, vand = t0, vxor = t0;
-            for (int j = 1; j < cc.L; ++j) {
-                w = lits[cc.off + j];
-                uint32_t tj = S[(size_t)(w & LIT_VAR) * ntile + tile] ^ ((w >> 31) ? 0xffffffffu : 0u);
-                vor |= tj; vand &= tj; vxor ^= tj;
-            }
-            uint32_t carry = cc.type == AFS_OR ? vor : cc.type == AFS_XOR ? ~(vxor ^ ((cc.k & 1) ? 0xffffffffu : 0u))
-                                                                          : (vor & ~vand);
+            const uint32_t* lw = lits + cc.off;
+            uint32_t vor[TPT], vand[TPT], vxor[TPT];
 #pragma unroll
-            for (int p = 0; p < PLANES; ++p) {
-                uint32_t t = plane[p] & carry;
-                plane[p] ^= carry;
-                carry = t;
-            }
-            any = true;
-        }
-        if (any) {
-            for (int r = 0; r < 32; ++r) {
-                int cnt = 0;
+            for (int k = 0; k < TPT; ++k) { vor[k] = 0u; vand[k] = 0xffffffffu; vxor[k] = 0u; }
+            for (int j = 0; j < cc.L; ++j) {
+                const uint32_t w = lw[j];
+                const uint32_t flipm = (w >> 31) ? 0xffffffffu : 0u;
+                const SWords<TPT> sw = ld_swords<TPT>(S + (size_t)(w & LIT_VAR) * ntile + tile0);
 #pragma unroll
-                for (int p = 0; p < PLANES; ++p) cnt |= (int)((plane[p] >> r) & 1u) << p;
-                if (cnt) atomicAdd(&s_cnt[tl][r], cnt);
+                for (int k = 0; k < TPT; ++k) {
+                    const uint32_t tj = sw.w[k] ^ flipm;
+                    vor[k] |= tj; vand[k] &= tj; vxor[k] ^= tj;
+                }
             }
+            const uint32_t par = (cc.k & 1) ? 0xffffffffu : 0u;
+#pragma unroll
+            for (int k = 0; k < TPT; ++k)
+                T[k] = cc.type == AFS_OR ? vor[k] : cc.type == AFS_XOR ? ~(vxor[k] ^ par) : (vor[k] & ~vand[k]);
         }
+#pragma unroll
+        for (int k = 0; k < TPT; ++k) cnt[k] += bit_column_sums(T[k], lane);
     }
+#pragma unroll
+    for (int k = 0; k < TPT; ++k)
+        if (cnt[k]) atomicAdd(&s_cnt[k][lane], cnt[k]);
     __syncthreads();
-    {
-        const int t2 = threadIdx.x >> 5, r = threadIdx.x & 31;
-        const int tile2 = blockIdx.y * SATP_TG + t2;
-        int cnt = s_cnt[t2][r];
-        if (tile2 < ntile && cnt) atomicAdd(&sat[tile2 * 32 + r], cnt);
+    if (threadIdx.x < TPT * 32) {
+        const int k = threadIdx.x >> 5, r = threadIdx.x & 31;
+        const int v = s_cnt[k][r];
+        if (v) atomicAdd(&sat[(tile0 + k) * 32 + r], v);
     }
 }
 

@@ -184,13 +184,7 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
                         T = cc.type == AFS_OR ? vor : cc.type == AFS_XOR ? ~(vxor ^ ((cc.k & 1) ? 0xffffffffu : 0u))
                                                                          : (vor & ~vand);
                     }
-                    if (__any_sync(FULL, T != 0u)) {
-#pragma unroll 8
-                        for (int r = 0; r < 32; ++r) {
-                            const unsigned bal = __ballot_sync(FULL, (T >> r) & 1u);
-                            if (lane == r) satcnt += __popc(bal);
-                        }
-                    }
+                    satcnt += bit_column_sums(T, lane);
                 } else {
                     const int i0 = (it - n_push - n_cnt) * RES_VCH;
                     for (int i = i0; i < min(i0 + RES_VCH, ve - vb); ++i) {

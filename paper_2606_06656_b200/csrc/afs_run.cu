@@ -248,21 +248,17 @@ static afs_status launch_sat_pull(afs_problem* P, const uint32_t* S, int Bp, int
 {
     if (P->n_pull == 0) return AFS_OK;
     const int ntile = Bp / 32;
-    const int gy = (ntile + SATP_TG - 1) / SATP_TG;
-    // enough chunks to fill the chip, at most 1023 clauses each
-    long long want = (long long)P->sm_count * 8 * SATP_CPB / gy;
-    if (want < 1) want = 1;
-    int chunk = (int)((P->n_pull + want - 1) / want);
-    if (chunk < 15) chunk = 15;
-    if (chunk > 1023) chunk = 1023;
-    const int nchunks = (int)((P->n_pull + chunk - 1) / chunk);
-    dim3 grid((nchunks + SATP_CPB - 1) / SATP_CPB, gy);
+    const int tpt = ntile % 4 == 0 ? 4 : ntile % 2 == 0 ? 2 : 1;
+    const int gy = ntile / tpt;
     const int m = (int)P->n_pull;
+    int gx = (m + 255) / 256;                               // 8 warps x 32 clauses per CTA and pass
+    const int cap = (P->sm_count * 8 + gy - 1) / gy;        // enough CTAs to fill the chip, grid-stride beyond
+    if (gx > cap) gx = cap < 1 ? 1 : cap;
+    dim3 grid(gx, gy);
     ProfSpan span(P, 2, st);
-    if (chunk <= 15) k_sat_pull<4><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, chunk, S, ntile, sat);
-    else if (chunk <= 63) k_sat_pull<6><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, chunk, S, ntile, sat);
-    else if (chunk <= 255) k_sat_pull<8><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, chunk, S, ntile, sat);
-    else k_sat_pull<10><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, chunk, S, ntile, sat);
+    if (tpt == 4) k_sat_pull<4><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, S, ntile, sat);
+    else if (tpt == 2) k_sat_pull<2><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, S, ntile, sat);
+    else k_sat_pull<1><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, S, ntile, sat);
     P->last_launches++;
     return AFS_OK;
 }
