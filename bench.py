@@ -44,8 +44,8 @@ def kernel_class_of_constraints(inst):
         l = int(L[c])
         if (prod[c] or ty[c] == W.AFS_NAE) and l <= 5:
             out[c] = "var"
-        elif prod[c] or (two[c] and l <= 32):
-            out[c] = "med%d" % (0 if l <= 8 else 1 if l <= 16 else 2 if l <= 32 else 3 if l <= 64 else 4)
+        elif prod[c] or two[c]:
+            out[c] = "med0"
         elif cnt[c] and l <= 64:
             out[c] = "cmed"
         else:
@@ -247,9 +247,9 @@ def run_cuda(args):
 
     cfg = args.config
     inst = W.config(cfg)
+    from paper_2606_06656_b200 import shard
     if world > 1:   # every rank its own start points (weak scaling), same instance
-        rng = np.random.Generator(np.random.PCG64(W.BASE_SEED + 1000 * (rank + 1) + cfg))
-        inst.X0 = rng.uniform(-1, 1, size=inst.X0.shape).astype(np.float32)
+        inst.X0 = shard.rank_start_points(W.BASE_SEED, cfg, rank, inst.X0.shape)
     pgd_steps = inst.steps if args.pgd_steps is None else args.pgd_steps
     lr = float(np.float32(inst.lr))
     P = afs.Problem.from_instance(inst, device=local)
@@ -295,13 +295,9 @@ def run_cuda(args):
     dev_ms = sum(a.elapsed_time(b) for a, b in evs)
     launches = P.info("launches") * args.steps
     resident = P.info("resident")
-    t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        # the one exchange of the sharded job (DESIGN.md multi-GPU): best counts of every rank
-        gathered = [torch.empty_like(out["best_sat"]) for _ in range(world)]
-        dist.all_gather(gathered, out["best_sat"])
-    dev_ms = float(t.item())
+    dev_ms = shard.max_over_ranks(dev_ms, device="cuda")
+    # the one exchange of the sharded job: best counts of every rank
+    _, job_best = shard.gather_best(out["best_sat"])
     units = float(inst.B) * pgd_steps * args.steps * world
     value = units / (dev_ms * 1e-3)
 
@@ -323,10 +319,7 @@ def run_cuda(args):
         dt = time.perf_counter() - t0
         if i > 0:
             e2e_t += dt
-    t2 = torch.tensor([e2e_t], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t2, op=dist.ReduceOp.MAX)
-    e2e_value = float(inst.B) * pgd_steps * n_e2e * world / float(t2.item())
+    e2e_value = float(inst.B) * pgd_steps * n_e2e * world / shard.max_over_ranks(e2e_t, device="cuda")
     h2d = inst.B * inst.n * 4 + (inst.n if inst.mask is not None else 0)
     d2h = inst.B * inst.n * 4 + inst.B * inst.n + 8 * inst.B
 
@@ -396,7 +389,7 @@ def run_cuda(args):
                             path="resident" if resident else "streaming", parallelism="restarts x%d" % world),
                 literal_evals_per_sec=value * inst.nnz,
                 wall_ms_per_step=1e3 * wall / args.steps,
-                gpu_launches=int(launches),
+                gpu_launches=int(launches), best_sat_max=int(job_best[2]),
                 e2e=dict(value=e2e_value, unit="restart-steps/s", h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h)),
                 roofline=roof, cpu_baseline=cpu, clocks=clocks)
     print(json.dumps(line))

@@ -77,8 +77,8 @@ typedef enum {
  *   k        host    int32[n_cons]; EK: exactly k; CARD: at least k; XOR: required parity (1 = odd); otherwise ignored
  *   device           CUDA device ordinal
  *   out              receives the handle (NULL on error)
- * Limits of this build: count-type constraints (AMO/EO/EK/NAE/CARD and OR longer than 64) up to L = 1151
- * literals, otherwise AFS_ERR_UNSUPPORTED.
+ * Limits of this build: EK / CARD up to L = 1151 literals, otherwise AFS_ERR_UNSUPPORTED; the other types have no
+ * length limit.
  */
 AFS_API afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const int64_t* row_ptr, const int32_t* lits,
                               const int32_t* types, const int32_t* k, int32_t device, afs_problem** out);
@@ -165,7 +165,7 @@ AFS_API afs_status afs_set_option(afs_problem* p, int32_t what, int64_t value);
  * recent afs_pgd_run* call per kernel class into ms[0..n) / launches[0..n) (host arrays, n <= AFS_KERNEL_CLASSES;
  * the caller zeroes them), and forgets the spans.  Classes:
  *   0 tile-resident PGD kernel      1 variable pass (pull gradients + S6 + S7 + S8)    2 pull-clause counts (S9)
- *   3 EK/CARD with L <= 64          4..8 medium buckets (padded 8, 16, 32, 64, two-pass product)
+ *   3 EK/CARD with L <= 64          4 medium class (prefix x suffix bodies; 5..8 unused)
  *   9..17 long-constraint kernel, 1..9 rows of 128 pmf cells                              18 boundary (layout changes,
  *   final count, fills)
  */

@@ -17,16 +17,13 @@ constexpr uint32_t LIT_VAR = 0x7fffffffu;
 // ---- execution classes (decided at create; S0 of the path) ---------------------------------------------------
 //  PULL : OR / XOR / NAE with L <= PULL_MAX_LEN.  No gradient is materialised: the variable pass recomputes each
 //         occurrence's leave-one-out product from the other literals (deterministic by construction).
-//  MED  : thread per (constraint, restart), prefix/suffix in registers: OR/XOR L<=64, NAE/EO/AMO L<=32;
-//         OR/XOR longer than 64 run a two-pass running-product kernel (scratch row = prefix storage).
+//  MED  : thread per (constraint, restart): OR / XOR beyond the pull lengths and NAE / EO / AMO of any length;
+//         prefix states stored per literal in private rows (aux), suffix carried backwards in registers.
 //  CMED : EK / CARD with L <= 64: thread per (constraint, restart), the pmf in the warp's shared-memory buffer.
 //  LONG : warp per (constraint, restart), count-basis DP + stable-direction leave-one-out recurrences:
-//         EK/CARD longer than 64, and NAE/EO/AMO too long for MED.
+//         EK/CARD longer than 64.
 constexpr int PULL_MAX_LEN = 5;
-constexpr int MED_MAX_PROD = 64;
-constexpr int MED_MAX_TWO = 32;
 constexpr int LONG_MAX_LEN = 1151;   // 9 rows x 128 cells hold q_0..q_L
-constexpr int MED_BUCKETS = 5;       // padded lengths 8, 16, 32, 64; bucket 4 = OR/XOR longer than 64 (two-pass kernel)
 constexpr int LONG_BUCKETS = 9;      // NR = 1..9 rows of 128 pmf cells
 
 // pull streams (S0 output for the PULL class).  Per variable its occurrences are grouped into RUNS of equal
@@ -68,7 +65,7 @@ struct CountCon {      // generic forward CSR entry for the count-only kernel: 1
 };
 
 // ---- tile-resident kernel (afs_resident.cuh): static split of one tile's work over the C CTAs of a cluster ----------
-struct ResItem {       // one MED-class constraint: code 0..4 = MED bucket; idx into d_med
+struct ResItem {       // one MED-class constraint: idx into d_med (code unused)
     uint32_t code;
     uint32_t idx;
 };
@@ -81,6 +78,8 @@ struct ResPlan {
     int32_t* d_cm_begin = nullptr;     // [C+1] ranges of d_cm_items
     int32_t* d_cm_items = nullptr;     // CMED constraints (indices into d_cm), each rank's heaviest first
     int32_t* d_pc_begin = nullptr;     // [C+1] ranges of the pull clauses whose counts the rank takes
+    // capacities (max over ranks) of the index streams a CTA may stage in shared memory
+    int cap_words = 0, cap_runs = 0, cap_own = 0, cap_plits = 0, cap_cm = 0, cap_push = 0;
 };
 
 // ---- per-launch device timing (afs_set_option 1, afs_profile_read): CUDA events on the caller's stream around the
@@ -104,6 +103,7 @@ struct Workspace {
     int64_t sat_rows = 0;
     void* XT[2] = {nullptr, nullptr};      // real [n][Bp]
     void* scratch = nullptr;               // real [nslots][Bp]
+    void* aux[2] = {nullptr, nullptr};     // real [med_nnz][Bp] prefix states of the MED class
     int32_t* sat_hist = nullptr;           // [sat_rows][Bp]
     int32_t* best_sat[2] = {nullptr, nullptr};
     int32_t* best_step[2] = {nullptr, nullptr};
@@ -147,7 +147,8 @@ struct afs_problem {
     afs::MedCon* d_med = nullptr;       // sorted by bucket
     uint32_t* d_med_lits = nullptr;
     int32_t* d_med_slots = nullptr;
-    int32_t med_begin[afs::MED_BUCKETS + 1] = {0};
+    int64_t med_nnz = 0;                // literals of the MED class = rows of the aux buffers
+    bool med_two = false;               // some MED constraint carries a two-component prefix state (NAE / EO / AMO)
 
     afs::LongCon* d_long = nullptr;     // sorted by bucket (NR), longest first inside a bucket
     uint32_t* d_long_lits = nullptr;

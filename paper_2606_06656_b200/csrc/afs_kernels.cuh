@@ -247,120 +247,123 @@ __device__ __forceinline__ void cm_body(const LongCon& lc, const uint32_t* __res
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// MED class: thread = (constraint, restart); y gathered once into registers; division-free leave-one-out by
-// prefix / suffix products (OR, XOR, NAE) or a two-state prefix / suffix pmf (EO, AMO).  S1-S3, S5, S9.
-//   OR   FE = 2 prod u - 1                 dFE/dy_j = prod_{i!=j} u_i                      (u = (1+y)/2)
+// MED class: OR / XOR beyond the pull lengths and NAE / EO / AMO of any length; thread = (constraint, restart).
+// Division-free leave-one-out by prefix x suffix (BASELINE.json subsystem (2)): a forward pass over the literals
+// writes the prefix state in front of literal j to a private row (aux0 / aux1, one row per literal of the class), a
+// backward pass carries the suffix state in registers, combines and writes dFE/dy_j (times the literal sign, S5) to
+// the literal's scratch row.  State: OR / XOR the running product (u = (1+y)/2 resp. y); NAE the products of u and
+// of p = (1-y)/2; EO / AMO the pmf of the true count truncated to {0, 1} (count basis, G10; d_t of P:L52):
+//   OR   FE = 2 prod u - 1                 dFE/dy_j = prod_{i!=j} u_i
 //   XOR  FE = s prod y                     dFE/dy_j = s prod_{i!=j} y_i                    (s = +1 odd parity, -1 even)
-//   NAE  FE = 2 prod u + 2 prod p - 1      dFE/dy_j = prod_{i!=j} u_i - prod_{i!=j} p_i     (p = (1-y)/2)
+//   NAE  FE = 2 prod u + 2 prod p - 1      dFE/dy_j = prod_{i!=j} u_i - prod_{i!=j} p_i
 //   EO   FE = 1 - 2 q_1                    dFE/dy_j = q_0^(-j) - q_1^(-j)
 //   AMO  FE = 1 - 2 (q_0 + q_1)            dFE/dy_j = - q_1^(-j)
-// (count basis, G10; d_t of P:L52).  The gradient written to scratch already carries the literal sign (S5).
+// Two short dynamic loops, no register arrays: any length, a few hundred bytes of code.
 // ------------------------------------------------------------------------------------------------------------------
-template <typename real, int LP, typename XL, typename SW>
+template <typename real, typename XL, typename SW>
 __device__ __forceinline__ void med_body(const MedCon& mc, const uint32_t* __restrict__ lc,
-                                         const int32_t* __restrict__ sc, const XL& xl, const SW& sw, int& satcnt,
-                                         real& fe)
+                                         const int32_t* __restrict__ sc, const XL& xl, const SW& sw, const SW& ax0,
+                                         const SW& ax1, int& satcnt, real& fe)
 {
-    const real half = real(0.5), one = real(1);
-    real y[LP];
-    unsigned long long negmask = 0ull;
+    const real half = real(0.5), one = real(1), zero = real(0);
+    const int L = mc.L, row0 = mc.off;
+    const int type = mc.type;
     int t = 0;
-#pragma unroll
-    for (int j = 0; j < LP; ++j) {
-        real v = one;   // padding literal: constant False (y = +1), neutral for every type below
-        if (j < mc.L) {
-            uint32_t w = lc[j];
-            real x = xl(w & LIT_VAR);
-            bool neg = (w >> 31) != 0;
-            t += ((x < real(0)) != neg) ? 1 : 0;
-            v = neg ? -x : x;
-            if (neg) negmask |= 1ull << j;
-        }
-        y[j] = v;
-    }
-    satcnt += pred(mc.type, mc.L, mc.k, t) ? 1 : 0;
-    fe = real(0);
-    if (mc.type == AFS_OR || mc.type == AFS_XOR) {
-        const bool is_or = mc.type == AFS_OR;
+    if (type == AFS_OR || type == AFS_XOR) {
+        const bool is_or = type == AFS_OR;
         const real s = is_or ? one : ((mc.k & 1) ? one : -one);
-        real g[LP];
         real pre = one;
-#pragma unroll
-        for (int j = 0; j < LP; ++j) {
-            real f = is_or ? half + half * y[j] : y[j];
-            y[j] = f;
-            g[j] = pre;
-            pre *= f;
+#pragma unroll 2
+        for (int j = 0; j < L; ++j) {
+            const uint32_t w = lc[j];
+            const real x = xl(w & LIT_VAR);
+            const bool neg = (w >> 31) != 0;
+            t += ((x < zero) != neg) ? 1 : 0;
+            const real y = neg ? -x : x;
+            ax0.put(row0 + j, pre);
+            pre = mul_rn(pre, is_or ? fma(half, y, half) : y);
         }
-        fe = is_or ? real(2) * pre - one : s * pre;
+        fe = is_or ? fma(real(2), pre, -one) : mul_rn(s, pre);
         real suf = s;
-#pragma unroll
-        for (int j = LP - 1; j >= 0; --j) {
-            g[j] *= suf;
-            suf *= y[j];
+#pragma unroll 2
+        for (int j = L - 1; j >= 0; --j) {
+            const uint32_t w = lc[j];
+            const real x = xl(w & LIT_VAR);
+            const bool neg = (w >> 31) != 0;
+            const real y = neg ? -x : x;
+            const real g = mul_rn(ax0.get(row0 + j), suf);
+            sw.put(sc[j], neg ? -g : g);
+            suf = mul_rn(suf, is_or ? fma(half, y, half) : y);
         }
-#pragma unroll
-        for (int j = 0; j < LP; ++j)
-            if (j < mc.L) sw.put(sc[j], ((negmask >> j) & 1ull) ? -g[j] : g[j]);
-    } else {
-        if constexpr (LP <= 32) {
-            if (mc.type == AFS_NAE) {
-                real gu[LP], gp[LP];
-                real pu = one, pp = one;
-#pragma unroll
-                for (int j = 0; j < LP; ++j) {
-                    // a padding literal must be neutral in BOTH chains: treat it as absent (factor 1)
-                    real u = j < mc.L ? half + half * y[j] : one;
-                    real p = j < mc.L ? half - half * y[j] : one;
-                    gu[j] = pu; gp[j] = pp;
-                    pu *= u; pp *= p;
-                }
-                fe = real(2) * pu + real(2) * pp - one;
-                real su = one, sp = one;
-#pragma unroll
-                for (int j = LP - 1; j >= 0; --j) {
-                    real u = j < mc.L ? half + half * y[j] : one;
-                    real p = j < mc.L ? half - half * y[j] : one;
-                    gu[j] = gu[j] * su - gp[j] * sp;
-                    su *= u; sp *= p;
-                }
-#pragma unroll
-                for (int j = 0; j < LP; ++j)
-                    if (j < mc.L) sw.put(sc[j], ((negmask >> j) & 1ull) ? -gu[j] : gu[j]);
-            } else {   // EO, AMO: pmf of the true count truncated to {0, 1}
-                real P0[LP], P1[LP];
-                real a0 = one, a1 = real(0);
-#pragma unroll
-                for (int j = 0; j < LP; ++j) {
-                    real u = half + half * y[j], p = half - half * y[j];
-                    P0[j] = a0; P1[j] = a1;
-                    a1 = a1 * u + a0 * p;
-                    a0 = a0 * u;
-                }
-                const bool is_eo = mc.type == AFS_EO;
-                fe = is_eo ? one - real(2) * a1 : one - real(2) * (a0 + a1);
-                real s0 = one, s1 = real(0);
-#pragma unroll
-                for (int j = LP - 1; j >= 0; --j) {
-                    real u = half + half * y[j], p = half - half * y[j];
-                    real q0 = P0[j] * s0;
-                    real q1 = P1[j] * s0 + P0[j] * s1;
-                    P0[j] = is_eo ? q0 - q1 : -q1;
-                    s1 = s1 * u + s0 * p;
-                    s0 = s0 * u;
-                }
-#pragma unroll
-                for (int j = 0; j < LP; ++j)
-                    if (j < mc.L) sw.put(sc[j], ((negmask >> j) & 1ull) ? -P0[j] : P0[j]);
-            }
+    } else if (type == AFS_NAE) {
+        real pu = one, pp = one;
+#pragma unroll 2
+        for (int j = 0; j < L; ++j) {
+            const uint32_t w = lc[j];
+            const real x = xl(w & LIT_VAR);
+            const bool neg = (w >> 31) != 0;
+            t += ((x < zero) != neg) ? 1 : 0;
+            const real y = neg ? -x : x;
+            ax0.put(row0 + j, pu);
+            ax1.put(row0 + j, pp);
+            pu = mul_rn(pu, fma(half, y, half));
+            pp = mul_rn(pp, fma(-half, y, half));
+        }
+        fe = fma(real(2), pu, fma(real(2), pp, -one));
+        real su = one, sp = one;
+#pragma unroll 2
+        for (int j = L - 1; j >= 0; --j) {
+            const uint32_t w = lc[j];
+            const real x = xl(w & LIT_VAR);
+            const bool neg = (w >> 31) != 0;
+            const real y = neg ? -x : x;
+            const real g = fma(ax0.get(row0 + j), su, -mul_rn(ax1.get(row0 + j), sp));
+            sw.put(sc[j], neg ? -g : g);
+            su = mul_rn(su, fma(half, y, half));
+            sp = mul_rn(sp, fma(-half, y, half));
+        }
+    } else {   // EO, AMO
+        const bool is_eo = type == AFS_EO;
+        real a0 = one, a1 = zero;
+#pragma unroll 2
+        for (int j = 0; j < L; ++j) {
+            const uint32_t w = lc[j];
+            const real x = xl(w & LIT_VAR);
+            const bool neg = (w >> 31) != 0;
+            t += ((x < zero) != neg) ? 1 : 0;
+            const real y = neg ? -x : x;
+            const real u = fma(half, y, half), p = fma(-half, y, half);
+            ax0.put(row0 + j, a0);
+            ax1.put(row0 + j, a1);
+            a1 = fma(a1, u, mul_rn(a0, p));
+            a0 = mul_rn(a0, u);
+        }
+        fe = is_eo ? fma(real(-2), a1, one) : fma(real(-2), a0 + a1, one);
+        real s0 = one, s1 = zero;
+#pragma unroll 2
+        for (int j = L - 1; j >= 0; --j) {
+            const uint32_t w = lc[j];
+            const real x = xl(w & LIT_VAR);
+            const bool neg = (w >> 31) != 0;
+            const real y = neg ? -x : x;
+            const real u = fma(half, y, half), p = fma(-half, y, half);
+            const real P0 = ax0.get(row0 + j), P1 = ax1.get(row0 + j);
+            const real q0 = mul_rn(P0, s0);
+            const real q1 = fma(P1, s0, mul_rn(P0, s1));
+            const real g = is_eo ? q0 - q1 : -q1;
+            sw.put(sc[j], neg ? -g : g);
+            s1 = fma(s1, u, mul_rn(s0, p));
+            s0 = mul_rn(s0, u);
         }
     }
+    satcnt += pred(type, L, mc.k, t) ? 1 : 0;
 }
 
-template <typename real, int LP>
+template <typename real>
 __global__ void __launch_bounds__(128) k_med(const MedCon* __restrict__ cons, int c_begin, int c_end,
                                              const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
                                              const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
+                                             real* __restrict__ aux0, real* __restrict__ aux1,
                                              int32_t* __restrict__ sat, real* __restrict__ fe_out)
 {
     __shared__ int s_sat[4][32];
@@ -368,11 +371,11 @@ __global__ void __launch_bounds__(128) k_med(const MedCon* __restrict__ cons, in
     const int b = blockIdx.y * 32 + lane;
     int satcnt = 0;
     const XGlobal<real> xl{XT, Bp, b};
-    const SGlobal<real> sc{scratch, Bp, b};
+    const SGlobal<real> sc{scratch, Bp, b}, a0{aux0, Bp, b}, a1{aux1, Bp, b};
     for (int c = c_begin + blockIdx.x * 4 + warp; c < c_end; c += gridDim.x * 4) {
         const MedCon mc = cons[c];
         real fe;
-        med_body<real, LP>(mc, lits + mc.off, slots + mc.off, xl, sc, satcnt, fe);
+        med_body<real>(mc, lits + mc.off, slots + mc.off, xl, sc, a0, a1, satcnt, fe);
         if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
     }
     if (sat) {
@@ -403,69 +406,6 @@ __global__ void __launch_bounds__(128) k_cmed(const LongCon* __restrict__ cons, 
         const LongCon lc = cons[c];
         real fe;
         cm_body<real>(lc, lits + lc.off, slots + lc.off, xl, sc, q, satcnt, fe, fe_out != nullptr);
-        if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
-    }
-    if (sat) {
-        s_sat[warp][lane] = satcnt;
-        __syncthreads();
-        if (warp == 0) {
-            int tot = s_sat[0][lane] + s_sat[1][lane] + s_sat[2][lane] + s_sat[3][lane];
-            if (tot) atomicAdd(&sat[b], tot);
-        }
-    }
-}
-
-// OR / XOR longer than 64 literals: two passes, the scratch row of each literal holds the running prefix product
-// between them (no extra memory, no division).
-template <typename real, typename XL, typename SW>
-__device__ __forceinline__ void prod_long_body(const MedCon& mc, const uint32_t* __restrict__ lc,
-                                               const int32_t* __restrict__ sc, const XL& xl, const SW& sw, int& satcnt,
-                                               real& fe)
-{
-    const real half = real(0.5), one = real(1);
-    const bool is_or = mc.type == AFS_OR;
-    const real s = is_or ? one : ((mc.k & 1) ? one : -one);
-    real pre = one;
-    int t = 0;
-    for (int j = 0; j < mc.L; ++j) {
-        uint32_t w = lc[j];
-        real x = xl(w & LIT_VAR);
-        bool neg = (w >> 31) != 0;
-        t += ((x < real(0)) != neg) ? 1 : 0;
-        real yj = neg ? -x : x;
-        sw.put(sc[j], pre);
-        pre *= is_or ? half + half * yj : yj;
-    }
-    satcnt += pred(mc.type, mc.L, mc.k, t) ? 1 : 0;
-    fe = is_or ? real(2) * pre - one : s * pre;
-    real suf = s;
-    for (int j = mc.L - 1; j >= 0; --j) {
-        uint32_t w = lc[j];
-        real x = xl(w & LIT_VAR);
-        bool neg = (w >> 31) != 0;
-        real yj = neg ? -x : x;
-        real g = sw.get(sc[j]) * suf;
-        sw.put(sc[j], neg ? -g : g);
-        suf *= is_or ? half + half * yj : yj;
-    }
-}
-
-template <typename real>
-__global__ void __launch_bounds__(128) k_prod_long(const MedCon* __restrict__ cons, int c_begin, int c_end,
-                                                   const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
-                                                   const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
-                                                   int32_t* __restrict__ sat, real* __restrict__ fe_out)
-{
-    __shared__ int s_sat[4][32];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int b = blockIdx.y * 32 + lane;
-    int satcnt = 0;
-    const XGlobal<real> xl{XT, Bp, b};
-    const SGlobal<real> sc{scratch, Bp, b};
-    for (int c = c_begin + blockIdx.x * 4 + warp; c < c_end; c += gridDim.x * 4) {
-        const MedCon mc = cons[c];
-        real fe;
-        prod_long_body<real>(mc, lits + mc.off, slots + mc.off, xl, sc, satcnt, fe);
         if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
     }
     if (sat) {

@@ -35,7 +35,6 @@ static afs_status upload(T** dst, const std::vector<T>& src)
     return AFS_OK;
 }
 
-static int med_bucket(int64_t L) { return L <= 8 ? 0 : L <= 16 ? 1 : L <= 32 ? 2 : L <= 64 ? 3 : 4; }
 
 // leave-one-out pmf indices that enter dFE/dy_j = sum_t d_t q_t^(-j), d_t = (sp_t - sp_{t+1})/2
 static void long_targets(int type, int L, int k, LongCon& c)
@@ -85,8 +84,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
                 if (stamp[v] == c) return AFS_ERR_DUP_VAR;
                 stamp[v] = c;
             }
-            bool count_type = !(ty == AFS_OR || ty == AFS_XOR);
-            if (count_type && L > LONG_MAX_LEN) unsupported = true;
+            if ((ty == AFS_EK || ty == AFS_CARD) && L > LONG_MAX_LEN) unsupported = true;
         }
     }
     if (unsupported) return AFS_ERR_UNSUPPORTED;
@@ -112,8 +110,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
             int ty = types[c];
             bool prod = (ty == AFS_OR || ty == AFS_XOR);
             if ((prod || ty == AFS_NAE) && L <= PULL_MAX_LEN) cls[c] = C_PULL;
-            else if (prod) cls[c] = C_MED;   // any length: beyond MED_MAX_PROD the two-pass product kernel takes it
-            else if ((ty == AFS_NAE || ty == AFS_EO || ty == AFS_AMO) && L <= MED_MAX_TWO) cls[c] = C_MED;
+            else if (prod || ty == AFS_NAE || ty == AFS_EO || ty == AFS_AMO) cls[c] = C_MED;   // any length
             else if ((ty == AFS_EK || ty == AFS_CARD) && L <= CM_MAX_LEN) cls[c] = C_CMED;
             else cls[c] = C_LONG;
         }
@@ -195,29 +192,24 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
         {
             std::vector<int> ids;
             for (int c = 0; c < m; ++c) if (cls[c] == C_MED) ids.push_back(c);
-            auto bucket_of = [&](int c) { return med_bucket(row_ptr[c + 1] - row_ptr[c]); };
+            // longest first: the grid-stride loops and the resident kernel's work counter take the heavy ones early
             std::stable_sort(ids.begin(), ids.end(), [&](int a, int b) {
-                int ba = bucket_of(a), bb = bucket_of(b);
-                if (ba != bb) return ba < bb;
-                return types[a] < types[b];     // homogeneous warps inside a bucket
+                return (row_ptr[a + 1] - row_ptr[a]) > (row_ptr[b + 1] - row_ptr[b]);
             });
-            int cur = 0;
-            P->med_begin[0] = 0;
             for (size_t i = 0; i < ids.size(); ++i) {
                 int c = ids[i];
-                int bk = bucket_of(c);
-                while (cur < bk) P->med_begin[++cur] = (int32_t)i;
                 MedCon mc;
                 int64_t L = row_ptr[c + 1] - row_ptr[c];
                 mc.off = (int32_t)med_lits.size(); mc.L = (int32_t)L;
                 mc.type = types[c]; mc.k = k[c];
+                if (types[c] != AFS_OR && types[c] != AFS_XOR) P->med_two = true;
                 for (int64_t e = row_ptr[c]; e < row_ptr[c + 1]; ++e) {
                     med_lits.push_back(lit_word(lits[e]));
                     med_slots.push_back(slot_of[e]);
                 }
                 med.push_back(mc);
             }
-            while (cur < MED_BUCKETS) P->med_begin[++cur] = (int32_t)ids.size();
+            P->med_nnz = (int64_t)med_lits.size();
             P->n_med = (int64_t)ids.size();
         }
         // ------------------------------------------------------------ long constraints (sorted by row count, longest first)
@@ -277,9 +269,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
             struct It { double cost; ResItem it; bool cm; };
             std::vector<It> its;
             for (size_t i = 0; i < med.size(); ++i) {
-                int bk = med_bucket(med[i].L);
-                double LP = bk < 4 ? (double)(8 << bk) : (double)med[i].L;
-                its.push_back({12.0 * LP, ResItem{(uint32_t)bk, (uint32_t)i}, false});
+                its.push_back({40.0 + 30.0 * med[i].L, ResItem{0u, (uint32_t)i}, false});
             }
             for (size_t i = 0; i < cmv.size(); ++i) {
                 const double L = cmv[i].L;
@@ -318,6 +308,17 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
                 }
                 ibeg[C] = (int32_t)flat.size();
                 cbeg[C] = (int32_t)cflat.size();
+                for (int q = 0; q < C; ++q) {
+                    int plits = 0;
+                    for (const ResItem& it : per[q]) plits += med[it.idx].L;
+                    for (int32_t ci : perc[q]) plits += cmv[ci].L;
+                    rp.cap_words = std::max(rp.cap_words, pull_ptr[vbeg[q + 1]] - pull_ptr[vbeg[q]] + 32);
+                    rp.cap_runs = std::max(rp.cap_runs, run_ptr[vbeg[q + 1]] - run_ptr[vbeg[q]]);
+                    rp.cap_own = std::max(rp.cap_own, vbeg[q + 1] - vbeg[q]);
+                    rp.cap_plits = std::max(rp.cap_plits, plits);
+                    rp.cap_cm = std::max(rp.cap_cm, (int)perc[q].size());
+                    rp.cap_push = std::max(rp.cap_push, (int)per[q].size());
+                }
                 up(&rp.d_cm_begin, cbeg);
                 up(&rp.d_cm_items, cflat);
                 for (int q = 0; q <= C; ++q) pbeg[q] = (int32_t)((int64_t)pc.size() * q / C);

@@ -29,7 +29,7 @@ namespace afs {
 
 namespace cg = cooperative_groups;
 
-constexpr int RES_WARPS = 16;
+constexpr int RES_WARPS = 32;
 constexpr int RES_VCH = 2;   // variables per work item
 
 template <typename real>
@@ -48,6 +48,8 @@ template <typename real>
 struct ResArgs {
     int n, steps, C, Bp, ntile;
     int cm_bufs, cm_rows;        // pmf buffers of the CTA (warps 0..cm_bufs-1 own one), rows (cm_maxL + 1) of each
+    int meta;                    // 1: the rank's index streams are staged in shared memory at kernel start
+    int cap_words, cap_runs, cap_own, cap_plits, cap_cm, cap_push;   // capacities of the staged arrays (max over ranks)
     int64_t nslots;
     const int32_t* pull_ptr;
     const uint32_t* pull_words;
@@ -72,6 +74,9 @@ struct ResArgs {
     real* XT;                    // [ntile][n][32]
     real* G;                     // [ntile][n][32] pull part of the gradient
     real* scratch;               // [ntile][nslots][32]
+    real* aux0;                  // [ntile][med_nnz][32] prefix states of the MED bodies
+    real* aux1;
+    int64_t med_nnz;
     int32_t* sat_hist;           // [steps+1][Bp], zeroed
     uint32_t* best_bits;         // [n][ntile]
     int32_t* best_sat;           // [Bp]
@@ -83,22 +88,10 @@ struct ResArgs {
 template <typename real>
 __device__ __forceinline__ real ld_cg(const real* p) { return __ldcg(p); }
 
-template <typename real>
-__device__ __forceinline__ void res_push_item(const ResArgs<real>& a, const ResItem it, const XTile<real>& xl,
-                                              const STile<real>& sw, int& satcnt)
-{
-    real fe;
-    const MedCon mc = a.med[it.idx];
-    const uint32_t* lc = a.med_lits + mc.off;
-    const int32_t* sc = a.med_slots + mc.off;
-    switch (it.code) {
-    case 0: med_body<real, 8>(mc, lc, sc, xl, sw, satcnt, fe); break;
-    case 1: med_body<real, 16>(mc, lc, sc, xl, sw, satcnt, fe); break;
-    case 2: med_body<real, 32>(mc, lc, sc, xl, sw, satcnt, fe); break;
-    case 3: med_body<real, 64>(mc, lc, sc, xl, sw, satcnt, fe); break;
-    default: prod_long_body<real>(mc, lc, sc, xl, sw, satcnt, fe); break;
-    }
-}
+struct ResMed {   // staged MED item: the constraint record and its bucket
+    MedCon mc;
+    uint32_t code;
+};
 
 template <typename real>
 __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<real> a)
@@ -116,11 +109,24 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
     uint32_t* bestb = S + n;                                            // [n] sign words of the best iterate (rank 0)
     uint2* sbuf0 = reinterpret_cast<uint2*>(S + ((2 * n + 3) & ~3));     // 16-byte aligned
     uint2* sbuf = sbuf0 + warp * PULL_SBUF;
-    real* qcol = reinterpret_cast<real*>(sbuf0 + RES_WARPS * PULL_SBUF) + (size_t)warp * a.cm_rows * 32 + lane;
+    real* qbase = reinterpret_cast<real*>(sbuf0 + RES_WARPS * PULL_SBUF);
+    real* qcol = qbase + (size_t)warp * a.cm_rows * 32 + lane;
+    // staged index streams of this rank (a.meta): pull words and runs of the own variables, their stream offsets,
+    // literal words / slot ids / records of the own push items
+    uint32_t* smw = reinterpret_cast<uint32_t*>(qbase + (size_t)a.cm_bufs * a.cm_rows * 32);
+    uint32_t* smr = smw + a.cap_words;
+    int32_t* smpp = reinterpret_cast<int32_t*>(smr + a.cap_runs);
+    int32_t* smrp = smpp + a.cap_own + 1;
+    uint32_t* sml = reinterpret_cast<uint32_t*>(smrp + a.cap_own + 1);
+    int32_t* sms = reinterpret_cast<int32_t*>(sml + a.cap_plits);
+    int32_t* smo = sms + a.cap_plits;                                   // [cap_cm + cap_push + 1] offsets into sml / sms
+    LongCon* smcm = reinterpret_cast<LongCon*>(smo + a.cap_cm + a.cap_push + 1);
+    ResMed* smmed = reinterpret_cast<ResMed*>(smcm + a.cap_cm);
     real* XTt = a.XT + (size_t)tile * n * 32 + lane;
     real* Gt = a.G + (size_t)tile * n * 32 + lane;
     const XTile<real> xl{Xs + lane};
     const STile<real> sw{a.scratch + (size_t)tile * a.nslots * 32 + lane};
+    const STile<real> ax0{a.aux0 + (size_t)tile * a.med_nnz * 32 + lane}, ax1{a.aux1 + (size_t)tile * a.med_nnz * 32 + lane};
     const ColShared<real> xcol{(uint32_t)__cvta_generic_to_shared(Xs + lane)};
     const int vb = a.var_begin[rank], ve = a.var_begin[rank + 1];
     const int ib = a.item_begin[rank], n_push = a.item_begin[rank + 1] - ib;
@@ -131,6 +137,38 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
     const int b = tile * 32 + lane;
     const real one = real(1);
 
+    // base-adjusted views: indexed with the global (absolute) offsets whether staged or not
+    const uint32_t* words_v = a.pull_words;
+    const uint32_t* runs_v = a.runs;
+    const int32_t* pp_v = a.pull_ptr;
+    const int32_t* rp_v = a.run_ptr;
+    if (a.meta) {
+        const int wbase = a.pull_ptr[vb], wn = a.pull_ptr[ve] - wbase + 32;   // + the slack a staged chunk may read
+        const int rbase = a.run_ptr[vb], rn = a.run_ptr[ve] - rbase;
+        for (int i = tid; i < wn; i += NT) smw[i] = a.pull_words[wbase + i];
+        for (int i = tid; i < rn; i += NT) smr[i] = a.runs[rbase + i];
+        for (int i = tid; i <= ve - vb; i += NT) { smpp[i] = a.pull_ptr[vb + i]; smrp[i] = a.run_ptr[vb + i]; }
+        for (int i = tid; i < n_cm; i += NT) { const LongCon lc = a.cm[a.cm_items[mb + i]]; smcm[i] = lc; smo[i + 1] = lc.L; }
+        for (int i = tid; i < n_push; i += NT) {
+            const ResItem it = a.items[ib + i];
+            ResMed rm; rm.mc = a.med[it.idx]; rm.code = it.code;
+            smmed[i] = rm; smo[n_cm + i + 1] = rm.mc.L;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int off = 0;
+            smo[0] = 0;
+            for (int i = 1; i <= n_cm + n_push; ++i) { off += smo[i]; smo[i] = off; }
+        }
+        __syncthreads();
+        for (int i = warp; i < n_cm + n_push; i += RES_WARPS) {
+            const int o = smo[i], L = smo[i + 1] - o;
+            const uint32_t* gl = i < n_cm ? a.cm_lits + smcm[i].off : a.med_lits + smmed[i - n_cm].mc.off;
+            const int32_t* gs = i < n_cm ? a.cm_slots + smcm[i].off : a.med_slots + smmed[i - n_cm].mc.off;
+            for (int j = lane; j < L; j += 32) { sml[o + j] = gl[j]; sms[o + j] = gs[j]; }
+        }
+        words_v = smw - wbase; runs_v = smr - rbase; pp_v = smpp - vb; rp_v = smrp - vb;
+    }
     for (int i = lane; i < PULL_SBUF; i += 32) sbuf[i] = make_uint2(0u, 0u);
     for (int v = warp; v < n; v += RES_WARPS) {
         const real x = ld_cg(XTt + (size_t)v * 32);
@@ -154,9 +192,11 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
                     if (lane == 0) it = atomicAdd(&s_ctr_cm, 1);
                     it = __shfl_sync(FULL, it, 0);
                     if (it >= n_cm) break;
-                    const LongCon lc = a.cm[a.cm_items[mb + it]];
                     real fe;
-                    cm_body<real>(lc, a.cm_lits + lc.off, a.cm_slots + lc.off, xl, sw, qcol, satcnt, fe, false);
+                    const LongCon lc = a.meta ? smcm[it] : a.cm[a.cm_items[mb + it]];
+                    const uint32_t* lw = a.meta ? sml + smo[it] : a.cm_lits + lc.off;
+                    const int32_t* ls = a.meta ? sms + smo[it] : a.cm_slots + lc.off;
+                    cm_body<real>(lc, lw, ls, xl, sw, qcol, satcnt, fe, false);
                 }
             }
             for (;;) {
@@ -165,7 +205,13 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
                 it = __shfl_sync(FULL, it, 0);
                 if (it >= total) break;
                 if (it < n_push) {
-                    res_push_item<real>(a, a.items[ib + it], xl, sw, satcnt);
+                    ResMed rm;
+                    if (a.meta) rm = smmed[it];
+                    else { const ResItem ri = a.items[ib + it]; rm.mc = a.med[ri.idx]; rm.code = ri.code; }
+                    const uint32_t* lw = a.meta ? sml + smo[n_cm + it] : a.med_lits + rm.mc.off;
+                    const int32_t* ls = a.meta ? sms + smo[n_cm + it] : a.med_slots + rm.mc.off;
+                    real fe;
+                    med_body<real>(rm.mc, lw, ls, xl, sw, ax0, ax1, satcnt, fe);
                 } else if (it < n_push + n_cnt) {
                     // S9 of 32 pull clauses, lane <-> clause, bit r of T <-> restart r
                     const int c = cb + (it - n_push) * 32 + lane;
@@ -193,8 +239,8 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
                         real g[1] = {real(0)};
                         if (mk == 0) {
                             g[0] = (real)a.gconst[v];
-                            pull_variable<real, 1>(a.runs, a.run_ptr[v], a.run_ptr[v + 1], a.pull_words, a.pull_ptr[v],
-                                                   xcol, 32u * (uint32_t)sizeof(real), lane, sbuf, g);
+                            pull_variable<real, 1>(runs_v, rp_v[v], rp_v[v + 1], words_v, pp_v[v], xcol,
+                                                   32u * (uint32_t)sizeof(real), lane, sbuf, g);
                         }
                         Gt[(size_t)v * 32] = g[0];
                     }
@@ -250,6 +296,7 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
             const int sp = __ldcg(a.sat_hist + (size_t)t * a.Bp + b);
             if (sp > s_best_sat[lane]) { s_best_sat[lane] = sp; s_best_step[lane] = t; }
         }
+#pragma unroll 4
         for (int v = warp; v < n; v += RES_WARPS) {
             const real x = ld_cg(XTt + (size_t)v * 32);
             Xs[v * 32 + lane] = x;
@@ -316,12 +363,18 @@ __global__ void __launch_bounds__(256) k_res_out(const real* __restrict__ XT, co
     }
 }
 
-// dynamic shared memory of k_resident for n variables and cm_bufs pmf buffers of cm_rows rows
+// dynamic shared memory of k_resident for n variables and cm_bufs pmf buffers of cm_rows rows (without staged streams)
 template <typename real>
 inline size_t res_smem_bytes(int n, int cm_bufs, int cm_rows)
 {
     return (size_t)n * 32 * sizeof(real) + (size_t)((2 * n + 3) & ~3) * 4 + (size_t)RES_WARPS * PULL_SBUF * sizeof(uint2) +
            (size_t)cm_bufs * cm_rows * 32 * sizeof(real);
+}
+// bytes of the staged index streams of one rank, capacities as in ResArgs
+inline size_t res_meta_bytes(int cap_words, int cap_runs, int cap_own, int cap_plits, int cap_cm, int cap_push)
+{
+    return 4 * ((size_t)cap_words + cap_runs + 2 * ((size_t)cap_own + 1) + 2 * (size_t)cap_plits + cap_cm + cap_push + 1) +
+           sizeof(LongCon) * (size_t)cap_cm + sizeof(ResMed) * (size_t)cap_push + 16;
 }
 
 }  // namespace afs

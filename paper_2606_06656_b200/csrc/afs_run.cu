@@ -1,6 +1,7 @@
 // afs_run.cu -- workspace management, launch orchestration and the device entry points of include/afs.h.
 // Streaming path: per PGD step one launch per non-empty push bucket (medium / long constraints) plus one fused
 // variable pass; no host round trip inside the loop (everything is enqueued on the caller's stream).
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 
@@ -27,7 +28,7 @@ template <typename T> static void free_ptr(T*& p) { if (p) cudaFree(p); p = null
 void free_workspace(afs_problem* P)
 {
     Workspace& w = P->ws;
-    free_ptr(w.XT[0]); free_ptr(w.XT[1]); free_ptr(w.scratch);
+    free_ptr(w.XT[0]); free_ptr(w.XT[1]); free_ptr(w.scratch); free_ptr(w.aux[0]); free_ptr(w.aux[1]);
     free_ptr(w.sat_hist); free_ptr(w.best_sat[0]); free_ptr(w.best_sat[1]);
     free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.best_bits);
     free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.fe_cm); free_ptr(w.f_part);
@@ -102,6 +103,8 @@ static afs_status ensure_workspace(afs_problem* P, int Bp, size_t elem, int64_t 
     A((unsigned char**)&w.XT[0], n * nBp * nelem);
     A((unsigned char**)&w.XT[1], n * nBp * nelem);
     A((unsigned char**)&w.scratch, (size_t)P->nslots * nBp * nelem);
+    A((unsigned char**)&w.aux[0], (size_t)P->med_nnz * nBp * nelem);
+    A((unsigned char**)&w.aux[1], (size_t)(P->med_two ? P->med_nnz : 0) * nBp * nelem);
     A(&w.sat_hist, (size_t)nrows * nBp);
     A(&w.best_sat[0], (size_t)nBp); A(&w.best_sat[1], (size_t)nBp);
     A(&w.best_step[0], (size_t)nBp); A(&w.best_step[1], (size_t)nBp);
@@ -203,21 +206,13 @@ static afs_status launch_push(afs_problem* P, const real* XT, int Bp, real* scra
                                                         fe_cm, qrows);
         P->last_launches++;
     }
-    for (int bk = 0; bk < MED_BUCKETS; ++bk) {
-        int c0 = P->med_begin[bk], c1 = P->med_begin[bk + 1];
-        if (c1 <= c0) continue;
-        int gx = (c1 - c0 + 3) / 4;
+    if (P->n_med > 0) {
+        int gx = ((int)P->n_med + 3) / 4;
         int cap = (P->sm_count * 16 + tiles - 1) / tiles;   // enough CTAs to fill the chip, grid-stride beyond
         if (gx > cap) gx = cap < 1 ? 1 : cap;
-        dim3 grid(gx, tiles);
-        ProfSpan span(P, 4 + bk, st);
-        switch (bk) {
-        case 0: k_med<real, 8><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
-        case 1: k_med<real, 16><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
-        case 2: k_med<real, 32><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
-        case 3: k_med<real, 64><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
-        default: k_prod_long<real><<<grid, 128, 0, st>>>(P->d_med, c0, c1, P->d_med_lits, P->d_med_slots, XT, Bp, scratch, sat, fe_med); break;
-        }
+        ProfSpan span(P, 4, st);
+        k_med<real><<<dim3(gx, tiles), 128, 0, st>>>(P->d_med, 0, (int)P->n_med, P->d_med_lits, P->d_med_slots, XT, Bp, scratch,
+                                                    (real*)P->ws.aux[0], (real*)P->ws.aux[1], sat, fe_med);
         P->last_launches++;
     }
     afs_status s = AFS_OK;
@@ -354,25 +349,35 @@ static afs_status round_count_impl(afs_problem* P, const real* X, int32_t B, int
 // ----------------------------------------------------------------------------------------------------------------
 constexpr size_t RES_SMEM_MAX = 227 * 1024 - 512;
 
-// pmf buffers one CTA of the resident kernel can hold beside the tile (0 = does not fit)
+// Shared-memory layout of one CTA of the resident kernel for plan pi: the tile and its sign words always; then, as far
+// as the 227 KB go, the staged index streams of the rank (meta) and the pmf buffers of the EK / CARD bodies.
+// The streams are staged when at least min(4, RES_WARPS) pmf buffers still fit beside them (or none is needed).
+struct ResLayout { bool ok; int cm_bufs; int meta; size_t bytes; };
 template <typename real>
-static int resident_cm_bufs(const afs_problem* P)
+static ResLayout resident_layout(const afs_problem* P, int pi)
 {
+    const ResPlan& rp = P->res[pi];
     const size_t base = res_smem_bytes<real>(P->n, 0, 0);
-    if (base > RES_SMEM_MAX) return -1;
-    if (P->n_cm == 0) return 0;
-    const size_t per = (size_t)(P->cm_maxL + 1) * 32 * sizeof(real);
-    const size_t fit = (RES_SMEM_MAX - base) / per;
-    return fit == 0 ? -1 : (int)(fit > RES_WARPS ? RES_WARPS : fit);
+    if (base > RES_SMEM_MAX) return {false, 0, 0, 0};
+    const size_t per = P->n_cm > 0 ? (size_t)(P->cm_maxL + 1) * 32 * sizeof(real) : 0;
+    const size_t mb = res_meta_bytes(rp.cap_words, rp.cap_runs, rp.cap_own, rp.cap_plits, rp.cap_cm, rp.cap_push);
+    auto bufs = [&](size_t left) { return per == 0 ? 0 : (int)std::min<size_t>(RES_WARPS, left / per); };
+    if (base + mb <= RES_SMEM_MAX) {
+        const int nb = bufs(RES_SMEM_MAX - base - mb);
+        if (per == 0 || nb >= 4) return {true, nb, 1, base + mb + nb * per};
+    }
+    const int nb = bufs(RES_SMEM_MAX - base);
+    if (per != 0 && nb == 0) return {false, 0, 0, 0};
+    return {true, nb, 0, base + nb * per};
 }
 
 template <typename real>
 static int resident_plan(const afs_problem* P, int ntile)
 {
-    if (P->n_long > 0 || !P->res[0].d_var_begin || resident_cm_bufs<real>(P) < 0) return -1;
+    if (P->n_long > 0 || !P->res[0].d_var_begin) return -1;
     int pi = RES_PLANS - 1;
     while (pi > 0 && (long long)ntile * (1 << pi) > P->sm_count) --pi;
-    return pi;
+    return resident_layout<real>(P, pi).ok ? pi : -1;
 }
 
 template <typename real>
@@ -389,9 +394,13 @@ static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, i
     CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)(steps + 1) * Bp * sizeof(int32_t), st));
     ResArgs<real> a{};
     a.n = P->n; a.steps = steps; a.C = rp.C; a.Bp = Bp; a.ntile = ntile; a.nslots = P->nslots;
-    a.cm_bufs = resident_cm_bufs<real>(P); a.cm_rows = P->cm_maxL + 1;
+    const ResLayout lay = resident_layout<real>(P, pi);
+    a.cm_bufs = lay.cm_bufs; a.cm_rows = P->cm_maxL + 1; a.meta = lay.meta;
+    a.cap_words = rp.cap_words; a.cap_runs = rp.cap_runs; a.cap_own = rp.cap_own; a.cap_plits = rp.cap_plits;
+    a.cap_cm = rp.cap_cm; a.cap_push = rp.cap_push;
     a.cm_begin = rp.d_cm_begin; a.cm_items = rp.d_cm_items;
     a.G = (real*)w.XT[1];
+    a.aux0 = (real*)w.aux[0]; a.aux1 = (real*)w.aux[1]; a.med_nnz = P->med_nnz;
     a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
     a.gconst = P->d_pull_gconst; a.slot_ptr = P->d_slot_ptr;
     a.med = P->d_med; a.med_lits = P->d_med_lits; a.med_slots = P->d_med_slots;
@@ -401,7 +410,7 @@ static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, i
     a.XT = XT; a.scratch = (real*)w.scratch; a.sat_hist = w.sat_hist;
     a.best_bits = w.best_bits; a.best_sat = w.best_sat[0]; a.best_step = w.best_step[0];
     a.lr = lr; a.mask = mask;
-    const size_t smem = res_smem_bytes<real>(P->n, a.cm_bufs, a.cm_rows);
+    const size_t smem = lay.bytes;
     static bool attr_done[2] = {false, false};
     const int ti = sizeof(real) == 8 ? 1 : 0;
     if (!attr_done[ti]) {
