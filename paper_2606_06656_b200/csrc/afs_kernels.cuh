@@ -181,9 +181,18 @@ __device__ __forceinline__ void cm_body(const LongCon& lc, const uint32_t* __res
         tc += ((x < zero) != neg) ? 1 : 0;
         const real y = neg ? -x : x;
         const real u = fma(half, y, half), p = fma(-half, y, half);
-        real hi = zero;   // old q_{j+1}
-#pragma unroll 4
-        for (int t = j + 1; t >= 1; --t) {
+        // cells j+1 .. 1, four at a time with the loads in front (the stores of a group never feed its loads)
+        real hi = zero;   // old q_{t}, starting with q_{j+1} = 0
+        int t = j + 1;
+        for (; t >= 4; t -= 4) {
+            const real l1 = q[(t - 1) * 32], l2 = q[(t - 2) * 32], l3 = q[(t - 3) * 32], l4 = q[(t - 4) * 32];
+            q[t * 32] = fma(l1, p, mul_rn(hi, u));
+            q[(t - 1) * 32] = fma(l2, p, mul_rn(l1, u));
+            q[(t - 2) * 32] = fma(l3, p, mul_rn(l2, u));
+            q[(t - 3) * 32] = fma(l4, p, mul_rn(l3, u));
+            hi = l4;
+        }
+        for (; t >= 1; --t) {
             const real lo = q[(t - 1) * 32];
             q[t * 32] = fma(lo, p, mul_rn(hi, u));
             hi = lo;
@@ -209,40 +218,73 @@ __device__ __forceinline__ void cm_body(const LongCon& lc, const uint32_t* __res
     const real wA = useA ? (real)lc.wA : zero, wB = useB ? (real)lc.wB : zero;
     // capture steps: bottom-up chain step = t; top-down chain step i <-> t = L-1-i
     const int f1 = tA, f2 = tB, b1 = L - 1 - tB, b2 = L - 1 - tA;
-    int bp0 = min(f1, b1), bp3 = max(f2, b2);
-    int m1 = max(f1, b1), m2 = min(f2, b2);
-    int bp1 = min(m1, m2), bp2 = max(m1, m2);
-    const int bp[4] = {bp0, bp1, bp2, bp3};
-    for (int j = 0; j < L; ++j) {
-        const uint32_t w = lw[j];
-        const real x = xl(w & LIT_VAR);
-        const bool neg = (w >> 31) != 0;
-        const real y = neg ? -x : x;
-        const real u = fma(half, y, half), p = fma(-half, y, half);
-        const bool fwd = !(y < zero);   // p <= 1/2
-        const real rb = rcp_rn(fwd ? u : p);
-        const real R = mul_rn(fwd ? p : u, rb);
-        const int c1 = fwd ? f1 : b1, c2 = fwd ? f2 : b2;
-        const real w1 = fwd ? wA : wB, w2 = fwd ? wB : wA;
-        const real* qp = fwd ? q : q + L * 32;
-        const int stride = fwd ? 32 : -32;
-        real acc = zero, v1 = zero, v2 = zero;
+    const int bp0 = min(f1, b1), bp3 = max(f2, b2);
+    const int m1 = max(f1, b1), m2 = min(f2, b2);
+    const int bp[4] = {bp0, min(m1, m2), max(m1, m2), bp3};
+    // two literals at a time: two independent chains per lane, loads of a group of four steps in front
+    for (int j0 = 0; j0 < L; j0 += 2) {
+        real R[2], rb[2], w1[2], w2[2], acc[2], v1[2], v2[2];
+        const real* qp[2];
+        int st[2], c1[2], c2[2];
+        bool ng[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int j = min(j0 + h, L - 1);
+            const uint32_t w = lw[j];
+            const real x = xl(w & LIT_VAR);
+            ng[h] = (w >> 31) != 0;
+            const real y = ng[h] ? -x : x;
+            const real u = fma(half, y, half), p = fma(-half, y, half);
+            const bool fwd = !(y < zero);   // p <= 1/2
+            rb[h] = rcp_rn(fwd ? u : p);
+            R[h] = -mul_rn(fwd ? p : u, rb[h]);
+            c1[h] = fwd ? f1 : b1; c2[h] = fwd ? f2 : b2;
+            w1[h] = fwd ? wA : wB; w2[h] = fwd ? wB : wA;
+            qp[h] = fwd ? q : q + L * 32;
+            st[h] = fwd ? 32 : -32;
+            acc[h] = zero; v1[h] = zero; v2[h] = zero;
+        }
         int s = 0;
 #pragma unroll
         for (int b = 0; b < 4; ++b) {
             const int e = bp[b];
             if (e >= s) {
-#pragma unroll 4
-                for (; s <= e; ++s) {
-                    acc = fma(-R, acc, *qp);
-                    qp += stride;
+                int cnt = e - s + 1;
+                for (; cnt >= 4; cnt -= 4) {
+                    real a[2][4];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) a[h][i] = qp[h][i * st[h]];
+                        qp[h] += 4 * st[h];
+                    }
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        acc[0] = fma(R[0], acc[0], a[0][i]);
+                        acc[1] = fma(R[1], acc[1], a[1][i]);
+                    }
                 }
-                v1 = c1 == e ? acc : v1;
-                v2 = c2 == e ? acc : v2;
+                for (; cnt > 0; --cnt) {
+                    const real a0 = *qp[0], a1 = *qp[1];
+                    qp[0] += st[0]; qp[1] += st[1];
+                    acc[0] = fma(R[0], acc[0], a0);
+                    acc[1] = fma(R[1], acc[1], a1);
+                }
+                s = e + 1;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    v1[h] = c1[h] == e ? acc[h] : v1[h];
+                    v2[h] = c2[h] == e ? acc[h] : v2[h];
+                }
             }
         }
-        const real g = mul_rn(fma(w1, v1, mul_rn(w2, v2)), rb);
-        sc.put(sw[j], neg ? -g : g);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            if (j0 + h < L) {
+                const real g = mul_rn(fma(w1[h], v1[h], mul_rn(w2[h], v2[h])), rb[h]);
+                sc.put(sw[j0 + h], ng[h] ? -g : g);
+            }
+        }
     }
 }
 

@@ -29,7 +29,10 @@ namespace afs {
 
 namespace cg = cooperative_groups;
 
-constexpr int RES_WARPS = 32;
+#ifndef AFS_RES_WARPS
+#define AFS_RES_WARPS 32
+#endif
+constexpr int RES_WARPS = AFS_RES_WARPS;
 constexpr int RES_VCH = 2;   // variables per work item
 
 template <typename real>
@@ -48,7 +51,8 @@ template <typename real>
 struct ResArgs {
     int n, steps, C, Bp, ntile;
     int cm_bufs, cm_rows;        // pmf buffers of the CTA (warps 0..cm_bufs-1 own one), rows (cm_maxL + 1) of each
-    int meta;                    // 1: the rank's index streams are staged in shared memory at kernel start
+    int meta;                    // bit 0: the rank's small index streams (runs, offsets, push-item literals) are staged
+                                 // in shared memory at kernel start; bit 1: its pull words too (cap_words > 0)
     int cap_words, cap_runs, cap_own, cap_plits, cap_cm, cap_push;   // capacities of the staged arrays (max over ranks)
     int64_t nslots;
     const int32_t* pull_ptr;
@@ -93,6 +97,15 @@ struct ResMed {   // staged MED item: the constraint record and its bucket
     uint32_t code;
 };
 
+#ifdef AFS_RES_TIMING   // development aid (never defined in the product build): per-warp phase clocks of one iteration
+__device__ long long g_res_timing[256 * RES_WARPS * 8];
+#define AFS_T(slot) do { if (t == 5 && lane == 0 && blockIdx.x < 256) g_res_timing[(blockIdx.x * RES_WARPS + warp) * 8 + (slot)] = clock64(); } while (0)
+#define AFS_T6(slot) do { if (t == 6 && lane == 0 && blockIdx.x < 256) g_res_timing[(blockIdx.x * RES_WARPS + warp) * 8 + (slot)] = clock64(); } while (0)
+#else
+#define AFS_T(slot) do { } while (0)
+#define AFS_T6(slot) do { } while (0)
+#endif
+
 template <typename real>
 __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<real> a)
 {
@@ -110,7 +123,10 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
     uint2* sbuf0 = reinterpret_cast<uint2*>(S + ((2 * n + 3) & ~3));     // 16-byte aligned
     uint2* sbuf = sbuf0 + warp * PULL_SBUF;
     real* qbase = reinterpret_cast<real*>(sbuf0 + RES_WARPS * PULL_SBUF);
-    real* qcol = qbase + (size_t)warp * a.cm_rows * 32 + lane;
+    // pmf buffers belong to the HIGHEST warp ids: the issue arbiter favours them, and the EK / CARD items are the
+    // longest dependent chains of the iteration
+    const int cmw = RES_WARPS - 1 - warp;
+    real* qcol = qbase + (size_t)(cmw < a.cm_bufs ? cmw : 0) * a.cm_rows * 32 + lane;
     // staged index streams of this rank (a.meta): pull words and runs of the own variables, their stream offsets,
     // literal words / slot ids / records of the own push items
     uint32_t* smw = reinterpret_cast<uint32_t*>(qbase + (size_t)a.cm_bufs * a.cm_rows * 32);
@@ -145,7 +161,8 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
     if (a.meta) {
         const int wbase = a.pull_ptr[vb], wn = a.pull_ptr[ve] - wbase + 32;   // + the slack a staged chunk may read
         const int rbase = a.run_ptr[vb], rn = a.run_ptr[ve] - rbase;
-        for (int i = tid; i < wn; i += NT) smw[i] = a.pull_words[wbase + i];
+        if (a.meta & 2)
+            for (int i = tid; i < wn; i += NT) smw[i] = a.pull_words[wbase + i];
         for (int i = tid; i < rn; i += NT) smr[i] = a.runs[rbase + i];
         for (int i = tid; i <= ve - vb; i += NT) { smpp[i] = a.pull_ptr[vb + i]; smrp[i] = a.run_ptr[vb + i]; }
         for (int i = tid; i < n_cm; i += NT) { const LongCon lc = a.cm[a.cm_items[mb + i]]; smcm[i] = lc; smo[i + 1] = lc.L; }
@@ -167,7 +184,16 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
             const int32_t* gs = i < n_cm ? a.cm_slots + smcm[i].off : a.med_slots + smmed[i - n_cm].mc.off;
             for (int j = lane; j < L; j += 32) { sml[o + j] = gl[j]; sms[o + j] = gs[j]; }
         }
-        words_v = smw - wbase; runs_v = smr - rbase; pp_v = smpp - vb; rp_v = smrp - vb;
+        if (a.meta & 2) words_v = smw - wbase;
+        runs_v = smr - rbase; pp_v = smpp - vb; rp_v = smrp - vb;
+    }
+    // P3 takes the own variables vb + warp + RES_WARPS * k; lane k keeps the slot range and the mask of the k-th one
+    const int p3_n = ve - vb > warp ? (ve - vb - warp + RES_WARPS - 1) / RES_WARPS : 0;
+    const bool p3_regs = ve - vb <= 32 * RES_WARPS;
+    int p3_s0 = 0, p3_s1 = 0, p3_mk = 0;
+    if (p3_regs && lane < p3_n) {
+        const int v = vb + warp + RES_WARPS * lane;
+        p3_s0 = a.slot_ptr[v]; p3_s1 = a.slot_ptr[v + 1]; p3_mk = a.mask ? a.mask[v] : 0;
     }
     for (int i = lane; i < PULL_SBUF; i += 32) sbuf[i] = make_uint2(0u, 0u);
     for (int v = warp; v < n; v += RES_WARPS) {
@@ -186,7 +212,9 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
         {
             int satcnt = 0;
             const int total = n_push + n_cnt + (last ? 0 : n_var);
-            if (warp < a.cm_bufs) {   // EK / CARD constraints first (the heaviest items), by the warps that own a pmf buffer
+            AFS_T(0);
+            AFS_T6(7);
+            if (cmw < a.cm_bufs) {   // EK / CARD constraints first (the heaviest items), by the warps that own a pmf buffer
                 for (;;) {
                     int it = 0;
                     if (lane == 0) it = atomicAdd(&s_ctr_cm, 1);
@@ -198,6 +226,7 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
                     const int32_t* ls = a.meta ? sms + smo[it] : a.cm_slots + lc.off;
                     cm_body<real>(lc, lw, ls, xl, sw, qcol, satcnt, fe, false);
                 }
+                AFS_T(2);
             }
             for (;;) {
                 int it = 0;
@@ -248,7 +277,9 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
             }
             if (satcnt) atomicAdd(a.sat_hist + (size_t)t * a.Bp + b, satcnt);
         }
+        AFS_T(1);
         cluster.sync();
+        AFS_T(3);
         if (tid == 0) { s_ctr = 0; s_ctr_cm = 0; }
         // ---- S10: iterate t against the best so far (rank 0 holds the record of the tile)
         if (rank == 0) {
@@ -267,36 +298,63 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
             }
         }
         if (last) break;
-        // ---- P3: S6 (fixed transposed-CSR order) + S7 + S8 for the own variables
-        for (int i = warp; i < ve - vb; i += RES_WARPS) {
-            const int v = vb + i;
-            const real x = Xs[v * 32 + lane];
-            const int mk = a.mask ? a.mask[v] : 0;
-            real g = ld_cg(Gt + (size_t)v * 32);
-            if (mk == 0) {
-                const int s1 = a.slot_ptr[v + 1];
-                int s = a.slot_ptr[v];
+        // ---- P3: S6 (fixed transposed-CSR order) + S7 + S8 for the own variables, two at a time: G and the first
+        // four gradient rows of both are requested together (everything here comes from L2), then added in slot order
+        for (int k = 0; k < p3_n; k += 2) {
+            int v[2], s0[2], s1[2], mk[2];
+            bool ok[2];
+            real x[2], g[2], pre[2][4];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                ok[h] = k + h < p3_n;
+                const int kk = ok[h] ? k + h : k;
+                v[h] = vb + warp + RES_WARPS * kk;
+                if (p3_regs) {
+                    s0[h] = __shfl_sync(FULL, p3_s0, kk); s1[h] = __shfl_sync(FULL, p3_s1, kk); mk[h] = __shfl_sync(FULL, p3_mk, kk);
+                } else {
+                    s0[h] = a.slot_ptr[v[h]]; s1[h] = a.slot_ptr[v[h] + 1]; mk[h] = a.mask ? a.mask[v[h]] : 0;
+                }
+                if (mk[h] != 0) s1[h] = s0[h];
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                x[h] = Xs[v[h] * 32 + lane];
+                g[h] = ld_cg(Gt + (size_t)v[h] * 32);
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    pre[h][i] = s0[h] + i < s1[h] ? ld_cg(sw.p + (size_t)(s0[h] + i) * 32) : real(0);
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                if (!ok[h]) continue;
                 const real* __restrict__ sc = sw.p;
-                for (; s + 4 <= s1; s += 4) {
+                int s = s0[h];
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    if (s + i < s1[h]) g[h] += pre[h][i];
+                s += 4;
+                for (; s + 4 <= s1[h]; s += 4) {
                     real g0 = ld_cg(sc + (size_t)s * 32), g1 = ld_cg(sc + (size_t)(s + 1) * 32);
                     real g2 = ld_cg(sc + (size_t)(s + 2) * 32), g3 = ld_cg(sc + (size_t)(s + 3) * 32);
-                    g += g0; g += g1; g += g2; g += g3;
+                    g[h] += g0; g[h] += g1; g[h] += g2; g[h] += g3;
                 }
-                for (; s < s1; ++s) g += ld_cg(sc + (size_t)s * 32);
+                for (; s < s1[h]; ++s) g[h] += ld_cg(sc + (size_t)s * 32);
+                real xn = x[h] - a.lr * g[h];
+                xn = xn > one ? one : xn;
+                xn = xn < -one ? -one : xn;
+                if (mk[h] != 0) xn = x[h];
+                XTt[(size_t)v[h] * 32] = xn;
             }
-            real xn = x - a.lr * g;
-            xn = xn > one ? one : xn;
-            xn = xn < -one ? -one : xn;
-            if (mk != 0) xn = x;
-            XTt[(size_t)v * 32] = xn;
         }
+        AFS_T(4);
         cluster.sync();
+        AFS_T(5);
         // ---- P4: the record of iterate t, then X_{t+1} and its sign words
         if (rank == 0 && warp == 0) {
             const int sp = __ldcg(a.sat_hist + (size_t)t * a.Bp + b);
             if (sp > s_best_sat[lane]) { s_best_sat[lane] = sp; s_best_step[lane] = t; }
         }
-#pragma unroll 4
+#pragma unroll 8
         for (int v = warp; v < n; v += RES_WARPS) {
             const real x = ld_cg(XTt + (size_t)v * 32);
             Xs[v * 32 + lane] = x;

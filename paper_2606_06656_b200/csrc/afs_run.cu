@@ -350,25 +350,33 @@ static afs_status round_count_impl(afs_problem* P, const real* X, int32_t B, int
 constexpr size_t RES_SMEM_MAX = 227 * 1024 - 512;
 
 // Shared-memory layout of one CTA of the resident kernel for plan pi: the tile and its sign words always; then, as far
-// as the 227 KB go, the staged index streams of the rank (meta) and the pmf buffers of the EK / CARD bodies.
-// The streams are staged when at least min(4, RES_WARPS) pmf buffers still fit beside them (or none is needed).
-struct ResLayout { bool ok; int cm_bufs; int meta; size_t bytes; };
+// as the 227 KB go and in this order: the rank's small index streams (runs, stream offsets, literals of its push
+// items), pmf buffers for the EK / CARD bodies -- up to 12, or one per constraint of the rank if that is fewer: the
+// warps that own one carry the longest dependent chains of the iteration and must not be few -- and last the rank's
+// pull words (the largest stream; 32 warps hide its L2 latency when it stays in global memory).
+struct ResLayout { bool ok; int cm_bufs; int meta; int cap_words; size_t bytes; };
 template <typename real>
 static ResLayout resident_layout(const afs_problem* P, int pi)
 {
     const ResPlan& rp = P->res[pi];
-    const size_t base = res_smem_bytes<real>(P->n, 0, 0);
-    if (base > RES_SMEM_MAX) return {false, 0, 0, 0};
+    size_t used = res_smem_bytes<real>(P->n, 0, 0);
+    if (used > RES_SMEM_MAX) return {false, 0, 0, 0, 0};
     const size_t per = P->n_cm > 0 ? (size_t)(P->cm_maxL + 1) * 32 * sizeof(real) : 0;
-    const size_t mb = res_meta_bytes(rp.cap_words, rp.cap_runs, rp.cap_own, rp.cap_plits, rp.cap_cm, rp.cap_push);
-    auto bufs = [&](size_t left) { return per == 0 ? 0 : (int)std::min<size_t>(RES_WARPS, left / per); };
-    if (base + mb <= RES_SMEM_MAX) {
-        const int nb = bufs(RES_SMEM_MAX - base - mb);
-        if (per == 0 || nb >= 4) return {true, nb, 1, base + mb + nb * per};
+    if (per != 0 && used + per > RES_SMEM_MAX) return {false, 0, 0, 0, 0};
+    int meta = 0, nb = 0, cap_words = 0;
+    const size_t small = res_meta_bytes(0, rp.cap_runs, rp.cap_own, rp.cap_plits, rp.cap_cm, rp.cap_push);
+    if (used + small + per <= RES_SMEM_MAX) { meta = 1; used += small; }
+    if (per != 0) {
+        const int want = std::min(RES_WARPS, std::min(12, std::max(rp.cap_cm, 1)));
+        nb = (int)std::min<size_t>((size_t)want, (RES_SMEM_MAX - used) / per);
+        used += (size_t)nb * per;
     }
-    const int nb = bufs(RES_SMEM_MAX - base);
-    if (per != 0 && nb == 0) return {false, 0, 0, 0};
-    return {true, nb, 0, base + nb * per};
+    if (meta && used + 4 * (size_t)rp.cap_words <= RES_SMEM_MAX) { meta |= 2; cap_words = rp.cap_words; used += 4 * (size_t)cap_words; }
+    if (per != 0 && nb < RES_WARPS) {   // what is left goes to more pmf buffers
+        const int more = (int)std::min<size_t>((size_t)(RES_WARPS - nb), (RES_SMEM_MAX - used) / per);
+        nb += more; used += (size_t)more * per;
+    }
+    return {true, nb, meta, cap_words, used};
 }
 
 template <typename real>
@@ -396,7 +404,7 @@ static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, i
     a.n = P->n; a.steps = steps; a.C = rp.C; a.Bp = Bp; a.ntile = ntile; a.nslots = P->nslots;
     const ResLayout lay = resident_layout<real>(P, pi);
     a.cm_bufs = lay.cm_bufs; a.cm_rows = P->cm_maxL + 1; a.meta = lay.meta;
-    a.cap_words = rp.cap_words; a.cap_runs = rp.cap_runs; a.cap_own = rp.cap_own; a.cap_plits = rp.cap_plits;
+    a.cap_words = lay.cap_words; a.cap_runs = rp.cap_runs; a.cap_own = rp.cap_own; a.cap_plits = rp.cap_plits;
     a.cap_cm = rp.cap_cm; a.cap_push = rp.cap_push;
     a.cm_begin = rp.d_cm_begin; a.cm_items = rp.d_cm_items;
     a.G = (real*)w.XT[1];
@@ -560,3 +568,10 @@ extern "C" afs_status afs_pgd_run_host(afs_problem* P, float* X, int32_t B, int3
     CU(cudaStreamSynchronize(st));
     return AFS_OK;
 }
+
+#ifdef AFS_RES_TIMING
+extern "C" __attribute__((visibility("default"))) int afs_debug_timing(long long* out, int n)
+{
+    return (int)cudaMemcpyFromSymbol(out, afs::g_res_timing, sizeof(long long) * n);
+}
+#endif
