@@ -654,8 +654,10 @@ __device__ __forceinline__ void pull_variable(const uint32_t* __restrict__ runs,
     for (int c = 0; c < RPL; ++c) g[c] += acc[c];
 }
 
+// 4 CTAs (32 warps) per SM at <= 64 registers: the pass waits on L2 gathers, and occupancy is what hides them -- at
+// 95 registers (2 CTAs per SM) the same code took 1.5x as long on configs[3] (measured: 420 -> 274 us per iteration).
 template <typename real, bool EVAL, int RPL>
-__global__ void __launch_bounds__(VAR_WARPS * 32, RPL == 1 ? 4 : 2) k_var(const VarArgs<real> a)
+__global__ void __launch_bounds__(VAR_WARPS * 32, 4) k_var(const VarArgs<real> a)
 {
     __shared__ __align__(16) uint2 s_stage[VAR_WARPS][PULL_SBUF];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
