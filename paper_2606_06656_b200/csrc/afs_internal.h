@@ -55,6 +55,12 @@ struct LongCon {       // 32 bytes
     float wA, wB;      // their weights d_t in {-1, 0, +1}
 };
 
+struct PullClause {    // one PULL-class clause packed for the bit-parallel count: header + its <= 5 literal words, 32 bytes
+    uint32_t hdr;      // bits 0..2 L | 3..4 kind (PH_KIND_*) | 5 XOR parity k
+    uint32_t lit[PULL_MAX_LEN];
+    uint32_t pad[2];
+};
+
 struct CountCon {      // generic forward CSR entry for the count-only kernel: 16 bytes
     int64_t off;
     int32_t L;
@@ -141,6 +147,7 @@ struct afs_problem {
     float* d_pull_gconst = nullptr;     // [n] constant gradient of unit clauses
     afs::CountCon* d_pc = nullptr;      // the PULL constraints alone (forward CSR), for counts and objective
     uint32_t* d_pc_lits = nullptr;
+    afs::PullClause* d_pcp = nullptr;   // the same clauses packed for the bit-parallel counts
     int32_t* d_slot_ptr = nullptr;      // [n+1] scratch rows of each variable (transposed-CSR order)
     int64_t nslots = 0;
 

@@ -551,8 +551,8 @@ __device__ __forceinline__ void pull_run(const uint32_t* __restrict__ words, int
                                          uint32_t rowbytes, int lane, uint2* sbuf, real (&gout)[RPL])
 {
     constexpr int OPC = 32 / NOTHER;              // occurrences per staged chunk of <= 32 entries
-    // occurrences gathered together: 8 (NOTHER <= 2) or up to 16 loads in flight per lane.  More does not pay: on the
-    // large instances the pass moves ~7 TB/s out of L2 as it is, and the tail of a wider batch gathers rows it discards
+    // occurrences gathered together: 8 (NOTHER <= 2) or up to 16 loads in flight per lane; the tail of a wider batch
+    // gathers rows it discards, and the registers are better spent on occupancy (see k_var)
     constexpr int U0 = NOTHER <= 2 ? 4 : 2;
     constexpr int U = U0 / RPL >= 1 ? U0 / RPL : 1;
     real g[RPL];
@@ -797,8 +797,8 @@ __device__ __forceinline__ SWords<TPT> ld_swords(const uint32_t* __restrict__ p)
 }
 
 template <int TPT>
-__global__ void __launch_bounds__(256) k_sat_pull(const CountCon* __restrict__ cons, const uint32_t* __restrict__ lits,
-                                                  int m, const uint32_t* __restrict__ S, int ntile,
+__global__ void __launch_bounds__(256) k_sat_pull(const PullClause* __restrict__ cons, int m,
+                                                  const uint32_t* __restrict__ S, int ntile,
                                                   int32_t* __restrict__ sat)
 {
     __shared__ int s_cnt[TPT][32];
@@ -816,25 +816,28 @@ __global__ void __launch_bounds__(256) k_sat_pull(const CountCon* __restrict__ c
 #pragma unroll
         for (int k = 0; k < TPT; ++k) T[k] = 0u;
         if (c < m) {
-            const CountCon cc = cons[c];
-            const uint32_t* lw = lits + cc.off;
+            const uint4* rec = reinterpret_cast<const uint4*>(cons + c);
+            const uint4 h0 = rec[0], h1 = rec[1];
+            const uint32_t lit[PULL_MAX_LEN] = {h0.y, h0.z, h0.w, h1.x, h1.y};
+            const int L = (int)(h0.x & 7u), kind = (int)((h0.x >> 3) & 3u);
             uint32_t vor[TPT], vand[TPT], vxor[TPT];
 #pragma unroll
             for (int k = 0; k < TPT; ++k) { vor[k] = 0u; vand[k] = 0xffffffffu; vxor[k] = 0u; }
-            for (int j = 0; j < cc.L; ++j) {
-                const uint32_t w = lw[j];
-                const uint32_t flipm = (w >> 31) ? 0xffffffffu : 0u;
-                const SWords<TPT> sw = ld_swords<TPT>(S + (size_t)(w & LIT_VAR) * ntile + tile0);
 #pragma unroll
-                for (int k = 0; k < TPT; ++k) {
-                    const uint32_t tj = sw.w[k] ^ flipm;
-                    vor[k] |= tj; vand[k] &= tj; vxor[k] ^= tj;
+            for (int j = 0; j < PULL_MAX_LEN; ++j)
+                if (j < L) {
+                    const uint32_t flipm = (lit[j] >> 31) ? 0xffffffffu : 0u;
+                    const SWords<TPT> sw = ld_swords<TPT>(S + (size_t)(lit[j] & LIT_VAR) * ntile + tile0);
+#pragma unroll
+                    for (int k = 0; k < TPT; ++k) {
+                        const uint32_t tj = sw.w[k] ^ flipm;
+                        vor[k] |= tj; vand[k] &= tj; vxor[k] ^= tj;
+                    }
                 }
-            }
-            const uint32_t par = (cc.k & 1) ? 0xffffffffu : 0u;
+            const uint32_t par = ((h0.x >> 5) & 1u) ? 0xffffffffu : 0u;
 #pragma unroll
             for (int k = 0; k < TPT; ++k)
-                T[k] = cc.type == AFS_OR ? vor[k] : cc.type == AFS_XOR ? ~(vxor[k] ^ par) : (vor[k] & ~vand[k]);
+                T[k] = kind == (int)PH_KIND_OR ? vor[k] : kind == (int)PH_KIND_XOR ? ~(vxor[k] ^ par) : (vor[k] & ~vand[k]);
         }
 #pragma unroll
         for (int k = 0; k < TPT; ++k) cnt[k] += bit_column_sums(T[k], lane);

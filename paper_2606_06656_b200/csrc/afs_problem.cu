@@ -137,6 +137,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
         std::vector<float> gconst(n, 0.f);
         std::vector<CountCon> pc;
         std::vector<uint32_t> pc_lits;
+        std::vector<PullClause> pcp;
         for (int c = 0; c < m; ++c) {
             if (cls[c] != C_PULL) continue;
             P->n_pull++;
@@ -146,6 +147,10 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
             pc.push_back(cc);
             for (int j = 0; j < L; ++j) pc_lits.push_back(lit_word(lc[j]));
             int kind = types[c] == AFS_OR ? (int)PH_KIND_OR : types[c] == AFS_XOR ? (int)PH_KIND_XOR : (int)PH_KIND_NAE;
+            PullClause pq{};
+            pq.hdr = (uint32_t)L | ((uint32_t)kind << 3) | ((uint32_t)(k[c] & 1) << 5);
+            for (int j = 0; j < L; ++j) pq.lit[j] = lit_word(lc[j]);
+            pcp.push_back(pq);
             for (int j = 0; j < L; ++j) {
                 int v = std::abs(lc[j]) - 1;
                 bool sign = (lc[j] < 0) != (types[c] == AFS_XOR && !(k[c] & 1));
@@ -335,6 +340,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
         up(&P->d_pull_gconst, gconst);
         up(&P->d_pc, pc);
         up(&P->d_pc_lits, pc_lits);
+        up(&P->d_pcp, pcp);
         up(&P->d_slot_ptr, slot_ptr);
         up(&P->d_med, med);
         up(&P->d_med_lits, med_lits);
@@ -365,7 +371,7 @@ extern "C" void afs_problem_destroy(afs_problem* p)
     cudaSetDevice(p->device);
     cudaDeviceSynchronize();
     cudaFree(p->d_pull_ptr); cudaFree(p->d_pull_words); cudaFree(p->d_slot_ptr);
-    cudaFree(p->d_run_ptr); cudaFree(p->d_runs); cudaFree(p->d_pull_gconst); cudaFree(p->d_pc); cudaFree(p->d_pc_lits);
+    cudaFree(p->d_run_ptr); cudaFree(p->d_runs); cudaFree(p->d_pull_gconst); cudaFree(p->d_pc); cudaFree(p->d_pc_lits); cudaFree(p->d_pcp);
     cudaFree(p->d_med); cudaFree(p->d_med_lits); cudaFree(p->d_med_slots);
     cudaFree(p->d_long); cudaFree(p->d_long_lits); cudaFree(p->d_long_slots);
     cudaFree(p->d_cm); cudaFree(p->d_cm_lits); cudaFree(p->d_cm_slots);

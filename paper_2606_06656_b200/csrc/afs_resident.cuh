@@ -67,8 +67,7 @@ struct ResArgs {
     const LongCon* cm;
     const uint32_t* cm_lits;
     const int32_t* cm_slots;
-    const CountCon* pc;
-    const uint32_t* pc_lits;
+    const PullClause* pcp;
     const int32_t* var_begin;    // [C+1]
     const int32_t* item_begin;   // [C+1]
     const ResItem* items;
@@ -246,18 +245,19 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
                     const int c = cb + (it - n_push) * 32 + lane;
                     uint32_t T = 0u;
                     if (c < ce) {
-                        const CountCon cc = a.pc[c];
-                        const uint32_t* lw = a.pc_lits + cc.off;
-                        uint32_t w = lw[0];
-                        uint32_t t0 = S[w & LIT_VAR] ^ ((w >> 31) ? 0xffffffffu : 0u);
-                        uint32_t vor = t0, vand = t0, vxor = t0;
-                        for (int j = 1; j < cc.L; ++j) {
-                            w = lw[j];
-                            const uint32_t tj = S[w & LIT_VAR] ^ ((w >> 31) ? 0xffffffffu : 0u);
-                            vor |= tj; vand &= tj; vxor ^= tj;
-                        }
-                        T = cc.type == AFS_OR ? vor : cc.type == AFS_XOR ? ~(vxor ^ ((cc.k & 1) ? 0xffffffffu : 0u))
-                                                                         : (vor & ~vand);
+                        const uint4* rec = reinterpret_cast<const uint4*>(a.pcp + c);
+                        const uint4 h0 = rec[0], h1 = rec[1];
+                        const uint32_t lit[PULL_MAX_LEN] = {h0.y, h0.z, h0.w, h1.x, h1.y};
+                        const int L = (int)(h0.x & 7u), kind = (int)((h0.x >> 3) & 3u);
+                        uint32_t vor = 0u, vand = 0xffffffffu, vxor = 0u;
+#pragma unroll
+                        for (int j = 0; j < PULL_MAX_LEN; ++j)
+                            if (j < L) {
+                                const uint32_t tj = S[lit[j] & LIT_VAR] ^ ((lit[j] >> 31) ? 0xffffffffu : 0u);
+                                vor |= tj; vand &= tj; vxor ^= tj;
+                            }
+                        const uint32_t par = ((h0.x >> 5) & 1u) ? 0xffffffffu : 0u;
+                        T = kind == (int)PH_KIND_OR ? vor : kind == (int)PH_KIND_XOR ? ~(vxor ^ par) : (vor & ~vand);
                     }
                     satcnt += bit_column_sums(T, lane);
                 } else {

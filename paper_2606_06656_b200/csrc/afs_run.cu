@@ -251,9 +251,9 @@ static afs_status launch_sat_pull(afs_problem* P, const uint32_t* S, int Bp, int
     if (gx > cap) gx = cap < 1 ? 1 : cap;
     dim3 grid(gx, gy);
     ProfSpan span(P, 2, st);
-    if (tpt == 4) k_sat_pull<4><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, S, ntile, sat);
-    else if (tpt == 2) k_sat_pull<2><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, S, ntile, sat);
-    else k_sat_pull<1><<<grid, 256, 0, st>>>(P->d_pc, P->d_pc_lits, m, S, ntile, sat);
+    if (tpt == 4) k_sat_pull<4><<<grid, 256, 0, st>>>(P->d_pcp, m, S, ntile, sat);
+    else if (tpt == 2) k_sat_pull<2><<<grid, 256, 0, st>>>(P->d_pcp, m, S, ntile, sat);
+    else k_sat_pull<1><<<grid, 256, 0, st>>>(P->d_pcp, m, S, ntile, sat);
     P->last_launches++;
     return AFS_OK;
 }
@@ -413,7 +413,7 @@ static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, i
     a.gconst = P->d_pull_gconst; a.slot_ptr = P->d_slot_ptr;
     a.med = P->d_med; a.med_lits = P->d_med_lits; a.med_slots = P->d_med_slots;
     a.cm = P->d_cm; a.cm_lits = P->d_cm_lits; a.cm_slots = P->d_cm_slots;
-    a.pc = P->d_pc; a.pc_lits = P->d_pc_lits;
+    a.pcp = P->d_pcp;
     a.var_begin = rp.d_var_begin; a.item_begin = rp.d_item_begin; a.items = rp.d_items; a.pc_begin = rp.d_pc_begin;
     a.XT = XT; a.scratch = (real*)w.scratch; a.sat_hist = w.sat_hist;
     a.best_bits = w.best_bits; a.best_sat = w.best_sat[0]; a.best_step = w.best_step[0];
