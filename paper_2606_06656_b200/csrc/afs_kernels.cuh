@@ -551,8 +551,9 @@ __device__ __forceinline__ void pull_run(const uint32_t* __restrict__ words, int
                                          uint32_t rowbytes, int lane, uint2* sbuf, real (&gout)[RPL])
 {
     constexpr int OPC = 32 / NOTHER;              // occurrences per staged chunk of <= 32 entries
-    // occurrences gathered together: 8 (NOTHER <= 2) or up to 16 loads in flight per lane; the tail of a wider batch
-    // gathers rows it discards, and the registers are better spent on occupancy (see k_var)
+    // occurrences gathered together: 8 (NOTHER <= 2) or up to 16 loads in flight per lane.  Wider batches were measured
+    // slower at the same register count (configs[3]: 272 -> 320 us per iteration with twice the batch): their tails
+    // gather rows that are discarded, and occupancy already hides the latency (see k_var)
     constexpr int U0 = NOTHER <= 2 ? 4 : 2;
     constexpr int U = U0 / RPL >= 1 ? U0 / RPL : 1;
     real g[RPL];
