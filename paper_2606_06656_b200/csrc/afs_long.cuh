@@ -241,7 +241,9 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
                 const real y = neg ? -x : x;
                 const real u = real(0.5) + real(0.5) * y, p = real(0.5) - real(0.5) * y;
                 const bool fwd = !(y < real(0));             // p <= 1/2: type A
-                const real R = fwd ? p / u : u / p;          // in [0, 1]; the divisor is >= 1/2; 0 on the boundary
+                // in [0, 1]; the divisor is >= 1/2; 0 on the boundary.  Correctly rounded reciprocal times the numerator
+                // (one MUFU + two corrections instead of the IEEE division sequence; <= 1 ulp from the quotient)
+                const real R = (fwd ? p : u) * recip(fwd ? u : p);
                 AAll[r * QS + j] = fwd ? R : -R;             // the sign bit is the direction (-0.0 for y = -1)
             }
             unsigned bal = __ballot_sync(FULLM, tr);
