@@ -230,28 +230,45 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
     {
         const int r = tid % RPC;
         const unsigned pat = RPC == 8 ? 0x01010101u : RPC == 4 ? 0x11111111u : RPC == 2 ? 0x55555555u : 0xffffffffu;
-        for (int idx = tid; idx < ((L * RPC + NT - 1) / NT) * NT; idx += NT) {
-            int j = idx / RPC;
-            bool tr = false;
-            if (j < L) {
-                uint32_t w = lw[j];
-                real x = XT[(size_t)(w & LIT_VAR) * Bp + bg * RPC + r];
-                bool neg = (w >> 31) != 0;
-                tr = (x < real(0)) != neg;
-                const real y = neg ? -x : x;
-                const real u = real(0.5) + real(0.5) * y, p = real(0.5) - real(0.5) * y;
-                const bool fwd = !(y < real(0));             // p <= 1/2: type A
-                // in [0, 1]; the divisor is >= 1/2; 0 on the boundary.  Correctly rounded reciprocal times the numerator
-                // (one MUFU + two corrections instead of the IEEE division sequence; <= 1 ulp from the quotient)
-                const real R = (fwd ? p : u) * recip(fwd ? u : p);
-                AAll[r * QS + j] = fwd ? R : -R;             // the sign bit is the direction (-0.0 for y = -1)
+        // four rounds of the block at a time: the literal words first, then the four gathers, so that a thread has four
+        // dependent (word -> row) pairs in flight instead of one
+        const int rounds = (L * RPC + NT - 1) / NT;
+        int truec = 0;   // lanes < RPC: true literals of restart `lane` seen by this warp
+        for (int r0 = 0; r0 < rounds; r0 += 4) {
+            uint32_t w[4];
+            real x[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int j = (tid + (r0 + k) * NT) / RPC;
+                w[k] = j < L ? lw[j] : 0u;
             }
-            unsigned bal = __ballot_sync(FULLM, tr);
-            if (lane < RPC) {
-                int add = __popc(bal & (pat << lane));
-                if (add) atomicAdd(&s_cnt[lane], add);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int j = (tid + (r0 + k) * NT) / RPC;
+                x[k] = j < L ? XT[(size_t)(w[k] & LIT_VAR) * Bp + bg * RPC + r] : real(0);
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                if (r0 + k < rounds) {   // block-uniform
+                    const int j = (tid + (r0 + k) * NT) / RPC;
+                    bool tr = false;
+                    if (j < L) {
+                        const bool neg = (w[k] >> 31) != 0;
+                        tr = (x[k] < real(0)) != neg;
+                        const real y = neg ? -x[k] : x[k];
+                        const real u = real(0.5) + real(0.5) * y, p = real(0.5) - real(0.5) * y;
+                        const bool fwd = !(y < real(0));             // p <= 1/2: type A
+                        // in [0, 1]; the divisor is >= 1/2; 0 on the boundary.  Correctly rounded reciprocal times the
+                        // numerator (one MUFU + two corrections instead of the IEEE division sequence; <= 1 ulp off)
+                        const real R = (fwd ? p : u) * recip(fwd ? u : p);
+                        AAll[r * QS + j] = fwd ? R : -R;             // the sign bit is the direction (-0.0 for y = -1)
+                    }
+                    const unsigned bal = __ballot_sync(FULLM, tr);
+                    if (lane < RPC) truec += __popc(bal & (pat << lane));
+                }
             }
         }
+        if (lane < RPC && truec) atomicAdd(&s_cnt[lane], truec);
     }
     __syncthreads();
     const int b = bg * RPC + warp;
