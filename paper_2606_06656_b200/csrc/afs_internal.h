@@ -160,6 +160,13 @@ struct afs_problem {
     afs::LongCon* d_long = nullptr;     // sorted by bucket (NR), longest first inside a bucket
     uint32_t* d_long_lits = nullptr;
     int32_t* d_long_slots = nullptr;
+    // the same class with the literals of the run's fixed variables folded away (k_long_fold, once per afs_pgd_run with
+    // a mask): compacted literal / slot lists at the same offsets, L and k reduced, targets recomputed
+    afs::LongCon* d_long_f = nullptr;
+    uint32_t* d_long_lits_f = nullptr;
+    int32_t* d_long_slots_f = nullptr;
+    int64_t long_nnz = 0;
+    bool long_folded = false;           // the launches of the current call use the folded lists
     int32_t long_begin[afs::LONG_BUCKETS + 1] = {0};
     int32_t long_maxL[afs::LONG_BUCKETS] = {0};
 

@@ -159,7 +159,10 @@ static afs_status launch_long_rpc(afs_problem* P, int bucket, const real* XT, in
     long long blocks = (long long)(c1 - c0) * (Bp / RPC);
     if (blocks > 0x7fffffffLL) return AFS_ERR_UNSUPPORTED;
     ProfSpan span(P, 8 + NR, st);
-    k_long<real, NR, RPC><<<(unsigned)blocks, RPC * 32, smem, st>>>(P->d_long, c0, P->d_long_lits, P->d_long_slots, XT,
+    const bool fo = P->long_folded;
+    k_long<real, NR, RPC><<<(unsigned)blocks, RPC * 32, smem, st>>>(fo ? P->d_long_f : P->d_long, c0,
+                                                                    fo ? P->d_long_lits_f : P->d_long_lits,
+                                                                    fo ? P->d_long_slots_f : P->d_long_slots, XT,
                                                                     Bp, scratch, sat, fe, LS, QS);
     P->last_launches++;
     return AFS_OK;
@@ -265,6 +268,7 @@ static afs_status enter(afs_problem* P, int32_t B)
     if ((unsigned long long)P->n * (unsigned long long)(((B + 31) / 32) * 32) * 8ull >= (1ull << 32)) return AFS_ERR_UNSUPPORTED;
     if (cudaSetDevice(P->device) != cudaSuccess) { (void)cudaGetLastError(); return AFS_ERR_CUDA; }
     P->last_launches = 0;
+    P->long_folded = false;
     P->prof.on = false;
     P->prof.spans.clear();
     P->prof.used = 0;
@@ -474,6 +478,12 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     CU(cudaMemsetAsync(w.best_step[0], 0, (size_t)Bp * sizeof(int32_t), st));
     P->last_launches++;
     const int gx = var_grid_x(P->n);
+    if (mask && P->n_long > 0 && steps > 0) {   // the fixed variables' literals leave the long constraints for this run
+        k_long_fold<<<(unsigned)((P->n_long + 3) / 4), 128, 0, st>>>(P->d_long, P->d_long_lits, P->d_long_slots, (int)P->n_long,
+                                                                   mask, P->d_long_f, P->d_long_lits_f, P->d_long_slots_f);
+        P->last_launches++;
+        P->long_folded = true;
+    }
     for (int t = 0; t < steps; ++t) {
         P->prof.on = P->prof.stride > 0 && t % P->prof.stride == 0;
         const real* Xin = XT[t & 1];
@@ -496,6 +506,7 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
         if ((s = launch_sat_pull(P, w.S[t & 1], Bp, sat_cur, st)) != AFS_OK) return s;
     }
     P->prof.on = false;
+    P->long_folded = false;
     // the last iterate: count only, then fold and write out
     const real* Xfin = XT[steps & 1];
     int32_t* sat_fin = w.sat_hist + (size_t)steps * Bp;
