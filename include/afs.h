@@ -172,6 +172,17 @@ AFS_API afs_status afs_set_option(afs_problem* p, int32_t what, int64_t value);
 #define AFS_KERNEL_CLASSES 19
 AFS_API afs_status afs_profile_read(afs_problem* p, double* ms, int64_t* launches, int32_t n);
 
+/*
+ * afs_profile_flops -- after afs_profile_read: adds to flops[0..n) (host, caller-zeroed) the STATE-DEPENDENT
+ * algorithmic flops the timed launches of each class had to do, as counted by the kernels themselves, and forgets
+ * them.  Only the long-constraint kernels (classes 9..17) count: per (constraint, restart) 6 Leff Keff, the survey's
+ * figure evaluated on the Leff literals that are strictly inside the cube at that iterate, with the
+ * threshold left after the boundary literals that are true; 0 where the expansion is constant there.  Literals on the
+ * boundary (clipped iterates, fixed variables) are exact shifts of the pmf and cost no arithmetic, so
+ * the state-independent 6 L K over-counts what these kernels have to do.  Other classes add nothing.
+ */
+AFS_API afs_status afs_profile_flops(afs_problem* p, double* flops, int32_t n);
+
 /* Static, never NULL. */
 AFS_API const char* afs_status_string(afs_status s);
 

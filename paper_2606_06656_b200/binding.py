@@ -21,7 +21,7 @@ EXPORTS = (
     "afs_problem_create", "afs_problem_destroy", "afs_coeffs", "afs_eval_grad", "afs_eval_grad_f64",
     "afs_round_count", "afs_round_count_f64", "afs_pgd_run", "afs_pgd_run_f64", "afs_pgd_run_host",
     "afs_problem_info", "afs_set_option", "afs_status_string", "afs_abi_version", "afs_last_error_message",
-    "afs_profile_read",
+    "afs_profile_read", "afs_profile_flops",
 )
 
 _lib = None
@@ -68,6 +68,8 @@ def lib():
     L.afs_set_option.restype = C.c_int
     L.afs_profile_read.argtypes = [vp, vp, vp, i32]
     L.afs_profile_read.restype = C.c_int
+    L.afs_profile_flops.argtypes = [vp, vp, i32]
+    L.afs_profile_flops.restype = C.c_int
     L.afs_status_string.argtypes = [C.c_int]
     L.afs_status_string.restype = C.c_char_p
     L.afs_abi_version.restype = i32
@@ -151,6 +153,12 @@ class Problem:
         cnt = np.zeros(len(self.KERNEL_CLASSES), dtype=np.int64)
         _chk(lib().afs_profile_read(self._h, ms.ctypes.data, cnt.ctypes.data, len(ms)), "afs_profile_read")
         return {k: (float(m), int(c)) for k, m, c in zip(self.KERNEL_CLASSES, ms, cnt) if c}
+
+    def profile_flops(self):
+        """afs_profile_flops: {class name: state-dependent algorithmic flops of the launches last read}, non-zero only."""
+        fl = np.zeros(len(self.KERNEL_CLASSES), dtype=np.float64)
+        _chk(lib().afs_profile_flops(self._h, fl.ctypes.data, len(fl)), "afs_profile_flops")
+        return {k: float(v) for k, v in zip(self.KERNEL_CLASSES, fl) if v}
 
     # ------------------------------------------------------------------ helpers
     def _dev(self):

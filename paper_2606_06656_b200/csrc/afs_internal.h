@@ -98,6 +98,8 @@ struct Profiler {
     size_t used = 0;
     struct Span { int cls, e0, e1; };
     std::vector<Span> spans;
+    unsigned long long* d_work = nullptr;   // [PROF_CLASSES][32] state-dependent algorithmic flops counted by the kernels
+    double work[PROF_CLASSES] = {0};        // of the timed launches (k_long only), summed at afs_profile_read
 };
 
 // records cudaGetErrorString(e) + location for afs_last_error_message()

@@ -250,7 +250,8 @@ template <typename real, int NR, int RPC>
 __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ cons, int c_begin,
                                                    const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
                                                    const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
-                                                   int32_t* __restrict__ sat, real* __restrict__ fe_out, int LS, int QS)
+                                                   int32_t* __restrict__ sat, real* __restrict__ fe_out, int LS, int QS,
+                                                   unsigned long long* __restrict__ work)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     real* RcAll = reinterpret_cast<real*>(smem_raw);              // [RPC][LS]  ratios in list order
@@ -413,6 +414,17 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
     __syncwarp();
     // ---- S3 + S5: leave-one-out
     const bool useA = lc.wA != 0.f, useB = lc.wB != 0.f;
+    // timing mode only: the state-dependent algorithmic work of this (constraint, restart) -- 6 Leff Keff flops, the
+    // survey's count for a pmf of Leff interior literals with the threshold left after the nB0 true boundary literals
+    if (work && lane == 0) {
+        const int keff = lc.k - nB0;
+        const bool live = (useA || useB) && Leff > 0 && keff >= (lc.type == AFS_EK ? 0 : 1) && keff <= Leff;
+        if (live) {
+            int K = min(keff, Leff - keff + 1) + 1;
+            K = K < 1 ? 1 : K;
+            atomicAdd(work + (blockIdx.x & 31u), 6ull * (unsigned long long)Leff * (unsigned long long)K);   // 32 slots
+        }
+    }
     // capture points in true-count index space, t1 <= t2 (equal if only one is used)
     int t1 = lc.tA, t2 = lc.tB;
     real w1 = (real)lc.wA, w2 = (real)lc.wB;

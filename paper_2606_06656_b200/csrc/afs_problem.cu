@@ -388,6 +388,7 @@ extern "C" void afs_problem_destroy(afs_problem* p)
     }
     afs::free_workspace(p);
     for (cudaEvent_t e : p->prof.pool) cudaEventDestroy(e);
+    cudaFree(p->prof.d_work);
     (void)cudaGetLastError();
     delete p;
 }

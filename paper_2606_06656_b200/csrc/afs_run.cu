@@ -69,6 +69,21 @@ extern "C" afs_status afs_profile_read(afs_problem* P, double* ms, int64_t* laun
     }
     pr.spans.clear();
     pr.used = 0;
+    if (pr.d_work) {
+        unsigned long long h[PROF_CLASSES * 32];
+        CU(cudaMemcpy(h, pr.d_work, sizeof(h), cudaMemcpyDeviceToHost));
+        CU(cudaMemset(pr.d_work, 0, sizeof(h)));
+        for (int c = 0; c < PROF_CLASSES; ++c)
+            for (int i = 0; i < 32; ++i) pr.work[c] += (double)h[c * 32 + i];
+    }
+    return AFS_OK;
+}
+
+extern "C" afs_status afs_profile_flops(afs_problem* P, double* flops, int32_t n)
+{
+    if (!P || !flops || n < 0 || n > PROF_CLASSES) return AFS_ERR_INVALID_ARG;
+    for (int c = 0; c < n; ++c) { flops[c] += P->prof.work[c]; }
+    for (int c = 0; c < PROF_CLASSES; ++c) P->prof.work[c] = 0.0;
     return AFS_OK;
 }
 
@@ -160,10 +175,18 @@ static afs_status launch_long_rpc(afs_problem* P, int bucket, const real* XT, in
     if (blocks > 0x7fffffffLL) return AFS_ERR_UNSUPPORTED;
     ProfSpan span(P, 8 + NR, st);
     const bool fo = P->long_folded;
+    unsigned long long* work = nullptr;
+    if (P->prof.on) {
+        if (!P->prof.d_work) {
+            CU(cudaMalloc((void**)&P->prof.d_work, sizeof(unsigned long long) * PROF_CLASSES * 32));
+            CU(cudaMemsetAsync(P->prof.d_work, 0, sizeof(unsigned long long) * PROF_CLASSES * 32, st));
+        }
+        work = P->prof.d_work + (8 + NR) * 32;
+    }
     k_long<real, NR, RPC><<<(unsigned)blocks, RPC * 32, smem, st>>>(fo ? P->d_long_f : P->d_long, c0,
                                                                     fo ? P->d_long_lits_f : P->d_long_lits,
                                                                     fo ? P->d_long_slots_f : P->d_long_slots, XT,
-                                                                    Bp, scratch, sat, fe, LS, QS);
+                                                                    Bp, scratch, sat, fe, LS, QS, work);
     P->last_launches++;
     return AFS_OK;
 }

@@ -348,6 +348,12 @@ def test_profile_read_times_every_kernel_class_of_a_run(afs):
     prof = P.profile_read()
     assert prof["var"][1] == 3 and prof["var"][0] > 0          # iterations 0, 2, 4
     assert any(k.startswith("long") for k in prof) and "resident" not in prof
+    fl = P.profile_flops()                                     # counted by the long kernels of the timed launches
+    assert fl and all(k.startswith("long") and v > 0 for k, v in fl.items())
+    # never more than the state-independent 6 L K of the constraints, summed over restarts and timed launches
+    lens = inst.lengths()[inst.lengths() > 64].astype(float)
+    assert sum(fl.values()) <= 6 * (lens * (lens / 2 + 2)).sum() * inst.B * 3
+    assert P.profile_flops() == {}
     assert P.profile_read() == {}                              # spans are consumed
     P.set_option(1, 0)
     X2 = dev(inst.X0)
