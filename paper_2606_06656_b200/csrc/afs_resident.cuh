@@ -50,7 +50,7 @@ struct STile {   // scratch[tile][slot][32] in global memory
 template <typename real>
 struct ResArgs {
     int n, steps, C, Bp, ntile;
-    int cm_bufs, cm_rows;        // pmf buffers of the CTA (warps 0..cm_bufs-1 own one), rows (cm_maxL + 1) of each
+    int cm_bufs, cm_rows;        // pmf buffers of the CTA (the cm_bufs highest warps own one), rows (cm_maxL + 1) of each
     int meta;                    // bit 0: the rank's small index streams (runs, offsets, push-item literals) are staged
                                  // in shared memory at kernel start; bit 1: its pull words too (cap_words > 0)
     int cap_words, cap_runs, cap_own, cap_plits, cap_cm, cap_push;   // capacities of the staged arrays (max over ranks)
@@ -122,8 +122,8 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
     uint2* sbuf0 = reinterpret_cast<uint2*>(S + ((2 * n + 3) & ~3));     // 16-byte aligned
     uint2* sbuf = sbuf0 + warp * PULL_SBUF;
     real* qbase = reinterpret_cast<real*>(sbuf0 + RES_WARPS * PULL_SBUF);
-    // pmf buffers belong to the HIGHEST warp ids: the issue arbiter favours them, and the EK / CARD items are the
-    // longest dependent chains of the iteration
+    // pmf buffers belong to the highest warp ids, three per scheduler when there are twelve (the EK / CARD items are
+    // the longest dependent chains of the iteration; which warp ids own them made no measurable difference)
     const int cmw = RES_WARPS - 1 - warp;
     real* qcol = qbase + (size_t)(cmw < a.cm_bufs ? cmw : 0) * a.cm_rows * 32 + lane;
     // staged index streams of this rank (a.meta): pull words and runs of the own variables, their stream offsets,
