@@ -111,14 +111,19 @@ def algorithmic_work(inst):
 
 def load_traffic(workload, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, copied from an
-    `ncu --set full` capture into profiles/traffic.json (the capture and its command are named there); else None."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+    `ncu --set full` capture into profiles/traffic.csv (the capture and its command are named there); else None."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(path):
         return None
     try:
-        return json.load(open(path)).get(workload, {}).get(kernel, {}).get("dram_bytes_per_launch")
+        import csv
+        with open(path, newline="") as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload and row["kernel"] == kernel:
+                    return int(row["dram_bytes_per_launch"])
     except Exception:
         return None
+    return None
 
 
 def load_peaks():
