@@ -371,6 +371,45 @@ def test_profile_read_times_every_kernel_class_of_a_run(afs):
     P.close()
 
 
+def test_fixed_variables_folded_on_device_equal_a_hand_folded_instance(afs):
+    """k_long_fold (literals of the run's fixed variables leave the long constraints, k drops by the fixed true ones)
+    against the same folding done by hand on the host: identical fp64 trajectories and counts."""
+    import torch
+    rng = np.random.default_rng(11)
+    n = 500
+    rows, types, ks = [], [], []
+    for L in (70, 96, 128, 129, 200, 257, 300, 420):
+        for ty in (W.AFS_CARD, W.AFS_EK):
+            v = rng.choice(n, size=L, replace=False)
+            sg = 1 - 2 * rng.integers(0, 2, size=L)
+            rows.append((sg * (v + 1)).astype(np.int32)); types.append(ty); ks.append(int(rng.integers(L // 4, 3 * L // 4)))
+    mask = np.zeros(n, np.int8)
+    fix = rng.choice(n, size=n // 2, replace=False)
+    mask[fix] = 1 - 2 * rng.integers(0, 2, size=fix.size)
+    frows, fks = [], []
+    for lits, ty, k in zip(rows, types, ks):
+        mv = mask[np.abs(lits) - 1].astype(int)
+        ftrue = int(np.sum((mv != 0) & ((mv < 0) != (lits < 0))))
+        keep = lits[mv == 0]
+        k2 = k - ftrue
+        if ty == W.AFS_CARD:
+            k2 = min(max(k2, 0), len(keep) + 1)
+        elif k2 < 0 or k2 > len(keep):
+            k2 = len(keep) + 1                                   # EK that cannot hold any more
+        frows.append(keep); fks.append(k2)
+    a = W.generate._pack("fold_a", n, rows, types, ks, None, 11)
+    b = W.generate._pack("fold_b", n, frows, types, fks, None, 11)
+    X0 = rng.uniform(-1, 1, (21, n))
+    Pa, Pb = afs.Problem.from_instance(a), afs.Problem.from_instance(b)
+    Xa, Xb = dev(X0), dev(X0)
+    oa = Pa.pgd_run(Xa, 15, 0.1, mask=dev(mask))
+    ob = Pb.pgd_run(Xb, 15, 0.1, mask=dev(mask))
+    assert (Xa - Xb).abs().max().item() < 1e-10
+    assert torch.equal(oa["best_sat"], ob["best_sat"]) and torch.equal(oa["best_step"], ob["best_step"])
+    assert torch.equal(oa["best_assign"], ob["best_assign"])
+    Pa.close(); Pb.close()
+
+
 def test_host_entry_point_equals_device_entry_point(afs):
     import torch
     inst = case_long(10)
