@@ -483,6 +483,28 @@ def test_duplicate_constraints_equal_doubled_step_fp64_build(afs):
     Pa.close(); Pb.close()
 
 
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
+def test_full_size_instances_fp64_trajectory_20_steps_on_sampled_restarts(afs, cfg):
+    """BASELINE.json: "first-20-step PGD trajectories within 1e-3 in an fp64 verification build", on the full-size
+    instances; the oracle runs the sampled restarts one by one (8 restarts x 20 steps; the sample is the first 8)."""
+    import torch
+    inst = W.config(cfg)
+    nb = 8
+    X0 = inst.X0[:nb].astype(np.float64)
+    P = afs.Problem.from_instance(inst)
+    mask = None if inst.mask is None else dev(inst.mask)
+    X = dev(X0, torch.float64)
+    out = P.pgd_run(X, 20, LR, mask=mask)
+    torch.cuda.synchronize()
+    o = ref.pgd_run(inst, X0, 20, LR, mask=inst.mask)
+    d = np.abs(X.cpu().numpy() - o["X"]).max()
+    assert d <= 1e-3, d
+    assert d <= 1e-8, d                              # what the arithmetic actually delivers
+    assert np.array_equal(out["best_sat"].cpu().numpy(), o["best_sat"])
+    assert np.array_equal(out["best_step"].cpu().numpy(), o["best_step"])
+    P.close()
+
+
 # ------------------------------------------------------------------------------------------------ full BASELINE.json sizes
 FULL = {0: dict(sample=64, steps=200), 1: dict(sample=48, steps=500), 2: dict(sample=48, steps=1000),
         3: dict(sample=24, steps=300), 4: dict(sample=4, steps=20)}
