@@ -319,7 +319,8 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
     real* Rc = RcAll + warp * LS;
     real* Aw = AAll + warp * QS;
     uint16_t* inv = InvAll + warp * LS;
-    // ---- lists: [B interior, pad | A interior, pad | A boundary | B boundary]
+    // ---- lists: [B interior, pad | A interior, pad]; the boundary literals share two slots behind them (send: y = +1,
+    // send + 1: y = -1), because all literals of one kind get the same gradient
     int nBr = 0, nAr = 0, nA0 = 0;
     for (int j0 = 0; j0 < L; j0 += 32) {
         const int j = j0 + lane;
@@ -334,23 +335,20 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
     const int nBr4 = (nBr + 3) & ~3, nAr4 = (nAr + 3) & ~3, send = nBr4 + nAr4, Leff = nBr + nAr;
     {
         const unsigned lt = (1u << lane) - 1u;
-        int pBr = 0, pAr = nBr4, pA0 = send, pB0 = send + nA0;
+        int pBr = 0, pAr = nBr4;
         for (int j0 = 0; j0 < L; j0 += 32) {
             const int j = j0 + lane;
             const bool act = j < L;
             const real rs = Aw[act ? j : 0];
             const bool isB = signbit(rs), intr = rs != real(0);
-            const bool cBr = act && isB && intr, cAr = act && !isB && intr, cA0 = act && !isB && !intr,
-                       cB0 = act && isB && !intr;
-            const unsigned mBr = __ballot_sync(FULLM, cBr), mAr = __ballot_sync(FULLM, cAr),
-                           mA0 = __ballot_sync(FULLM, cA0), mB0 = __ballot_sync(FULLM, cB0);
-            int pos = cBr ? pBr + __popc(mBr & lt) : cAr ? pAr + __popc(mAr & lt)
-                    : cA0 ? pA0 + __popc(mA0 & lt) : pB0 + __popc(mB0 & lt);
+            const bool cBr = act && isB && intr, cAr = act && !isB && intr;
+            const unsigned mBr = __ballot_sync(FULLM, cBr), mAr = __ballot_sync(FULLM, cAr);
+            const int pos = cBr ? pBr + __popc(mBr & lt) : cAr ? pAr + __popc(mAr & lt) : send + (isB ? 1 : 0);
             if (act) {
                 inv[j] = (uint16_t)pos;
                 if (intr) Rc[pos] = fabs(rs);
             }
-            pBr += __popc(mBr); pAr += __popc(mAr); pA0 += __popc(mA0); pB0 += __popc(mB0);
+            pBr += __popc(mBr); pAr += __popc(mAr);
         }
         if (lane < nBr4 - nBr) Rc[nBr + lane] = real(0);
         if (lane < nAr4 - nAr) Rc[nBr4 + nAr + lane] = real(0);
@@ -438,7 +436,7 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
         auto qat = [&](int tau) -> real { return (tau >= 0 && tau <= Leff) ? qr[tau] : real(0); };
         const real gA0 = w1 * qat(t1 - nB0) + w2 * qat(t2 - nB0);
         const real gB0 = w1 * qat(t1 + 1 - nB0) + w2 * qat(t2 + 1 - nB0);
-        for (int e = lane; e < nA0 + nB0; e += 32) Rc[send + e] = e < nA0 ? gA0 : gB0;
+        if (lane < 2) Rc[send + lane] = lane == 0 ? gA0 : gB0;
     }
     // interior literals: q^(-j)_t = qred^(-j)_{t - nB0}, qred^(-j) has degree Leff - 1
     int c1 = t1 - nB0, c2 = t2 - nB0;

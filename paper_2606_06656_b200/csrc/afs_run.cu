@@ -197,7 +197,7 @@ static afs_status launch_long(afs_problem* P, int bucket, const real* XT, int Bp
 {
     if (P->long_begin[bucket + 1] <= P->long_begin[bucket]) return AFS_OK;
     int Lmax = P->long_maxL[bucket];
-    int LS = ((Lmax + 6 + 31) / 32) * 32;            // list order: L entries + at most 6 neutral ones
+    int LS = ((Lmax + 8 + 31) / 32) * 32;            // list order: L entries + at most 6 neutral ones + 2 boundary slots
     int QS = ((Lmax + 1 + 3 + 3) / 4) * 4 + 4;       // pmf q_0..q_L behind an offset of at most 3
     const size_t per_restart = (size_t)LS * (sizeof(real) + sizeof(uint16_t)) + (size_t)QS * sizeof(real);
     // restarts per CTA: 8 keeps whole 32-byte sectors in the gather (fp32); 4 packs more warps per SM for the longest rows
