@@ -270,7 +270,10 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
         if (lng.empty()) {
             std::vector<double> vcost(n);
             for (int v = 0; v < n; ++v)
-                vcost[v] = 6.0 * (pull_ptr[v + 1] - pull_ptr[v]) + 2.0 * (slot_ptr[v + 1] - slot_ptr[v]) + 24.0;
+                // warp-instructions, from the source-level counts of the resident kernel: ~10 per staged pull word,
+                // ~30 per run, ~60 per variable, plus the P3 share (~8 per gradient row)
+                vcost[v] = 10.0 * (pull_ptr[v + 1] - pull_ptr[v]) + 30.0 * (run_ptr[v + 1] - run_ptr[v]) +
+                           8.0 * (slot_ptr[v + 1] - slot_ptr[v]) + 60.0;
             struct It { double cost; ResItem it; bool cm; };
             std::vector<It> its;
             for (size_t i = 0; i < med.size(); ++i) {
@@ -279,7 +282,8 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
             for (size_t i = 0; i < cmv.size(); ++i) {
                 const double L = cmv[i].L;
                 const double chain = std::max({(double)cmv[i].tA, (double)cmv[i].tB, L - 1 - cmv[i].tA, L - 1 - cmv[i].tB}) + 1;
-                its.push_back({2.0 * L * L + L * (40.0 + 4.0 * chain), ResItem{0u, (uint32_t)i}, true});
+                // forward pmf ~4.2 per cell (L^2 / 2 cells), chains ~5 per step and pair of literals, ~50 per literal
+                its.push_back({2.1 * L * L + L * (50.0 + 2.5 * chain), ResItem{0u, (uint32_t)i}, true});
             }
             std::stable_sort(its.begin(), its.end(), [](const It& x, const It& y) { return x.cost > y.cost; });
             for (int pi = 0; pi < RES_PLANS; ++pi) {
