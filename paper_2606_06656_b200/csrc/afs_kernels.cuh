@@ -9,7 +9,7 @@
 namespace afs {
 
 constexpr unsigned FULL = 0xffffffffu;
-constexpr int VAR_WARPS = 8;   // warps per CTA in the variable pass
+constexpr int VAR_WARPS = 4;   // warps per CTA in the variable pass (8 CTAs per SM; measured 2-3 % ahead of 8 warps x 4 CTAs)
 constexpr int VAR_VPW = 4;     // consecutive variables per warp
 
 // Is the constraint true when t of its L literals are true?  (Table 2; XOR parity k, G2)
@@ -655,10 +655,10 @@ __device__ __forceinline__ void pull_variable(const uint32_t* __restrict__ runs,
     for (int c = 0; c < RPL; ++c) g[c] += acc[c];
 }
 
-// 4 CTAs (32 warps) per SM at <= 64 registers: the pass waits on L2 gathers, and occupancy is what hides them -- at
+// 32 warps per SM at <= 64 registers: the pass waits on L2 gathers, and occupancy is what hides them -- at
 // 95 registers (2 CTAs per SM) the same code took 1.5x as long on configs[3] (measured: 420 -> 274 us per iteration).
 template <typename real, bool EVAL, int RPL>
-__global__ void __launch_bounds__(VAR_WARPS * 32, 4) k_var(const VarArgs<real> a)
+__global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const VarArgs<real> a)
 {
     __shared__ __align__(16) uint2 s_stage[VAR_WARPS][PULL_SBUF];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
