@@ -555,7 +555,9 @@ __device__ __forceinline__ void pull_run(const uint32_t* __restrict__ words, int
     // slower at the same register count (configs[3]: 272 -> 320 us per iteration with twice the batch): their tails
     // gather rows that are discarded, and occupancy already hides the latency (see k_var)
     constexpr int U0 = NOTHER <= 2 ? 4 : 2;
-    constexpr int U = U0 / RPL >= 1 ? U0 / RPL : 1;
+    // one sub-tile per lane (the resident kernel): four occurrences per batch whatever their length -- fewer, longer
+    // loop bodies (configs[1]: 80.6 -> 67.3 us per iteration against 2 for the 3- and 4-literal runs; 8/5/4: 69.9)
+    constexpr int U = RPL == 1 ? 4 : (U0 / RPL >= 1 ? U0 / RPL : 1);
     real g[RPL];
 #pragma unroll
     for (int c = 0; c < RPL; ++c) g[c] = real(0);
