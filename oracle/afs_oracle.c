@@ -253,18 +253,27 @@ static int check_instance(int n, int64_t m, const int64_t *row_ptr, const int32_
                           const int32_t *types, const int32_t *k)
 {
     if (n < 1 || m < 0) return -1;
-    for (int64_t c = 0; c < m; ++c) {
+    /* G8: the multilinear expansion assumes distinct variables inside a constraint, so the
+     * same variable twice is rejected.  seen[v] = 1 + the last constraint that used variable v. */
+    int64_t *seen = (int64_t *)calloc((size_t)n, sizeof(int64_t));
+    if (!seen) return -1;
+    int bad = 0;
+    for (int64_t c = 0; c < m && !bad; ++c) {
         int64_t L = row_ptr[c + 1] - row_ptr[c];
-        if (L < 1 || types[c] < 0 || types[c] > 6) return -1;
-        if (types[c] == ORC_NAE && L < 2) return -1;                    /* G6 */
-        if ((types[c] == ORC_EK || types[c] == ORC_CARD) && (k[c] < 0 || k[c] > L + 1)) return -1;
-        if (types[c] == ORC_XOR && (k[c] < 0 || k[c] > 1)) return -1;
+        if (L < 1 || types[c] < 0 || types[c] > 6) { bad = 1; break; }
+        if (types[c] == ORC_NAE && L < 2) { bad = 1; break; }            /* G6 */
+        if ((types[c] == ORC_EK || types[c] == ORC_CARD) && (k[c] < 0 || k[c] > L + 1)) { bad = 1; break; }
+        if (types[c] == ORC_XOR && (k[c] < 0 || k[c] > 1)) { bad = 1; break; }
         for (int64_t e = row_ptr[c]; e < row_ptr[c + 1]; ++e) {
             int32_t l = lits[e];
-            if (l == 0 || l > n || l < -n) return -1;
+            if (l == 0 || l > n || l < -n) { bad = 1; break; }
+            int32_t v = (l < 0 ? -l : l) - 1;
+            if (seen[v] == c + 1) { bad = 1; break; }                    /* G8 */
+            seen[v] = c + 1;
         }
     }
-    return 0;
+    free(seen);
+    return bad ? -1 : 0;
 }
 
 static int eval_one(int n, int64_t m, const int64_t *row_ptr, const int32_t *lits,

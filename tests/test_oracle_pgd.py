@@ -121,3 +121,19 @@ def test_evaluators_give_the_same_trajectory():
     t1 = ref.pgd_run(inst, inst.X0, 10, LR, evaluator=1, want_traj=True)["traj"]
     t2 = ref.pgd_run(inst, inst.X0, 10, LR, evaluator=2, want_traj=True)["traj"]
     assert np.abs(t0 - t1).max() < 1e-12 and np.abs(t1 - t2).max() < 1e-12
+
+
+def test_same_variable_twice_in_one_constraint_is_rejected():
+    # G8: the multilinear expansion assumes distinct variables; the oracle refuses, like afs_problem_create
+    ok = W.Instance("ok", 4, np.array([0, 3, 5], np.int64), np.array([1, -2, 3, 2, -4], np.int32),
+                    np.array([W.AFS_OR, W.AFS_XOR], np.int32), np.array([0, 1], np.int32))
+    X = np.zeros((1, 4))
+    ref.eval_grad(ok, X)                                       # the same variable in two constraints is fine
+    for lits in ([1, -2, 1, 2, -4], [1, -2, -1, 2, -4], [1, -2, 3, 4, -4]):
+        bad = W.Instance("dup", 4, ok.row_ptr.copy(), np.array(lits, np.int32), ok.types.copy(), ok.k.copy())
+        with pytest.raises(ValueError):
+            ref.eval_grad(bad, X)
+        with pytest.raises(ValueError):
+            ref.round_count(bad, X)
+        with pytest.raises(ValueError):
+            ref.pgd_run(bad, X, 1, LR)
