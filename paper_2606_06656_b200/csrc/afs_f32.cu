@@ -1,0 +1,12 @@
+// afs_f32.cu -- the fp32 device entry points of include/afs.h (the product path)
+#include "afs_run.cuh"
+
+using namespace afs;
+
+extern "C" afs_status afs_eval_grad(afs_problem* p, const float* X, int32_t B, float* F, float* G, void* stream)
+{ return eval_grad_impl<float>(p, X, B, F, G, stream); }
+extern "C" afs_status afs_round_count(afs_problem* p, const float* X, int32_t B, int8_t* assign, int32_t* sat, void* stream)
+{ return round_count_impl<float>(p, X, B, assign, sat, stream); }
+extern "C" afs_status afs_pgd_run(afs_problem* p, float* X, int32_t B, int32_t steps, float lr, const int8_t* mask,
+                                  int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
+{ return pgd_run_impl<float>(p, X, B, steps, lr, mask, best_assign, best_sat, best_step, stream); }

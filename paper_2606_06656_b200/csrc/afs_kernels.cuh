@@ -4,7 +4,6 @@
 // BASELINE.json.  P:Lnn = PAPER.md line nn.
 #pragma once
 #include "afs_internal.h"
-#include "afs_long.cuh"
 
 namespace afs {
 
@@ -968,10 +967,5 @@ __global__ void __launch_bounds__(256) k_finalize(const FinArgs<real> a)
     }
 }
 
-__global__ void k_fill_i32(int32_t* p, size_t n, int32_t v)
-{
-    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) p[i] = v;
-}
 
 }  // namespace afs

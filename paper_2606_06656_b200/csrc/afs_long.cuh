@@ -203,49 +203,6 @@ __device__ __forceinline__ bool long_pred(int type, int L, int k, int t)
     }
 }
 
-// Folding of the run's fixed variables (G16), once per afs_pgd_run with a mask: a literal of a fixed
-// variable is a constant of the run -- true or false for every restart and every iteration -- so it leaves the list,
-// a fixed true one lowers k by one, and the gradient row of its slot is never read (a fixed variable does not move).
-// warp = constraint; the compacted lists keep the constraint's offset.  EK / CARD only (the LONG class).
-__global__ void __launch_bounds__(128) k_long_fold(const LongCon* __restrict__ cons, const uint32_t* __restrict__ lits,
-                                                   const int32_t* __restrict__ slots, int n_long,
-                                                   const int8_t* __restrict__ mask, LongCon* __restrict__ cons_f,
-                                                   uint32_t* __restrict__ lits_f, int32_t* __restrict__ slots_f)
-{
-    const int lane = threadIdx.x & 31;
-    const int c = blockIdx.x * 4 + (threadIdx.x >> 5);
-    if (c >= n_long) return;
-    LongCon lc = cons[c];
-    const unsigned lt = (1u << lane) - 1u;
-    int out = 0, ftrue = 0;
-    for (int j0 = 0; j0 < lc.L; j0 += 32) {
-        const int j = j0 + lane;
-        const bool act = j < lc.L;
-        const uint32_t w = act ? lits[lc.off + j] : 0u;
-        const int mk = act ? (int)mask[w & LIT_VAR] : 0;
-        const bool fixed = act && mk != 0;
-        const bool keep = act && !fixed;
-        ftrue += __popc(__ballot_sync(0xffffffffu, fixed && ((mk < 0) != ((w >> 31) != 0))));   // True is -1
-        const unsigned m = __ballot_sync(0xffffffffu, keep);
-        if (keep) {
-            const int pos = out + __popc(m & lt);
-            lits_f[lc.off + pos] = w;
-            slots_f[lc.off + pos] = slots[lc.off + j];
-        }
-        out += __popc(m);
-    }
-    if (lane == 0) {
-        lc.L = out;
-        lc.k -= ftrue;
-        lc.tA = lc.tB = 0;
-        lc.wA = lc.wB = 0.f;
-        // d_t of P:L52 on the folded constraint: CARD >= k: +1 at k-1;  EK: +1 at k-1, -1 at k (indices 0..L-1 only)
-        if (lc.k - 1 >= 0 && lc.k - 1 <= out - 1) { lc.tA = lc.k - 1; lc.wA = 1.f; }
-        if (lc.type == AFS_EK && lc.k >= 0 && lc.k <= out - 1) { lc.tB = lc.k; lc.wB = -1.f; }
-        cons_f[c] = lc;
-    }
-}
-
 template <typename real, int NR, int RPC>
 __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ cons, int c_begin,
                                                    const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,

@@ -29,10 +29,7 @@ namespace afs {
 
 namespace cg = cooperative_groups;
 
-#ifndef AFS_RES_WARPS
-#define AFS_RES_WARPS 32
-#endif
-constexpr int RES_WARPS = AFS_RES_WARPS;
+constexpr int RES_WARPS = 32;
 constexpr int RES_VCH = 1;   // variables per work item (measured on configs[1]: 1 -> 80.4, 2 -> 84.1, 4 -> 83.1 us/iteration)
 
 template <typename real>
@@ -96,14 +93,6 @@ struct ResMed {   // staged MED item: the constraint record and its bucket
     uint32_t code;
 };
 
-#ifdef AFS_RES_TIMING   // development aid (never defined in the product build): per-warp phase clocks of one iteration
-__device__ long long g_res_timing[256 * RES_WARPS * 8];
-#define AFS_T(slot) do { if (t == 5 && lane == 0 && blockIdx.x < 256) g_res_timing[(blockIdx.x * RES_WARPS + warp) * 8 + (slot)] = clock64(); } while (0)
-#define AFS_T6(slot) do { if (t == 6 && lane == 0 && blockIdx.x < 256) g_res_timing[(blockIdx.x * RES_WARPS + warp) * 8 + (slot)] = clock64(); } while (0)
-#else
-#define AFS_T(slot) do { } while (0)
-#define AFS_T6(slot) do { } while (0)
-#endif
 
 template <typename real>
 __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<real> a)
@@ -211,8 +200,6 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
         {
             int satcnt = 0;
             const int total = n_push + n_cnt + (last ? 0 : n_var);
-            AFS_T(0);
-            AFS_T6(7);
             if (cmw < a.cm_bufs) {   // EK / CARD constraints first (the heaviest items), by the warps that own a pmf buffer
                 for (;;) {
                     int it = 0;
@@ -225,7 +212,6 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
                     const int32_t* ls = a.meta ? sms + smo[it] : a.cm_slots + lc.off;
                     cm_body<real>(lc, lw, ls, xl, sw, qcol, satcnt, fe, false);
                 }
-                AFS_T(2);
             }
             for (;;) {
                 int it = 0;
@@ -277,9 +263,7 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
             }
             if (satcnt) atomicAdd(a.sat_hist + (size_t)t * a.Bp + b, satcnt);
         }
-        AFS_T(1);
         cluster.sync();
-        AFS_T(3);
         if (tid == 0) { s_ctr = 0; s_ctr_cm = 0; }
         // ---- S10: iterate t against the best so far (rank 0 holds the record of the tile)
         if (rank == 0) {
@@ -346,9 +330,7 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
                 XTt[(size_t)v[h] * 32] = xn;
             }
         }
-        AFS_T(4);
         cluster.sync();
-        AFS_T(5);
         // ---- P4: the record of iterate t, then X_{t+1} and its sign words
         if (rank == 0 && warp == 0) {
             const int sp = __ldcg(a.sat_hist + (size_t)t * a.Bp + b);

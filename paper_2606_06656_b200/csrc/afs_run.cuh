@@ -1,0 +1,320 @@
+// afs_run.cuh -- launch orchestration of the device entry points of include/afs.h, templated on the arithmetic type;
+// instantiated by afs_f32.cu (the product) and afs_f64.cu (the fp64 verification build).
+// Streaming path: per PGD step one launch per non-empty push bucket (medium / long constraints) plus one fused
+// variable pass; no host round trip inside the loop (everything is enqueued on the caller's stream).
+#pragma once
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+
+#include "afs_kernels.cuh"
+#include "afs_resident.cuh"
+#include "afs_launch.h"
+
+namespace afs {
+
+static int var_grid_x(int n) { return (n + VAR_WARPS * VAR_VPW - 1) / (VAR_WARPS * VAR_VPW); }
+
+// variable pass: as many 32-restart sub-tiles per lane as the batch allows (4, 2 or 1)
+template <typename real, bool EVAL>
+static void launch_var(const VarArgs<real>& a, int gx, int tiles, cudaStream_t st)
+{
+    if (sizeof(real) == 4 && tiles % 4 == 0) k_var<real, EVAL, 4><<<dim3(gx, tiles / 4), VAR_WARPS * 32, 0, st>>>(a);
+    else if (tiles % 2 == 0) k_var<real, EVAL, 2><<<dim3(gx, tiles / 2), VAR_WARPS * 32, 0, st>>>(a);
+    else k_var<real, EVAL, 1><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
+}
+
+// ----------------------------------------------------------------------------------------------------------------
+// push phase: gradients of the medium and long constraints of iterate XT into scratch (+ counts, + FE)
+// ----------------------------------------------------------------------------------------------------------------
+template <typename real>
+static afs_status launch_push(afs_problem* P, const real* XT, int Bp, real* scratch, int32_t* sat, real* fe_med,
+                              real* fe_cm, real* fe_long, cudaStream_t st)
+{
+    const int tiles = Bp / 32;
+    if (P->n_cm > 0) {
+        const int c0 = 0, c1 = (int)P->n_cm;
+        int gx = (c1 - c0 + 3) / 4;
+        int cap = (P->sm_count * 16 + tiles - 1) / tiles;
+        if (gx > cap) gx = cap < 1 ? 1 : cap;
+        const int qrows = P->cm_maxL + 1;
+        const size_t smem = (size_t)4 * qrows * 32 * sizeof(real);
+        // kernel attributes are per device and per instantiation: set before every launch (cheap), never cached
+        if (smem > 48 * 1024)
+            CU(cudaFuncSetAttribute(k_cmed<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ProfSpan span(P, 3, st);
+        k_cmed<real><<<dim3(gx, tiles), 128, smem, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat,
+                                                        fe_cm, qrows);
+        P->last_launches++;
+    }
+    if (P->n_med > 0) {
+        int gx = ((int)P->n_med + 3) / 4;
+        int cap = (P->sm_count * 16 + tiles - 1) / tiles;   // enough CTAs to fill the chip, grid-stride beyond
+        if (gx > cap) gx = cap < 1 ? 1 : cap;
+        ProfSpan span(P, 4, st);
+        k_med<real><<<dim3(gx, tiles), 128, 0, st>>>(P->d_med, 0, (int)P->n_med, P->d_med_lits, P->d_med_slots, XT, Bp, scratch,
+                                                    (real*)P->ws.aux[0], (real*)P->ws.aux[1], sat, fe_med);
+        P->last_launches++;
+    }
+    if (P->n_long > 0) return launch_long_all<real>(P, XT, Bp, scratch, sat, fe_long, st);
+    return AFS_OK;
+}
+
+template <typename real>
+static afs_status launch_count(afs_problem* P, const real* XT, int Bp, int32_t* sat, cudaStream_t st)
+{
+    CU(cudaMemsetAsync(sat, 0, (size_t)Bp * sizeof(int32_t), st));
+    if (P->m > 0) {
+        const int tiles = Bp / 32;
+        int gx = (P->m + 7) / 8;
+        int cap = (P->sm_count * 8 + tiles - 1) / tiles;
+        if (gx > cap) gx = cap < 1 ? 1 : cap;
+        ProfSpan span(P, 18, st);
+        k_count<real><<<dim3(gx, tiles), 256, 0, st>>>(P->d_count, P->d_count_lits, P->m, XT, Bp, sat);
+        P->last_launches++;
+    }
+    return AFS_OK;
+}
+
+// ----------------------------------------------------------------------------------------------------------------
+template <typename real>
+static afs_status eval_grad_impl(afs_problem* P, const real* X, int32_t B, real* F, real* G, void* stream)
+{
+    afs_status s = enter(P, B);
+    if (s != AFS_OK) return s;
+    if (!X) return AFS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int Bp = ((B + 31) / 32) * 32;
+    if ((s = ensure_workspace(P, Bp, sizeof(real), 2)) != AFS_OK) return s;
+    if ((s = ensure_eval_buffers(P, Bp, sizeof(real))) != AFS_OK) return s;
+    Workspace& w = P->ws;
+    const int wBp = Bp;   // kernels run on the first Bp columns with row stride Bp
+    real* XT = (real*)w.XT[0];
+    real* GT = (real*)w.XT[1];
+    real* scratch = (real*)w.scratch;
+    real* fe_med = (real*)w.fe_med; real* fe_long = (real*)w.fe_long; real* fe_cm = (real*)w.fe_cm;
+    real* fpart = (real*)w.f_part;
+    dim3 tg((P->n + 31) / 32, Bp / 32);
+    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, wBp, nullptr);
+    P->last_launches++;
+    if ((s = launch_push<real>(P, XT, wBp, scratch, nullptr, fe_med, fe_cm, fe_long, st)) != AFS_OK) return s;
+    VarArgs<real> a{};
+    a.n = P->n; a.Bp = wBp; a.t = 0;
+    a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
+    a.gconst = P->d_pull_gconst; a.slot_ptr = P->d_slot_ptr;
+    a.scratch = scratch; a.Xin = XT; a.Xout = nullptr; a.lr = real(0); a.mask = nullptr;
+    a.GT = GT;
+    const int gx = var_grid_x(P->n);
+    if (G) {
+        launch_var<real, true>(a, gx, Bp / 32, st);
+        P->last_launches++;
+    }
+    if (F) {
+        const int fgx = fe_pull_grid_x(P);
+        k_fe_pull<real><<<dim3(fgx, Bp / 32), 256, 0, st>>>(P->d_pc, P->d_pc_lits, (int)P->n_pull, XT, wBp, fpart);
+        k_reduce_F<real><<<(B + 127) / 128, 128, 0, st>>>(fpart, fgx * 8, fe_med, (int)P->n_med, fe_cm, (int)P->n_cm,
+                                                         fe_long, (int)P->n_long, wBp, B, F);
+        P->last_launches += 2;
+    }
+    if (G) {
+        k_transpose_out<real><<<tg, 256, 0, st>>>(GT, G, B, P->n, wBp);
+        P->last_launches++;
+    }
+    CU(cudaGetLastError());
+    return AFS_OK;
+}
+
+template <typename real>
+static afs_status round_count_impl(afs_problem* P, const real* X, int32_t B, int8_t* assign, int32_t* sat, void* stream)
+{
+    afs_status s = enter(P, B);
+    if (s != AFS_OK) return s;
+    if (!X || !sat) return AFS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int Bp = ((B + 31) / 32) * 32;
+    if ((s = ensure_workspace(P, Bp, sizeof(real), 2)) != AFS_OK) return s;
+    Workspace& w = P->ws;
+    real* XT = (real*)w.XT[0];
+    dim3 tg((P->n + 31) / 32, Bp / 32);
+    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, Bp, nullptr);
+    P->last_launches++;
+    if ((s = launch_count<real>(P, XT, Bp, w.sat_hist, st)) != AFS_OK) return s;
+    CU(cudaMemcpyAsync(sat, w.sat_hist, (size_t)B * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    if (assign) {
+        k_assign_out<real><<<tg, 256, 0, st>>>(XT, assign, B, P->n, Bp);
+        P->last_launches++;
+    }
+    CU(cudaGetLastError());
+    return AFS_OK;
+}
+
+// ----------------------------------------------------------------------------------------------------------------
+// tile-resident path: one launch for the whole run.  Eligible when no constraint needs the CTA-cooperative LONG
+// kernel and the tile X[n][32] plus the rank's gradient rows fit the 227 KB of shared memory.
+// ----------------------------------------------------------------------------------------------------------------
+constexpr size_t RES_SMEM_MAX = 227 * 1024 - 512;
+
+// Shared-memory layout of one CTA of the resident kernel for plan pi: the tile and its sign words always; then, as far
+// as the 227 KB go and in this order: the rank's small index streams (runs, stream offsets, literals of its push
+// items), pmf buffers for the EK / CARD bodies -- up to 12, or one per constraint of the rank if that is fewer: the
+// warps that own one carry the longest dependent chains of the iteration and must not be few -- and last the rank's
+// pull words (the largest stream; 32 warps hide its L2 latency when it stays in global memory).
+struct ResLayout { bool ok; int cm_bufs; int meta; int cap_words; size_t bytes; };
+template <typename real>
+static ResLayout resident_layout(const afs_problem* P, int pi)
+{
+    const ResPlan& rp = P->res[pi];
+    size_t used = res_smem_bytes<real>(P->n, 0, 0);
+    if (used > RES_SMEM_MAX) return {false, 0, 0, 0, 0};
+    const size_t per = P->n_cm > 0 ? (size_t)(P->cm_maxL + 1) * 32 * sizeof(real) : 0;
+    if (per != 0 && used + per > RES_SMEM_MAX) return {false, 0, 0, 0, 0};
+    int meta = 0, nb = 0, cap_words = 0;
+    const size_t small = res_meta_bytes(0, rp.cap_runs, rp.cap_own, rp.cap_plits, rp.cap_cm, rp.cap_push);
+    if (used + small + per <= RES_SMEM_MAX) { meta = 1; used += small; }
+    if (per != 0) {
+        const int want = std::min(RES_WARPS, std::min(12, std::max(rp.cap_cm, 1)));
+        nb = (int)std::min<size_t>((size_t)want, (RES_SMEM_MAX - used) / per);
+        used += (size_t)nb * per;
+    }
+    if (meta && used + 4 * (size_t)rp.cap_words <= RES_SMEM_MAX) { meta |= 2; cap_words = rp.cap_words; used += 4 * (size_t)cap_words; }
+    if (per != 0 && nb < RES_WARPS) {   // what is left goes to more pmf buffers
+        const int more = (int)std::min<size_t>((size_t)(RES_WARPS - nb), (RES_SMEM_MAX - used) / per);
+        nb += more; used += (size_t)more * per;
+    }
+    return {true, nb, meta, cap_words, used};
+}
+
+template <typename real>
+static int resident_plan(const afs_problem* P, int ntile)
+{
+    if (P->n_long > 0 || !P->res[0].d_var_begin) return -1;
+    int pi = RES_PLANS - 1;
+    while (pi > 0 && (long long)ntile * (1 << pi) > P->sm_count) --pi;
+    return resident_layout<real>(P, pi).ok ? pi : -1;
+}
+
+template <typename real>
+static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, int32_t steps, real lr,
+                                   const int8_t* mask, int8_t* best_assign, int32_t* best_sat, int32_t* best_step,
+                                   cudaStream_t st)
+{
+    Workspace& w = P->ws;
+    const int Bp = ((B + 31) / 32) * 32, ntile = Bp / 32;
+    const ResPlan& rp = P->res[pi];
+    real* XT = (real*)w.XT[0];
+    dim3 tg((P->n + 31) / 32, ntile);
+    k_res_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, mask);
+    CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)(steps + 1) * Bp * sizeof(int32_t), st));
+    ResArgs<real> a{};
+    a.n = P->n; a.steps = steps; a.C = rp.C; a.Bp = Bp; a.ntile = ntile; a.nslots = P->nslots;
+    const ResLayout lay = resident_layout<real>(P, pi);
+    a.cm_bufs = lay.cm_bufs; a.cm_rows = P->cm_maxL + 1; a.meta = lay.meta;
+    a.cap_words = lay.cap_words; a.cap_runs = rp.cap_runs; a.cap_own = rp.cap_own; a.cap_plits = rp.cap_plits;
+    a.cap_cm = rp.cap_cm; a.cap_push = rp.cap_push;
+    a.cm_begin = rp.d_cm_begin; a.cm_items = rp.d_cm_items;
+    a.G = (real*)w.XT[1];
+    a.aux0 = (real*)w.aux[0]; a.aux1 = (real*)w.aux[1]; a.med_nnz = P->med_nnz;
+    a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
+    a.gconst = P->d_pull_gconst; a.slot_ptr = P->d_slot_ptr;
+    a.med = P->d_med; a.med_lits = P->d_med_lits; a.med_slots = P->d_med_slots;
+    a.cm = P->d_cm; a.cm_lits = P->d_cm_lits; a.cm_slots = P->d_cm_slots;
+    a.pcp = P->d_pcp;
+    a.var_begin = rp.d_var_begin; a.item_begin = rp.d_item_begin; a.items = rp.d_items; a.pc_begin = rp.d_pc_begin;
+    a.XT = XT; a.scratch = (real*)w.scratch; a.sat_hist = w.sat_hist;
+    a.best_bits = w.best_bits; a.best_sat = w.best_sat[0]; a.best_step = w.best_step[0];
+    a.lr = lr; a.mask = mask;
+    const size_t smem = lay.bytes;
+    CU(cudaFuncSetAttribute(k_resident<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RES_SMEM_MAX));
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(ntile * rp.C));
+    cfg.blockDim = dim3(RES_WARPS * 32);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)rp.C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    P->prof.on = P->prof.stride > 0;
+    {
+        ProfSpan span(P, 0, st);
+        CU(cudaLaunchKernelEx(&cfg, k_resident<real>, a));
+    }
+    P->prof.on = false;
+    k_res_out<real><<<tg, 256, 0, st>>>(XT, w.best_bits, w.best_sat[0], w.best_step[0], B, P->n, ntile, X, best_assign,
+                                        best_sat, best_step);
+    P->last_launches += 3;
+    P->last_resident = 1;
+    CU(cudaGetLastError());
+    return AFS_OK;
+}
+
+template <typename real>
+static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps, real lr, const int8_t* mask,
+                               int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
+{
+    afs_status s = enter(P, B);
+    if (s != AFS_OK) return s;
+    if (!X || steps < 0 || !std::isfinite((double)lr)) return AFS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int Bp = ((B + 31) / 32) * 32;
+    const int plan = P->opt_mode == 1 ? -1 : resident_plan<real>(P, Bp / 32);
+    if (P->opt_mode == 2 && plan < 0) return AFS_ERR_UNSUPPORTED;
+    if ((s = ensure_workspace(P, Bp, sizeof(real), (int64_t)steps + 1)) != AFS_OK) return s;
+    Workspace& w = P->ws;
+    P->last_resident = 0;
+    if (plan >= 0) return pgd_run_resident<real>(P, plan, X, B, steps, lr, mask, best_assign, best_sat, best_step, st);
+    real* XT[2] = {(real*)w.XT[0], (real*)w.XT[1]};
+    real* scratch = (real*)w.scratch;
+    const int tiles = Bp / 32;
+    dim3 tg((P->n + 31) / 32, tiles);
+    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT[0], B, P->n, Bp, mask);
+    P->last_launches++;
+    CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)(steps + 1) * Bp * sizeof(int32_t), st));
+    launch_fill_i32(w.best_sat[0], (size_t)Bp, -1, st);
+    CU(cudaMemsetAsync(w.best_step[0], 0, (size_t)Bp * sizeof(int32_t), st));
+    P->last_launches++;
+    const int gx = var_grid_x(P->n);
+    if (mask && P->n_long > 0 && steps > 0) {   // the fixed variables' literals leave the long constraints for this run
+        if ((s = launch_long_fold(P, mask, st)) != AFS_OK) return s;
+    }
+    for (int t = 0; t < steps; ++t) {
+        P->prof.on = P->prof.stride > 0 && t % P->prof.stride == 0;
+        const real* Xin = XT[t & 1];
+        int32_t* sat_cur = w.sat_hist + (size_t)t * Bp;
+        if ((s = launch_push<real>(P, Xin, Bp, scratch, sat_cur, nullptr, nullptr, nullptr, st)) != AFS_OK) return s;
+        VarArgs<real> a{};
+        a.n = P->n; a.Bp = Bp; a.t = t;
+        a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
+        a.gconst = P->d_pull_gconst; a.slot_ptr = P->d_slot_ptr;
+        a.scratch = scratch; a.Xin = Xin; a.Xout = XT[(t + 1) & 1]; a.lr = lr; a.mask = mask;
+        a.sat_prev = t > 0 ? w.sat_hist + (size_t)(t - 1) * Bp : nullptr;
+        a.best_sat_in = w.best_sat[t & 1]; a.best_sat_out = w.best_sat[(t + 1) & 1];
+        a.best_step_in = w.best_step[t & 1]; a.best_step_out = w.best_step[(t + 1) & 1];
+        a.S_prev = w.S[(t + 1) & 1]; a.S_cur = w.S[t & 1]; a.best_bits = w.best_bits;
+        {
+            ProfSpan span(P, 1, st);
+            launch_var<real, false>(a, gx, tiles, st);
+        }
+        P->last_launches++;
+        if ((s = launch_sat_pull(P, w.S[t & 1], Bp, sat_cur, st)) != AFS_OK) return s;
+    }
+    P->prof.on = false;
+    P->long_folded = false;
+    // the last iterate: count only, then fold and write out
+    const real* Xfin = XT[steps & 1];
+    int32_t* sat_fin = w.sat_hist + (size_t)steps * Bp;
+    if ((s = launch_count<real>(P, Xfin, Bp, sat_fin, st)) != AFS_OK) return s;
+    FinArgs<real> f{};
+    f.n = P->n; f.B = B; f.Bp = Bp; f.steps = steps; f.XT = Xfin;
+    f.sat_prev = steps >= 1 ? w.sat_hist + (size_t)(steps - 1) * Bp : nullptr;
+    f.sat_fin = sat_fin;
+    f.best_sat_in = w.best_sat[steps & 1]; f.best_step_in = w.best_step[steps & 1];
+    f.S_prev = w.S[(steps + 1) & 1]; f.best_bits = w.best_bits;
+    f.X = X; f.best_assign = best_assign; f.best_sat = best_sat; f.best_step = best_step;
+    k_finalize<real><<<tg, 256, 0, st>>>(f);
+    P->last_launches++;
+    CU(cudaGetLastError());
+    return AFS_OK;
+}
+
+}  // namespace afs
