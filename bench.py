@@ -3,6 +3,10 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl reference]
 
+Without --config the run times configs[1], [2], [3] and [4] of BASELINE.json one after the other in one process: the
+top-level line is the largest of them (configs[4], named in config.workload) and `per_config` carries value, e2e,
+roofline, cpu_baseline, ms_per_step and clocks of each.  --config I times that one configuration alone.
+
 A bench "step" is ONE afs_pgd_run call: the whole hot path (S1..S10 of DESIGN.md) over one batch of B restarts for
 the configuration's PGD iteration count.  metric = PGD restart-steps per second = B * pgd_iterations / time.
 `value` is measured with X0 already resident in HBM (CUDA events on the launching stream, max over ranks);
@@ -95,8 +99,10 @@ def algorithmic_work(inst):
         sel = cls == name
         if name == "var":
             continue
-        # gather X rows of the literals once + write one gradient per literal + the literal CSR
-        work[name] = (float(f[sel].sum()) * B, float(L[sel].sum()) * (B * 8 + 8))
+        # compulsory HBM bytes of a materialising kernel: every X element its literals touch once (at most the whole
+        # iterate) + its literal CSR.  Per-literal gradient rows are scratch traffic the design has to avoid
+        # (SURVEY.md 8(d)), not algorithmic bytes.
+        work[name] = (float(f[sel].sum()) * B, min(float(L[sel].sum()), float(inst.n)) * B * 4 + float(L[sel].sum()) * 8)
     pull = cls == "var"
     pushed = float(L[~pull].sum())
     # variable pass: pull clauses, one add per materialised literal gradient, 5 flops per variable for S7-S9;
@@ -132,6 +138,19 @@ def load_peaks():
         p = json.load(open(path))
         return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+_FP32_PEAK = {}
+
+
+def fp32_peak(device: int, peaks):
+    """(measured, derived) plain-FP32 FMA peak in TFLOP/s.  Measured: the library's own FMA micro-benchmark kernel
+    (afs_fp32_fma_peak: independent FFMA chains on every SM, best of 5, CUDA events) on this box, now; derived:
+    148 SMs x 128 lanes x 2 flop x sm_max_mhz, the upper bound the measured figure is checked against."""
+    if device not in _FP32_PEAK:
+        import paper_2606_06656_b200 as afs
+        _FP32_PEAK[device] = afs.fp32_fma_peak(device)
+    return _FP32_PEAK[device], 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
 
 
 # --------------------------------------------------------------------------------------------- clocks
@@ -209,7 +228,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    cfg = args.config
+    cfg = HEADLINE if args.config is None else args.config     # the workload the CUDA arm's headline names
     inst = W.config(cfg)
     from oracle import ref
     for _ in range(args.warmup):
@@ -234,28 +253,14 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------------------------- CUDA arm
-def run_cuda(args):
+def measure_config(cfg, args, afs, shard, rank, world, local, peaks):
+    """Time configs[cfg]: `value` (device-resident inputs, CUDA events), `e2e` (host buffers through afs_pgd_run_host),
+    the roofline of its dominant kernel and of the whole PGD iteration, and the oracle beside it.  Returns the JSON
+    line of that configuration (rank 0; other ranks return None after taking part in the collectives)."""
     import torch
     import torch.distributed as dist
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    from paper_2606_06656_b200 import build as afs_build
-    if rank == 0:
-        afs_build.build()
-    if world > 1:
-        dist.barrier()
-    import paper_2606_06656_b200 as afs
-
-    cfg = args.config
     inst = W.config(cfg)
-    from paper_2606_06656_b200 import shard
     if world > 1:   # every rank its own start points (weak scaling), same instance
         inst.X0 = shard.rank_start_points(W.BASE_SEED, cfg, rank, inst.X0.shape)
     pgd_steps = inst.steps if args.pgd_steps is None else args.pgd_steps
@@ -332,15 +337,13 @@ def run_cuda(args):
     d2h = inst.B * inst.n * 4 + inst.B * inst.n + 8 * inst.B
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return 0
+        P.close()
+        return None
 
     # ---- roofline of the dominant kernel: its launches timed live with CUDA events on the launching stream
     # (afs_set_option(1, stride) + afs_profile_read), in a second pass so that the events do not sit in `value`
-    peaks = load_peaks()
     work = algorithmic_work(inst)
-    fp32_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12          # TFLOP/s, DESIGN.md section 7
+    fp32_meas, fp32_derived = fp32_peak(local, peaks)
     stride = max(1, pgd_steps // 64)
     P.set_option(1, stride)
     prof, counted = {}, {}
@@ -356,25 +359,27 @@ def run_cuda(args):
     # actually see; the state-independent 6 L K stays beside it as `static_formula`.
     static_work = dict(work)
     for k, fl in counted.items():
-        if k in prof and prof[k][1] > 0:
+        if k in prof and prof[k][1] > 0 and k in work:
             work[k] = (fl / prof[k][1], work[k][1])
     if counted:
-        step_f = work["step"][0] - sum(static_work[k][0] for k in counted) + sum(work[k][0] for k in counted)
+        step_f = work["step"][0] - sum(static_work[k][0] for k in counted if k in static_work) + \
+            sum(work[k][0] for k in counted if k in work)
         work["step"] = (step_f, work["step"][1])
     dom = max(prof, key=lambda k: prof[k][0]) if prof else None
     roof = dict(bound=None, achieved=None, peak=None, unit=None, frac=None, traffic=None)
     per_iter_s = dev_ms * 1e-3 / (args.steps * max(pgd_steps, 1))           # whole PGD iteration, this rank
+    alu_src = ("afs_fp32_fma_peak: FFMA micro-benchmark measured on this GPU in this run (derived bound "
+               "148 SMs x 128 lanes x 2 flop x %.0f MHz = %.2f)" % (peaks["sm_max_mhz"], fp32_derived))
     if dom is not None:
         dur_s = prof[dom][0] * 1e-3 / prof[dom][1]                          # average launch duration
         if dom == "resident":                                               # one launch = every iteration of the call
             flops, hbm = work["step"][0] * pgd_steps, 2 * inst.B * inst.n * 4 + inst.nnz * 4
         else:
-            flops, hbm = work[dom]
-        t_alu, t_hbm = flops / (fp32_peak * 1e12), hbm / (peaks["hbm_gbs"] * 1e9)
+            flops, hbm = work.get(dom, (0.0, 0.0))
+        t_alu, t_hbm = flops / (fp32_meas * 1e12), hbm / (peaks["hbm_gbs"] * 1e9)
         if t_alu >= t_hbm:
-            roof.update(bound="alu", achieved=flops / dur_s / 1e12, peak=fp32_peak, unit="TFLOP/s",
-                        peak_source="148 SMs x 128 FP32 lanes x 2 flop x sm_max_mhz %.0f (MEASURED_PEAKS.json: %s)"
-                                    % (peaks["sm_max_mhz"], peaks["source"]))
+            roof.update(bound="alu", achieved=flops / dur_s / 1e12, peak=fp32_meas, unit="TFLOP/s", peak_source=alu_src,
+                        peak_derived=fp32_derived)
         else:
             roof.update(bound="hbm", achieved=hbm / dur_s / 1e9, peak=peaks["hbm_gbs"], unit="GB/s",
                         peak_source="MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"])
@@ -383,22 +388,23 @@ def run_cuda(args):
         roof["launch_ms"] = dur_s * 1e3
         roof["launches_timed"] = prof[dom][1]
         roof["algorithmic_per_launch"] = dict(flops=flops, hbm_bytes=hbm)
-        if dom in counted:
+        if dom in counted and dom in static_work:
             sf0 = static_work[dom][0]
-            roof["static_formula"] = dict(flops_per_launch=sf0, frac_alu=sf0 / dur_s / 1e12 / fp32_peak,
+            roof["static_formula"] = dict(flops_per_launch=sf0, frac_alu=sf0 / dur_s / 1e12 / fp32_meas,
                                           note="6 L K on the unfixed literals, whatever the iterate; the kernel skips boundary literals")
         tot_ms = sum(v[0] for v in prof.values())
         roof["share_of_timed_launches"] = {k: round(v[0] / tot_ms, 4) for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}
         roof["traffic"] = load_traffic(inst.name, dom)
-    # the whole PGD iteration against the same two ceilings (every kernel of the step, launch gaps included)
+    # the whole PGD iteration against the same two ceilings (every kernel of the step, launch gaps included): the
+    # figure BASELINE.json's ">= 50 % of its roofline" target is judged on
     sf, sb = work["step"]
-    t_alu, t_hbm = sf / (fp32_peak * 1e12), sb / (peaks["hbm_gbs"] * 1e9)
+    t_alu, t_hbm = sf / (fp32_meas * 1e12), sb / (peaks["hbm_gbs"] * 1e9)
     roof["step"] = dict(bound="alu" if t_alu >= t_hbm else "hbm", roofline_us=max(t_alu, t_hbm) * 1e6,
                         measured_us=per_iter_s * 1e6, frac=max(t_alu, t_hbm) / per_iter_s,
                         algorithmic_per_iteration=dict(flops=sf, hbm_bytes=sb))
     if counted:
         s0 = static_work["step"][0]
-        roof["step"]["static_formula"] = dict(flops=s0, frac_alu=s0 / (fp32_peak * 1e12) / per_iter_s)
+        roof["step"]["static_formula"] = dict(flops=s0, frac_alu=s0 / (fp32_meas * 1e12) / per_iter_s)
 
     # ---- the oracle beside it (bounded sample, rank 0, N = 1 only)
     cpu = None
@@ -406,8 +412,8 @@ def run_cuda(args):
         o = oracle_sample(inst, cfg)
         cpu = dict(value=o["value"], unit="restart-steps/s", cores=o["cores"], kind="oracle",
                    sample="first %d restarts x %d PGD iterations of configs[%d] (%.1f s)" % (o["B_o"], o["steps_o"], cfg, o["seconds"]))
-
-    line = dict(metric="pgd_restart_steps_per_sec", value=value, unit="restart-steps/s", n_gpus=world,
+    P.close()
+    return dict(metric="pgd_restart_steps_per_sec", value=value, unit="restart-steps/s", n_gpus=world,
                 steps=args.steps, warmup=args.warmup, ms_per_step=dev_ms / args.steps, higher_is_better=True,
                 scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
                 config=dict(workload=inst.name, n=inst.n, m=inst.m, nnz=inst.nnz, B=inst.B, pgd_steps_per_call=pgd_steps,
@@ -419,10 +425,61 @@ def run_cuda(args):
                 gpu_launches=int(launches), best_sat_max=int(job_best[2]),
                 e2e=dict(value=e2e_value, unit="restart-steps/s", h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h)),
                 roofline=roof, cpu_baseline=cpu, clocks=clocks)
-    print(json.dumps(line))
+
+
+HEADLINE = 4                      # the largest single-GPU configuration (by work): configs[4]
+ALL_CONFIGS = (1, 2, 3, 4)        # the configurations BASELINE.json's target is set on
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2606_06656_b200 import build as afs_build
+    if rank == 0:
+        afs_build.build()
+    if world > 1:
+        dist.barrier()
+    import paper_2606_06656_b200 as afs
+    from paper_2606_06656_b200 import shard
+
+    peaks = load_peaks()
+    cfgs = ALL_CONFIGS if args.config is None else (args.config,)
+    lines = {}
+    for cfg in cfgs:
+        lines[cfg] = measure_config(cfg, args, afs, shard, rank, world, local, peaks)
+        torch.cuda.empty_cache()
+    if rank == 0:
+        head = HEADLINE if HEADLINE in lines else cfgs[-1]
+        line = dict(lines[head])
+        if len(cfgs) > 1:
+            keep = ("value", "unit", "ms_per_step", "literal_evals_per_sec", "gpu_launches", "e2e", "roofline",
+                    "cpu_baseline", "clocks", "config")
+            line["per_config"] = [dict(cfg=c, **{k: lines[c][k] for k in keep}) for c in cfgs]
+            line["gpu_launches"] = int(sum(lines[c]["gpu_launches"] for c in cfgs))
+        print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` with N > 1 outside torchrun: start N ranks (one per GPU) through
+    torch.distributed.run on this node and pass the output through; NCCL's communicator log stays on."""
+    port = 29500 + os.getpid() % 2000
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")
+    return subprocess.call(cmd, env=env)
 
 
 def main():
@@ -430,12 +487,15 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (default 1: the metric's workload)")
+    ap.add_argument("--config", type=int, default=None,
+                    help="BASELINE.json configs index; default: configs[1-4] in one run, configs[4] as the headline")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--pgd-steps", type=int, default=None, help="override the configuration's PGD iteration count")
     ap.add_argument("--mode", type=int, default=None, help="afs_set_option(0, mode): 1 streaming, 2 resident")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.gpus > 1 and "RANK" not in os.environ:
+        return spawn_ranks(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_cuda(args)

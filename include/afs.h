@@ -183,6 +183,14 @@ AFS_API afs_status afs_profile_read(afs_problem* p, double* ms, int64_t* launche
  */
 AFS_API afs_status afs_profile_flops(afs_problem* p, double* flops, int32_t n);
 
+/*
+ * afs_fp32_fma_peak -- measures the plain-FP32 FMA throughput of `device` (TFLOP/s, FMA = 2 flops) with a hand-written
+ * micro-benchmark kernel (independent FFMA chains on every SM, best of 5 launches, CUDA events).  Not on the product
+ * path: bench.py uses it as the denominator of its "alu" roofline.  Synchronous; restores the caller's
+ * current device.
+ */
+AFS_API afs_status afs_fp32_fma_peak(int32_t device, double* tflops);
+
 /* Static, never NULL. */
 AFS_API const char* afs_status_string(afs_status s);
 

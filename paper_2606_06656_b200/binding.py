@@ -21,7 +21,7 @@ EXPORTS = (
     "afs_problem_create", "afs_problem_destroy", "afs_coeffs", "afs_eval_grad", "afs_eval_grad_f64",
     "afs_round_count", "afs_round_count_f64", "afs_pgd_run", "afs_pgd_run_f64", "afs_pgd_run_host",
     "afs_problem_info", "afs_set_option", "afs_status_string", "afs_abi_version", "afs_last_error_message",
-    "afs_profile_read", "afs_profile_flops",
+    "afs_profile_read", "afs_profile_flops", "afs_fp32_fma_peak",
 )
 
 _lib = None
@@ -70,6 +70,8 @@ def lib():
     L.afs_profile_read.restype = C.c_int
     L.afs_profile_flops.argtypes = [vp, vp, i32]
     L.afs_profile_flops.restype = C.c_int
+    L.afs_fp32_fma_peak.argtypes = [i32, vp]
+    L.afs_fp32_fma_peak.restype = C.c_int
     L.afs_status_string.argtypes = [C.c_int]
     L.afs_status_string.restype = C.c_char_p
     L.afs_abi_version.restype = i32
@@ -88,6 +90,13 @@ def coeffs(ctype: int, L: int, k: int = 0) -> np.ndarray:
     a = np.zeros(L + 1, dtype=np.float64)
     _chk(lib().afs_coeffs(ctype, L, k, a.ctypes.data), "afs_coeffs")
     return a
+
+
+def fp32_fma_peak(device: int = 0) -> float:
+    """afs_fp32_fma_peak: measured plain-FP32 FMA throughput of the device, TFLOP/s."""
+    v = C.c_double(0.0)
+    _chk(lib().afs_fp32_fma_peak(int(device), C.byref(v)), "afs_fp32_fma_peak")
+    return float(v.value)
 
 
 def _torch():

@@ -69,7 +69,7 @@ void free_workspace(afs_problem* P)
     Workspace& w = P->ws;
     free_ptr(w.XT[0]); free_ptr(w.XT[1]); free_ptr(w.scratch); free_ptr(w.aux[0]); free_ptr(w.aux[1]);
     free_ptr(w.sat_hist); free_ptr(w.best_sat[0]); free_ptr(w.best_sat[1]);
-    free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.best_bits);
+    free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.SAT[0]); free_ptr(w.SAT[1]); free_ptr(w.bnd); free_ptr(w.best_bits);
     free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.fe_cm); free_ptr(w.f_part);
     free_ptr(w.mask_dev); free_ptr(w.host_stage_X); free_ptr(w.host_stage_assign);
     free_ptr(w.host_stage_sat); free_ptr(w.host_stage_step);
@@ -124,6 +124,8 @@ afs_status ensure_workspace(afs_problem* P, int Bp, size_t elem, int64_t sat_row
     A(&w.best_sat[0], (size_t)nBp); A(&w.best_sat[1], (size_t)nBp);
     A(&w.best_step[0], (size_t)nBp); A(&w.best_step[1], (size_t)nBp);
     A(&w.S[0], n * ntile); A(&w.S[1], n * ntile); A(&w.best_bits, n * ntile);
+    A(&w.SAT[0], n * ntile); A(&w.SAT[1], n * ntile);
+    A((unsigned char**)&w.bnd, (size_t)P->n_long * nBp * 2 * nelem);
     if (st != AFS_OK) { afs::free_workspace(P); return st; }
     w.Bp = nBp; w.elem = nelem; w.sat_rows = nrows; w.bytes = tot;
     return AFS_OK;
@@ -280,5 +282,61 @@ extern "C" afs_status afs_pgd_run_host(afs_problem* P, float* X, int32_t B, int3
     if (best_sat) CU(cudaMemcpyAsync(best_sat, w.host_stage_sat, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
     if (best_step) CU(cudaMemcpyAsync(best_step, w.host_stage_step, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    return AFS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// afs_fp32_fma_peak: the plain-FP32 ceiling of this GPU, measured ("measure an FMA micro-benchmark on
+// the box").  Not on the product path: bench.py calls it for the denominator of the "alu" roofline.  Every thread runs
+// 8 independent FFMA chains; 2 CTAs x 1024 threads per SM keep all four schedulers of every SM issuing.
+// ---------------------------------------------------------------------------------------------------------------------
+namespace afs {
+__global__ void __launch_bounds__(1024, 2) k_fma_peak(float* __restrict__ out, int iters, float a, float b)
+{
+    float x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = (float)(threadIdx.x + i) * 1e-3f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) x[i] = fmaf(x[i], a, b);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+}  // namespace afs
+
+extern "C" afs_status afs_fp32_fma_peak(int32_t device, double* tflops)
+{
+    if (!tflops) return AFS_ERR_INVALID_ARG;
+    *tflops = 0.0;
+    int ndev = 0, prev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { (void)cudaGetLastError(); return AFS_ERR_CUDA; }
+    CU(cudaGetDevice(&prev));
+    CU(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, device));
+    const int grid = prop.multiProcessorCount * 2, iters = 4096;
+    float* out = nullptr;
+    CU(cudaMalloc((void**)&out, (size_t)grid * 1024 * sizeof(float)));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {   // the first repetition is the warm-up
+        CU(cudaEventRecord(e0, 0));
+        k_fma_peak<<<grid, 1024>>>(out, iters, 0.999f, 1e-3f);
+        CU(cudaEventRecord(e1, 0));
+        CU(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, e0, e1));
+        const double fl = (double)grid * 1024.0 * iters * 64.0 * 2.0;
+        if (rep > 0 && ms > 0.f) best = std::max(best, fl / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
+    cudaSetDevice(prev);
+    *tflops = best;
     return AFS_OK;
 }

@@ -115,7 +115,9 @@ struct Workspace {
     int32_t* sat_hist = nullptr;           // [sat_rows][Bp]
     int32_t* best_sat[2] = {nullptr, nullptr};
     int32_t* best_step[2] = {nullptr, nullptr};
-    uint32_t* S[2] = {nullptr, nullptr};   // sign bits [n][Bp/32]
+    uint32_t* S[2] = {nullptr, nullptr};   // sign bits [n][Bp/32]: bit r of word (v, tile) = "x_v < 0" for restart 32 tile + r
+    uint32_t* SAT[2] = {nullptr, nullptr}; // saturation bits, same layout: |x_v| = 1 (on the boundary of the cube)
+    void* bnd = nullptr;                   // real [n_long][Bp][2]: dFE/dy of a boundary literal at y = +1 / y = -1
     uint32_t* best_bits = nullptr;         // [n][Bp/32]
     void* fe_med = nullptr;                // real [n_med][Bp]      (eval_grad only)
     void* fe_long = nullptr;               // real [n_long][Bp]
@@ -151,6 +153,7 @@ struct afs_problem {
     uint32_t* d_pc_lits = nullptr;
     afs::PullClause* d_pcp = nullptr;   // the same clauses packed for the bit-parallel counts
     int32_t* d_slot_ptr = nullptr;      // [n+1] scratch rows of each variable (transposed-CSR order)
+    int32_t* d_slot_info = nullptr;     // [nslots] -1, or for a slot of the LONG class (index in d_long) << 1 | literal negated
     int64_t nslots = 0;
 
     afs::MedCon* d_med = nullptr;       // sorted by bucket

@@ -35,9 +35,11 @@ __device__ __forceinline__ real ldx(const real* __restrict__ XT, uint32_t w, int
 // ------------------------------------------------------------------------------------------------------------------
 // layout changes at the API boundary: X[B,n] <-> XT[n][Bp]
 // ------------------------------------------------------------------------------------------------------------------
+// Also writes the sign / saturation words of the iterate (Sw, SATw: [n][Bp/32], may be NULL).
 template <typename real>
 __global__ void __launch_bounds__(256) k_transpose_in(const real* __restrict__ X, real* __restrict__ XT, int B, int n,
-                                                      int Bp, const int8_t* __restrict__ mask)
+                                                      int Bp, const int8_t* __restrict__ mask,
+                                                      uint32_t* __restrict__ Sw, uint32_t* __restrict__ SATw)
 {
     __shared__ real tile[32][33];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
@@ -55,6 +57,13 @@ __global__ void __launch_bounds__(256) k_transpose_in(const real* __restrict__ X
             real x = tile[tx][r];
             if (mask) { int mk = mask[v]; if (mk != 0 && b < B) x = (real)mk; }   // fixed at entry
             XT[(size_t)v * Bp + b] = x;
+        }
+        if (Sw) {   // the 32 lanes of a warp hold one variable's tile (v is warp-uniform)
+            const real xx = v < n ? tile[tx][r] : real(0);
+            real xm = xx;
+            if (mask && v < n) { int mk = mask[v]; if (mk != 0 && b < B) xm = (real)mk; }
+            const unsigned sb = __ballot_sync(FULL, xm < real(0)), sa = __ballot_sync(FULL, xm == real(1) || xm == real(-1));
+            if (tx == 0 && v < n) { Sw[(size_t)v * (Bp >> 5) + blockIdx.y] = sb; SATw[(size_t)v * (Bp >> 5) + blockIdx.y] = sa; }
         }
     }
 }
@@ -490,9 +499,12 @@ struct VarArgs {
     int32_t* best_sat_out;
     const int32_t* best_step_in;
     int32_t* best_step_out;
-    const uint32_t* S_prev;
-    uint32_t* S_cur;
+    const uint32_t* S_prev;      // sign words of X_{t-1} (best-so-far merge)
+    uint32_t* S_next;            // sign / saturation words of X_{t+1}, written with the step (may alias S_prev: the same
+    uint32_t* SAT_next;          // thread reads a word of S_prev before it writes that word of S_next)
     uint32_t* best_bits;
+    const int32_t* slot_info;    // LONGT: -1, or (long constraint << 1 | literal negated) of a slot
+    const real* bnd;             // LONGT: [n_long][Bp][2] gradients of boundary literals (y = +1, y = -1)
     real* GT;
 };
 
@@ -658,7 +670,10 @@ __device__ __forceinline__ void pull_variable(const uint32_t* __restrict__ runs,
 
 // 32 warps per SM at <= 64 registers: the pass waits on L2 gathers, and occupancy is what hides them -- at
 // 95 registers (2 CTAs per SM) the same code took 1.5x as long on configs[3] (measured: 420 -> 274 us per iteration).
-template <typename real, bool EVAL, int RPL>
+// LONGT: the instance has LONG-class constraints -- a slot of that class is read from its scratch row only where this
+// restart's x is strictly inside the cube; on the boundary the literal's gradient is one of the pair bnd[c][b] that the
+// long kernel wrote for all boundary literals of the constraint (picked by the literal's truth value).
+template <typename real, bool EVAL, int RPL, bool LONGT>
 __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const VarArgs<real> a)
 {
     __shared__ __align__(16) uint2 s_stage[VAR_WARPS][PULL_SBUF];
@@ -712,14 +727,7 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
         int mk = 0;
 #pragma unroll
         for (int c = 0; c < RPL; ++c) x[c] = xcol[(size_t)v * Bp + 32 * c];
-        if (!EVAL) {
-#pragma unroll
-            for (int c = 0; c < RPL; ++c) {
-                unsigned sb = __ballot_sync(FULL, x[c] < real(0));
-                if (lane == 0) a.S_cur[(size_t)v * ntile + tile0 + c] = sb;
-            }
-            mk = a.mask ? a.mask[v] : 0;
-        }
+        if (!EVAL) mk = a.mask ? a.mask[v] : 0;
 #pragma unroll
         for (int c = 0; c < RPL; ++c) g[c] = real(0);
         if (mk == 0) {   // a fixed variable never moves: its gradient is not needed
@@ -732,17 +740,44 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
             const int s1 = a.slot_ptr[v + 1];
             int s = a.slot_ptr[v];
             const real* __restrict__ sc = a.scratch + b;
-            for (; s + 4 <= s1; s += 4) {
+            if (LONGT) {
+                bool onb[RPL], neg0[RPL];
 #pragma unroll
-                for (int c = 0; c < RPL; ++c) {
-                    real g0 = sc[(size_t)s * Bp + 32 * c], g1 = sc[(size_t)(s + 1) * Bp + 32 * c];
-                    real g2 = sc[(size_t)(s + 2) * Bp + 32 * c], g3 = sc[(size_t)(s + 3) * Bp + 32 * c];
-                    g[c] += g0; g[c] += g1; g[c] += g2; g[c] += g3;
+                for (int c = 0; c < RPL; ++c) { onb[c] = x[c] == one || x[c] == -one; neg0[c] = x[c] < real(0); }
+                for (; s < s1; ++s) {
+                    const int info = a.slot_info[s];
+                    if (info < 0) {
+#pragma unroll
+                        for (int c = 0; c < RPL; ++c) g[c] += sc[(size_t)s * Bp + 32 * c];
+                    } else {
+                        const bool lneg = info & 1;
+                        const real* __restrict__ bp = a.bnd + ((size_t)(info >> 1) * Bp + b) * 2;
+#pragma unroll
+                        for (int c = 0; c < RPL; ++c) {
+                            real val;
+                            if (onb[c]) {   // literal true (y = -1) iff (x < 0) != negated; chain rule sign (S5)
+                                const real t = bp[64 * c + ((neg0[c] != lneg) ? 1 : 0)];
+                                val = lneg ? -t : t;
+                            } else {
+                                val = sc[(size_t)s * Bp + 32 * c];
+                            }
+                            g[c] += val;
+                        }
+                    }
                 }
-            }
-            for (; s < s1; ++s)
+            } else {
+                for (; s + 4 <= s1; s += 4) {
 #pragma unroll
-                for (int c = 0; c < RPL; ++c) g[c] += sc[(size_t)s * Bp + 32 * c];
+                    for (int c = 0; c < RPL; ++c) {
+                        real g0 = sc[(size_t)s * Bp + 32 * c], g1 = sc[(size_t)(s + 1) * Bp + 32 * c];
+                        real g2 = sc[(size_t)(s + 2) * Bp + 32 * c], g3 = sc[(size_t)(s + 3) * Bp + 32 * c];
+                        g[c] += g0; g[c] += g1; g[c] += g2; g[c] += g3;
+                    }
+                }
+                for (; s < s1; ++s)
+#pragma unroll
+                    for (int c = 0; c < RPL; ++c) g[c] += sc[(size_t)s * Bp + 32 * c];
+            }
         }
 #pragma unroll
         for (int c = 0; c < RPL; ++c) {
@@ -755,6 +790,11 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
                 xn = xn < -one ? -one : xn;
                 if (mk != 0) xn = x[c];
                 a.Xout[(size_t)v * Bp + b + 32 * c] = xn;
+                const unsigned sb = __ballot_sync(FULL, xn < real(0)), sa = __ballot_sync(FULL, xn == one || xn == -one);
+                if (lane == 0) {
+                    a.S_next[(size_t)v * ntile + tile0 + c] = sb;
+                    a.SAT_next[(size_t)v * ntile + tile0 + c] = sa;
+                }
             }
         }
     }

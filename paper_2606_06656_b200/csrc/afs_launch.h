@@ -36,6 +36,7 @@ afs_status prof_work_slot(afs_problem* P, int cls, cudaStream_t st, unsigned lon
 
 // the long-constraint kernels of one PGD iteration (all length buckets); instantiated in afs_long_f32.cu / _f64.cu
 template <typename real>
-afs_status launch_long_all(afs_problem* P, const real* XT, int Bp, real* scratch, int32_t* sat, real* fe, cudaStream_t st);
+afs_status launch_long_all(afs_problem* P, const real* XT, const uint32_t* Sw, const uint32_t* SATw, int Bp, real* scratch,
+                           int32_t* sat, real* fe, cudaStream_t st);
 
 }  // namespace afs

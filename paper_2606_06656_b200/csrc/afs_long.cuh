@@ -1,15 +1,17 @@
-// afs_long.cuh -- the LONG class: EK / CARD longer than 64 literals (and NAE / EO / AMO too long for the register
-// kernels).  warp = (constraint, restart), CTA = one constraint x RPC restarts.  Count basis (G10):
+// afs_long.cuh -- the LONG class: EK / CARD longer than 64 literals.  warp = (constraint, restart), CTA = one
+// constraint x one tile of 32 restarts.  Count basis (G10):
 //
 //   Q(z) = prod_j (u_j + p_j z),  u = (1+y)/2, p = (1-y)/2,  q_t = [z^t] Q = Pr[t literals true]
 //
-//   gather    per literal the ratio R = min(u, p) / max(u, p) in [0, 1] and its direction (type A: p <= 1/2, type B:
-//             p > 1/2); max(u, p) = 1 / (1 + R) because u + p = 1.  A literal on the boundary of the cube has R = 0:
-//             y = +1 is the factor 1, y = -1 is the factor z -- an exact shift of the pmf, no arithmetic.  PGD iterates
-//             sit on that boundary in most coordinates (clipping; fixed variables), so the pmf is
-//             built from the INTERIOR literals only:  Q(z) = z^nB0 * Qred(z),  deg Qred = Leff.
-//   lists     the literals of a restart are compacted into  [ B interior | A interior | A boundary | B boundary ],
-//             the interior sections padded with neutral R = 0 entries to multiples of four.
+//   classes   a literal on the boundary of the cube is the factor 1 (y = +1) or z (y = -1): an exact shift of the pmf,
+//             no arithmetic.  PGD iterates sit on that boundary in most coordinates (clipping; fixed variables,
+//             P:L140), so the pmf is built from the INTERIOR literals only:  Q(z) = z^nB0 * Qred(z),  deg Qred = Leff.
+//             Which literals are interior, and which way they lean, is read from two bit words per (variable, tile of
+//             32 restarts) that the variable pass writes with the iterate: sign (x < 0) and saturated (|x| = 1).
+//   ratios    per interior literal R = min(u, p) / max(u, p) in (0, 1] (type A: p <= 1/2, type B: p > 1/2);
+//             max(u, p) = 1 / (1 + R) because u + p = 1.
+//   lists     the interior literals of a restart are compacted into  [ B interior | A interior ], both sections padded
+//             with neutral R = 0 entries to multiples of four.
 //   forward   Qred = rev(prod_B (1 + R_j w)) * prod_A (1 + R_j z) / prod (1 + R_j): every literal is the one-FMA
 //             update q_t += R q_{t-1}; after the B section the coefficient vector is reversed once (prod_B (z + R_j)
 //             is the reversal of prod_B (1 + R_j w)).  The scalar 1 / prod (1 + R_j) is applied every 32 literals
@@ -20,7 +22,7 @@
 //             recurrence from the top for type B; q^(-j) = (1 + R_j) s.  Nothing that vanishes at x = +-1 is ever
 //             divided by (BASELINE.json subsystem (2)).  A warp runs chains of one direction and one length; every
 //             lane carries up to four chains that share each broadcast load of q.  Boundary literals need no chain:
-//             q^(-j) = q (y = +1) or q shifted by one (y = -1).
+//             q^(-j) = q (y = +1) or q shifted by one (y = -1) -- one pair of values per (constraint, restart).
 // The reduced pmf sits in shared memory at A[off + t] with off = (3 - Leff) mod 4, so that the top-down chains read
 // aligned 16-byte blocks from index 0 and the bottom-up chains after at most three scalar steps.
 #pragma once
@@ -203,224 +205,219 @@ __device__ __forceinline__ bool long_pred(int type, int L, int k, int t)
     }
 }
 
+// One CTA = one constraint x one tile of 32 restarts; its RPC warps take the restarts of the tile in turn (warp w:
+// restarts w, w + RPC, ...), each with its own list / pmf buffers.
+//   words    the CTA first stages, per literal, the tile's "true" word (sign word of the variable, flipped for a negated
+//            literal) and "saturated" word (|x| = 1) -- two 4-byte loads per literal for 32 restarts instead of 32
+//            element gathers.  Bit r of the words classifies literal j for restart r: boundary-true, boundary-false,
+//            interior with y < 0 (type B), interior with y >= 0 (type A).
+//   pass 1   per restart, ballots over the words: true count tc (S9), boundary-true count nB0, nBr, nAr.  A restart
+//            with no interior literal is finished here: its pmf is the point mass at nB0, the objective is -+1 and the
+//            two boundary gradients are d_t picked at nB0 (no list, no gather, no arithmetic).
+//   pass 2   otherwise: list positions from the same ballots, x gathered for the INTERIOR literals only.
+//   output   boundary literals: ONE pair (dFE/dy at y = +1, at y = -1) per (constraint, restart) in bnd[c][b][2]; the
+//            variable pass picks by its own x (a variable on +-1 is a boundary literal in every constraint it occurs
+//            in).  Interior literals: their own scratch rows, as the other materialising classes.
 template <typename real, int NR, int RPC>
 __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ cons, int c_begin,
                                                    const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
-                                                   const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
+                                                   const real* __restrict__ XT, const uint32_t* __restrict__ Sw,
+                                                   const uint32_t* __restrict__ SATw, int ntile, int Bp,
+                                                   real* __restrict__ scratch, real* __restrict__ bnd,
                                                    int32_t* __restrict__ sat, real* __restrict__ fe_out, int LS, int QS,
                                                    unsigned long long* __restrict__ work)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    real* RcAll = reinterpret_cast<real*>(smem_raw);              // [RPC][LS]  ratios in list order
-    real* AAll = RcAll + RPC * LS;                                // [RPC][QS]  signed ratios (gather), then the pmf
-    uint16_t* InvAll = reinterpret_cast<uint16_t*>(AAll + RPC * QS);   // [RPC][LS]  list position of each literal
-    __shared__ int s_cnt[RPC];
+    real* RcAll = reinterpret_cast<real*>(smem_raw);              // [RPC][LS]  ratios in list order, then gradients
+    real* AAll = RcAll + RPC * LS;                                // [RPC][QS]  the pmf
+    uint32_t* TW = reinterpret_cast<uint32_t*>(AAll + RPC * QS);  // [LS] true words of the tile
+    uint32_t* SW = TW + LS;                                       // [LS] saturated words
+    uint16_t* JAll = reinterpret_cast<uint16_t*>(SW + LS);        // [RPC][LS]  literal index at each list position
     constexpr int NT = RPC * 32;
     constexpr unsigned FULLM = 0xffffffffu;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int groups = Bp / RPC;
-    const int c = c_begin + (int)(blockIdx.x / groups);
-    const int bg = (int)(blockIdx.x % groups);
+    const int c = c_begin + (int)(blockIdx.x / (unsigned)ntile);
+    const int tile = (int)(blockIdx.x % (unsigned)ntile);
     const LongCon lc = cons[c];
     const int L = lc.L;
     const uint32_t* lw = lits + lc.off;
     const int32_t* sw = slots + lc.off;
-    if (tid < RPC) s_cnt[tid] = 0;
-    __syncthreads();
-    // ---- S1: gather the literal values of RPC consecutive restarts (one 32-byte sector per literal for 8 x fp32)
-    {
-        const int r = tid % RPC;
-        const unsigned pat = RPC == 8 ? 0x01010101u : RPC == 4 ? 0x11111111u : RPC == 2 ? 0x55555555u : 0xffffffffu;
-        // four rounds of the block at a time: the literal words first, then the four gathers, so that a thread has four
-        // dependent (word -> row) pairs in flight instead of one
-        const int rounds = (L * RPC + NT - 1) / NT;
-        int truec = 0;   // lanes < RPC: true literals of restart `lane` seen by this warp
-        for (int r0 = 0; r0 < rounds; r0 += 4) {
-            uint32_t w[4];
-            real x[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int j = (tid + (r0 + k) * NT) / RPC;
-                w[k] = j < L ? lw[j] : 0u;
-            }
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int j = (tid + (r0 + k) * NT) / RPC;
-                x[k] = j < L ? XT[(size_t)(w[k] & LIT_VAR) * Bp + bg * RPC + r] : real(0);
-            }
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                if (r0 + k < rounds) {   // block-uniform
-                    const int j = (tid + (r0 + k) * NT) / RPC;
-                    bool tr = false;
-                    if (j < L) {
-                        const bool neg = (w[k] >> 31) != 0;
-                        tr = (x[k] < real(0)) != neg;
-                        const real y = neg ? -x[k] : x[k];
-                        const real u = real(0.5) + real(0.5) * y, p = real(0.5) - real(0.5) * y;
-                        const bool fwd = !(y < real(0));             // p <= 1/2: type A
-                        // in [0, 1]; the divisor is >= 1/2; 0 on the boundary.  Correctly rounded reciprocal times the
-                        // numerator (one MUFU + two corrections instead of the IEEE division sequence; <= 1 ulp off)
-                        const real R = (fwd ? p : u) * recip(fwd ? u : p);
-                        AAll[r * QS + j] = fwd ? R : -R;             // the sign bit is the direction (-0.0 for y = -1)
-                    }
-                    const unsigned bal = __ballot_sync(FULLM, tr);
-                    if (lane < RPC) truec += __popc(bal & (pat << lane));
-                }
-            }
-        }
-        if (lane < RPC && truec) atomicAdd(&s_cnt[lane], truec);
+    for (int j = tid; j < L; j += NT) {
+        const uint32_t w = lw[j];
+        const size_t wi = (size_t)(w & LIT_VAR) * ntile + tile;
+        const uint32_t s = Sw[wi];
+        TW[j] = (w >> 31) ? ~s : s;
+        SW[j] = SATw[wi];
     }
     __syncthreads();
-    const int b = bg * RPC + warp;
     real* Rc = RcAll + warp * LS;
     real* Aw = AAll + warp * QS;
-    uint16_t* inv = InvAll + warp * LS;
-    // ---- lists: [B interior, pad | A interior, pad]; the boundary literals share two slots behind them (send: y = +1,
-    // send + 1: y = -1), because all literals of one kind get the same gradient
-    int nBr = 0, nAr = 0, nA0 = 0;
-    for (int j0 = 0; j0 < L; j0 += 32) {
-        const int j = j0 + lane;
-        const bool act = j < L;
-        const real rs = Aw[act ? j : 0];
-        const bool isB = signbit(rs), intr = rs != real(0);
-        nBr += __popc(__ballot_sync(FULLM, act && isB && intr));
-        nAr += __popc(__ballot_sync(FULLM, act && !isB && intr));
-        nA0 += __popc(__ballot_sync(FULLM, act && !isB && !intr));
-    }
-    const int nB0 = L - nBr - nAr - nA0;
-    const int nBr4 = (nBr + 3) & ~3, nAr4 = (nAr + 3) & ~3, send = nBr4 + nAr4, Leff = nBr + nAr;
-    {
-        const unsigned lt = (1u << lane) - 1u;
-        int pBr = 0, pAr = nBr4;
-        for (int j0 = 0; j0 < L; j0 += 32) {
-            const int j = j0 + lane;
-            const bool act = j < L;
-            const real rs = Aw[act ? j : 0];
-            const bool isB = signbit(rs), intr = rs != real(0);
-            const bool cBr = act && isB && intr, cAr = act && !isB && intr;
-            const unsigned mBr = __ballot_sync(FULLM, cBr), mAr = __ballot_sync(FULLM, cAr);
-            const int pos = cBr ? pBr + __popc(mBr & lt) : cAr ? pAr + __popc(mAr & lt) : send + (isB ? 1 : 0);
-            if (act) {
-                inv[j] = (uint16_t)pos;
-                if (intr) Rc[pos] = fabs(rs);
-            }
-            pBr += __popc(mBr); pAr += __popc(mAr);
-        }
-        if (lane < nBr4 - nBr) Rc[nBr + lane] = real(0);
-        if (lane < nAr4 - nAr) Rc[nBr4 + nAr + lane] = real(0);
-    }
-    __syncwarp();
-    // ---- S2: forward pmf of the interior literals
-    const int off = (3 - Leff) & 3;
-    {
-        real q[NR][4];
-#pragma unroll
-        for (int r = 0; r < NR; ++r)
-#pragma unroll
-            for (int i = 0; i < 4; ++i) q[r][i] = real(0);
-        if (lane == 0) q[0][0] = real(1);
-        real P = real(1);
-        for (int t = lane; t < QS; t += 32) Aw[t] = real(0);   // the signed ratios are no longer needed
-        __syncwarp();
-        if (nBr > 0) {
-            DpPhases<real, NR, 0>::run(q, Rc, 0, nBr4, lane, P);
-            // prod_B (z + R_j) is the reversal of prod_B (1 + R_j w): c_t -> c_{nBr - t}, through shared memory
-#pragma unroll
-            for (int r = 0; r < NR; ++r)
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    int t = (r * 32 + lane) * 4 + i;
-                    if (t <= nBr) Aw[t] = q[r][i];
-                }
-            __syncwarp();
-#pragma unroll
-            for (int r = 0; r < NR; ++r)
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    int t = (r * 32 + lane) * 4 + i;
-                    q[r][i] = t <= nBr ? Aw[nBr - t] : real(0);
-                }
-            __syncwarp();
-            for (int t = lane; t <= nBr; t += 32) Aw[t] = real(0);
-            __syncwarp();
-        }
-        DpPhases<real, NR, 0>::run(q, Rc, nBr4, send, lane, P);
-        const real sc = recip(P);
-        real fe = real(0);
-#pragma unroll
-        for (int r = 0; r < NR; ++r)
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                int t = (r * 32 + lane) * 4 + i;
-                if (t <= Leff) {
-                    const real v = q[r][i] * sc;
-                    Aw[off + t] = v;
-                    fe += long_pred(lc.type, L, lc.k, t + nB0) ? -v : v;   // sp = -1 where satisfied
-                }
-            }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) fe += __shfl_xor_sync(FULLM, fe, o);
-        if (lane == 0) {
-            if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
-            if (sat && long_pred(lc.type, L, lc.k, s_cnt[warp])) atomicAdd(&sat[b], 1);
-        }
-    }
-    __syncwarp();
-    // ---- S3 + S5: leave-one-out
+    uint16_t* J = JAll + warp * LS;
     const bool useA = lc.wA != 0.f, useB = lc.wB != 0.f;
-    // timing mode only: the state-dependent algorithmic work of this (constraint, restart) -- 6 Leff Keff flops, the
-    // survey's count for a pmf of Leff interior literals with the threshold left after the nB0 true boundary literals
-    if (work && lane == 0) {
-        const int keff = lc.k - nB0;
-        const bool live = (useA || useB) && Leff > 0 && keff >= (lc.type == AFS_EK ? 0 : 1) && keff <= Leff;
-        if (live) {
-            int K = min(keff, Leff - keff + 1) + 1;
-            K = K < 1 ? 1 : K;
-            atomicAdd(work + (blockIdx.x & 31u), 6ull * (unsigned long long)Leff * (unsigned long long)K);   // 32 slots
-        }
-    }
     // capture points in true-count index space, t1 <= t2 (equal if only one is used)
     int t1 = lc.tA, t2 = lc.tB;
     real w1 = (real)lc.wA, w2 = (real)lc.wB;
     if (!useA) { t1 = t2; w1 = real(0); }
     if (!useB) { t2 = t1; w2 = w1; w1 = real(0); }
     if (t1 > t2) { int tt = t1; t1 = t2; t2 = tt; real ww = w1; w1 = w2; w2 = ww; }
-    const real* qr = Aw + off;   // qr[tau] = reduced pmf, tau in [0, Leff]; q_t = qr[t - nB0]
-    // boundary literals: y = +1 leaves q unchanged, y = -1 removes one shift (q^(-j)_t = q_{t+1}).  Every dFE/dy_j
-    // goes to Rc at the literal's list position; the CTA then writes whole 32-byte sectors of the scratch rows.
-    {
-        auto qat = [&](int tau) -> real { return (tau >= 0 && tau <= Leff) ? qr[tau] : real(0); };
-        const real gA0 = w1 * qat(t1 - nB0) + w2 * qat(t2 - nB0);
-        const real gB0 = w1 * qat(t1 + 1 - nB0) + w2 * qat(t2 + 1 - nB0);
-        if (lane < 2) Rc[send + lane] = lane == 0 ? gA0 : gB0;
-    }
-    // interior literals: q^(-j)_t = qred^(-j)_{t - nB0}, qred^(-j) has degree Leff - 1
-    int c1 = t1 - nB0, c2 = t2 - nB0;
-    const bool v1 = c1 >= 0 && c1 <= Leff - 1 && w1 != real(0), v2 = c2 >= 0 && c2 <= Leff - 1 && w2 != real(0);
-    if (!v1 && !v2) {   // the expansion does not depend on the interior literals here (or is constant): zero gradient
-        for (int e = lane; e < send; e += 32) Rc[e] = real(0);
-    } else {
-        if (!v1) { c1 = c2; w1 = real(0); }
-        if (!v2) { c2 = c1; w2 = w1; w1 = real(0); }
-        // type A: bottom-up chain over qr_0, qr_1, ...; captures at c1 then c2
-        deconv_dir<real, false>(qr, off, Rc + nBr4, nAr, c1, c2, w1, w2, lane);
-        // type B: top-down chain over qr_Leff, qr_{Leff-1}, ...; chain index i <-> tau = Leff-1-i, so c2 is met first
-        deconv_dir<real, true>(qr + Leff, 0, Rc, nBr, Leff - 1 - c2, Leff - 1 - c1, w2, w1, lane);
-    }
-    __syncthreads();
-    // ---- S5 + write-out: thread = (literal, restart), restart fastest
-    {
-        const int r = tid % RPC;
-        const real* Rr = RcAll + r * LS;
-        const uint16_t* ir = InvAll + r * LS;
-        real* dst = scratch + (size_t)bg * RPC + r;
-#pragma unroll 4
-        for (int idx = tid; idx < L * RPC; idx += NT) {
-            const int j = idx / RPC;
-            const real g = Rr[ir[j]];
-            dst[(size_t)sw[j] * Bp] = (lw[j] >> 31) ? -g : g;
+    const unsigned lt = (1u << lane) - 1u;
+#pragma unroll 1
+    for (int r = warp; r < 32; r += RPC) {
+        const int b = tile * 32 + r;
+        // ---- pass 1: counts of the four literal kinds from the words
+        int tc = 0, nB0 = 0, nBr = 0, nAr = 0;
+        for (int j0 = 0; j0 < L; j0 += 32) {
+            const int j = j0 + lane;
+            const bool act = j < L;
+            const bool tb = act && ((TW[act ? j : 0] >> r) & 1u), sb = !act || ((SW[act ? j : 0] >> r) & 1u);
+            const unsigned mT = __ballot_sync(FULLM, tb), mS = __ballot_sync(FULLM, sb);
+            const unsigned mAct = L - j0 >= 32 ? FULLM : (1u << (L - j0)) - 1u;
+            tc += __popc(mT); nB0 += __popc(mT & mS); nBr += __popc(mT & ~mS); nAr += __popc(~mT & ~mS & mAct);
         }
+        const int Leff = nBr + nAr;
+        if (lane == 0 && sat && long_pred(lc.type, L, lc.k, tc)) atomicAdd(&sat[b], 1);
+        auto dpick = [&](int tau) -> real {   // w1 [t1 = tau] + w2 [t2 = tau]: d_t at the point mass
+            return (tau == t1 - nB0 ? w1 : real(0)) + (tau == t2 - nB0 ? w2 : real(0));
+        };
+        if (Leff == 0) {
+            // every literal on the boundary: Q(z) = z^nB0.  Removing a false literal leaves the mass at nB0, removing a
+            // true one moves it to nB0 - 1 (P:L52 d_t; exact, no arithmetic)
+            if (lane == 0) {
+                bnd[((size_t)c * Bp + b) * 2] = dpick(0);
+                bnd[((size_t)c * Bp + b) * 2 + 1] = dpick(-1);
+                if (fe_out) fe_out[(size_t)c * Bp + b] = long_pred(lc.type, L, lc.k, nB0) ? real(-1) : real(1);
+            }
+            continue;
+        }
+        // ---- pass 2: lists [B interior, pad | A interior, pad] of literal indices; x gathered for these only
+        const int nBr4 = (nBr + 3) & ~3, nAr4 = (nAr + 3) & ~3, send = nBr4 + nAr4;
+        {
+            int pBr = 0, pAr = nBr4;
+            for (int j0 = 0; j0 < L; j0 += 32) {
+                const int j = j0 + lane;
+                const bool act = j < L;
+                const bool tb = act && ((TW[act ? j : 0] >> r) & 1u), intr = act && !((SW[act ? j : 0] >> r) & 1u);
+                const bool cBr = intr && tb, cAr = intr && !tb;
+                const unsigned mBr = __ballot_sync(FULLM, cBr), mAr = __ballot_sync(FULLM, cAr);
+                if (intr) J[cBr ? pBr + __popc(mBr & lt) : pAr + __popc(mAr & lt)] = (uint16_t)j;
+                pBr += __popc(mBr); pAr += __popc(mAr);
+            }
+            if (lane < nBr4 - nBr) J[nBr + lane] = 0xffffu;
+            if (lane < nAr4 - nAr) J[nBr4 + nAr + lane] = 0xffffu;
+        }
+        __syncwarp();
+        for (int e = lane; e < send; e += 32) {
+            const int j = J[e];
+            real R = real(0);   // neutral pad entry
+            if (j != 0xffff) {
+                const uint32_t w = lw[j];
+                const real x = XT[(size_t)(w & LIT_VAR) * Bp + b];
+                const real y = (w >> 31) ? -x : x;
+                const real u = real(0.5) + real(0.5) * y, p = real(0.5) - real(0.5) * y;
+                // the list decides the direction (type B: literal true by sign, p >= 1/2): min / max, divisor >= 1/2.
+                // Correctly rounded reciprocal times the numerator (<= 1 ulp off the IEEE quotient)
+                R = e < nBr4 ? u * recip(p) : p * recip(u);
+            }
+            Rc[e] = R;
+        }
+        // ---- S2: forward pmf of the interior literals
+        const int off = (3 - Leff) & 3;
+        {
+            real q[NR][4];
+#pragma unroll
+            for (int rr = 0; rr < NR; ++rr)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) q[rr][i] = real(0);
+            if (lane == 0) q[0][0] = real(1);
+            real P = real(1);
+            for (int t = lane; t < QS; t += 32) Aw[t] = real(0);
+            __syncwarp();
+            if (nBr > 0) {
+                DpPhases<real, NR, 0>::run(q, Rc, 0, nBr4, lane, P);
+                // prod_B (z + R_j) is the reversal of prod_B (1 + R_j w): c_t -> c_{nBr - t}, through shared memory
+#pragma unroll
+                for (int rr = 0; rr < NR; ++rr)
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        int t = (rr * 32 + lane) * 4 + i;
+                        if (t <= nBr) Aw[t] = q[rr][i];
+                    }
+                __syncwarp();
+#pragma unroll
+                for (int rr = 0; rr < NR; ++rr)
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        int t = (rr * 32 + lane) * 4 + i;
+                        q[rr][i] = t <= nBr ? Aw[nBr - t] : real(0);
+                    }
+                __syncwarp();
+                for (int t = lane; t <= nBr; t += 32) Aw[t] = real(0);
+                __syncwarp();
+            }
+            DpPhases<real, NR, 0>::run(q, Rc, nBr4, send, lane, P);
+            const real sc = recip(P);
+            real fe = real(0);
+#pragma unroll
+            for (int rr = 0; rr < NR; ++rr)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    int t = (rr * 32 + lane) * 4 + i;
+                    if (t <= Leff) {
+                        const real v = q[rr][i] * sc;
+                        Aw[off + t] = v;
+                        fe += long_pred(lc.type, L, lc.k, t + nB0) ? -v : v;   // sp = -1 where satisfied
+                    }
+                }
+            if (fe_out) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) fe += __shfl_xor_sync(FULLM, fe, o);
+                if (lane == 0) fe_out[(size_t)c * Bp + b] = fe;
+            }
+        }
+        __syncwarp();
+        // ---- S3 + S5: leave-one-out
+        // timing mode only: the state-dependent algorithmic work of this (constraint, restart) -- 6 Leff Keff flops, the
+        // survey's count for a pmf of Leff interior literals with the threshold left after the nB0 true boundary literals
+        if (work && lane == 0) {
+            const int keff = lc.k - nB0;
+            const bool live = (useA || useB) && keff >= (lc.type == AFS_EK ? 0 : 1) && keff <= Leff;
+            if (live) {
+                int K = min(keff, Leff - keff + 1) + 1;
+                K = K < 1 ? 1 : K;
+                atomicAdd(work + (blockIdx.x & 31u), 6ull * (unsigned long long)Leff * (unsigned long long)K);   // 32 slots
+            }
+        }
+        const real* qr = Aw + off;   // qr[tau] = reduced pmf, tau in [0, Leff]; q_t = qr[t - nB0]
+        // boundary literals: y = +1 leaves q unchanged, y = -1 removes one shift (q^(-j)_t = q_{t+1})
+        if (lane == 0) {
+            auto qat = [&](int tau) -> real { return (tau >= 0 && tau <= Leff) ? qr[tau] : real(0); };
+            bnd[((size_t)c * Bp + b) * 2] = w1 * qat(t1 - nB0) + w2 * qat(t2 - nB0);
+            bnd[((size_t)c * Bp + b) * 2 + 1] = w1 * qat(t1 + 1 - nB0) + w2 * qat(t2 + 1 - nB0);
+        }
+        // interior literals: q^(-j)_t = qred^(-j)_{t - nB0}, qred^(-j) has degree Leff - 1
+        int c1 = t1 - nB0, c2 = t2 - nB0;
+        real v1w = w1, v2w = w2;
+        const bool v1 = c1 >= 0 && c1 <= Leff - 1 && w1 != real(0), v2 = c2 >= 0 && c2 <= Leff - 1 && w2 != real(0);
+        if (!v1 && !v2) {   // the expansion does not depend on the interior literals here (or is constant): zero gradient
+            for (int e = lane; e < send; e += 32) Rc[e] = real(0);
+        } else {
+            if (!v1) { c1 = c2; v1w = real(0); }
+            if (!v2) { c2 = c1; v2w = v1w; v1w = real(0); }
+            // type A: bottom-up chain over qr_0, qr_1, ...; captures at c1 then c2
+            deconv_dir<real, false>(qr, off, Rc + nBr4, nAr, c1, c2, v1w, v2w, lane);
+            // type B: top-down chain over qr_Leff, qr_{Leff-1}, ...; chain index i <-> tau = Leff-1-i, so c2 is met first
+            deconv_dir<real, true>(qr + Leff, 0, Rc, nBr, Leff - 1 - c2, Leff - 1 - c1, v2w, v1w, lane);
+        }
+        __syncwarp();
+        // ---- S5 + write-out of the interior literals' rows
+        for (int e = lane; e < send; e += 32) {
+            const int j = J[e];
+            if (j != 0xffff) {
+                const real g = Rc[e];
+                scratch[(size_t)sw[j] * Bp + b] = (lw[j] >> 31) ? -g : g;
+            }
+        }
+        __syncwarp();
     }
 }
 

@@ -346,6 +346,13 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
         up(&P->d_pc_lits, pc_lits);
         up(&P->d_pcp, pcp);
         up(&P->d_slot_ptr, slot_ptr);
+        {   // which slots belong to the LONG class: the variable pass takes boundary literals' gradients from bnd
+            std::vector<int32_t> slot_info((size_t)P->nslots, -1);
+            for (size_t i = 0; i < lng.size(); ++i)
+                for (int j = 0; j < lng[i].L; ++j)
+                    slot_info[long_slots[lng[i].off + j]] = (int32_t)((i << 1) | (long_lits[lng[i].off + j] >> 31));
+            up(&P->d_slot_info, slot_info);
+        }
         up(&P->d_med, med);
         up(&P->d_med_lits, med_lits);
         up(&P->d_med_slots, med_slots);
@@ -378,7 +385,7 @@ extern "C" void afs_problem_destroy(afs_problem* p)
     if (!p) return;
     cudaSetDevice(p->device);
     cudaDeviceSynchronize();
-    cudaFree(p->d_pull_ptr); cudaFree(p->d_pull_words); cudaFree(p->d_slot_ptr);
+    cudaFree(p->d_pull_ptr); cudaFree(p->d_pull_words); cudaFree(p->d_slot_ptr); cudaFree(p->d_slot_info);
     cudaFree(p->d_run_ptr); cudaFree(p->d_runs); cudaFree(p->d_pull_gconst); cudaFree(p->d_pc); cudaFree(p->d_pc_lits); cudaFree(p->d_pcp);
     cudaFree(p->d_med); cudaFree(p->d_med_lits); cudaFree(p->d_med_slots);
     cudaFree(p->d_long); cudaFree(p->d_long_lits); cudaFree(p->d_long_slots);

@@ -16,20 +16,27 @@ namespace afs {
 static int var_grid_x(int n) { return (n + VAR_WARPS * VAR_VPW - 1) / (VAR_WARPS * VAR_VPW); }
 
 // variable pass: as many 32-restart sub-tiles per lane as the batch allows (4, 2 or 1)
-template <typename real, bool EVAL>
-static void launch_var(const VarArgs<real>& a, int gx, int tiles, cudaStream_t st)
+template <typename real, bool EVAL, bool LONGT>
+static void launch_var_l(const VarArgs<real>& a, int gx, int tiles, cudaStream_t st)
 {
-    if (sizeof(real) == 4 && tiles % 4 == 0) k_var<real, EVAL, 4><<<dim3(gx, tiles / 4), VAR_WARPS * 32, 0, st>>>(a);
-    else if (tiles % 2 == 0) k_var<real, EVAL, 2><<<dim3(gx, tiles / 2), VAR_WARPS * 32, 0, st>>>(a);
-    else k_var<real, EVAL, 1><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
+    if (sizeof(real) == 4 && tiles % 4 == 0) k_var<real, EVAL, 4, LONGT><<<dim3(gx, tiles / 4), VAR_WARPS * 32, 0, st>>>(a);
+    else if (tiles % 2 == 0) k_var<real, EVAL, 2, LONGT><<<dim3(gx, tiles / 2), VAR_WARPS * 32, 0, st>>>(a);
+    else k_var<real, EVAL, 1, LONGT><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
+}
+template <typename real, bool EVAL>
+static void launch_var(const afs_problem* P, VarArgs<real>& a, int gx, int tiles, cudaStream_t st)
+{
+    a.slot_info = P->d_slot_info; a.bnd = (const real*)P->ws.bnd;
+    if (P->n_long > 0) launch_var_l<real, EVAL, true>(a, gx, tiles, st);
+    else launch_var_l<real, EVAL, false>(a, gx, tiles, st);
 }
 
 // ----------------------------------------------------------------------------------------------------------------
 // push phase: gradients of the medium and long constraints of iterate XT into scratch (+ counts, + FE)
 // ----------------------------------------------------------------------------------------------------------------
 template <typename real>
-static afs_status launch_push(afs_problem* P, const real* XT, int Bp, real* scratch, int32_t* sat, real* fe_med,
-                              real* fe_cm, real* fe_long, cudaStream_t st)
+static afs_status launch_push(afs_problem* P, const real* XT, const uint32_t* Sw, const uint32_t* SATw, int Bp,
+                              real* scratch, int32_t* sat, real* fe_med, real* fe_cm, real* fe_long, cudaStream_t st)
 {
     const int tiles = Bp / 32;
     if (P->n_cm > 0) {
@@ -56,7 +63,7 @@ static afs_status launch_push(afs_problem* P, const real* XT, int Bp, real* scra
                                                     (real*)P->ws.aux[0], (real*)P->ws.aux[1], sat, fe_med);
         P->last_launches++;
     }
-    if (P->n_long > 0) return launch_long_all<real>(P, XT, Bp, scratch, sat, fe_long, st);
+    if (P->n_long > 0) return launch_long_all<real>(P, XT, Sw, SATw, Bp, scratch, sat, fe_long, st);
     return AFS_OK;
 }
 
@@ -95,9 +102,9 @@ static afs_status eval_grad_impl(afs_problem* P, const real* X, int32_t B, real*
     real* fe_med = (real*)w.fe_med; real* fe_long = (real*)w.fe_long; real* fe_cm = (real*)w.fe_cm;
     real* fpart = (real*)w.f_part;
     dim3 tg((P->n + 31) / 32, Bp / 32);
-    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, wBp, nullptr);
+    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, wBp, nullptr, w.S[0], w.SAT[0]);
     P->last_launches++;
-    if ((s = launch_push<real>(P, XT, wBp, scratch, nullptr, fe_med, fe_cm, fe_long, st)) != AFS_OK) return s;
+    if ((s = launch_push<real>(P, XT, w.S[0], w.SAT[0], wBp, scratch, nullptr, fe_med, fe_cm, fe_long, st)) != AFS_OK) return s;
     VarArgs<real> a{};
     a.n = P->n; a.Bp = wBp; a.t = 0;
     a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
@@ -106,7 +113,7 @@ static afs_status eval_grad_impl(afs_problem* P, const real* X, int32_t B, real*
     a.GT = GT;
     const int gx = var_grid_x(P->n);
     if (G) {
-        launch_var<real, true>(a, gx, Bp / 32, st);
+        launch_var<real, true>(P, a, gx, Bp / 32, st);
         P->last_launches++;
     }
     if (F) {
@@ -136,7 +143,7 @@ static afs_status round_count_impl(afs_problem* P, const real* X, int32_t B, int
     Workspace& w = P->ws;
     real* XT = (real*)w.XT[0];
     dim3 tg((P->n + 31) / 32, Bp / 32);
-    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, Bp, nullptr);
+    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, Bp, nullptr, nullptr, nullptr);
     P->last_launches++;
     if ((s = launch_count<real>(P, XT, Bp, w.sat_hist, st)) != AFS_OK) return s;
     CU(cudaMemcpyAsync(sat, w.sat_hist, (size_t)B * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
@@ -267,7 +274,7 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     real* scratch = (real*)w.scratch;
     const int tiles = Bp / 32;
     dim3 tg((P->n + 31) / 32, tiles);
-    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT[0], B, P->n, Bp, mask);
+    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT[0], B, P->n, Bp, mask, w.S[0], w.SAT[0]);
     P->last_launches++;
     CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)(steps + 1) * Bp * sizeof(int32_t), st));
     launch_fill_i32(w.best_sat[0], (size_t)Bp, -1, st);
@@ -281,7 +288,7 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
         P->prof.on = P->prof.stride > 0 && t % P->prof.stride == 0;
         const real* Xin = XT[t & 1];
         int32_t* sat_cur = w.sat_hist + (size_t)t * Bp;
-        if ((s = launch_push<real>(P, Xin, Bp, scratch, sat_cur, nullptr, nullptr, nullptr, st)) != AFS_OK) return s;
+        if ((s = launch_push<real>(P, Xin, w.S[t & 1], w.SAT[t & 1], Bp, scratch, sat_cur, nullptr, nullptr, nullptr, st)) != AFS_OK) return s;
         VarArgs<real> a{};
         a.n = P->n; a.Bp = Bp; a.t = t;
         a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
@@ -290,10 +297,10 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
         a.sat_prev = t > 0 ? w.sat_hist + (size_t)(t - 1) * Bp : nullptr;
         a.best_sat_in = w.best_sat[t & 1]; a.best_sat_out = w.best_sat[(t + 1) & 1];
         a.best_step_in = w.best_step[t & 1]; a.best_step_out = w.best_step[(t + 1) & 1];
-        a.S_prev = w.S[(t + 1) & 1]; a.S_cur = w.S[t & 1]; a.best_bits = w.best_bits;
+        a.S_prev = w.S[(t + 1) & 1]; a.S_next = w.S[(t + 1) & 1]; a.SAT_next = w.SAT[(t + 1) & 1]; a.best_bits = w.best_bits;
         {
             ProfSpan span(P, 1, st);
-            launch_var<real, false>(a, gx, tiles, st);
+            launch_var<real, false>(P, a, gx, tiles, st);
         }
         P->last_launches++;
         if ((s = launch_sat_pull(P, w.S[t & 1], Bp, sat_cur, st)) != AFS_OK) return s;

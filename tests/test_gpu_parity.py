@@ -296,9 +296,11 @@ def case_no_long(B=37):
 @pytest.mark.parametrize("name,B", [("cnf", 70), ("random_cnf", 64), ("mixed", 45), ("xor", 96), ("no_long", 37),
                                     ("mixed", 300), ("cnf", 1200), ("mixed", 1024), ("xor", 4800)])
 def test_resident_kernel_equals_streaming_path(afs, name, B):
-    """The one-launch tile-resident kernel runs the same arithmetic as the per-phase streaming kernels: iterates,
-    best counts, steps and assignments are bit-identical, for every cluster size the batch selects, with and without
-    a mask."""
+    """The one-launch tile-resident kernel runs the same constraint bodies as the per-phase streaming kernels, for
+    every cluster size the batch selects, with and without a mask.  fp64 build: iterates within 1e-12 and every integer
+    output (best_sat, best_step, best_assign) identical.  fp32: the two kernels inline the bodies into different
+    surroundings, so a product may be contracted into an FMA in one and not in the other -- iterates within 2e-6, and
+    the integer outputs identical for every restart whose iterates agree to the bit (the large majority)."""
     import torch
     inst = case_no_long(B) if name == "no_long" else CASES[name](B)
     P = afs.Problem.from_instance(inst)
@@ -306,20 +308,27 @@ def test_resident_kernel_equals_streaming_path(afs, name, B):
     mask = np.zeros(inst.n, np.int8)
     fix = rng.choice(inst.n, size=inst.n // 3, replace=False)
     mask[fix] = 1 - 2 * rng.integers(0, 2, size=fix.size)
-    for steps, mk in ((0, None), (1, None), (12, None), (12, dev(mask))):
-        res = {}
-        for mode in (1, 2):
-            P.set_option(0, mode)
-            X = dev(inst.X0)
-            out = P.pgd_run(X, steps, LR, mask=mk)
-            torch.cuda.synchronize()
-            assert P.info("resident") == (1 if mode == 2 else 0)
-            res[mode] = [X.cpu().numpy()] + [out[k].cpu().numpy() for k in ("best_sat", "best_step", "best_assign")]
-        # X: the two kernels inline the same constraint bodies into different surroundings, so a product may be
-        # contracted into an FMA in one and not in the other: agreement to a few ulp, not to the bit
-        assert np.abs(res[1][0] - res[2][0]).max() <= 2e-6
-        for a, b in zip(res[1][1:3], res[2][1:3]):
-            assert np.mean(a != b) <= 0.01
+    for dtype in (torch.float64, torch.float32):
+        for steps, mk in ((0, None), (1, None), (12, None), (12, dev(mask))):
+            res = {}
+            for mode in (1, 2):
+                P.set_option(0, mode)
+                X = dev(inst.X0, dtype)
+                out = P.pgd_run(X, steps, LR, mask=mk)
+                torch.cuda.synchronize()
+                assert P.info("resident") == (1 if mode == 2 else 0)
+                res[mode] = [X.cpu().numpy()] + [out[k].cpu().numpy() for k in ("best_sat", "best_step", "best_assign")]
+            dX = np.abs(res[1][0] - res[2][0])
+            if dtype == torch.float64:
+                assert dX.max() <= 1e-12, dX.max()
+                for a, b in zip(res[1][1:], res[2][1:]):
+                    assert np.array_equal(a, b)
+            else:
+                assert dX.max() <= 2e-6, dX.max()
+                same = dX.max(axis=1) == 0
+                assert same.mean() >= 0.5
+                for a, b in zip(res[1][1:], res[2][1:]):
+                    assert np.array_equal(a[same], b[same])
     P.set_option(0, 0)
     X = dev(inst.X0)
     P.pgd_run(X, 3, LR)
