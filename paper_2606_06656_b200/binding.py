@@ -153,7 +153,7 @@ class Problem:
     def set_option(self, what: int, value: int):
         _chk(lib().afs_set_option(self._h, what, value), "afs_set_option")
 
-    KERNEL_CLASSES = (["resident", "var", "sat_pull", "cmed"] + ["med%d" % i for i in range(5)] +
+    KERNEL_CLASSES = (["resident", "var", "sat_pull", "cmed", "med0", "long_scan", "glong", "med3", "med4"] +
                       ["long%d" % (i + 1) for i in range(9)] + ["boundary"])
 
     def profile_read(self):

@@ -69,7 +69,9 @@ void free_workspace(afs_problem* P)
     Workspace& w = P->ws;
     free_ptr(w.XT[0]); free_ptr(w.XT[1]); free_ptr(w.scratch); free_ptr(w.aux[0]); free_ptr(w.aux[1]);
     free_ptr(w.sat_hist); free_ptr(w.best_sat[0]); free_ptr(w.best_sat[1]);
-    free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.SAT[0]); free_ptr(w.SAT[1]); free_ptr(w.bnd); free_ptr(w.best_bits);
+    free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.SAT[0]); free_ptr(w.SAT[1]); free_ptr(w.bnd); free_ptr(w.GL);
+    for (int k = 0; k < 4; ++k) free_ptr(w.long_items[k]);
+    free_ptr(w.long_count); free_ptr(w.best_bits);
     free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.fe_cm); free_ptr(w.f_part);
     free_ptr(w.mask_dev); free_ptr(w.host_stage_X); free_ptr(w.host_stage_assign);
     free_ptr(w.host_stage_sat); free_ptr(w.host_stage_step);
@@ -126,7 +128,11 @@ afs_status ensure_workspace(afs_problem* P, int Bp, size_t elem, int64_t sat_row
     A(&w.S[0], n * ntile); A(&w.S[1], n * ntile); A(&w.best_bits, n * ntile);
     A(&w.SAT[0], n * ntile); A(&w.SAT[1], n * ntile);
     A((unsigned char**)&w.bnd, (size_t)P->n_long * nBp * 2 * nelem);
+    A((unsigned char**)&w.GL, (P->n_long > 0 ? n : 0) * nBp * nelem);
+    for (int k = 0; k < 4; ++k) A(&w.long_items[k], (size_t)P->n_long * nBp);
+    A(&w.long_count, (size_t)8);
     if (st != AFS_OK) { afs::free_workspace(P); return st; }
+    CU(cudaMemset(w.long_count, 0, 8 * sizeof(int)));
     w.Bp = nBp; w.elem = nelem; w.sat_rows = nrows; w.bytes = tot;
     return AFS_OK;
 }

@@ -117,7 +117,10 @@ struct Workspace {
     int32_t* best_step[2] = {nullptr, nullptr};
     uint32_t* S[2] = {nullptr, nullptr};   // sign bits [n][Bp/32]: bit r of word (v, tile) = "x_v < 0" for restart 32 tile + r
     uint32_t* SAT[2] = {nullptr, nullptr}; // saturation bits, same layout: |x_v| = 1 (on the boundary of the cube)
+    void* GL = nullptr;                    // real [n][Bp]: the LONG class's share of the gradient (k_glong -> k_var)
     void* bnd = nullptr;                   // real [n_long][Bp][2]: dFE/dy of a boundary literal at y = +1 / y = -1
+    uint4* long_items[4] = {nullptr, nullptr, nullptr, nullptr};   // work lists of the long-constraint kernels, by size class
+    int* long_count = nullptr;             // [2][4] their lengths, two sets used alternately
     uint32_t* best_bits = nullptr;         // [n][Bp/32]
     void* fe_med = nullptr;                // real [n_med][Bp]      (eval_grad only)
     void* fe_long = nullptr;               // real [n_long][Bp]
@@ -153,8 +156,10 @@ struct afs_problem {
     uint32_t* d_pc_lits = nullptr;
     afs::PullClause* d_pcp = nullptr;   // the same clauses packed for the bit-parallel counts
     int32_t* d_slot_ptr = nullptr;      // [n+1] scratch rows of each variable (transposed-CSR order)
-    int32_t* d_slot_info = nullptr;     // [nslots] -1, or for a slot of the LONG class (index in d_long) << 1 | literal negated
-    int64_t nslots = 0;
+    int32_t* d_lslot_ptr = nullptr;     // [n+1] rows of the LONG class of each variable, relative to row nslots_a
+    int32_t* d_lslot_info = nullptr;    // per LONG-class row: (index in d_long) << 1 | literal negated
+    int64_t nslots = 0;                 // all scratch rows: [0, nslots_a) MED / CMED literals, [nslots_a, nslots) LONG literals
+    int64_t nslots_a = 0;
 
     afs::MedCon* d_med = nullptr;       // sorted by bucket
     uint32_t* d_med_lits = nullptr;
@@ -172,6 +177,8 @@ struct afs_problem {
     int32_t* d_long_slots_f = nullptr;
     int64_t long_nnz = 0;
     bool long_folded = false;           // the launches of the current call use the folded lists
+    uint64_t long_iter = 0;             // launches of the long-constraint pass so far (parity selects the counter set)
+    int long_occ[2][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}};   // resident CTAs per SM of the item kernels (per type, size class)
     int32_t long_begin[afs::LONG_BUCKETS + 1] = {0};
     int32_t long_maxL[afs::LONG_BUCKETS] = {0};
 

@@ -4,10 +4,10 @@
 // BASELINE.json.  P:Lnn = PAPER.md line nn.
 #pragma once
 #include "afs_internal.h"
+#include "afs_bits.cuh"
 
 namespace afs {
 
-constexpr unsigned FULL = 0xffffffffu;
 constexpr int VAR_WARPS = 4;   // warps per CTA in the variable pass (8 CTAs per SM; measured 2-3 % ahead of 8 warps x 4 CTAs)
 constexpr int VAR_VPW = 4;     // consecutive variables per warp
 
@@ -503,10 +503,13 @@ struct VarArgs {
     uint32_t* S_next;            // sign / saturation words of X_{t+1}, written with the step (may alias S_prev: the same
     uint32_t* SAT_next;          // thread reads a word of S_prev before it writes that word of S_next)
     uint32_t* best_bits;
-    const int32_t* slot_info;    // LONGT: -1, or (long constraint << 1 | literal negated) of a slot
-    const real* bnd;             // LONGT: [n_long][Bp][2] gradients of boundary literals (y = +1, y = -1)
+    const real* GL;              // LONGT: [n][Bp] the LONG class's share of the gradient (k_glong)
     real* GT;
 };
+
+template <typename real> struct Pair;
+template <> struct Pair<float> { typedef float2 type; };
+template <> struct Pair<double> { typedef double2 type; };
 
 __device__ __forceinline__ float flip(float x, uint32_t signbit) { return __int_as_float(__float_as_int(x) ^ (int)signbit); }
 __device__ __forceinline__ double flip(double x, uint32_t signbit) { return signbit ? -x : x; }
@@ -670,9 +673,7 @@ __device__ __forceinline__ void pull_variable(const uint32_t* __restrict__ runs,
 
 // 32 warps per SM at <= 64 registers: the pass waits on L2 gathers, and occupancy is what hides them -- at
 // 95 registers (2 CTAs per SM) the same code took 1.5x as long on configs[3] (measured: 420 -> 274 us per iteration).
-// LONGT: the instance has LONG-class constraints -- a slot of that class is read from its scratch row only where this
-// restart's x is strictly inside the cube; on the boundary the literal's gradient is one of the pair bnd[c][b] that the
-// long kernel wrote for all boundary literals of the constraint (picked by the literal's truth value).
+// LONGT: the instance has LONG-class constraints; their share of the gradient comes summed from k_glong.
 template <typename real, bool EVAL, int RPL, bool LONGT>
 __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const VarArgs<real> a)
 {
@@ -740,43 +741,20 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
             const int s1 = a.slot_ptr[v + 1];
             int s = a.slot_ptr[v];
             const real* __restrict__ sc = a.scratch + b;
-            if (LONGT) {
-                bool onb[RPL], neg0[RPL];
+            for (; s + 4 <= s1; s += 4) {
 #pragma unroll
-                for (int c = 0; c < RPL; ++c) { onb[c] = x[c] == one || x[c] == -one; neg0[c] = x[c] < real(0); }
-                for (; s < s1; ++s) {
-                    const int info = a.slot_info[s];
-                    if (info < 0) {
-#pragma unroll
-                        for (int c = 0; c < RPL; ++c) g[c] += sc[(size_t)s * Bp + 32 * c];
-                    } else {
-                        const bool lneg = info & 1;
-                        const real* __restrict__ bp = a.bnd + ((size_t)(info >> 1) * Bp + b) * 2;
-#pragma unroll
-                        for (int c = 0; c < RPL; ++c) {
-                            real val;
-                            if (onb[c]) {   // literal true (y = -1) iff (x < 0) != negated; chain rule sign (S5)
-                                const real t = bp[64 * c + ((neg0[c] != lneg) ? 1 : 0)];
-                                val = lneg ? -t : t;
-                            } else {
-                                val = sc[(size_t)s * Bp + 32 * c];
-                            }
-                            g[c] += val;
-                        }
-                    }
+                for (int c = 0; c < RPL; ++c) {
+                    real g0 = sc[(size_t)s * Bp + 32 * c], g1 = sc[(size_t)(s + 1) * Bp + 32 * c];
+                    real g2 = sc[(size_t)(s + 2) * Bp + 32 * c], g3 = sc[(size_t)(s + 3) * Bp + 32 * c];
+                    g[c] += g0; g[c] += g1; g[c] += g2; g[c] += g3;
                 }
-            } else {
-                for (; s + 4 <= s1; s += 4) {
+            }
+            for (; s < s1; ++s)
 #pragma unroll
-                    for (int c = 0; c < RPL; ++c) {
-                        real g0 = sc[(size_t)s * Bp + 32 * c], g1 = sc[(size_t)(s + 1) * Bp + 32 * c];
-                        real g2 = sc[(size_t)(s + 2) * Bp + 32 * c], g3 = sc[(size_t)(s + 3) * Bp + 32 * c];
-                        g[c] += g0; g[c] += g1; g[c] += g2; g[c] += g3;
-                    }
-                }
-                for (; s < s1; ++s)
+                for (int c = 0; c < RPL; ++c) g[c] += sc[(size_t)s * Bp + 32 * c];
+            if (LONGT) {   // the LONG class's share of dF/dx_v, summed by k_glong in its own fixed order
 #pragma unroll
-                    for (int c = 0; c < RPL; ++c) g[c] += sc[(size_t)s * Bp + 32 * c];
+                for (int c = 0; c < RPL; ++c) g[c] += a.GL[(size_t)v * Bp + b + 32 * c];
             }
         }
 #pragma unroll
@@ -801,31 +779,62 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
 }
 
 // ------------------------------------------------------------------------------------------------------------------
+// S6 for the LONG class: GL[v][b] = sum over the LONG-class literals of v, in transposed-CSR order.  warp = (variable,
+// tile), lane <-> restart.  A literal's gradient is its scratch row only where this restart's x_v is strictly inside the
+// cube; on the boundary it is one of the pair bnd[c][b] that the long kernels wrote for ALL boundary literals of the
+// constraint, picked by the literal's truth value (a variable on +-1 is a boundary literal in every constraint it
+// occurs in).  Eight literals per round, their loads issued together: the pass waits on L2 / HBM latency, not on issue.
+// ------------------------------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void __launch_bounds__(256) k_glong(int n, int ntile, int Bp, const int32_t* __restrict__ lslot_ptr,
+                                               const int32_t* __restrict__ lslot_info, const real* __restrict__ Xin,
+                                               const real* __restrict__ lrows /* scratch + nslots_a * Bp */,
+                                               const real* __restrict__ bnd, const int8_t* __restrict__ mask,
+                                               real* __restrict__ GL)
+{
+    const int lane = threadIdx.x & 31;
+    const long long wid = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (wid >= (long long)n * ntile) return;
+    const int v = (int)(wid / ntile), tile = (int)(wid % ntile);
+    if (mask && mask[v] != 0) return;   // a fixed variable never moves: its gradient is not needed
+    const int b = tile * 32 + lane;
+    const real x = Xin[(size_t)v * Bp + b];
+    const bool onb = x == real(1) || x == real(-1);
+    const int neg0 = x < real(0) ? 1 : 0;
+    const real* __restrict__ rows = lrows + b;
+    const real* __restrict__ bb = bnd + (size_t)b * 2;
+    const int s0 = lslot_ptr[v], s1 = lslot_ptr[v + 1];
+    real g = real(0);
+    for (int sb0 = s0; sb0 < s1; sb0 += 32) {
+        const int myinfo = sb0 + lane < s1 ? lslot_info[sb0 + lane] : 0;   // 32 descriptors with one coalesced load
+        const int cnt = min(32, s1 - sb0);
+        for (int k = 0; k < cnt; k += 8) {
+            real t[8];
+            int ln[8];
+#pragma unroll
+            for (int h = 0; h < 8; ++h) {
+                const int kk = k + h < cnt ? k + h : k;
+                const int info = __shfl_sync(FULL, myinfo, kk);
+                ln[h] = info & 1;
+                // literal true (y = -1) iff (x < 0) != negated: the second element of the pair
+                const real* p = onb ? bb + (size_t)(info >> 1) * Bp * 2 + (neg0 ^ ln[h]) : rows + (size_t)(sb0 + kk) * Bp;
+                t[h] = *p;
+            }
+#pragma unroll
+            for (int h = 0; h < 8; ++h)
+                if (k + h < cnt) g += (onb && ln[h]) ? -t[h] : t[h];   // chain rule sign (S5); the rows carry it already
+        }
+    }
+    GL[(size_t)v * Bp + b] = g;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
 // S9 for the PULL class, bit-parallel over restarts: the sign words S[v][tile] (bit r = "x_v < 0" for restart
 // tile*32 + r) written by the variable pass give the truth of 32 restarts of a clause with a few logic ops.
 // thread = (clause, group of TPT restart tiles), lane <-> clause: the literal words are read once, the TPT sign words
 // of a literal are one 4*TPT-byte load, and every load of a clause is independent of the others.  The per-restart
 // totals come from a butterfly transposition (bit_column_sums: lane r collects restart r).  Integers only.
 // ------------------------------------------------------------------------------------------------------------------
-// Column sums of a 32 x 32 bit matrix held one row per lane: returns, in lane r, the number of lanes whose word has
-// bit r set.  Five butterfly steps; after step s a lane keeps the 32 >> s columns whose low s bits match its own lane
-// index, as packed (s+1)-bit counters.
-__device__ __forceinline__ int bit_column_sums(uint32_t w, int lane)
-{
-    uint32_t o;
-    o = __shfl_xor_sync(FULL, w, 1);
-    w = (lane & 1) ? ((w >> 1) & 0x55555555u) + ((o >> 1) & 0x55555555u) : (w & 0x55555555u) + (o & 0x55555555u);
-    o = __shfl_xor_sync(FULL, w, 2);
-    w = (lane & 2) ? ((w >> 2) & 0x33333333u) + ((o >> 2) & 0x33333333u) : (w & 0x33333333u) + (o & 0x33333333u);
-    o = __shfl_xor_sync(FULL, w, 4);
-    w = (lane & 4) ? ((w >> 4) & 0x0f0f0f0fu) + ((o >> 4) & 0x0f0f0f0fu) : (w & 0x0f0f0f0fu) + (o & 0x0f0f0f0fu);
-    o = __shfl_xor_sync(FULL, w, 8);
-    w = (lane & 8) ? ((w >> 8) & 0x00ff00ffu) + ((o >> 8) & 0x00ff00ffu) : (w & 0x00ff00ffu) + (o & 0x00ff00ffu);
-    o = __shfl_xor_sync(FULL, w, 16);
-    w = (lane & 16) ? (w >> 16) + (o >> 16) : (w & 0xffffu) + (o & 0xffffu);
-    return (int)w;
-}
-
 template <int TPT>
 struct SWords { uint32_t w[TPT]; };
 template <int TPT>

@@ -2,6 +2,8 @@
 // objects so that the fp32 product kernels and the fp64 verification build compile in parallel): error macro, the
 // per-launch profiler span, and the non-template helpers defined once in afs_common.cu.
 #pragma once
+#include <algorithm>
+
 #include "afs_internal.h"
 
 #define CU(x)                                \

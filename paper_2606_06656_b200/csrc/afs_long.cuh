@@ -27,6 +27,7 @@
 // aligned 16-byte blocks from index 0 and the bottom-up chains after at most three scalar steps.
 #pragma once
 #include "afs_internal.h"
+#include "afs_bits.cuh"
 
 namespace afs {
 
@@ -205,102 +206,245 @@ __device__ __forceinline__ bool long_pred(int type, int L, int k, int t)
     }
 }
 
-// One CTA = one constraint x one tile of 32 restarts; its RPC warps take the restarts of the tile in turn (warp w:
-// restarts w, w + RPC, ...), each with its own list / pmf buffers.
-//   words    the CTA first stages, per literal, the tile's "true" word (sign word of the variable, flipped for a negated
-//            literal) and "saturated" word (|x| = 1) -- two 4-byte loads per literal for 32 restarts instead of 32
-//            element gathers.  Bit r of the words classifies literal j for restart r: boundary-true, boundary-false,
-//            interior with y < 0 (type B), interior with y >= 0 (type A).
-//   pass 1   per restart, ballots over the words: true count tc (S9), boundary-true count nB0, nBr, nAr.  A restart
-//            with no interior literal is finished here: its pmf is the point mass at nB0, the objective is -+1 and the
-//            two boundary gradients are d_t picked at nB0 (no list, no gather, no arithmetic).
-//   pass 2   otherwise: list positions from the same ballots, x gathered for the INTERIOR literals only.
-//   output   boundary literals: ONE pair (dFE/dy at y = +1, at y = -1) per (constraint, restart) in bnd[c][b][2]; the
-//            variable pass picks by its own x (a variable on +-1 is a boundary literal in every constraint it occurs
-//            in).  Interior literals: their own scratch rows, as the other materialising classes.
-template <typename real, int NR, int RPC>
-__global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ cons, int c_begin,
-                                                   const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
-                                                   const real* __restrict__ XT, const uint32_t* __restrict__ Sw,
-                                                   const uint32_t* __restrict__ SATw, int ntile, int Bp,
-                                                   real* __restrict__ scratch, real* __restrict__ bnd,
-                                                   int32_t* __restrict__ sat, real* __restrict__ fe_out, int LS, int QS,
-                                                   unsigned long long* __restrict__ work)
+// Forward pmf of the interior literals of one restart (list ratios Rc[0, send), nBr of them type B), NRR rows of 128
+// cells in registers; leaves the reduced pmf at Aw[off + t], t = 0..Leff, and returns this lane's share of
+// FE = sum_t sp_t q_t (sp = -1 where the constraint holds with t + nB0 true literals).
+template <typename real, int NRR>
+__device__ __forceinline__ real long_forward(const LongCon& lc, const int L, real* __restrict__ Rc, real* __restrict__ Aw,
+                                             const int nBr, const int nBr4, const int send, const int Leff, const int nB0,
+                                             const int off, const int lane, const int QS)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    real* RcAll = reinterpret_cast<real*>(smem_raw);              // [RPC][LS]  ratios in list order, then gradients
-    real* AAll = RcAll + RPC * LS;                                // [RPC][QS]  the pmf
-    uint32_t* TW = reinterpret_cast<uint32_t*>(AAll + RPC * QS);  // [LS] true words of the tile
-    uint32_t* SW = TW + LS;                                       // [LS] saturated words
-    uint16_t* JAll = reinterpret_cast<uint16_t*>(SW + LS);        // [RPC][LS]  literal index at each list position
-    constexpr int NT = RPC * 32;
     constexpr unsigned FULLM = 0xffffffffu;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int c = c_begin + (int)(blockIdx.x / (unsigned)ntile);
-    const int tile = (int)(blockIdx.x % (unsigned)ntile);
+    real q[NRR][4];
+#pragma unroll
+    for (int rr = 0; rr < NRR; ++rr)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) q[rr][i] = real(0);
+    if (lane == 0) q[0][0] = real(1);
+    real P = real(1);
+    for (int t = lane; t < min(QS, Leff + 12); t += 32) Aw[t] = real(0);   // cells the reversal, the pmf and the chains' blocks touch
+    __syncwarp();
+    if (nBr > 0) {
+        DpPhases<real, NRR, 0>::run(q, Rc, 0, nBr4, lane, P);
+        // prod_B (z + R_j) is the reversal of prod_B (1 + R_j w): c_t -> c_{nBr - t}, through shared memory
+#pragma unroll
+        for (int rr = 0; rr < NRR; ++rr)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                int t = (rr * 32 + lane) * 4 + i;
+                if (t <= nBr) Aw[t] = q[rr][i];
+            }
+        __syncwarp();
+#pragma unroll
+        for (int rr = 0; rr < NRR; ++rr)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                int t = (rr * 32 + lane) * 4 + i;
+                q[rr][i] = t <= nBr ? Aw[nBr - t] : real(0);
+            }
+        __syncwarp();
+        for (int t = lane; t <= nBr; t += 32) Aw[t] = real(0);
+        __syncwarp();
+    }
+    DpPhases<real, NRR, 0>::run(q, Rc, nBr4, send, lane, P);
+    const real sc = recip(P);
+    real fe = real(0);
+#pragma unroll
+    for (int rr = 0; rr < NRR; ++rr)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            int t = (rr * 32 + lane) * 4 + i;
+            if (t <= Leff) {
+                const real v = q[rr][i] * sc;
+                Aw[off + t] = v;
+                fe += long_pred(lc.type, L, lc.k, t + nB0) ? -v : v;
+            }
+        }
+    (void)FULLM;
+    return fe;
+}
+
+// The same for Leff <= 31: one pmf cell per lane (cell t in lane t), two instructions per literal.  No rescaling on
+// the way: the un-normalised coefficients grow by at most 2 per literal (R <= 1), 2^31 in all.
+template <typename real>
+__device__ __forceinline__ real long_forward_tiny(const LongCon& lc, const int L, const real* __restrict__ Rc,
+                                                  real* __restrict__ Aw, const int nBr, const int nBr4, const int nAr,
+                                                  const int Leff, const int nB0, const int off, const int lane)
+{
+    constexpr unsigned FULLM = 0xffffffffu;
+    real q = lane == 0 ? real(1) : real(0), P = real(1);
+    for (int e = 0; e < nBr; ++e) {
+        const real R = Rc[e];
+        real lo = __shfl_up_sync(FULLM, q, 1);
+        if (lane == 0) lo = real(0);
+        q = fma(R, lo, q);
+        P = fma(P, R, P);
+    }
+    if (nBr > 0) {   // prod_B (z + R_j) is the reversal of prod_B (1 + R_j w)
+        const real rv = __shfl_sync(FULLM, q, (nBr - lane) & 31);
+        q = lane <= nBr ? rv : real(0);
+    }
+    for (int e = 0; e < nAr; ++e) {
+        const real R = Rc[nBr4 + e];
+        real lo = __shfl_up_sync(FULLM, q, 1);
+        if (lane == 0) lo = real(0);
+        q = fma(R, lo, q);
+        P = fma(P, R, P);
+    }
+    const real v = q * recip(P);
+    Aw[lane] = real(0); Aw[32 + lane] = real(0);   // cells the pmf (offset <= 3) and the chains' 16-byte blocks touch
+    __syncwarp();
+    real fe = real(0);
+    if (lane <= Leff) {
+        Aw[off + lane] = v;
+        fe = long_pred(lc.type, L, lc.k, lane + nB0) ? -v : v;
+    }
+    return fe;
+}
+
+// Two kernels per PGD iteration.
+//
+// k_long_scan   warp = (constraint, tile of 32 restarts).  Lane <-> literal: the tile's "true" word (sign word of the
+//               variable, flipped for a negated literal) and "saturated" word (|x| = 1) of 32 literals at a time -- two
+//               4-byte loads per literal for 32 restarts instead of 32 element gathers -- give three 32 x 32 bit
+//               matrices (boundary-true, interior-true = type B, interior-false = type A) whose column sums (butterfly,
+//               lane r <-> restart r afterwards) are nB0, nBr, nAr of every restart.  Then, lane <-> restart:
+//                 S9   the constraint holds for nB0 + nBr true literals -> integer add to sat[b];
+//                 Leff = nBr + nAr = 0 (every literal on the boundary): Q(z) = z^nB0, the objective is -+1 and the two
+//                      boundary gradients are d_t picked at nB0 -- finished here, no list, no gather, no
+//                      arithmetic;
+//                 otherwise the pair (constraint, restart) is appended to the work list of its size class (rows of 128
+//                      pmf cells that Leff needs); the order of a list does not enter any result.
+// k_long_items  warp = one work-list entry.  Interior literals found from the same words (one restart's bits), x gathered
+//               for these only, forward pmf, leave-one-out chains.
+// Output of both: boundary literals get ONE pair (dFE/dy at y = +1, at y = -1) per (constraint, restart) in
+// bnd[c][b][2]; the variable pass picks by its own x (a variable on +-1 is a boundary literal in every constraint it
+// occurs in).  Interior literals get their own scratch rows, as in the other materialising classes.
+constexpr int LONG_CLASSES = 4;
+__host__ __device__ constexpr int long_class_rows(int cls) { return cls == 0 ? 1 : cls == 1 ? 3 : cls == 2 ? 5 : 9; }
+// largest Leff of a class: its rows hold cells 0 .. 128 rows - 1, the padded list may run 6 entries beyond Leff
+__host__ __device__ constexpr int long_class_maxleff(int cls) { return 128 * long_class_rows(cls) - 8; }
+
+struct LongLists {
+    uint4* items[LONG_CLASSES];   // (constraint, restart, nB0 | nBr << 16, nAr)
+    int* count;                   // [2][LONG_CLASSES]: set (t & 1) is filled by iteration t, the other one reset
+};
+
+template <typename real>
+__global__ void __launch_bounds__(128) k_long_scan(const LongCon* __restrict__ cons, int n_long,
+                                                   const uint32_t* __restrict__ lits,
+                                                   const uint32_t* __restrict__ Sw, const uint32_t* __restrict__ SATw,
+                                                   int ntile, int Bp, real* __restrict__ bnd, int32_t* __restrict__ sat,
+                                                   real* __restrict__ fe_out, LongLists wl, int set)
+{
+    const int lane = threadIdx.x & 31;
+    const long long wid = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
+    if (blockIdx.x == 0 && threadIdx.x < LONG_CLASSES) wl.count[(set ^ 1) * LONG_CLASSES + threadIdx.x] = 0;
+    if (wid >= (long long)n_long * ntile) return;
+    const int c = (int)(wid / ntile), tile = (int)(wid % ntile);
     const LongCon lc = cons[c];
     const int L = lc.L;
     const uint32_t* lw = lits + lc.off;
-    const int32_t* sw = slots + lc.off;
-    for (int j = tid; j < L; j += NT) {
-        const uint32_t w = lw[j];
-        const size_t wi = (size_t)(w & LIT_VAR) * ntile + tile;
-        const uint32_t s = Sw[wi];
-        TW[j] = (w >> 31) ? ~s : s;
-        SW[j] = SATw[wi];
+    int nB0 = 0, nBr = 0, nAr = 0;
+    for (int j0 = 0; j0 < L; j0 += 32) {
+        const int j = j0 + lane;
+        uint32_t tw = 0u, sw = 0xffffffffu;
+        if (j < L) {
+            const uint32_t w = lw[j];
+            const size_t wi = (size_t)(w & LIT_VAR) * ntile + tile;
+            const uint32_t s = Sw[wi];
+            tw = (w >> 31) ? ~s : s;
+            sw = SATw[wi];
+        }
+        nB0 += bit_column_sums(tw & sw, lane);
+        nBr += bit_column_sums(tw & ~sw, lane);
+        nAr += bit_column_sums(~tw & ~sw, lane);
     }
-    __syncthreads();
+    // lane <-> restart from here on
+    const int b = tile * 32 + lane;
+    const int Leff = nBr + nAr;
+    if (sat && long_pred(lc.type, L, lc.k, nB0 + nBr)) atomicAdd(&sat[b], 1);
+    if (Leff == 0) {
+        // removing a false literal leaves the point mass at nB0, removing a true one moves it to nB0 - 1
+        const int tA = lc.tA - nB0, tB = lc.tB - nB0;
+        const real wA = (real)lc.wA, wB = (real)lc.wB;
+        real* o = bnd + ((size_t)c * Bp + b) * 2;
+        o[0] = (tA == 0 ? wA : real(0)) + (tB == 0 ? wB : real(0));
+        o[1] = (tA == -1 ? wA : real(0)) + (tB == -1 ? wB : real(0));
+        if (fe_out) fe_out[(size_t)c * Bp + b] = long_pred(lc.type, L, lc.k, nB0) ? real(-1) : real(1);
+    }
+    const int cls = Leff == 0 ? -1 : Leff <= long_class_maxleff(0) ? 0 : Leff <= long_class_maxleff(1) ? 1
+                  : Leff <= long_class_maxleff(2) ? 2 : 3;
+    const unsigned lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int k = 0; k < LONG_CLASSES; ++k) {
+        const unsigned m = __ballot_sync(FULL, cls == k);
+        if (m) {
+            int base = 0;
+            if (lane == 0) base = atomicAdd(&wl.count[set * LONG_CLASSES + k], __popc(m));
+            base = __shfl_sync(FULL, base, 0);
+            if (cls == k) wl.items[k][base + __popc(m & lt)] = make_uint4((unsigned)c, (unsigned)b, (unsigned)nB0 | ((unsigned)nBr << 16), (unsigned)nAr);
+        }
+    }
+}
+
+// WPC warps per CTA, each with its own list / pmf buffers of LS / QS entries; persistent over the class's work list.
+template <typename real, int NR, int WPC>
+__global__ void __launch_bounds__(WPC * 32) k_long_items(const LongCon* __restrict__ cons,
+                                                         const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
+                                                         const real* __restrict__ XT, const uint32_t* __restrict__ Sw,
+                                                         const uint32_t* __restrict__ SATw, int ntile, int Bp,
+                                                         real* __restrict__ scratch, real* __restrict__ bnd,
+                                                         real* __restrict__ fe_out, const uint4* __restrict__ items,
+                                                         const int* __restrict__ count, int LS, int QS,
+                                                         unsigned long long* __restrict__ work)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    real* RcAll = reinterpret_cast<real*>(smem_raw);              // [WPC][LS]  ratios in list order, then gradients
+    real* AAll = RcAll + WPC * LS;                                // [WPC][QS]  the pmf
+    uint16_t* JAll = reinterpret_cast<uint16_t*>(AAll + WPC * QS);   // [WPC][LS]  literal index at each list position
+    constexpr unsigned FULLM = 0xffffffffu;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     real* Rc = RcAll + warp * LS;
     real* Aw = AAll + warp * QS;
     uint16_t* J = JAll + warp * LS;
-    const bool useA = lc.wA != 0.f, useB = lc.wB != 0.f;
-    // capture points in true-count index space, t1 <= t2 (equal if only one is used)
-    int t1 = lc.tA, t2 = lc.tB;
-    real w1 = (real)lc.wA, w2 = (real)lc.wB;
-    if (!useA) { t1 = t2; w1 = real(0); }
-    if (!useB) { t2 = t1; w2 = w1; w1 = real(0); }
-    if (t1 > t2) { int tt = t1; t1 = t2; t2 = tt; real ww = w1; w1 = w2; w2 = ww; }
     const unsigned lt = (1u << lane) - 1u;
+    const int n_items = *count;
 #pragma unroll 1
-    for (int r = warp; r < 32; r += RPC) {
-        const int b = tile * 32 + r;
-        // ---- pass 1: counts of the four literal kinds from the words
-        int tc = 0, nB0 = 0, nBr = 0, nAr = 0;
-        for (int j0 = 0; j0 < L; j0 += 32) {
-            const int j = j0 + lane;
-            const bool act = j < L;
-            const bool tb = act && ((TW[act ? j : 0] >> r) & 1u), sb = !act || ((SW[act ? j : 0] >> r) & 1u);
-            const unsigned mT = __ballot_sync(FULLM, tb), mS = __ballot_sync(FULLM, sb);
-            const unsigned mAct = L - j0 >= 32 ? FULLM : (1u << (L - j0)) - 1u;
-            tc += __popc(mT); nB0 += __popc(mT & mS); nBr += __popc(mT & ~mS); nAr += __popc(~mT & ~mS & mAct);
-        }
+    for (int it = blockIdx.x * WPC + warp; it < n_items; it += gridDim.x * WPC) {
+        const uint4 ent = items[it];
+        const int c = (int)ent.x, b = (int)ent.y, tile = b >> 5, r = b & 31;
+        const int nB0 = (int)(ent.z & 0xffffu), nBr = (int)(ent.z >> 16), nAr = (int)ent.w;
+        const LongCon lc = cons[c];
+        const int L = lc.L;
+        const uint32_t* lw = lits + lc.off;
+        const int32_t* sw = slots + lc.off;
         const int Leff = nBr + nAr;
-        if (lane == 0 && sat && long_pred(lc.type, L, lc.k, tc)) atomicAdd(&sat[b], 1);
-        auto dpick = [&](int tau) -> real {   // w1 [t1 = tau] + w2 [t2 = tau]: d_t at the point mass
-            return (tau == t1 - nB0 ? w1 : real(0)) + (tau == t2 - nB0 ? w2 : real(0));
-        };
-        if (Leff == 0) {
-            // every literal on the boundary: Q(z) = z^nB0.  Removing a false literal leaves the mass at nB0, removing a
-            // true one moves it to nB0 - 1 (P:L52 d_t; exact, no arithmetic)
-            if (lane == 0) {
-                bnd[((size_t)c * Bp + b) * 2] = dpick(0);
-                bnd[((size_t)c * Bp + b) * 2 + 1] = dpick(-1);
-                if (fe_out) fe_out[(size_t)c * Bp + b] = long_pred(lc.type, L, lc.k, nB0) ? real(-1) : real(1);
-            }
-            continue;
-        }
-        // ---- pass 2: lists [B interior, pad | A interior, pad] of literal indices; x gathered for these only
+        // lists [B interior, pad | A interior, pad] of literal indices, from this restart's bits of the words; two groups
+        // of 32 literals per round with their loads in front.  x is gathered for the listed literals only.
         const int nBr4 = (nBr + 3) & ~3, nAr4 = (nAr + 3) & ~3, send = nBr4 + nAr4;
         {
             int pBr = 0, pAr = nBr4;
-            for (int j0 = 0; j0 < L; j0 += 32) {
-                const int j = j0 + lane;
-                const bool act = j < L;
-                const bool tb = act && ((TW[act ? j : 0] >> r) & 1u), intr = act && !((SW[act ? j : 0] >> r) & 1u);
-                const bool cBr = intr && tb, cAr = intr && !tb;
-                const unsigned mBr = __ballot_sync(FULLM, cBr), mAr = __ballot_sync(FULLM, cAr);
-                if (intr) J[cBr ? pBr + __popc(mBr & lt) : pAr + __popc(mAr & lt)] = (uint16_t)j;
-                pBr += __popc(mBr); pAr += __popc(mAr);
+            for (int j0 = 0; j0 < L; j0 += 64) {
+                uint32_t w[2], sg[2], st[2];
+#pragma unroll
+                for (int h = 0; h < 2; ++h) { const int j = j0 + 32 * h + lane; w[h] = j < L ? lw[j] : 0u; }
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int j = j0 + 32 * h + lane;
+                    const size_t wi = (size_t)(w[h] & LIT_VAR) * ntile + tile;
+                    sg[h] = j < L ? Sw[wi] : 0u;
+                    st[h] = j < L ? SATw[wi] : 0xffffffffu;
+                }
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int j = j0 + 32 * h + lane;
+                    const bool tb = (((sg[h] >> r) ^ (w[h] >> 31)) & 1u) != 0, intr = ((st[h] >> r) & 1u) == 0;
+                    const bool cBr = intr && tb, cAr = intr && !tb;
+                    const unsigned mBr = __ballot_sync(FULLM, cBr), mAr = __ballot_sync(FULLM, cAr);
+                    if (intr) J[cBr ? pBr + __popc(mBr & lt) : pAr + __popc(mAr & lt)] = (uint16_t)j;
+                    pBr += __popc(mBr); pAr += __popc(mAr);
+                }
             }
             if (lane < nBr4 - nBr) J[nBr + lane] = 0xffffu;
             if (lane < nAr4 - nAr) J[nBr4 + nAr + lane] = 0xffffu;
@@ -323,51 +467,9 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
         // ---- S2: forward pmf of the interior literals
         const int off = (3 - Leff) & 3;
         {
-            real q[NR][4];
-#pragma unroll
-            for (int rr = 0; rr < NR; ++rr)
-#pragma unroll
-                for (int i = 0; i < 4; ++i) q[rr][i] = real(0);
-            if (lane == 0) q[0][0] = real(1);
-            real P = real(1);
-            for (int t = lane; t < QS; t += 32) Aw[t] = real(0);
-            __syncwarp();
-            if (nBr > 0) {
-                DpPhases<real, NR, 0>::run(q, Rc, 0, nBr4, lane, P);
-                // prod_B (z + R_j) is the reversal of prod_B (1 + R_j w): c_t -> c_{nBr - t}, through shared memory
-#pragma unroll
-                for (int rr = 0; rr < NR; ++rr)
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        int t = (rr * 32 + lane) * 4 + i;
-                        if (t <= nBr) Aw[t] = q[rr][i];
-                    }
-                __syncwarp();
-#pragma unroll
-                for (int rr = 0; rr < NR; ++rr)
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        int t = (rr * 32 + lane) * 4 + i;
-                        q[rr][i] = t <= nBr ? Aw[nBr - t] : real(0);
-                    }
-                __syncwarp();
-                for (int t = lane; t <= nBr; t += 32) Aw[t] = real(0);
-                __syncwarp();
-            }
-            DpPhases<real, NR, 0>::run(q, Rc, nBr4, send, lane, P);
-            const real sc = recip(P);
-            real fe = real(0);
-#pragma unroll
-            for (int rr = 0; rr < NR; ++rr)
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    int t = (rr * 32 + lane) * 4 + i;
-                    if (t <= Leff) {
-                        const real v = q[rr][i] * sc;
-                        Aw[off + t] = v;
-                        fe += long_pred(lc.type, L, lc.k, t + nB0) ? -v : v;   // sp = -1 where satisfied
-                    }
-                }
+            real fe;
+            if (NR == 1 && Leff <= 31) fe = long_forward_tiny<real>(lc, L, Rc, Aw, nBr, nBr4, nAr, Leff, nB0, off, lane);
+            else fe = long_forward<real, NR>(lc, L, Rc, Aw, nBr, nBr4, send, Leff, nB0, off, lane, QS);
             if (fe_out) {
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) fe += __shfl_xor_sync(FULLM, fe, o);
@@ -376,6 +478,13 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
         }
         __syncwarp();
         // ---- S3 + S5: leave-one-out
+        const bool useA = lc.wA != 0.f, useB = lc.wB != 0.f;
+        // capture points in true-count index space, t1 <= t2 (equal if only one is used)
+        int t1 = lc.tA, t2 = lc.tB;
+        real w1 = (real)lc.wA, w2 = (real)lc.wB;
+        if (!useA) { t1 = t2; w1 = real(0); }
+        if (!useB) { t2 = t1; w2 = w1; w1 = real(0); }
+        if (t1 > t2) { int tt = t1; t1 = t2; t2 = tt; real ww = w1; w1 = w2; w2 = ww; }
         // timing mode only: the state-dependent algorithmic work of this (constraint, restart) -- 6 Leff Keff flops, the
         // survey's count for a pmf of Leff interior literals with the threshold left after the nB0 true boundary literals
         if (work && lane == 0) {
@@ -396,17 +505,16 @@ __global__ void __launch_bounds__(RPC * 32) k_long(const LongCon* __restrict__ c
         }
         // interior literals: q^(-j)_t = qred^(-j)_{t - nB0}, qred^(-j) has degree Leff - 1
         int c1 = t1 - nB0, c2 = t2 - nB0;
-        real v1w = w1, v2w = w2;
         const bool v1 = c1 >= 0 && c1 <= Leff - 1 && w1 != real(0), v2 = c2 >= 0 && c2 <= Leff - 1 && w2 != real(0);
         if (!v1 && !v2) {   // the expansion does not depend on the interior literals here (or is constant): zero gradient
             for (int e = lane; e < send; e += 32) Rc[e] = real(0);
         } else {
-            if (!v1) { c1 = c2; v1w = real(0); }
-            if (!v2) { c2 = c1; v2w = v1w; v1w = real(0); }
+            if (!v1) { c1 = c2; w1 = real(0); }
+            if (!v2) { c2 = c1; w2 = w1; w1 = real(0); }
             // type A: bottom-up chain over qr_0, qr_1, ...; captures at c1 then c2
-            deconv_dir<real, false>(qr, off, Rc + nBr4, nAr, c1, c2, v1w, v2w, lane);
+            deconv_dir<real, false>(qr, off, Rc + nBr4, nAr, c1, c2, w1, w2, lane);
             // type B: top-down chain over qr_Leff, qr_{Leff-1}, ...; chain index i <-> tau = Leff-1-i, so c2 is met first
-            deconv_dir<real, true>(qr + Leff, 0, Rc, nBr, Leff - 1 - c2, Leff - 1 - c1, v2w, v1w, lane);
+            deconv_dir<real, true>(qr + Leff, 0, Rc, nBr, Leff - 1 - c2, Leff - 1 - c1, w2, w1, lane);
         }
         __syncwarp();
         // ---- S5 + write-out of the interior literals' rows

@@ -1,62 +1,71 @@
 // afs_long_launch.cuh -- launches of the long-constraint kernels (afs_long.cuh), one translation unit per arithmetic
-// type (afs_long_f32.cu, afs_long_f64.cu) so that their many instantiations compile beside the rest of the library.
+// type (afs_long_f32.cu, afs_long_f64.cu) so that their instantiations compile beside the rest of the library.
 #pragma once
 #include "afs_long.cuh"
 #include "afs_launch.h"
 
 namespace afs {
 
-template <typename real, int NR, int RPC>
-static afs_status launch_long_rpc(afs_problem* P, int bucket, const real* XT, const uint32_t* Sw, const uint32_t* SATw,
-                                  int Bp, real* scratch, int32_t* sat, real* fe, cudaStream_t st, int LS, int QS,
-                                  size_t smem)
+template <typename real, int CLS>
+static afs_status launch_long_items(afs_problem* P, const LongLists& wl, int set, const real* XT, const uint32_t* Sw,
+                                    const uint32_t* SATw, int Bp, real* scratch, real* fe, cudaStream_t st)
 {
-    int c0 = P->long_begin[bucket], c1 = P->long_begin[bucket + 1];
-    if (smem > 48 * 1024)   // per device and per instantiation: set before every launch, never cached
-        CU(cudaFuncSetAttribute(k_long<real, NR, RPC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const int ntile = Bp / 32;
-    long long blocks = (long long)(c1 - c0) * ntile;
-    if (blocks > 0x7fffffffLL) return AFS_ERR_UNSUPPORTED;
+    constexpr int NR = long_class_rows(CLS);
+    constexpr int WPC = sizeof(real) == 8 ? 4 : 8;
+    int Lmax = 0;
+    for (int i = 0; i < LONG_BUCKETS; ++i) Lmax = std::max(Lmax, P->long_maxL[i]);
+    if (CLS > 0 && Lmax <= long_class_maxleff(CLS - 1)) return AFS_OK;   // no constraint can reach this class
+    const int LS = 128 * NR, QS = 128 * NR + 8;
+    const size_t smem = (size_t)WPC * ((size_t)LS * (sizeof(real) + sizeof(uint16_t)) + (size_t)QS * sizeof(real));
+    auto kern = k_long_items<real, NR, WPC>;
+    const int ti = sizeof(real) == 8 ? 1 : 0;
+    if (smem > 48 * 1024)   // per device and per instantiation: set before every launch, never cached process-wide
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (P->long_occ[ti][CLS] == 0) {   // per handle, hence per device
+        int occ = 0;
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, WPC * 32, smem));
+        if (occ < 1) return AFS_ERR_UNSUPPORTED;
+        P->long_occ[ti][CLS] = occ;
+    }
+    // persistent over the work list; never more CTAs than the list can hold entries for
+    long long cap = ((long long)P->n_long * Bp + WPC - 1) / WPC;
+    const int grid = (int)std::min<long long>((long long)P->sm_count * P->long_occ[ti][CLS], cap < 1 ? 1 : cap);
     ProfSpan span(P, 8 + NR, st);
     const bool fo = P->long_folded;
     unsigned long long* work = nullptr;
     { afs_status ws = prof_work_slot(P, 8 + NR, st, &work); if (ws != AFS_OK) return ws; }
-    k_long<real, NR, RPC><<<(unsigned)blocks, RPC * 32, smem, st>>>(fo ? P->d_long_f : P->d_long, c0,
-                                                                    fo ? P->d_long_lits_f : P->d_long_lits,
-                                                                    fo ? P->d_long_slots_f : P->d_long_slots, XT, Sw, SATw,
-                                                                    ntile, Bp, scratch, (real*)P->ws.bnd, sat, fe, LS, QS,
-                                                                    work);
+    kern<<<grid, WPC * 32, smem, st>>>(fo ? P->d_long_f : P->d_long, fo ? P->d_long_lits_f : P->d_long_lits,
+                                        fo ? P->d_long_slots_f : P->d_long_slots, XT, Sw, SATw, Bp / 32, Bp, scratch,
+                                        (real*)P->ws.bnd, fe, wl.items[CLS], wl.count + set * LONG_CLASSES + CLS, LS, QS,
+                                        work);
     P->last_launches++;
     return AFS_OK;
-}
-
-template <typename real, int NR>
-static afs_status launch_long(afs_problem* P, int bucket, const real* XT, const uint32_t* Sw, const uint32_t* SATw, int Bp,
-                              real* scratch, int32_t* sat, real* fe, cudaStream_t st)
-{
-    if (P->long_begin[bucket + 1] <= P->long_begin[bucket]) return AFS_OK;
-    int Lmax = P->long_maxL[bucket];
-    int LS = ((Lmax + 8 + 31) / 32) * 32;            // list order: L entries + at most 6 neutral ones
-    int QS = ((Lmax + 1 + 3 + 3) / 4) * 4 + 4;       // pmf q_0..q_L behind an offset of at most 3
-    const size_t per_restart = (size_t)LS * (sizeof(real) + sizeof(uint16_t)) + (size_t)QS * sizeof(real);
-    const size_t words = (size_t)LS * 8;             // true + saturated words of the tile
-    // warps per CTA (restarts in flight): 8, or 4 where that packs more warps on an SM (the longest rows in fp64)
-    const size_t budget = 227 * 1024;
-    const int w8 = (int)(budget / (8 * per_restart + words + 1024)) * 8, w4 = (int)(budget / (4 * per_restart + words + 1024)) * 4;
-    if (w4 == 0) return AFS_ERR_UNSUPPORTED;
-    if (w8 >= w4 || w8 >= 32)
-        return launch_long_rpc<real, NR, 8>(P, bucket, XT, Sw, SATw, Bp, scratch, sat, fe, st, LS, QS, 8 * per_restart + words);
-    return launch_long_rpc<real, NR, 4>(P, bucket, XT, Sw, SATw, Bp, scratch, sat, fe, st, LS, QS, 4 * per_restart + words);
 }
 
 template <typename real>
 afs_status launch_long_all(afs_problem* P, const real* XT, const uint32_t* Sw, const uint32_t* SATw, int Bp, real* scratch,
                            int32_t* sat, real* fe, cudaStream_t st)
 {
-    afs_status s = AFS_OK;
-#define LONG_CASE(NRV) if (s == AFS_OK) s = launch_long<real, NRV>(P, NRV - 1, XT, Sw, SATw, Bp, scratch, sat, fe, st);
-    LONG_CASE(1) LONG_CASE(2) LONG_CASE(3) LONG_CASE(4) LONG_CASE(5) LONG_CASE(6) LONG_CASE(7) LONG_CASE(8) LONG_CASE(9)
-#undef LONG_CASE
+    if (P->n_long == 0) return AFS_OK;
+    LongLists wl;
+    for (int k = 0; k < LONG_CLASSES; ++k) wl.items[k] = P->ws.long_items[k];
+    wl.count = P->ws.long_count;
+    const int set = (int)(P->long_iter++ & 1);
+    const bool fo = P->long_folded;
+    const int ntile = Bp / 32;
+    const long long warps = (long long)P->n_long * ntile;
+    if ((warps + 3) / 4 > 0x7fffffffLL) return AFS_ERR_UNSUPPORTED;
+    {
+        ProfSpan span(P, 5, st);
+        k_long_scan<real><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(fo ? P->d_long_f : P->d_long, (int)P->n_long,
+                                                                      fo ? P->d_long_lits_f : P->d_long_lits, Sw, SATw, ntile,
+                                                                      Bp, (real*)P->ws.bnd, sat, fe, wl, set);
+        P->last_launches++;
+    }
+    afs_status s = launch_long_items<real, 0>(P, wl, set, XT, Sw, SATw, Bp, scratch, fe, st);
+    if (s == AFS_OK) s = launch_long_items<real, 1>(P, wl, set, XT, Sw, SATw, Bp, scratch, fe, st);
+    if (s == AFS_OK) s = launch_long_items<real, 2>(P, wl, set, XT, Sw, SATw, Bp, scratch, fe, st);
+    if (s == AFS_OK) s = launch_long_items<real, 3>(P, wl, set, XT, Sw, SATw, Bp, scratch, fe, st);
     return s;
 }
 

@@ -115,18 +115,27 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
             else cls[c] = C_LONG;
         }
         // ------------------------------------------------------------ scratch slots, transposed-CSR order
-        // slot order: by variable, then constraint id, then position (a stable counting sort over the forward CSR)
-        std::vector<int32_t> slot_ptr(n + 1, 0);
+        // slot order: by variable, then constraint id, then position (a stable counting sort over the forward CSR).
+        // Two row ranges: the rows of MED / CMED literals first ([0, nslots_a), slot_ptr), then the rows of the LONG
+        // class ([nslots_a, nslots), lslot_ptr): the latter are read through their own pass (k_glong), which takes
+        // boundary literals' gradients from the per-(constraint, restart) pairs instead of the rows.
+        auto is_long_cls = [&](int c) { return cls[c] == C_LONG; };
+        std::vector<int32_t> slot_ptr(n + 1, 0), lslot_ptr(n + 1, 0);
         for (int c = 0; c < m; ++c)
             if (cls[c] != C_PULL)
-                for (int64_t e = row_ptr[c]; e < row_ptr[c + 1]; ++e) slot_ptr[std::abs(lits[e])]++;
-        for (int v = 0; v < n; ++v) slot_ptr[v + 1] += slot_ptr[v];
-        P->nslots = slot_ptr[n];
-        std::vector<int32_t> fill(slot_ptr.begin(), slot_ptr.end() - 1);
+                for (int64_t e = row_ptr[c]; e < row_ptr[c + 1]; ++e) (is_long_cls(c) ? lslot_ptr : slot_ptr)[std::abs(lits[e])]++;
+        for (int v = 0; v < n; ++v) { slot_ptr[v + 1] += slot_ptr[v]; lslot_ptr[v + 1] += lslot_ptr[v]; }
+        const int64_t nslots_a = slot_ptr[n];
+        P->nslots = nslots_a + lslot_ptr[n];
+        P->nslots_a = nslots_a;
+        std::vector<int32_t> fill(slot_ptr.begin(), slot_ptr.end() - 1), lfill(lslot_ptr.begin(), lslot_ptr.end() - 1);
         std::vector<int32_t> slot_of((size_t)P->nnz, -1);
         for (int c = 0; c < m; ++c)
             if (cls[c] != C_PULL)
-                for (int64_t e = row_ptr[c]; e < row_ptr[c + 1]; ++e) slot_of[e] = fill[std::abs(lits[e]) - 1]++;
+                for (int64_t e = row_ptr[c]; e < row_ptr[c + 1]; ++e) {
+                    const int v = std::abs(lits[e]) - 1;
+                    slot_of[e] = is_long_cls(c) ? (int32_t)(nslots_a + lfill[v]++) : fill[v]++;
+                }
 
         auto lit_word = [](int32_t l) -> uint32_t { return (uint32_t)(std::abs(l) - 1) | (l < 0 ? LIT_NEG : 0u); };
 
@@ -346,12 +355,13 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
         up(&P->d_pc_lits, pc_lits);
         up(&P->d_pcp, pcp);
         up(&P->d_slot_ptr, slot_ptr);
-        {   // which slots belong to the LONG class: the variable pass takes boundary literals' gradients from bnd
-            std::vector<int32_t> slot_info((size_t)P->nslots, -1);
+        {   // per LONG-class row (in lslot order): (index in d_long) << 1 | literal negated
+            std::vector<int32_t> lslot_info((size_t)lslot_ptr[n], 0);
             for (size_t i = 0; i < lng.size(); ++i)
                 for (int j = 0; j < lng[i].L; ++j)
-                    slot_info[long_slots[lng[i].off + j]] = (int32_t)((i << 1) | (long_lits[lng[i].off + j] >> 31));
-            up(&P->d_slot_info, slot_info);
+                    lslot_info[long_slots[lng[i].off + j] - nslots_a] = (int32_t)((i << 1) | (long_lits[lng[i].off + j] >> 31));
+            up(&P->d_lslot_info, lslot_info);
+            up(&P->d_lslot_ptr, lslot_ptr);
         }
         up(&P->d_med, med);
         up(&P->d_med_lits, med_lits);
@@ -385,7 +395,7 @@ extern "C" void afs_problem_destroy(afs_problem* p)
     if (!p) return;
     cudaSetDevice(p->device);
     cudaDeviceSynchronize();
-    cudaFree(p->d_pull_ptr); cudaFree(p->d_pull_words); cudaFree(p->d_slot_ptr); cudaFree(p->d_slot_info);
+    cudaFree(p->d_pull_ptr); cudaFree(p->d_pull_words); cudaFree(p->d_slot_ptr); cudaFree(p->d_lslot_info); cudaFree(p->d_lslot_ptr);
     cudaFree(p->d_run_ptr); cudaFree(p->d_runs); cudaFree(p->d_pull_gconst); cudaFree(p->d_pc); cudaFree(p->d_pc_lits); cudaFree(p->d_pcp);
     cudaFree(p->d_med); cudaFree(p->d_med_lits); cudaFree(p->d_med_slots);
     cudaFree(p->d_long); cudaFree(p->d_long_lits); cudaFree(p->d_long_slots);

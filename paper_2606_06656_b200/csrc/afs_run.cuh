@@ -24,11 +24,22 @@ static void launch_var_l(const VarArgs<real>& a, int gx, int tiles, cudaStream_t
     else k_var<real, EVAL, 1, LONGT><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
 }
 template <typename real, bool EVAL>
-static void launch_var(const afs_problem* P, VarArgs<real>& a, int gx, int tiles, cudaStream_t st)
+static void launch_var(afs_problem* P, VarArgs<real>& a, int gx, int tiles, cudaStream_t st)
 {
-    a.slot_info = P->d_slot_info; a.bnd = (const real*)P->ws.bnd;
-    if (P->n_long > 0) launch_var_l<real, EVAL, true>(a, gx, tiles, st);
-    else launch_var_l<real, EVAL, false>(a, gx, tiles, st);
+    if (P->n_long > 0) {   // the LONG class's share first (k_glong), from the pairs and rows the long kernels just wrote
+        const long long warps = (long long)P->n * tiles;
+        real* GL = (real*)P->ws.GL;
+        {
+            ProfSpan span(P, 6, st);
+            k_glong<real><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P->n, tiles, a.Bp, P->d_lslot_ptr, P->d_lslot_info, a.Xin,
+                                                                     a.scratch + (size_t)P->nslots_a * a.Bp,
+                                                                     (const real*)P->ws.bnd, EVAL ? nullptr : a.mask, GL);
+        }
+        a.GL = GL;
+        launch_var_l<real, EVAL, true>(a, gx, tiles, st);
+    } else {
+        launch_var_l<real, EVAL, false>(a, gx, tiles, st);
+    }
 }
 
 // ----------------------------------------------------------------------------------------------------------------
