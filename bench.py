@@ -37,7 +37,8 @@ import workloads as W  # noqa: E402
 # --------------------------------------------------------------------------------------------- algorithmic work
 def kernel_class_of_constraints(inst):
     """The library's execution classes (afs_internal.h), restated so that algorithmic work can be attributed to the
-    kernel that does it: names are Problem.KERNEL_CLASSES ('var' holds the pull clauses)."""
+    kernel that does it: names are Problem.KERNEL_CLASSES ('var' holds the pull clauses; 'long' is the group of
+    launches that serve the LONG class in one iteration: long_scan, long1/3/5/9 by pmf size, glong)."""
     L = inst.lengths()
     ty = inst.types
     prod = (ty == W.AFS_OR) | (ty == W.AFS_XOR)
@@ -53,7 +54,7 @@ def kernel_class_of_constraints(inst):
         elif cnt[c] and l <= 64:
             out[c] = "cmed"
         else:
-            out[c] = "long%d" % ((l + 1 + 127) // 128)
+            out[c] = "long"
     return out
 
 
@@ -354,6 +355,20 @@ def measure_config(cfg, args, afs, shard, rank, world, local, peaks):
         for k, fl in P.profile_flops().items():          # state-dependent flops counted by the long-constraint kernels
             counted[k] = counted.get(k, 0.0) + fl
     P.set_option(1, 0)
+    # the launches that serve the LONG class in one iteration count as one kernel group
+    grp = [k for k in prof if k.startswith("long") or k == "glong"]
+    if grp:
+        iters = max(prof[k][1] for k in grp)
+        prof["long"] = [sum(prof[k][0] for k in grp), iters]
+        long_parts = {k: round(prof[k][0] / prof[k][1] * 1e3, 2) for k in grp}      # mean us per launch
+        for k in grp:
+            del prof[k]
+        if "var" in prof and "glong" in long_parts:      # the variable pass's span brackets k_glong too
+            prof["var"][0] = max(prof["var"][0] - long_parts["glong"] * 1e-3 * prof["var"][1], 0.0)
+        fl = sum(v for k, v in counted.items() if k.startswith("long"))
+        counted = {"long": fl} if fl else {}
+    else:
+        long_parts = None
     # Long EK/CARD kernels: literals on the boundary of the cube (clipped iterates, fixed variables) are exact shifts
     # and cost no arithmetic, so their algorithmic flops are the 6 Leff Keff the kernels count at the iterates they
     # actually see; the state-independent 6 L K stays beside it as `static_formula`.
@@ -385,6 +400,8 @@ def measure_config(cfg, args, afs, shard, rank, world, local, peaks):
                         peak_source="MEASURED_PEAKS.json hbm_gbs (%s)" % peaks["source"])
         roof["frac"] = roof["achieved"] / roof["peak"]
         roof["kernel"] = dom
+        if dom == "long":
+            roof["kernel_group_us_per_launch"] = long_parts
         roof["launch_ms"] = dur_s * 1e3
         roof["launches_timed"] = prof[dom][1]
         roof["algorithmic_per_launch"] = dict(flops=flops, hbm_bytes=hbm)

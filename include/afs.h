@@ -153,6 +153,10 @@ AFS_API int64_t afs_problem_info(const afs_problem* p, int32_t what);
  *   0 execution mode of afs_pgd_run: 0 auto, 1 force the streaming (one launch per phase per step) path,
  *     2 force the tile-resident path (AFS_ERR_UNSUPPORTED at run time if the instance does not fit)
  *   1 per-launch timing stride (see afs_profile_read); 0 = off
+ *   2 streaming path: every `value` PGD iterations the restarts whose iterate did not change in the last step (a fixed
+ *     point of the deterministic PGD map: they can never move again) are retired with their final results and the
+ *     remaining ones compacted, so that later iterations work on the active restarts only.  Results are
+ *     bit-identical to value = 0 (never), which tests use as the reference.  Default 32.
  * Returns AFS_ERR_INVALID_ARG for unknown options or values.
  */
 AFS_API afs_status afs_set_option(afs_problem* p, int32_t what, int64_t value);

@@ -6,6 +6,7 @@
 
 #include "afs_kernels.cuh"
 #include "afs_launch.h"
+#include "afs_retire.cuh"
 
 using namespace afs;
 
@@ -67,11 +68,13 @@ template <typename T> static void free_ptr(T*& p) { if (p) cudaFree(p); p = null
 void free_workspace(afs_problem* P)
 {
     Workspace& w = P->ws;
-    free_ptr(w.XT[0]); free_ptr(w.XT[1]); free_ptr(w.scratch); free_ptr(w.aux[0]); free_ptr(w.aux[1]);
+    free_ptr(w.XT[0]); free_ptr(w.XT[1]); free_ptr(w.XT[2]); free_ptr(w.scratch); free_ptr(w.aux[0]); free_ptr(w.aux[1]);
     free_ptr(w.sat_hist); free_ptr(w.best_sat[0]); free_ptr(w.best_sat[1]);
-    free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.SAT[0]); free_ptr(w.SAT[1]); free_ptr(w.bnd); free_ptr(w.GL);
+    free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.S[2]); free_ptr(w.SAT[0]); free_ptr(w.SAT[1]); free_ptr(w.SAT[2]);
+    free_ptr(w.bnd); free_ptr(w.GL); free_ptr(w.best_bits[1]); free_ptr(w.orig[0]); free_ptr(w.orig[1]); free_ptr(w.moved);
+    free_ptr(w.rs); free_ptr(w.rt_src); free_ptr(w.rt_imp); free_ptr(w.rt_ret); free_ptr(w.rt_ret_sat); free_ptr(w.rt_ret_step);
     for (int k = 0; k < 4; ++k) free_ptr(w.long_items[k]);
-    free_ptr(w.long_count); free_ptr(w.best_bits);
+    free_ptr(w.long_count); free_ptr(w.best_bits[0]);
     free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.fe_cm); free_ptr(w.f_part);
     free_ptr(w.mask_dev); free_ptr(w.host_stage_X); free_ptr(w.host_stage_assign);
     free_ptr(w.host_stage_sat); free_ptr(w.host_stage_step);
@@ -119,14 +122,19 @@ afs_status ensure_workspace(afs_problem* P, int Bp, size_t elem, int64_t sat_row
     const size_t n = (size_t)P->n, ntile = (size_t)nBp / 32;
     A((unsigned char**)&w.XT[0], n * nBp * nelem);
     A((unsigned char**)&w.XT[1], n * nBp * nelem);
+    A((unsigned char**)&w.XT[2], n * nBp * nelem);
     A((unsigned char**)&w.scratch, (size_t)P->nslots * nBp * nelem);
     A((unsigned char**)&w.aux[0], (size_t)P->med_nnz * nBp * nelem);
     A((unsigned char**)&w.aux[1], (size_t)(P->med_two ? P->med_nnz : 0) * nBp * nelem);
     A(&w.sat_hist, (size_t)nrows * nBp);
     A(&w.best_sat[0], (size_t)nBp); A(&w.best_sat[1], (size_t)nBp);
     A(&w.best_step[0], (size_t)nBp); A(&w.best_step[1], (size_t)nBp);
-    A(&w.S[0], n * ntile); A(&w.S[1], n * ntile); A(&w.best_bits, n * ntile);
-    A(&w.SAT[0], n * ntile); A(&w.SAT[1], n * ntile);
+    A(&w.S[0], n * ntile); A(&w.S[1], n * ntile); A(&w.S[2], n * ntile);
+    A(&w.best_bits[0], n * ntile); A(&w.best_bits[1], n * ntile);
+    A(&w.SAT[0], n * ntile); A(&w.SAT[1], n * ntile); A(&w.SAT[2], n * ntile);
+    A(&w.orig[0], (size_t)nBp); A(&w.orig[1], (size_t)nBp); A(&w.moved, (size_t)nBp);
+    A(&w.rs, (size_t)1); A(&w.rt_src, (size_t)nBp); A(&w.rt_imp, (size_t)nBp); A(&w.rt_ret, (size_t)nBp);
+    A(&w.rt_ret_sat, (size_t)nBp); A(&w.rt_ret_step, (size_t)nBp);
     A((unsigned char**)&w.bnd, (size_t)P->n_long * nBp * 2 * nelem);
     A((unsigned char**)&w.GL, (P->n_long > 0 ? n : 0) * nBp * nelem);
     for (int k = 0; k < 4; ++k) A(&w.long_items[k], (size_t)P->n_long * nBp);
@@ -157,7 +165,7 @@ afs_status ensure_eval_buffers(afs_problem* P, int Bp, size_t elem)
 }
 
 // S9 of the PULL class from the sign words of the iterate (bit-parallel over restarts)
-afs_status launch_sat_pull(afs_problem* P, const uint32_t* S, int Bp, int32_t* sat, cudaStream_t st)
+afs_status launch_sat_pull(afs_problem* P, const uint32_t* S, int Bp, int32_t* sat, const RunState* rs, cudaStream_t st)
 {
     if (P->n_pull == 0) return AFS_OK;
     const int ntile = Bp / 32;
@@ -169,9 +177,9 @@ afs_status launch_sat_pull(afs_problem* P, const uint32_t* S, int Bp, int32_t* s
     if (gx > cap) gx = cap < 1 ? 1 : cap;
     dim3 grid(gx, gy);
     ProfSpan span(P, 2, st);
-    if (tpt == 4) k_sat_pull<4><<<grid, 256, 0, st>>>(P->d_pcp, m, S, ntile, sat);
-    else if (tpt == 2) k_sat_pull<2><<<grid, 256, 0, st>>>(P->d_pcp, m, S, ntile, sat);
-    else k_sat_pull<1><<<grid, 256, 0, st>>>(P->d_pcp, m, S, ntile, sat);
+    if (tpt == 4) k_sat_pull<4><<<grid, 256, 0, st>>>(P->d_pcp, m, S, ntile, sat, rs);
+    else if (tpt == 2) k_sat_pull<2><<<grid, 256, 0, st>>>(P->d_pcp, m, S, ntile, sat, rs);
+    else k_sat_pull<1><<<grid, 256, 0, st>>>(P->d_pcp, m, S, ntile, sat, rs);
     P->last_launches++;
     return AFS_OK;
 }

@@ -10,6 +10,8 @@
 
 namespace afs {
 
+struct RunState;
+
 // ---- literal word: bit 31 = negated literal, bits 0..30 = variable index -------------------------------------
 constexpr uint32_t LIT_NEG = 0x80000000u;
 constexpr uint32_t LIT_VAR = 0x7fffffffu;
@@ -109,19 +111,28 @@ struct Workspace {
     // all sized for (Bp, steps) below; grown on demand
     int32_t Bp = 0;
     int64_t sat_rows = 0;
-    void* XT[2] = {nullptr, nullptr};      // real [n][Bp]
+    void* XT[3] = {nullptr, nullptr, nullptr};   // real [n][Bp]: X_t, X_{t+1} and the target of a compaction, in rotation
     void* scratch = nullptr;               // real [nslots][Bp]
     void* aux[2] = {nullptr, nullptr};     // real [med_nnz][Bp] prefix states of the MED class
     int32_t* sat_hist = nullptr;           // [sat_rows][Bp]
     int32_t* best_sat[2] = {nullptr, nullptr};
     int32_t* best_step[2] = {nullptr, nullptr};
-    uint32_t* S[2] = {nullptr, nullptr};   // sign bits [n][Bp/32]: bit r of word (v, tile) = "x_v < 0" for restart 32 tile + r
-    uint32_t* SAT[2] = {nullptr, nullptr}; // saturation bits, same layout: |x_v| = 1 (on the boundary of the cube)
+    uint32_t* S[3] = {nullptr, nullptr, nullptr};   // sign bits [n][Bp/32]: bit r of word (v, tile) = "x_v < 0" for restart 32 tile + r
+    uint32_t* SAT[3] = {nullptr, nullptr, nullptr}; // saturation bits, same layout: |x_v| = 1 (on the boundary of the cube)
     void* GL = nullptr;                    // real [n][Bp]: the LONG class's share of the gradient (k_glong -> k_var)
     void* bnd = nullptr;                   // real [n_long][Bp][2]: dFE/dy of a boundary literal at y = +1 / y = -1
     uint4* long_items[4] = {nullptr, nullptr, nullptr, nullptr};   // work lists of the long-constraint kernels, by size class
     int* long_count = nullptr;             // [2][4] their lengths, two sets used alternately
-    uint32_t* best_bits = nullptr;         // [n][Bp/32]
+    uint32_t* best_bits[2] = {nullptr, nullptr};   // [n][Bp/32]
+    // retirement of restarts at a fixed point (afs_retire.cuh)
+    afs::RunState* rs = nullptr;
+    int32_t* orig[2] = {nullptr, nullptr}; // [Bp] caller's restart index of every working column, -1 = none
+    int32_t* moved = nullptr;              // [Bp] the column changed in the step a retirement follows
+    int32_t* rt_src = nullptr;             // [Bp] plan: old column of every new one
+    uint8_t* rt_imp = nullptr;             // [Bp] plan: the pending iterate improved the column's best
+    int32_t* rt_ret = nullptr;             // [Bp] plan: frozen columns, with their final best record
+    int32_t* rt_ret_sat = nullptr;
+    int32_t* rt_ret_step = nullptr;
     void* fe_med = nullptr;                // real [n_med][Bp]      (eval_grad only)
     void* fe_long = nullptr;               // real [n_long][Bp]
     void* fe_cm = nullptr;                 // real [n_cm][Bp]
@@ -194,10 +205,16 @@ struct afs_problem {
     int64_t n_pull = 0, n_med = 0, n_long = 0, n_cm = 0;
     afs::ResPlan res[afs::RES_PLANS];
 
+    // the library's own second stream: per iteration the pull-clause counts (which need only the sign words of X_t)
+    // run beside the variable pass; forked from and joined to the caller's stream with events, never synchronised
+    cudaStream_t aux_stream = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+
     // ---- run state -----------------------------------------------------------------------------------------
     afs::Workspace ws;
     int64_t last_launches = 0;
     int32_t opt_mode = 0;
+    int32_t retire_every = 32;          // streaming path: retire restarts at a fixed point every this many iterations (0 = never)
     int32_t last_resident = 0;
     afs::Profiler prof;
 };

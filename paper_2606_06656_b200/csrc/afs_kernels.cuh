@@ -5,6 +5,7 @@
 #pragma once
 #include "afs_internal.h"
 #include "afs_bits.cuh"
+#include "afs_retire.cuh"
 
 namespace afs {
 
@@ -112,9 +113,11 @@ __global__ void __launch_bounds__(256) k_assign_out(const real* __restrict__ XT,
 // ------------------------------------------------------------------------------------------------------------------
 template <typename real>
 __global__ void __launch_bounds__(256) k_count(const CountCon* __restrict__ cons, const uint32_t* __restrict__ lits,
-                                               int m, const real* __restrict__ XT, int Bp, int32_t* __restrict__ sat)
+                                               int m, const real* __restrict__ XT, int Bp, int32_t* __restrict__ sat,
+                                               const RunState* __restrict__ rs)
 {
     __shared__ int s_sat[8][32];
+    if (tile_idle(rs, blockIdx.y)) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.y * 32 + lane;
     int cnt = 0;
@@ -414,9 +417,11 @@ __global__ void __launch_bounds__(128) k_med(const MedCon* __restrict__ cons, in
                                              const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
                                              const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
                                              real* __restrict__ aux0, real* __restrict__ aux1,
-                                             int32_t* __restrict__ sat, real* __restrict__ fe_out)
+                                             int32_t* __restrict__ sat, real* __restrict__ fe_out,
+                                             const RunState* __restrict__ rs)
 {
     __shared__ int s_sat[4][32];
+    if (tile_idle(rs, blockIdx.y)) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.y * 32 + lane;
     int satcnt = 0;
@@ -442,10 +447,12 @@ template <typename real>
 __global__ void __launch_bounds__(128) k_cmed(const LongCon* __restrict__ cons, int c_begin, int c_end,
                                               const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
                                               const real* __restrict__ XT, int Bp, real* __restrict__ scratch,
-                                              int32_t* __restrict__ sat, real* __restrict__ fe_out, int qrows)
+                                              int32_t* __restrict__ sat, real* __restrict__ fe_out, int qrows,
+                                              const RunState* __restrict__ rs)
 {
     extern __shared__ __align__(16) unsigned char cm_smem[];
     __shared__ int s_sat[4][32];
+    if (tile_idle(rs, blockIdx.y)) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.y * 32 + lane;
     int satcnt = 0;
@@ -494,7 +501,8 @@ struct VarArgs {
     real* Xout;
     real lr;
     const int8_t* mask;
-    const int32_t* sat_prev;
+    const int32_t* sat_prev;     // counts of X_{t-1}, or NULL when there is nothing to merge
+    int32_t* sat_zero;           // the count row of X_{t+1} (ring of three), zeroed here; may be NULL
     const int32_t* best_sat_in;
     int32_t* best_sat_out;
     const int32_t* best_step_in;
@@ -504,6 +512,8 @@ struct VarArgs {
     uint32_t* SAT_next;          // thread reads a word of S_prev before it writes that word of S_next)
     uint32_t* best_bits;
     const real* GL;              // LONGT: [n][Bp] the LONG class's share of the gradient (k_glong)
+    const RunState* rs;          // tile groups behind the active restarts return at once (afs_retire.cuh); may be NULL
+    int32_t* moved;              // non-NULL on the iterations a retirement follows: moved[b] = 1 if any x_v changed
     real* GT;
 };
 
@@ -688,6 +698,7 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
     uint2* sbuf = s_stage[warp];
     for (int i = lane; i < PULL_SBUF; i += 32) sbuf[i] = make_uint2(0u, 0u);   // slack slots must stay valid offsets
     __syncwarp();
+    if (tile_idle(a.rs, tile0)) return;
     const int vbeg = (blockIdx.x * VAR_WARPS + warp) * VAR_VPW;
     const int vend = min(vbeg + VAR_VPW, a.n);
     // ---- S10: did the previous iterate improve on the best so far?
@@ -698,7 +709,7 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
 #pragma unroll
     for (int c = 0; c < RPL; ++c) {
         imp[c] = false; impmask[c] = 0u; sprev[c] = 0;
-        if (!EVAL && a.t > 0) {
+        if (!EVAL && a.sat_prev != nullptr) {
             sprev[c] = a.sat_prev[b + 32 * c];
             imp[c] = sprev[c] > a.best_sat_in[b + 32 * c];
             impmask[c] = __ballot_sync(FULL, imp[c]);
@@ -718,6 +729,7 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
             if (v == 0) {
 #pragma unroll
                 for (int c = 0; c < RPL; ++c) {
+                    if (a.sat_zero) a.sat_zero[b + 32 * c] = 0;
                     int bs = a.best_sat_in[b + 32 * c], stp = a.best_step_in[b + 32 * c];
                     a.best_sat_out[b + 32 * c] = imp[c] ? sprev[c] : bs;
                     a.best_step_out[b + 32 * c] = imp[c] ? a.t - 1 : stp;
@@ -768,6 +780,7 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
                 xn = xn < -one ? -one : xn;
                 if (mk != 0) xn = x[c];
                 a.Xout[(size_t)v * Bp + b + 32 * c] = xn;
+                if (a.moved && xn != x[c]) a.moved[b + 32 * c] = 1;
                 const unsigned sb = __ballot_sync(FULL, xn < real(0)), sa = __ballot_sync(FULL, xn == one || xn == -one);
                 if (lane == 0) {
                     a.S_next[(size_t)v * ntile + tile0 + c] = sb;
@@ -790,12 +803,13 @@ __global__ void __launch_bounds__(256) k_glong(int n, int ntile, int Bp, const i
                                                const int32_t* __restrict__ lslot_info, const real* __restrict__ Xin,
                                                const real* __restrict__ lrows /* scratch + nslots_a * Bp */,
                                                const real* __restrict__ bnd, const int8_t* __restrict__ mask,
-                                               real* __restrict__ GL)
+                                               real* __restrict__ GL, const RunState* __restrict__ rs)
 {
     const int lane = threadIdx.x & 31;
     const long long wid = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (wid >= (long long)n * ntile) return;
     const int v = (int)(wid / ntile), tile = (int)(wid % ntile);
+    if (tile_idle(rs, tile)) return;
     if (mask && mask[v] != 0) return;   // a fixed variable never moves: its gradient is not needed
     const int b = tile * 32 + lane;
     const real x = Xin[(size_t)v * Bp + b];
@@ -850,11 +864,12 @@ __device__ __forceinline__ SWords<TPT> ld_swords(const uint32_t* __restrict__ p)
 template <int TPT>
 __global__ void __launch_bounds__(256) k_sat_pull(const PullClause* __restrict__ cons, int m,
                                                   const uint32_t* __restrict__ S, int ntile,
-                                                  int32_t* __restrict__ sat)
+                                                  int32_t* __restrict__ sat, const RunState* __restrict__ rs)
 {
     __shared__ int s_cnt[TPT][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int tile0 = blockIdx.y * TPT;
+    if (tile_idle(rs, tile0)) return;
     if (threadIdx.x < TPT * 32) s_cnt[threadIdx.x >> 5][threadIdx.x & 31] = 0;
     __syncthreads();
     int cnt[TPT];
@@ -965,6 +980,8 @@ struct FinArgs {
     int8_t* best_assign;
     int32_t* best_sat;
     int32_t* best_step;
+    const RunState* rs;           // only the tiles of active restarts are written (the others were written at retirement)
+    const int32_t* orig;          // caller's restart index of every column, -1 = none (pads)
 };
 
 template <typename real>
@@ -974,10 +991,11 @@ __global__ void __launch_bounds__(256) k_finalize(const FinArgs<real> a)
     __shared__ unsigned s_bits[32];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int v0 = blockIdx.x * 32, tileb = blockIdx.y, b0 = tileb * 32, ntile = a.Bp >> 5;
+    if (tile_idle(a.rs, tileb)) return;
     const int b = b0 + tx;
     int best = a.best_sat_in[b], bstep = a.best_step_in[b];
     bool imp1 = false;
-    if (a.steps >= 1) {
+    if (a.sat_prev != nullptr) {
         int sp = a.sat_prev[b];
         imp1 = sp > best;
         if (imp1) { best = sp; bstep = a.steps - 1; }
@@ -1004,15 +1022,16 @@ __global__ void __launch_bounds__(256) k_finalize(const FinArgs<real> a)
     }
     __syncthreads();
     for (int r = ty; r < 32; r += 8) {
-        int bb = b0 + r, v = v0 + tx;
-        if (bb < a.B && v < a.n) {
+        const int bb = a.orig[b0 + r], v = v0 + tx;
+        if (bb >= 0 && v < a.n) {
             if (a.X) a.X[(size_t)bb * a.n + v] = tile[tx][r];
             if (a.best_assign) a.best_assign[(size_t)bb * a.n + v] = ((s_bits[tx] >> r) & 1u) ? -1 : 1;
         }
     }
-    if (blockIdx.x == 0 && ty == 0 && b < a.B) {
-        if (a.best_sat) a.best_sat[b] = best;
-        if (a.best_step) a.best_step[b] = bstep;
+    const int ob = a.orig[b];
+    if (blockIdx.x == 0 && ty == 0 && ob >= 0) {
+        if (a.best_sat) a.best_sat[ob] = best;
+        if (a.best_step) a.best_step[ob] = bstep;
     }
 }
 

@@ -18,6 +18,7 @@
 
 namespace afs {
 
+struct RunState;
 void free_workspace(afs_problem* P);
 int prof_mark(afs_problem* P, cudaStream_t st);
 struct ProfSpan {   // brackets the launches enqueued during its lifetime
@@ -31,7 +32,7 @@ inline int fe_pull_parts(const afs_problem* P) { return fe_pull_grid_x(P) * 8; }
 afs_status ensure_workspace(afs_problem* P, int Bp, size_t elem, int64_t sat_rows);
 afs_status ensure_eval_buffers(afs_problem* P, int Bp, size_t elem);
 afs_status enter(afs_problem* P, int32_t B);
-afs_status launch_sat_pull(afs_problem* P, const uint32_t* S, int Bp, int32_t* sat, cudaStream_t st);
+afs_status launch_sat_pull(afs_problem* P, const uint32_t* S, int Bp, int32_t* sat, const RunState* rs, cudaStream_t st);
 afs_status launch_fill_i32(int32_t* p, size_t n, int32_t v, cudaStream_t st);
 afs_status launch_long_fold(afs_problem* P, const int8_t* mask, cudaStream_t st);
 afs_status prof_work_slot(afs_problem* P, int cls, cudaStream_t st, unsigned long long** out);
@@ -39,6 +40,6 @@ afs_status prof_work_slot(afs_problem* P, int cls, cudaStream_t st, unsigned lon
 // the long-constraint kernels of one PGD iteration (all length buckets); instantiated in afs_long_f32.cu / _f64.cu
 template <typename real>
 afs_status launch_long_all(afs_problem* P, const real* XT, const uint32_t* Sw, const uint32_t* SATw, int Bp, real* scratch,
-                           int32_t* sat, real* fe, cudaStream_t st);
+                           int32_t* sat, real* fe, const RunState* rs, cudaStream_t st);
 
 }  // namespace afs

@@ -28,6 +28,7 @@
 #pragma once
 #include "afs_internal.h"
 #include "afs_bits.cuh"
+#include "afs_retire.cuh"
 
 namespace afs {
 
@@ -335,13 +336,15 @@ __global__ void __launch_bounds__(128) k_long_scan(const LongCon* __restrict__ c
                                                    const uint32_t* __restrict__ lits,
                                                    const uint32_t* __restrict__ Sw, const uint32_t* __restrict__ SATw,
                                                    int ntile, int Bp, real* __restrict__ bnd, int32_t* __restrict__ sat,
-                                                   real* __restrict__ fe_out, LongLists wl, int set)
+                                                   real* __restrict__ fe_out, LongLists wl, int set,
+                                                   const RunState* __restrict__ rs)
 {
     const int lane = threadIdx.x & 31;
     const long long wid = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
     if (blockIdx.x == 0 && threadIdx.x < LONG_CLASSES) wl.count[(set ^ 1) * LONG_CLASSES + threadIdx.x] = 0;
     if (wid >= (long long)n_long * ntile) return;
     const int c = (int)(wid / ntile), tile = (int)(wid % ntile);
+    if (tile_idle(rs, tile)) return;
     const LongCon lc = cons[c];
     const int L = lc.L;
     const uint32_t* lw = lits + lc.off;

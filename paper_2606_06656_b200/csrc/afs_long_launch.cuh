@@ -44,7 +44,7 @@ static afs_status launch_long_items(afs_problem* P, const LongLists& wl, int set
 
 template <typename real>
 afs_status launch_long_all(afs_problem* P, const real* XT, const uint32_t* Sw, const uint32_t* SATw, int Bp, real* scratch,
-                           int32_t* sat, real* fe, cudaStream_t st)
+                           int32_t* sat, real* fe, const RunState* rs, cudaStream_t st)
 {
     if (P->n_long == 0) return AFS_OK;
     LongLists wl;
@@ -59,7 +59,7 @@ afs_status launch_long_all(afs_problem* P, const real* XT, const uint32_t* Sw, c
         ProfSpan span(P, 5, st);
         k_long_scan<real><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(fo ? P->d_long_f : P->d_long, (int)P->n_long,
                                                                       fo ? P->d_long_lits_f : P->d_long_lits, Sw, SATw, ntile,
-                                                                      Bp, (real*)P->ws.bnd, sat, fe, wl, set);
+                                                                      Bp, (real*)P->ws.bnd, sat, fe, wl, set, rs);
         P->last_launches++;
     }
     afs_status s = launch_long_items<real, 0>(P, wl, set, XT, Sw, SATw, Bp, scratch, fe, st);

@@ -379,6 +379,13 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
         up(&P->d_count, cnt);
         up(&P->d_count_lits, cnt_lits);
         if (st != AFS_OK) { afs_problem_destroy(P); return st; }
+        if (cudaStreamCreateWithFlags(&P->aux_stream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&P->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+            (void)cudaGetLastError();
+            afs_problem_destroy(P);
+            return AFS_ERR_CUDA;
+        }
         CUDA_TRY(cudaDeviceSynchronize());
     } catch (const std::bad_alloc&) {
         afs_problem_destroy(P);
@@ -408,6 +415,9 @@ extern "C" void afs_problem_destroy(afs_problem* p)
         cudaFree(p->res[i].d_cm_begin); cudaFree(p->res[i].d_cm_items);
     }
     afs::free_workspace(p);
+    if (p->aux_stream) cudaStreamDestroy(p->aux_stream);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
     for (cudaEvent_t e : p->prof.pool) cudaEventDestroy(e);
     cudaFree(p->prof.d_work);
     (void)cudaGetLastError();
@@ -437,6 +447,7 @@ extern "C" afs_status afs_set_option(afs_problem* p, int32_t what, int64_t value
     if (!p) return AFS_ERR_INVALID_ARG;
     if (what == 0 && value >= 0 && value <= 2) { p->opt_mode = (int32_t)value; return AFS_OK; }
     if (what == 1 && value >= 0 && value <= (1 << 20)) { p->prof.stride = (int)value; return AFS_OK; }
+    if (what == 2 && value >= 0 && value <= (1 << 20)) { p->retire_every = (int32_t)value; return AFS_OK; }
     return AFS_ERR_INVALID_ARG;
 }
 

@@ -24,7 +24,7 @@ static void launch_var_l(const VarArgs<real>& a, int gx, int tiles, cudaStream_t
     else k_var<real, EVAL, 1, LONGT><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
 }
 template <typename real, bool EVAL>
-static void launch_var(afs_problem* P, VarArgs<real>& a, int gx, int tiles, cudaStream_t st)
+static void launch_var(afs_problem* P, VarArgs<real>& a, int gx, int tiles, const RunState* rs, cudaStream_t st)
 {
     if (P->n_long > 0) {   // the LONG class's share first (k_glong), from the pairs and rows the long kernels just wrote
         const long long warps = (long long)P->n * tiles;
@@ -33,7 +33,7 @@ static void launch_var(afs_problem* P, VarArgs<real>& a, int gx, int tiles, cuda
             ProfSpan span(P, 6, st);
             k_glong<real><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P->n, tiles, a.Bp, P->d_lslot_ptr, P->d_lslot_info, a.Xin,
                                                                      a.scratch + (size_t)P->nslots_a * a.Bp,
-                                                                     (const real*)P->ws.bnd, EVAL ? nullptr : a.mask, GL);
+                                                                     (const real*)P->ws.bnd, EVAL ? nullptr : a.mask, GL, rs);
         }
         a.GL = GL;
         launch_var_l<real, EVAL, true>(a, gx, tiles, st);
@@ -47,7 +47,8 @@ static void launch_var(afs_problem* P, VarArgs<real>& a, int gx, int tiles, cuda
 // ----------------------------------------------------------------------------------------------------------------
 template <typename real>
 static afs_status launch_push(afs_problem* P, const real* XT, const uint32_t* Sw, const uint32_t* SATw, int Bp,
-                              real* scratch, int32_t* sat, real* fe_med, real* fe_cm, real* fe_long, cudaStream_t st)
+                              real* scratch, int32_t* sat, real* fe_med, real* fe_cm, real* fe_long, const RunState* rs,
+                              cudaStream_t st)
 {
     const int tiles = Bp / 32;
     if (P->n_cm > 0) {
@@ -62,7 +63,7 @@ static afs_status launch_push(afs_problem* P, const real* XT, const uint32_t* Sw
             CU(cudaFuncSetAttribute(k_cmed<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ProfSpan span(P, 3, st);
         k_cmed<real><<<dim3(gx, tiles), 128, smem, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat,
-                                                        fe_cm, qrows);
+                                                        fe_cm, qrows, rs);
         P->last_launches++;
     }
     if (P->n_med > 0) {
@@ -71,15 +72,15 @@ static afs_status launch_push(afs_problem* P, const real* XT, const uint32_t* Sw
         if (gx > cap) gx = cap < 1 ? 1 : cap;
         ProfSpan span(P, 4, st);
         k_med<real><<<dim3(gx, tiles), 128, 0, st>>>(P->d_med, 0, (int)P->n_med, P->d_med_lits, P->d_med_slots, XT, Bp, scratch,
-                                                    (real*)P->ws.aux[0], (real*)P->ws.aux[1], sat, fe_med);
+                                                    (real*)P->ws.aux[0], (real*)P->ws.aux[1], sat, fe_med, rs);
         P->last_launches++;
     }
-    if (P->n_long > 0) return launch_long_all<real>(P, XT, Sw, SATw, Bp, scratch, sat, fe_long, st);
+    if (P->n_long > 0) return launch_long_all<real>(P, XT, Sw, SATw, Bp, scratch, sat, fe_long, rs, st);
     return AFS_OK;
 }
 
 template <typename real>
-static afs_status launch_count(afs_problem* P, const real* XT, int Bp, int32_t* sat, cudaStream_t st)
+static afs_status launch_count(afs_problem* P, const real* XT, int Bp, int32_t* sat, const RunState* rs, cudaStream_t st)
 {
     CU(cudaMemsetAsync(sat, 0, (size_t)Bp * sizeof(int32_t), st));
     if (P->m > 0) {
@@ -88,7 +89,7 @@ static afs_status launch_count(afs_problem* P, const real* XT, int Bp, int32_t* 
         int cap = (P->sm_count * 8 + tiles - 1) / tiles;
         if (gx > cap) gx = cap < 1 ? 1 : cap;
         ProfSpan span(P, 18, st);
-        k_count<real><<<dim3(gx, tiles), 256, 0, st>>>(P->d_count, P->d_count_lits, P->m, XT, Bp, sat);
+        k_count<real><<<dim3(gx, tiles), 256, 0, st>>>(P->d_count, P->d_count_lits, P->m, XT, Bp, sat, rs);
         P->last_launches++;
     }
     return AFS_OK;
@@ -115,7 +116,7 @@ static afs_status eval_grad_impl(afs_problem* P, const real* X, int32_t B, real*
     dim3 tg((P->n + 31) / 32, Bp / 32);
     k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, wBp, nullptr, w.S[0], w.SAT[0]);
     P->last_launches++;
-    if ((s = launch_push<real>(P, XT, w.S[0], w.SAT[0], wBp, scratch, nullptr, fe_med, fe_cm, fe_long, st)) != AFS_OK) return s;
+    if ((s = launch_push<real>(P, XT, w.S[0], w.SAT[0], wBp, scratch, nullptr, fe_med, fe_cm, fe_long, nullptr, st)) != AFS_OK) return s;
     VarArgs<real> a{};
     a.n = P->n; a.Bp = wBp; a.t = 0;
     a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
@@ -124,7 +125,7 @@ static afs_status eval_grad_impl(afs_problem* P, const real* X, int32_t B, real*
     a.GT = GT;
     const int gx = var_grid_x(P->n);
     if (G) {
-        launch_var<real, true>(P, a, gx, Bp / 32, st);
+        launch_var<real, true>(P, a, gx, Bp / 32, nullptr, st);
         P->last_launches++;
     }
     if (F) {
@@ -156,7 +157,7 @@ static afs_status round_count_impl(afs_problem* P, const real* X, int32_t B, int
     dim3 tg((P->n + 31) / 32, Bp / 32);
     k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, Bp, nullptr, nullptr, nullptr);
     P->last_launches++;
-    if ((s = launch_count<real>(P, XT, Bp, w.sat_hist, st)) != AFS_OK) return s;
+    if ((s = launch_count<real>(P, XT, Bp, w.sat_hist, nullptr, st)) != AFS_OK) return s;
     CU(cudaMemcpyAsync(sat, w.sat_hist, (size_t)B * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
     if (assign) {
         k_assign_out<real><<<tg, 256, 0, st>>>(XT, assign, B, P->n, Bp);
@@ -239,7 +240,7 @@ static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, i
     a.pcp = P->d_pcp;
     a.var_begin = rp.d_var_begin; a.item_begin = rp.d_item_begin; a.items = rp.d_items; a.pc_begin = rp.d_pc_begin;
     a.XT = XT; a.scratch = (real*)w.scratch; a.sat_hist = w.sat_hist;
-    a.best_bits = w.best_bits; a.best_sat = w.best_sat[0]; a.best_step = w.best_step[0];
+    a.best_bits = w.best_bits[0]; a.best_sat = w.best_sat[0]; a.best_step = w.best_step[0];
     a.lr = lr; a.mask = mask;
     const size_t smem = lay.bytes;
     CU(cudaFuncSetAttribute(k_resident<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RES_SMEM_MAX));
@@ -258,7 +259,7 @@ static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, i
         CU(cudaLaunchKernelEx(&cfg, k_resident<real>, a));
     }
     P->prof.on = false;
-    k_res_out<real><<<tg, 256, 0, st>>>(XT, w.best_bits, w.best_sat[0], w.best_step[0], B, P->n, ntile, X, best_assign,
+    k_res_out<real><<<tg, 256, 0, st>>>(XT, w.best_bits[0], w.best_sat[0], w.best_step[0], B, P->n, ntile, X, best_assign,
                                         best_sat, best_step);
     P->last_launches += 3;
     P->last_resident = 1;
@@ -277,17 +278,27 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     const int Bp = ((B + 31) / 32) * 32;
     const int plan = P->opt_mode == 1 ? -1 : resident_plan<real>(P, Bp / 32);
     if (P->opt_mode == 2 && plan < 0) return AFS_ERR_UNSUPPORTED;
-    if ((s = ensure_workspace(P, Bp, sizeof(real), (int64_t)steps + 1)) != AFS_OK) return s;
+    // count rows: the resident kernel keeps one per iterate, the streaming path a ring of three
+    if ((s = ensure_workspace(P, Bp, sizeof(real), plan >= 0 ? (int64_t)steps + 1 : 3)) != AFS_OK) return s;
     Workspace& w = P->ws;
     P->last_resident = 0;
     if (plan >= 0) return pgd_run_resident<real>(P, plan, X, B, steps, lr, mask, best_assign, best_sat, best_step, st);
-    real* XT[2] = {(real*)w.XT[0], (real*)w.XT[1]};
+    real* XT[3] = {(real*)w.XT[0], (real*)w.XT[1], (real*)w.XT[2]};
     real* scratch = (real*)w.scratch;
     const int tiles = Bp / 32;
     dim3 tg((P->n + 31) / 32, tiles);
+    // buffer roles, tracked here (they rotate at every step and at every compaction)
+    int xc = 0;              // XT[xc] = X_t
+    int sc_ = 0, sp_ = 1;    // S/SAT[sc_] = words of X_t, S[sp_] = sign words of X_{t-1}
+    int bc = 0;              // best_sat/best_step[bc] = record over the iterates merged so far
+    int bb = 0;              // best_bits[bb]
+    int oc = 0;              // orig[oc]
+    bool pending = false;    // iterate t-1 is counted but not merged yet (the variable pass of iteration t merges it)
+    RunState* rs = w.rs;
     k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT[0], B, P->n, Bp, mask, w.S[0], w.SAT[0]);
-    P->last_launches++;
-    CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)(steps + 1) * Bp * sizeof(int32_t), st));
+    k_run_init<<<(Bp + 255) / 256, 256, 0, st>>>(rs, B, Bp, w.orig[0], w.moved);
+    P->last_launches += 2;
+    CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)3 * Bp * sizeof(int32_t), st));
     launch_fill_i32(w.best_sat[0], (size_t)Bp, -1, st);
     CU(cudaMemsetAsync(w.best_step[0], 0, (size_t)Bp * sizeof(int32_t), st));
     P->last_launches++;
@@ -295,40 +306,77 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     if (mask && P->n_long > 0 && steps > 0) {   // the fixed variables' literals leave the long constraints for this run
         if ((s = launch_long_fold(P, mask, st)) != AFS_OK) return s;
     }
+    const int K = P->retire_every;   // 0: never
     for (int t = 0; t < steps; ++t) {
         P->prof.on = P->prof.stride > 0 && t % P->prof.stride == 0;
-        const real* Xin = XT[t & 1];
-        int32_t* sat_cur = w.sat_hist + (size_t)t * Bp;
-        if ((s = launch_push<real>(P, Xin, w.S[t & 1], w.SAT[t & 1], Bp, scratch, sat_cur, nullptr, nullptr, nullptr, st)) != AFS_OK) return s;
+        const bool retire = K > 0 && (t + 1) % K == 0 && t + 1 < steps;
+        const real* Xin = XT[xc];
+        const int xn = (xc + 1) % 3;
+        int32_t* sat_cur = w.sat_hist + (size_t)(t % 3) * Bp;
+        if ((s = launch_push<real>(P, Xin, w.S[sc_], w.SAT[sc_], Bp, scratch, sat_cur, nullptr, nullptr, nullptr, rs, st)) != AFS_OK) return s;
         VarArgs<real> a{};
         a.n = P->n; a.Bp = Bp; a.t = t;
         a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
         a.gconst = P->d_pull_gconst; a.slot_ptr = P->d_slot_ptr;
-        a.scratch = scratch; a.Xin = Xin; a.Xout = XT[(t + 1) & 1]; a.lr = lr; a.mask = mask;
-        a.sat_prev = t > 0 ? w.sat_hist + (size_t)(t - 1) * Bp : nullptr;
-        a.best_sat_in = w.best_sat[t & 1]; a.best_sat_out = w.best_sat[(t + 1) & 1];
-        a.best_step_in = w.best_step[t & 1]; a.best_step_out = w.best_step[(t + 1) & 1];
-        a.S_prev = w.S[(t + 1) & 1]; a.S_next = w.S[(t + 1) & 1]; a.SAT_next = w.SAT[(t + 1) & 1]; a.best_bits = w.best_bits;
+        a.scratch = scratch; a.Xin = Xin; a.Xout = XT[xn]; a.lr = lr; a.mask = mask;
+        a.sat_prev = pending ? w.sat_hist + (size_t)((t + 2) % 3) * Bp : nullptr;
+        a.sat_zero = w.sat_hist + (size_t)((t + 1) % 3) * Bp;
+        a.best_sat_in = w.best_sat[bc]; a.best_sat_out = w.best_sat[bc ^ 1];
+        a.best_step_in = w.best_step[bc]; a.best_step_out = w.best_step[bc ^ 1];
+        a.S_prev = w.S[sp_]; a.S_next = w.S[sp_]; a.SAT_next = w.SAT[sp_]; a.best_bits = w.best_bits[bb];
+        a.rs = rs; a.moved = retire ? w.moved : nullptr;
+        // S9 of the pull clauses needs only the (complete) sign words of X_t: it runs on the library's second stream
+        // beside the variable pass and is joined before anything reads the count row of X_t
+        const bool side = P->n_pull > 0;
+        if (side) {
+            CU(cudaEventRecord(P->ev_fork, st));
+            CU(cudaStreamWaitEvent(P->aux_stream, P->ev_fork, 0));
+            if ((s = launch_sat_pull(P, w.S[sc_], Bp, sat_cur, rs, P->aux_stream)) != AFS_OK) return s;
+            CU(cudaEventRecord(P->ev_join, P->aux_stream));
+        }
         {
             ProfSpan span(P, 1, st);
-            launch_var<real, false>(P, a, gx, tiles, st);
+            launch_var<real, false>(P, a, gx, tiles, rs, st);
         }
         P->last_launches++;
-        if ((s = launch_sat_pull(P, w.S[t & 1], Bp, sat_cur, st)) != AFS_OK) return s;
+        if (side) CU(cudaStreamWaitEvent(st, P->ev_join, 0));
+        bc ^= 1;
+        xc = xn;
+        { const int tmp = sc_; sc_ = sp_; sp_ = tmp; }   // S[sc_] = words of X_{t+1}, S[sp_] = words of X_t
+        pending = true;
+        if (retire) {
+            // iterate t is merged by the plan; frozen restarts leave with their results; the rest moves to the front
+            ProfSpan span(P, 18, st);
+            const int xf = (xc + 1) % 3, sf = 3 - sc_ - sp_;
+            k_retire_plan<<<1, 1024, 0, st>>>(rs, t, sat_cur, w.best_sat[bc], w.best_step[bc], w.orig[oc], w.moved,
+                                              w.best_sat[bc ^ 1], w.best_step[bc ^ 1], w.orig[oc ^ 1], w.rt_src, w.rt_imp,
+                                              w.rt_ret, w.rt_ret_sat, w.rt_ret_step);
+            k_retire_out<real><<<tg, 256, 0, st>>>(rs, P->n, Bp, XT[xc], w.S[sp_], w.best_bits[bb], w.rt_imp, w.rt_ret,
+                                                   w.rt_ret_sat, w.rt_ret_step, w.orig[oc], X, best_assign, best_sat,
+                                                   best_step);
+            k_compact<real><<<dim3((P->n + 7) / 8, tiles), 256, 0, st>>>(rs, P->n, Bp, w.rt_src, w.rt_imp, XT[xc], w.S[sp_],
+                                                                         w.best_bits[bb], XT[xf], w.S[sf], w.SAT[sf],
+                                                                         w.best_bits[bb ^ 1]);
+            P->last_launches += 3;
+            bc ^= 1; oc ^= 1; bb ^= 1; xc = xf;
+            sp_ = sc_; sc_ = sf;      // the words of X_t are not needed any more: the next pass has nothing to merge
+            pending = false;
+        }
     }
     P->prof.on = false;
     P->long_folded = false;
     // the last iterate: count only, then fold and write out
-    const real* Xfin = XT[steps & 1];
-    int32_t* sat_fin = w.sat_hist + (size_t)steps * Bp;
-    if ((s = launch_count<real>(P, Xfin, Bp, sat_fin, st)) != AFS_OK) return s;
+    const real* Xfin = XT[xc];
+    int32_t* sat_fin = w.sat_hist + (size_t)(steps % 3) * Bp;
+    if ((s = launch_count<real>(P, Xfin, Bp, sat_fin, rs, st)) != AFS_OK) return s;
     FinArgs<real> f{};
     f.n = P->n; f.B = B; f.Bp = Bp; f.steps = steps; f.XT = Xfin;
-    f.sat_prev = steps >= 1 ? w.sat_hist + (size_t)(steps - 1) * Bp : nullptr;
+    f.sat_prev = pending ? w.sat_hist + (size_t)((steps + 2) % 3) * Bp : nullptr;
     f.sat_fin = sat_fin;
-    f.best_sat_in = w.best_sat[steps & 1]; f.best_step_in = w.best_step[steps & 1];
-    f.S_prev = w.S[(steps + 1) & 1]; f.best_bits = w.best_bits;
+    f.best_sat_in = w.best_sat[bc]; f.best_step_in = w.best_step[bc];
+    f.S_prev = w.S[sp_]; f.best_bits = w.best_bits[bb];
     f.X = X; f.best_assign = best_assign; f.best_sat = best_sat; f.best_step = best_step;
+    f.rs = rs; f.orig = w.orig[oc];
     k_finalize<real><<<tg, 256, 0, st>>>(f);
     P->last_launches++;
     CU(cudaGetLastError());
