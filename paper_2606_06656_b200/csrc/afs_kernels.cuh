@@ -45,10 +45,12 @@ __global__ void __launch_bounds__(256) k_transpose_in(const real* __restrict__ X
     __shared__ real tile[32][33];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int v0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
+    // columns behind the batch (ragged last tile) are copies of the last restart: whatever a warp decides for its 32
+    // restarts together (e.g. which body to run) is then a function of the caller's X alone, and a resumed run repeats it
     for (int r = ty; r < 32; r += 8) {
-        int b = b0 + r, v = v0 + tx;
+        int b = min(b0 + r, B - 1), v = v0 + tx;
         real x = real(0);
-        if (b < B && v < n) x = X[(size_t)b * n + v] + real(0);   // + 0 turns -0.0 into +0.0 (G13)
+        if (v < n) x = X[(size_t)b * n + v] + real(0);   // + 0 turns -0.0 into +0.0 (G13)
         tile[r][tx] = x;
     }
     __syncthreads();
@@ -56,13 +58,13 @@ __global__ void __launch_bounds__(256) k_transpose_in(const real* __restrict__ X
         int v = v0 + r, b = b0 + tx;
         if (v < n) {
             real x = tile[tx][r];
-            if (mask) { int mk = mask[v]; if (mk != 0 && b < B) x = (real)mk; }   // fixed at entry
+            if (mask) { int mk = mask[v]; if (mk != 0) x = (real)mk; }   // fixed at entry
             XT[(size_t)v * Bp + b] = x;
         }
         if (Sw) {   // the 32 lanes of a warp hold one variable's tile (v is warp-uniform)
             const real xx = v < n ? tile[tx][r] : real(0);
             real xm = xx;
-            if (mask && v < n) { int mk = mask[v]; if (mk != 0 && b < B) xm = (real)mk; }
+            if (mask && v < n) { int mk = mask[v]; if (mk != 0) xm = (real)mk; }
             const unsigned sb = __ballot_sync(FULL, xm < real(0)), sa = __ballot_sync(FULL, xm == real(1) || xm == real(-1));
             if (tx == 0 && v < n) { Sw[(size_t)v * (Bp >> 5) + blockIdx.y] = sb; SATw[(size_t)v * (Bp >> 5) + blockIdx.y] = sa; }
         }
@@ -179,8 +181,11 @@ __device__ __forceinline__ double rcp_rn(double x) { return 1.0 / x; }
 template <typename real, typename XL, typename SW>
 __device__ __forceinline__ void cm_body(const LongCon& lc, const uint32_t* __restrict__ lw,
                                         const int32_t* __restrict__ sw, const XL& xl, const SW& sc,
-                                        real* __restrict__ q, int& satcnt, real& fe, const bool want_fe)
+                                        real* __restrict__ q, int& satcnt, real& fe, const bool want_fe,
+                                        const bool commit = true)
 {
+    // commit = false: this lane's restart was served by cm_body_small; it walks along (the loops are warp-uniform)
+    // but writes no result
     const real half = real(0.5), one = real(1), zero = real(0);
     const int L = lc.L;
     q[0] = one;
@@ -210,19 +215,21 @@ __device__ __forceinline__ void cm_body(const LongCon& lc, const uint32_t* __res
         }
         q[0] = mul_rn(hi, u);
     }
-    satcnt += pred(lc.type, L, lc.k, tc) ? 1 : 0;
-    fe = zero;
+    satcnt += (commit && pred(lc.type, L, lc.k, tc)) ? 1 : 0;
     if (want_fe) {
         real f = zero;
         for (int t = 0; t <= L; ++t) {
             const real v = q[t * 32];
             f += (lc.type == AFS_CARD ? t >= lc.k : t == lc.k) ? -v : v;   // sp_t = -1 where satisfied
         }
-        fe = f;
+        if (commit) fe = f;
+    } else if (commit) {
+        fe = zero;
     }
     const bool useA = lc.wA != 0.f, useB = lc.wB != 0.f;
     if (!useA && !useB) {   // constant expansion (CARD k = 0 or k = L+1, G5): zero gradient
-        for (int j = 0; j < L; ++j) sc.put(sw[j], zero);
+        for (int j = 0; j < L; ++j)
+            if (commit) sc.put(sw[j], zero);
         return;
     }
     const int tA = useA ? lc.tA : lc.tB, tB = useB ? lc.tB : lc.tA;   // tA <= tB
@@ -293,10 +300,115 @@ __device__ __forceinline__ void cm_body(const LongCon& lc, const uint32_t* __res
         for (int h = 0; h < 2; ++h) {
             if (j0 + h < L) {
                 const real g = mul_rn(fma(w1[h], v1[h], mul_rn(w2[h], v2[h])), rb[h]);
-                sc.put(sw[j0 + h], ng[h] ? -g : g);
+                if (commit) sc.put(sw[j0 + h], ng[h] ? -g : g);
             }
         }
     }
+}
+
+// The same constraint when few of its literals are strictly inside the cube -- the usual state of a PGD iterate after a
+// few dozen steps (clipping): a literal on the boundary is the factor 1 (y = +1) or z (y = -1) of
+// Q(z) = prod (u_j + p_j z), an exact shift, so only the interior literals (at most `cap` per restart, lane-private
+// lists in the same shared-memory buffer) go through the pmf and the chains; all boundary literals of a kind share one
+// gradient value.  The decision is per restart (lane), so that a restart's result never depends on which restarts share
+// its warp: returns the mask of lanes served here; lanes with more interior literals than the buffer holds write
+// nothing and are served by cm_body (commit = their complement).
+// Buffer rows: [0, cap] pmf | [cap+1, 2cap] y | [2cap+1, 3cap] gradients.
+template <typename real, typename XL, typename SW>
+__device__ __forceinline__ unsigned cm_body_small(const LongCon& lc, const uint32_t* __restrict__ lw,
+                                              const int32_t* __restrict__ sw, const XL& xl, const SW& sc,
+                                              real* __restrict__ q, const int qrows, int& satcnt, real& fe,
+                                              const bool want_fe)
+{
+    const real half = real(0.5), one = real(1), zero = real(0);
+    const int L = lc.L;
+    const int cap = min(12, (qrows - 1) / 3);
+    if (cap < 1) return 0u;
+    real* __restrict__ yl = q + (cap + 1) * 32;
+    real* __restrict__ gl = yl + cap * 32;
+    int nB0 = 0, nI = 0, tc = 0;
+    for (int j = 0; j < L; ++j) {
+        const uint32_t w = lw[j];
+        const real x = xl(w & LIT_VAR);
+        const bool neg = (w >> 31) != 0;
+        tc += ((x < zero) != neg) ? 1 : 0;
+        const real y = neg ? -x : x;
+        if (y == -one) ++nB0;
+        else if (y != one) { if (nI < cap) yl[nI * 32] = y; ++nI; }
+    }
+    const bool mine = nI <= cap;
+    const unsigned served = __ballot_sync(FULL, mine);
+    if (served == 0u) return 0u;
+    const int maxI = __reduce_max_sync(FULL, mine ? nI : 0);
+    satcnt += (mine && pred(lc.type, L, lc.k, tc)) ? 1 : 0;
+    // forward pmf of the interior literals; lanes with fewer of them append neutral factors (u = 1, p = 0: exact)
+    q[0] = one;
+    for (int t = 1; t <= maxI; ++t) q[t * 32] = zero;
+    for (int e = 0; e < maxI; ++e) {
+        const real y = (mine && e < nI) ? yl[e * 32] : one;
+        const real u = fma(half, y, half), p = fma(-half, y, half);
+        real hi = zero;
+        for (int t = e + 1; t >= 1; --t) {
+            const real lo = q[(t - 1) * 32];
+            q[t * 32] = fma(lo, p, mul_rn(hi, u));
+            hi = lo;
+        }
+        q[0] = mul_rn(hi, u);
+    }
+    if (want_fe) {
+        real f = zero;
+        for (int t = 0; t <= maxI; ++t) {
+            const real v = q[t * 32];
+            f += (lc.type == AFS_CARD ? t + nB0 >= lc.k : t + nB0 == lc.k) ? -v : v;   // sp = -1 where satisfied
+        }
+        if (mine) fe = f;
+    } else if (mine) {
+        fe = zero;
+    }
+    const real wA = (real)lc.wA, wB = (real)lc.wB;   // zero where the target is unused
+    const int cA = lc.tA - nB0, cB = lc.tB - nB0;    // targets inside the reduced pmf (true-count index minus the shift)
+    // boundary literals: removing a false one leaves q, removing a true one takes one shift away
+    real gA0, gB0;
+    {
+        const real a0 = (cA >= 0 && cA <= maxI) ? q[cA * 32] : zero, a1 = (cA + 1 >= 0 && cA + 1 <= maxI) ? q[(cA + 1) * 32] : zero;
+        const real b0 = (cB >= 0 && cB <= maxI) ? q[cB * 32] : zero, b1 = (cB + 1 >= 0 && cB + 1 <= maxI) ? q[(cB + 1) * 32] : zero;
+        gA0 = fma(wA, a0, mul_rn(wB, b0));
+        gB0 = fma(wA, a1, mul_rn(wB, b1));
+    }
+    // interior literals: leave-one-out in the stable direction (divisor max(u, p) >= 1/2), one chain per literal
+    for (int e = 0; e < maxI; ++e) {
+        const bool has = e < nI && mine;
+        const real y = has ? yl[e * 32] : one;
+        const real u = fma(half, y, half), p = fma(-half, y, half);
+        const bool fwd = !(y < zero);
+        const real rb = rcp_rn(fwd ? u : p);
+        const real R = -mul_rn(fwd ? p : u, rb);
+        real acc = zero, vA = zero, vB = zero;
+        for (int s = 0; s < maxI; ++s) {
+            const bool on = has && s <= nI - 1;
+            const int row = fwd ? s : nI - s;
+            const real a = on ? q[row * 32] : zero;
+            acc = fma(R, acc, a);
+            const int idx = fwd ? s : nI - 1 - s;        // index of q^(-j) this step completes
+            vA = (on && idx == cA) ? acc : vA;
+            vB = (on && idx == cB) ? acc : vB;
+        }
+        if (has) gl[e * 32] = mul_rn(fma(wA, vA, mul_rn(wB, vB)), rb);
+    }
+    // S5 + write-out in literal order
+    int e = 0;
+    for (int j = 0; j < L; ++j) {
+        const uint32_t w = lw[j];
+        const real x = xl(w & LIT_VAR);
+        const bool neg = (w >> 31) != 0;
+        const real y = neg ? -x : x;
+        real g;
+        if (y == one) g = gA0;
+        else if (y == -one) g = gB0;
+        else { g = gl[min(e, cap - 1) * 32]; ++e; }
+        if (mine) sc.put(sw[j], neg ? -g : g);
+    }
+    return served;
 }
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -462,7 +574,9 @@ __global__ void __launch_bounds__(128) k_cmed(const LongCon* __restrict__ cons, 
     for (int c = c_begin + blockIdx.x * 4 + warp; c < c_end; c += gridDim.x * 4) {
         const LongCon lc = cons[c];
         real fe;
-        cm_body<real>(lc, lits + lc.off, slots + lc.off, xl, sc, q, satcnt, fe, fe_out != nullptr);
+        const unsigned served = cm_body_small<real>(lc, lits + lc.off, slots + lc.off, xl, sc, q, qrows, satcnt, fe, fe_out != nullptr);
+        if (served != FULL)
+            cm_body<real>(lc, lits + lc.off, slots + lc.off, xl, sc, q, satcnt, fe, fe_out != nullptr, !((served >> lane) & 1u));
         if (fe_out) fe_out[(size_t)c * Bp + b] = fe;
     }
     if (sat) {

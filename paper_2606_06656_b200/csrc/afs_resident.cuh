@@ -210,7 +210,8 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
                     const LongCon lc = a.meta ? smcm[it] : a.cm[a.cm_items[mb + it]];
                     const uint32_t* lw = a.meta ? sml + smo[it] : a.cm_lits + lc.off;
                     const int32_t* ls = a.meta ? sms + smo[it] : a.cm_slots + lc.off;
-                    cm_body<real>(lc, lw, ls, xl, sw, qcol, satcnt, fe, false);
+                    const unsigned served = cm_body_small<real>(lc, lw, ls, xl, sw, qcol, a.cm_rows, satcnt, fe, false);
+                    if (served != FULL) cm_body<real>(lc, lw, ls, xl, sw, qcol, satcnt, fe, false, !((served >> lane) & 1u));
                 }
             }
             for (;;) {
@@ -355,10 +356,10 @@ __global__ void __launch_bounds__(256) k_res_in(const real* __restrict__ X, real
     __shared__ real tile[32][33];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int v0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
-    for (int r = ty; r < 32; r += 8) {
-        int b = b0 + r, v = v0 + tx;
+    for (int r = ty; r < 32; r += 8) {   // columns behind the batch: copies of the last restart (see k_transpose_in)
+        int b = min(b0 + r, B - 1), v = v0 + tx;
         real x = real(0);
-        if (b < B && v < n) x = X[(size_t)b * n + v] + real(0);
+        if (v < n) x = X[(size_t)b * n + v] + real(0);
         tile[r][tx] = x;
     }
     __syncthreads();
@@ -366,7 +367,7 @@ __global__ void __launch_bounds__(256) k_res_in(const real* __restrict__ X, real
         int v = v0 + r, b = b0 + tx;
         if (v < n) {
             real x = tile[tx][r];
-            if (mask) { int mk = mask[v]; if (mk != 0 && b < B) x = (real)mk; }
+            if (mask) { int mk = mask[v]; if (mk != 0) x = (real)mk; }
             XT[((size_t)blockIdx.y * n + v) * 32 + tx] = x;
         }
     }

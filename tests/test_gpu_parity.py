@@ -618,3 +618,31 @@ def test_retirement_with_everything_frozen_and_resume(afs):
     b = P.pgd_run(X2, 40, LR)
     assert torch.equal(Xa, X2) and torch.equal(a["best_sat"], b["best_sat"]) and torch.equal(a["best_assign"], b["best_assign"])
     P.close()
+
+
+@pytest.mark.parametrize("name,B", [("mixed", 77), ("long", 45), ("no_long", 70)])
+def test_a_restart_does_not_depend_on_the_restarts_beside_it(afs, name, B):
+    """P:L164 / L182: restarts are independent.  Whatever a kernel decides for the 32 restarts of a warp together (which
+    body to run, how far a loop goes) must not enter any single restart's arithmetic: a permuted batch, and a batch cut
+    to a ragged size, return the same bits restart by restart, on both paths and with 50 steps of drift behind them."""
+    import torch
+    inst = case_no_long(B) if name == "no_long" else CASES[name](B)
+    P = afs.Problem.from_instance(inst)
+    mask = None if inst.mask is None else dev(inst.mask)
+    perm = np.random.default_rng(3).permutation(B)
+    sub = perm[: B - 19]
+    for mode in ((1,) if name == "long" else (1, 2)):
+        P.set_option(0, mode)
+        X = dev(inst.X0)
+        o = P.pgd_run(X, 50, LR, mask=mask)
+        Xp = dev(inst.X0[perm])
+        op = P.pgd_run(Xp, 50, LR, mask=mask)
+        Xs = dev(inst.X0[sub])
+        os_ = P.pgd_run(Xs, 50, LR, mask=mask)
+        torch.cuda.synchronize()
+        assert np.array_equal(X.cpu().numpy()[perm], Xp.cpu().numpy())
+        assert np.array_equal(X.cpu().numpy()[sub], Xs.cpu().numpy())
+        for k in ("best_sat", "best_step", "best_assign"):
+            assert np.array_equal(o[k].cpu().numpy()[perm], op[k].cpu().numpy())
+            assert np.array_equal(o[k].cpu().numpy()[sub], os_[k].cpu().numpy())
+    P.close()
