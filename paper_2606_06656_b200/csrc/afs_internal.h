@@ -77,7 +77,7 @@ struct ResItem {       // one MED-class constraint: idx into d_med (code unused)
     uint32_t code;
     uint32_t idx;
 };
-constexpr int RES_PLANS = 4;   // cluster sizes 1, 2, 4, 8
+constexpr int RES_PLANS = 8;   // cluster sizes 1 .. 8 (plan i: i + 1 CTAs per tile)
 struct ResPlan {
     int C = 0;
     int32_t* d_var_begin = nullptr;    // [C+1] contiguous variable ranges, balanced by pull + reduction work

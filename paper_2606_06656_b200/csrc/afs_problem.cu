@@ -296,7 +296,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
             }
             std::stable_sort(its.begin(), its.end(), [](const It& x, const It& y) { return x.cost > y.cost; });
             for (int pi = 0; pi < RES_PLANS; ++pi) {
-                const int C = 1 << pi;
+                const int C = pi + 1;
                 ResPlan& rp = P->res[pi];
                 rp.C = C;
                 std::vector<int32_t> vbeg(C + 1, 0), ibeg(C + 1, 0), pbeg(C + 1, 0);

@@ -207,8 +207,8 @@ template <typename real>
 static int resident_plan(const afs_problem* P, int ntile)
 {
     if (P->n_long > 0 || !P->res[0].d_var_begin) return -1;
-    int pi = RES_PLANS - 1;
-    while (pi > 0 && (long long)ntile * (1 << pi) > P->sm_count) --pi;
+    int pi = RES_PLANS - 1;   // plan pi: pi + 1 CTAs per tile; the largest cluster size whose CTAs are all resident at once
+    while (pi > 0 && (long long)ntile * (pi + 1) > P->sm_count) --pi;
     return resident_layout<real>(P, pi).ok ? pi : -1;
 }
 

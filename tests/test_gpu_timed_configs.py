@@ -77,14 +77,14 @@ def mixed_n700():
     return W.mixed_pb(W.BASE_SEED + 41, n=700, n_or=2100, n_xor=140, n_eo=70, n_amo=70, n_card=35)
 
 
-@pytest.mark.parametrize("B,C", [(1024, 4), (2048, 2), (3200, 1), (1000, 4)])
+@pytest.mark.parametrize("B,C", [(1024, 4), (2048, 2), (3200, 1), (1000, 4), (672, 7), (928, 5), (1500, 3)])
 def test_resident_kernel_fp64_build_every_cluster_size_against_the_oracle(afs, B, C):
     """The one-launch tile-resident kernel (restarts are independent) with the cluster size the batch
     selects -- C = 4 is the plan bench.py times on configs[1] -- against the oracle on 8 sampled restarts, 20 steps."""
     inst = mixed_n700()
     rng = np.random.default_rng(B)
     X0 = rng.uniform(-1, 1, (B, inst.n)).astype(np.float32)
-    assert C == max(c for c in (1, 2, 4, 8) if ((B + 31) // 32) * c <= 148)     # the plan the library picks on 148 SMs
+    assert C == max(c for c in range(1, 9) if ((B + 31) // 32) * c <= 148)     # the plan the library picks on 148 SMs
     idx = sample_of(B, 8, B + 7)
     d, resident = run_full_batch_fp64(afs, inst, X0, 20, idx, mode=2)
     assert resident == 1
