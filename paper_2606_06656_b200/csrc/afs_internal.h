@@ -122,6 +122,8 @@ struct Workspace {
     void* GL = nullptr;                    // real [n][Bp]: the LONG class's share of the gradient (k_glong -> k_var)
     void* bnd = nullptr;                   // real [n_long][Bp][2]: dFE/dy of a boundary literal at y = +1 / y = -1
     uint4* long_items[4] = {nullptr, nullptr, nullptr, nullptr};   // work lists of the long-constraint kernels, by size class
+    uint32_t* long_MI = nullptr;           // [long_grows][Bp] per group of 32 literals and restart: interior-literal mask,
+    uint32_t* long_MT = nullptr;           //                  literal-true mask (k_long_scan -> k_long_items)
     int* long_count = nullptr;             // [2][4] their lengths, two sets used alternately
     uint32_t* best_bits[2] = {nullptr, nullptr};   // [n][Bp/32]
     // retirement of restarts at a fixed point (afs_retire.cuh)
@@ -186,6 +188,8 @@ struct afs_problem {
     afs::LongCon* d_long_f = nullptr;
     uint32_t* d_long_lits_f = nullptr;
     int32_t* d_long_slots_f = nullptr;
+    int32_t* d_long_goff = nullptr;     // [n_long] first mask row of each constraint (rows = groups of 32 literals)
+    int64_t long_grows = 0;             // mask rows in all
     int64_t long_nnz = 0;
     bool long_folded = false;           // the launches of the current call use the folded lists
     uint64_t long_iter = 0;             // launches of the long-constraint pass so far (parity selects the counter set)

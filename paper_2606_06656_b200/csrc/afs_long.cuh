@@ -337,7 +337,8 @@ __global__ void __launch_bounds__(128) k_long_scan(const LongCon* __restrict__ c
                                                    const uint32_t* __restrict__ Sw, const uint32_t* __restrict__ SATw,
                                                    int ntile, int Bp, real* __restrict__ bnd, int32_t* __restrict__ sat,
                                                    real* __restrict__ fe_out, LongLists wl, int set,
-                                                   const RunState* __restrict__ rs)
+                                                   const RunState* __restrict__ rs, const int32_t* __restrict__ goff,
+                                                   uint32_t* __restrict__ MI, uint32_t* __restrict__ MT)
 {
     const int lane = threadIdx.x & 31;
     const long long wid = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
@@ -348,7 +349,12 @@ __global__ void __launch_bounds__(128) k_long_scan(const LongCon* __restrict__ c
     const LongCon lc = cons[c];
     const int L = lc.L;
     const uint32_t* lw = lits + lc.off;
-    int nB0 = 0, nBr = 0, nAr = 0;
+    // per group of 32 literals the two bit matrices (literal true, literal interior) are transposed: lane r then holds
+    // restart r's bits over the group's literals; their popcounts are the counts, and the words themselves go to
+    // MI / MT[group][b] so that the item kernel finds the interior literals of a restart without touching the
+    // variables' words again (one coalesced row per group here instead of two scattered sectors per literal there)
+    int tc = 0, nBr = 0, nAr = 0;
+    const size_t mrow = (size_t)goff[c] * Bp + (size_t)tile * 32 + lane;
     for (int j0 = 0; j0 < L; j0 += 32) {
         const int j = j0 + lane;
         uint32_t tw = 0u, sw = 0xffffffffu;
@@ -359,10 +365,17 @@ __global__ void __launch_bounds__(128) k_long_scan(const LongCon* __restrict__ c
             tw = (w >> 31) ? ~s : s;
             sw = SATw[wi];
         }
-        nB0 += bit_column_sums(tw & sw, lane);
-        nBr += bit_column_sums(tw & ~sw, lane);
-        nAr += bit_column_sums(~tw & ~sw, lane);
+        const uint32_t tT = transpose32(tw, lane);
+        tc += __popc(tT);
+        uint32_t tI = 0u;
+        if (__any_sync(FULL, sw != 0xffffffffu)) {
+            tI = transpose32(~sw, lane);
+            nBr += __popc(tI & tT); nAr += __popc(tI & ~tT);
+            MT[mrow + (size_t)(j0 >> 5) * Bp] = tT;
+        }
+        MI[mrow + (size_t)(j0 >> 5) * Bp] = tI;
     }
+    const int nB0 = tc - nBr;
     // lane <-> restart from here on
     const int b = tile * 32 + lane;
     const int Leff = nBr + nAr;
@@ -400,7 +413,9 @@ __global__ void __launch_bounds__(WPC * 32) k_long_items(const LongCon* __restri
                                                          real* __restrict__ scratch, real* __restrict__ bnd,
                                                          real* __restrict__ fe_out, const uint4* __restrict__ items,
                                                          const int* __restrict__ count, int LS, int QS,
-                                                         unsigned long long* __restrict__ work)
+                                                         unsigned long long* __restrict__ work,
+                                                         const int32_t* __restrict__ goff, const uint32_t* __restrict__ MI,
+                                                         const uint32_t* __restrict__ MT)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     real* RcAll = reinterpret_cast<real*>(smem_raw);              // [WPC][LS]  ratios in list order, then gradients
@@ -416,38 +431,40 @@ __global__ void __launch_bounds__(WPC * 32) k_long_items(const LongCon* __restri
 #pragma unroll 1
     for (int it = blockIdx.x * WPC + warp; it < n_items; it += gridDim.x * WPC) {
         const uint4 ent = items[it];
-        const int c = (int)ent.x, b = (int)ent.y, tile = b >> 5, r = b & 31;
+        const int c = (int)ent.x, b = (int)ent.y;
         const int nB0 = (int)(ent.z & 0xffffu), nBr = (int)(ent.z >> 16), nAr = (int)ent.w;
         const LongCon lc = cons[c];
         const int L = lc.L;
         const uint32_t* lw = lits + lc.off;
         const int32_t* sw = slots + lc.off;
         const int Leff = nBr + nAr;
-        // lists [B interior, pad | A interior, pad] of literal indices, from this restart's bits of the words; two groups
-        // of 32 literals per round with their loads in front.  x is gathered for the listed literals only.
+        // lists [B interior, pad | A interior, pad] of literal indices, from the restart's masks the scan kernel wrote:
+        // lane <-> group of 32 literals, positions by a warp scan of the popcounts, every lane expands its own bits.
+        // x is gathered for the listed literals only.
         const int nBr4 = (nBr + 3) & ~3, nAr4 = (nAr + 3) & ~3, send = nBr4 + nAr4;
         {
             int pBr = 0, pAr = nBr4;
-            for (int j0 = 0; j0 < L; j0 += 64) {
-                uint32_t w[2], sg[2], st[2];
-#pragma unroll
-                for (int h = 0; h < 2; ++h) { const int j = j0 + 32 * h + lane; w[h] = j < L ? lw[j] : 0u; }
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int j = j0 + 32 * h + lane;
-                    const size_t wi = (size_t)(w[h] & LIT_VAR) * ntile + tile;
-                    sg[h] = j < L ? Sw[wi] : 0u;
-                    st[h] = j < L ? SATw[wi] : 0xffffffffu;
+            const int ngr = (L + 31) >> 5;
+            const size_t mrow = (size_t)goff[c] * Bp + b;
+            for (int g0 = 0; g0 < ngr; g0 += 32) {
+                const int g = g0 + lane;
+                uint32_t mi = 0u, mt = 0u;
+                if (g < ngr) {
+                    mi = MI[mrow + (size_t)g * Bp];
+                    if (mi) mt = MT[mrow + (size_t)g * Bp];
                 }
+                uint32_t mB = mi & mt, mA = mi & ~mt;
+                const int cB = __popc(mB), cA = __popc(mA);
+                int sB = cB, sA = cA;   // inclusive scans
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int j = j0 + 32 * h + lane;
-                    const bool tb = (((sg[h] >> r) ^ (w[h] >> 31)) & 1u) != 0, intr = ((st[h] >> r) & 1u) == 0;
-                    const bool cBr = intr && tb, cAr = intr && !tb;
-                    const unsigned mBr = __ballot_sync(FULLM, cBr), mAr = __ballot_sync(FULLM, cAr);
-                    if (intr) J[cBr ? pBr + __popc(mBr & lt) : pAr + __popc(mAr & lt)] = (uint16_t)j;
-                    pBr += __popc(mBr); pAr += __popc(mAr);
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int uB = __shfl_up_sync(FULLM, sB, o), uA = __shfl_up_sync(FULLM, sA, o);
+                    if (lane >= o) { sB += uB; sA += uA; }
                 }
+                int qB = pBr + sB - cB, qA = pAr + sA - cA;
+                while (mB) { J[qB++] = (uint16_t)(g * 32 + __ffs(mB) - 1); mB &= mB - 1; }
+                while (mA) { J[qA++] = (uint16_t)(g * 32 + __ffs(mA) - 1); mA &= mA - 1; }
+                pBr += __shfl_sync(FULLM, sB, 31); pAr += __shfl_sync(FULLM, sA, 31);
             }
             if (lane < nBr4 - nBr) J[nBr + lane] = 0xffffu;
             if (lane < nAr4 - nAr) J[nBr4 + nAr + lane] = 0xffffu;

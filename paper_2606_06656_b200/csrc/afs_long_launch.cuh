@@ -37,7 +37,7 @@ static afs_status launch_long_items(afs_problem* P, const LongLists& wl, int set
     kern<<<grid, WPC * 32, smem, st>>>(fo ? P->d_long_f : P->d_long, fo ? P->d_long_lits_f : P->d_long_lits,
                                         fo ? P->d_long_slots_f : P->d_long_slots, XT, Sw, SATw, Bp / 32, Bp, scratch,
                                         (real*)P->ws.bnd, fe, wl.items[CLS], wl.count + set * LONG_CLASSES + CLS, LS, QS,
-                                        work);
+                                        work, P->d_long_goff, P->ws.long_MI, P->ws.long_MT);
     P->last_launches++;
     return AFS_OK;
 }
@@ -59,7 +59,8 @@ afs_status launch_long_all(afs_problem* P, const real* XT, const uint32_t* Sw, c
         ProfSpan span(P, 5, st);
         k_long_scan<real><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(fo ? P->d_long_f : P->d_long, (int)P->n_long,
                                                                       fo ? P->d_long_lits_f : P->d_long_lits, Sw, SATw, ntile,
-                                                                      Bp, (real*)P->ws.bnd, sat, fe, wl, set, rs);
+                                                                      Bp, (real*)P->ws.bnd, sat, fe, wl, set, rs, P->d_long_goff, P->ws.long_MI,
+                                                                      P->ws.long_MT);
         P->last_launches++;
     }
     afs_status s = launch_long_items<real, 0>(P, wl, set, XT, Sw, SATw, Bp, scratch, fe, st);

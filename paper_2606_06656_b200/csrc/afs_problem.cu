@@ -370,6 +370,12 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
         up(&P->d_long_lits, long_lits);
         up(&P->d_long_slots, long_slots);
         P->long_nnz = (int64_t)long_lits.size();
+        {
+            std::vector<int32_t> goff(lng.size() + 1, 0);
+            for (size_t i = 0; i < lng.size(); ++i) goff[i + 1] = goff[i] + (lng[i].L + 31) / 32;
+            P->long_grows = goff[lng.size()];
+            up(&P->d_long_goff, goff);
+        }
         up(&P->d_long_f, lng);
         up(&P->d_long_lits_f, long_lits);
         up(&P->d_long_slots_f, long_slots);
@@ -406,7 +412,7 @@ extern "C" void afs_problem_destroy(afs_problem* p)
     cudaFree(p->d_run_ptr); cudaFree(p->d_runs); cudaFree(p->d_pull_gconst); cudaFree(p->d_pc); cudaFree(p->d_pc_lits); cudaFree(p->d_pcp);
     cudaFree(p->d_med); cudaFree(p->d_med_lits); cudaFree(p->d_med_slots);
     cudaFree(p->d_long); cudaFree(p->d_long_lits); cudaFree(p->d_long_slots);
-    cudaFree(p->d_long_f); cudaFree(p->d_long_lits_f); cudaFree(p->d_long_slots_f);
+    cudaFree(p->d_long_goff); cudaFree(p->d_long_f); cudaFree(p->d_long_lits_f); cudaFree(p->d_long_slots_f);
     cudaFree(p->d_cm); cudaFree(p->d_cm_lits); cudaFree(p->d_cm_slots);
     cudaFree(p->d_count); cudaFree(p->d_count_lits);
     for (int i = 0; i < afs::RES_PLANS; ++i) {
