@@ -449,3 +449,81 @@ int orc_pgd_run(int n, int64_t m, const int64_t *row_ptr, const int32_t *lits,
     }
     return err;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * PGD with per-restart convergence detection ("the small step size satisfies convergence criteria
+ * prematurely"; L152-L164: restarts converge at different times and "all batch elements must iterate together;
+ * idling converged elements waste compute"; the criterion itself is not printed: DESIGN.md reading G24).
+ *   A restart stops after the first step t -> t+1 with  max_v |X_{t+1}[v] - X_t[v]| < tol  (free coordinates); its
+ *   iterate stays X_{t+1} from then on, conv_step[b] = t+1 = the number of steps it took; -1 if it never stops within
+ *   max_steps.  Every iterate it reaches is rounded and counted (X_0 .. X_{conv_step}), best as in orc_pgd_run.
+ *   tol <= 0 never stops a restart: identical to orc_pgd_run.
+ * Outputs for the histograms of Fig. 4-5: final_sat[b] = satisfied constraints of the returned X
+ * (#unsatisfied = m - final_sat), final_F[b] = objective of the returned X ("energy"), conv_step[b] ("steps").
+ * ------------------------------------------------------------------------------------------ */
+int orc_pgd_run_conv(int n, int64_t m, const int64_t *row_ptr, const int32_t *lits,
+                     const int32_t *types, const int32_t *k, double *X, int B, int max_steps, double lr,
+                     const int8_t *mask, double tol, int8_t *best_assign, int32_t *best_sat, int32_t *best_step,
+                     int32_t *conv_step, int32_t *final_sat, double *final_F, int evaluator, int nthreads)
+{
+    if (check_instance(n, m, row_ptr, lits, types, k) || max_steps < 0) return -1;
+    int Lmax = max_len(m, row_ptr);
+    int err = 0;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+    (void)nthreads;
+#pragma omp parallel
+    {
+        double *ybuf = (double *)malloc((size_t)Lmax * sizeof(double));
+        double *gbuf = (double *)malloc((size_t)Lmax * sizeof(double));
+        double *g = (double *)malloc((size_t)n * sizeof(double));
+        int8_t *cur = (int8_t *)malloc((size_t)n);
+#pragma omp for schedule(dynamic, 1)
+        for (int b = 0; b < B; ++b) {
+            double *x = X + (size_t)b * n;
+            if (mask) for (int v = 0; v < n; ++v) if (mask[v]) x[v] = (double)mask[v];
+            int32_t best = -1, conv = -1, s = 0;
+            for (int t = 0; t <= max_steps; ++t) {
+                s = count_one(n, m, row_ptr, lits, types, k, x, cur);
+                if (s > best) {
+                    best = s;
+                    if (best_assign) memcpy(best_assign + (size_t)b * n, cur, (size_t)n);
+                    if (best_step) best_step[b] = t;
+                }
+                if (t == max_steps || conv >= 0) break;
+                int rc = eval_one(n, m, row_ptr, lits, types, k, x, NULL, g, evaluator, Lmax, ybuf, gbuf);
+                if (rc) {
+#pragma omp critical
+                    err = rc;
+                    break;
+                }
+                double delta = 0.0;
+                for (int v = 0; v < n; ++v) {
+                    if (mask && mask[v]) continue;
+                    double xn = x[v] - lr * g[v];
+                    if (xn > 1.0) xn = 1.0;
+                    if (xn < -1.0) xn = -1.0;
+                    double d = fabs(xn - x[v]);
+                    if (d > delta) delta = d;
+                    x[v] = xn;
+                }
+                if (delta < tol) conv = t + 1;
+            }
+            if (best_sat) best_sat[b] = best;
+            if (conv_step) conv_step[b] = conv;
+            if (final_sat) final_sat[b] = s;
+            if (final_F) {
+                double F = 0.0;
+                int rc = eval_one(n, m, row_ptr, lits, types, k, x, &F, NULL, evaluator, Lmax, ybuf, gbuf);
+                if (rc) {
+#pragma omp critical
+                    err = rc;
+                }
+                final_F[b] = F;
+            }
+        }
+        free(ybuf); free(gbuf); free(g); free(cur);
+    }
+    return err;
+}

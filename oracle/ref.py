@@ -32,6 +32,8 @@ def lib():
         L.orc_round_count.argtypes = inst + [f64p, C.c_int, i8p, i32p]
         L.orc_pgd_run.argtypes = inst + [f64p, C.c_int, C.c_int, C.c_double, i8p, i8p, i32p, i32p,
                                          f64p, i32p, C.c_int, C.c_int]
+        L.orc_pgd_run_conv.argtypes = inst + [f64p, C.c_int, C.c_int, C.c_double, i8p, C.c_double, i8p, i32p, i32p,
+                                              i32p, i32p, f64p, C.c_int, C.c_int]
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -136,3 +138,26 @@ def pgd_run(inst, X0, steps: int, lr: float, mask=None, evaluator: int = 2, want
     if want_traj:
         out["traj"] = traj
     return out
+
+
+def pgd_run_conv(inst, X0, max_steps: int, lr: float, tol: float, mask=None, evaluator: int = 2, nthreads: int = 0):
+    """PGD with per-restart convergence detection (orc_pgd_run_conv): a restart stops after the first step with
+    max|dX| < tol.  Returns dict(X, best_assign, best_sat, best_step, conv_step, final_sat, final_F)."""
+    X = np.array(X0, dtype=np.float64, order="C", copy=True)
+    B, n = X.shape
+    m8 = None if mask is None else np.ascontiguousarray(mask, dtype=np.int8)
+    best_assign = np.zeros((B, n), dtype=np.int8)
+    best_sat = np.zeros(B, dtype=np.int32)
+    best_step = np.zeros(B, dtype=np.int32)
+    conv_step = np.zeros(B, dtype=np.int32)
+    final_sat = np.zeros(B, dtype=np.int32)
+    final_F = np.zeros(B, dtype=np.float64)
+    keep, args = _inst_args(inst)
+    rc = lib().orc_pgd_run_conv(*args, _p(X, C.c_double), B, int(max_steps), float(lr), _p(m8, C.c_int8), float(tol),
+                                _p(best_assign, C.c_int8), _p(best_sat, C.c_int32), _p(best_step, C.c_int32),
+                                _p(conv_step, C.c_int32), _p(final_sat, C.c_int32), _p(final_F, C.c_double),
+                                evaluator, nthreads)
+    if rc:
+        raise ValueError("oracle error %d" % rc)
+    return dict(X=X, best_assign=best_assign, best_sat=best_sat, best_step=best_step, conv_step=conv_step,
+                final_sat=final_sat, final_F=final_F)
