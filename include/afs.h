@@ -132,6 +132,27 @@ AFS_API afs_status afs_pgd_run_f64(afs_problem* p, double* X, int32_t B, int32_t
                            int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* cuda_stream);
 
 /*
+ * afs_pgd_run_conv -- afs_pgd_run with per-restart convergence detection ("convergence criteria"; P:L152-L164:
+ * restarts converge at different times and idling converged batch elements waste compute; reading G24):
+ *   a restart STOPS after the first step t -> t+1 with max_v |X_{t+1}[v] - X_t[v]| < tol (free coordinates); its
+ *   iterate stays X_{t+1} and conv_step[b] = t+1, the number of steps it took (-1: never stopped within max_steps).
+ *   Every iterate a restart reaches is rounded and counted as in afs_pgd_run.  Stopped restarts are retired from the
+ *   working batch and the remaining ones compacted (no work is spent on them).  tol = 0 never stops a restart: the call
+ *   is afs_pgd_run and conv_step is -1 everywhere.  tol must be finite and >= 0.
+ * Extra outputs (device, may be NULL) -- the per-restart quantities of the paper's Fig. 4-5 histograms:
+ *   conv_step int32[B] ("steps")    final_sat int32[B] satisfied constraints of the returned X (#unsatisfied =
+ *   n_cons - final_sat)    final_F float[B] objective of the returned X ("energy")
+ * tol > 0 always takes the streaming path.  The fp32 entry decides |dX| < tol in fp32, the _f64 twin in fp64.
+ */
+AFS_API afs_status afs_pgd_run_conv(afs_problem* p, float* X, int32_t B, int32_t max_steps, float lr, const int8_t* mask,
+                                    float tol, int8_t* best_assign, int32_t* best_sat, int32_t* best_step,
+                                    int32_t* conv_step, int32_t* final_sat, float* final_F, void* cuda_stream);
+AFS_API afs_status afs_pgd_run_conv_f64(afs_problem* p, double* X, int32_t B, int32_t max_steps, double lr,
+                                        const int8_t* mask, double tol, int8_t* best_assign, int32_t* best_sat,
+                                        int32_t* best_step, int32_t* conv_step, int32_t* final_sat, double* final_F,
+                                        void* cuda_stream);
+
+/*
  * afs_pgd_run_host -- the same call with HOST buffers (all pointers host; pinned memory recommended): copies X
  * and mask to the device, runs afs_pgd_run, copies X, best_assign, best_sat, best_step back, synchronises.
  * This is the end-to-end entry point bench.py times ("e2e").  Output pointers may be NULL.

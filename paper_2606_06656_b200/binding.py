@@ -21,7 +21,7 @@ EXPORTS = (
     "afs_problem_create", "afs_problem_destroy", "afs_coeffs", "afs_eval_grad", "afs_eval_grad_f64",
     "afs_round_count", "afs_round_count_f64", "afs_pgd_run", "afs_pgd_run_f64", "afs_pgd_run_host",
     "afs_problem_info", "afs_set_option", "afs_status_string", "afs_abi_version", "afs_last_error_message",
-    "afs_profile_read", "afs_profile_flops", "afs_fp32_fma_peak",
+    "afs_profile_read", "afs_profile_flops", "afs_fp32_fma_peak", "afs_pgd_run_conv", "afs_pgd_run_conv_f64",
 )
 
 _lib = None
@@ -60,6 +60,10 @@ def lib():
     L.afs_pgd_run.restype = C.c_int
     L.afs_pgd_run_f64.argtypes = [vp, vp, i32, i32, C.c_double, vp, vp, vp, vp, vp]
     L.afs_pgd_run_f64.restype = C.c_int
+    L.afs_pgd_run_conv.argtypes = [vp, vp, i32, i32, C.c_float, vp, C.c_float, vp, vp, vp, vp, vp, vp, vp]
+    L.afs_pgd_run_conv.restype = C.c_int
+    L.afs_pgd_run_conv_f64.argtypes = [vp, vp, i32, i32, C.c_double, vp, C.c_double, vp, vp, vp, vp, vp, vp, vp]
+    L.afs_pgd_run_conv_f64.restype = C.c_int
     L.afs_pgd_run_host.argtypes = [vp, vp, i32, i32, C.c_float, vp, vp, vp, vp, vp]
     L.afs_pgd_run_host.restype = C.c_int
     L.afs_problem_info.argtypes = [vp, i32]
@@ -231,6 +235,25 @@ class Problem:
         _chk(fn(self._h, X.data_ptr(), B, int(steps), float(lr), mask.data_ptr() if mask is not None else None,
                 ba.data_ptr(), bs.data_ptr(), bt.data_ptr(), _stream_ptr(X.device)), "afs_pgd_run")
         return dict(X=X, best_assign=ba, best_sat=bs, best_step=bt)
+
+    def pgd_run_conv(self, X, max_steps: int, lr: float, tol: float, mask=None):
+        """afs_pgd_run_conv / _f64, in place on X. Returns dict(X, best_assign, best_sat, best_step, conv_step,
+        final_sat, final_F)."""
+        torch = _torch()
+        f64 = X.dtype == torch.float64
+        self._check_X(X, torch.float64 if f64 else torch.float32)
+        B = X.shape[0]
+        if mask is not None and not (mask.is_cuda and mask.dtype == torch.int8 and mask.numel() == self.n):
+            raise ValueError("mask must be a contiguous CUDA int8 tensor [n]")
+        ba = torch.empty((B, self.n), dtype=torch.int8, device=X.device)
+        i32 = lambda: torch.empty(B, dtype=torch.int32, device=X.device)
+        bs, bt, cs, fs = i32(), i32(), i32(), i32()
+        fF = torch.empty(B, dtype=X.dtype, device=X.device)
+        fn = lib().afs_pgd_run_conv_f64 if f64 else lib().afs_pgd_run_conv
+        _chk(fn(self._h, X.data_ptr(), B, int(max_steps), float(lr), mask.data_ptr() if mask is not None else None,
+                float(tol), ba.data_ptr(), bs.data_ptr(), bt.data_ptr(), cs.data_ptr(), fs.data_ptr(), fF.data_ptr(),
+                _stream_ptr(X.device)), "afs_pgd_run_conv")
+        return dict(X=X, best_assign=ba, best_sat=bs, best_step=bt, conv_step=cs, final_sat=fs, final_F=fF)
 
     def pgd_run_host(self, X, steps: int, lr: float, mask=None, out=None):
         """afs_pgd_run_host: X float32 [B,n] HOST tensor/array (pinned recommended), updated in place; H2D and D2H

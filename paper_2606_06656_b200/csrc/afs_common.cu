@@ -72,7 +72,7 @@ void free_workspace(afs_problem* P)
     free_ptr(w.sat_hist); free_ptr(w.best_sat[0]); free_ptr(w.best_sat[1]);
     free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.S[2]); free_ptr(w.SAT[0]); free_ptr(w.SAT[1]); free_ptr(w.SAT[2]);
     free_ptr(w.bnd); free_ptr(w.GL); free_ptr(w.best_bits[1]); free_ptr(w.orig[0]); free_ptr(w.orig[1]); free_ptr(w.moved);
-    free_ptr(w.rs); free_ptr(w.rt_src); free_ptr(w.rt_imp); free_ptr(w.rt_ret); free_ptr(w.rt_ret_sat); free_ptr(w.rt_ret_step);
+    free_ptr(w.rs); free_ptr(w.rt_src); free_ptr(w.rt_imp); free_ptr(w.rt_ret); free_ptr(w.rt_ret_sat); free_ptr(w.rt_ret_step); free_ptr(w.rt_ret_conv); free_ptr(w.conv[0]); free_ptr(w.conv[1]); free_ptr(w.delta);
     for (int k = 0; k < 4; ++k) free_ptr(w.long_items[k]);
     free_ptr(w.long_count); free_ptr(w.long_MI); free_ptr(w.long_MT); free_ptr(w.best_bits[0]);
     free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.fe_cm); free_ptr(w.f_part);
@@ -134,7 +134,8 @@ afs_status ensure_workspace(afs_problem* P, int Bp, size_t elem, int64_t sat_row
     A(&w.SAT[0], n * ntile); A(&w.SAT[1], n * ntile); A(&w.SAT[2], n * ntile);
     A(&w.orig[0], (size_t)nBp); A(&w.orig[1], (size_t)nBp); A(&w.moved, (size_t)nBp);
     A(&w.rs, (size_t)1); A(&w.rt_src, (size_t)nBp); A(&w.rt_imp, (size_t)nBp); A(&w.rt_ret, (size_t)nBp);
-    A(&w.rt_ret_sat, (size_t)nBp); A(&w.rt_ret_step, (size_t)nBp);
+    A(&w.rt_ret_sat, (size_t)nBp); A(&w.rt_ret_step, (size_t)nBp); A(&w.rt_ret_conv, (size_t)nBp);
+    A(&w.conv[0], (size_t)nBp); A(&w.conv[1], (size_t)nBp); A((unsigned long long**)&w.delta, (size_t)3 * nBp);
     A((unsigned char**)&w.bnd, (size_t)P->n_long * nBp * 2 * nelem);
     A((unsigned char**)&w.GL, (P->n_long > 0 ? n : 0) * nBp * nelem);
     for (int k = 0; k < 4; ++k) A(&w.long_items[k], (size_t)P->n_long * nBp);

@@ -135,6 +135,10 @@ struct Workspace {
     int32_t* rt_ret = nullptr;             // [Bp] plan: frozen columns, with their final best record
     int32_t* rt_ret_sat = nullptr;
     int32_t* rt_ret_step = nullptr;
+    int32_t* rt_ret_conv = nullptr;
+    // convergence detection (afs_pgd_run_conv)
+    int32_t* conv[2] = {nullptr, nullptr}; // [Bp] steps after which the column stopped, -1 = running
+    void* delta = nullptr;                 // [3][Bp] 8-byte cells: max |dX| of a step as order-preserving integer bits
     void* fe_med = nullptr;                // real [n_med][Bp]      (eval_grad only)
     void* fe_long = nullptr;               // real [n_long][Bp]
     void* fe_cm = nullptr;                 // real [n_cm][Bp]

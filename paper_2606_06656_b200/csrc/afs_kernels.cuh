@@ -626,10 +626,25 @@ struct VarArgs {
     uint32_t* SAT_next;          // thread reads a word of S_prev before it writes that word of S_next)
     uint32_t* best_bits;
     const real* GL;              // LONGT: [n][Bp] the LONG class's share of the gradient (k_glong)
+    // CONV (afs_pgd_run_conv): a restart stops after the first step with max_v |dX| < tol (G24)
+    real tol;
+    const int32_t* conv_in;      // [Bp] number of steps after which the restart stopped, -1 = still running
+    int32_t* conv_out;
+    const void* delta_prev;      // [Bp] DBits: max |dX| of the previous step, NULL = already folded into conv_in
+    void* delta_cur;             // [Bp] DBits: max |dX| of this step (integer atomicMax), zeroed by the previous pass
+    void* delta_zero;            // [Bp] the row of the next step
     const RunState* rs;          // tile groups behind the active restarts return at once (afs_retire.cuh); may be NULL
     int32_t* moved;              // non-NULL on the iterations a retirement follows: moved[b] = 1 if any x_v changed
     real* GT;
 };
+
+// |dX| as an order-preserving unsigned integer (non-negative IEEE values compare like their bit patterns), so that the
+// per-restart maximum over all variables is an integer atomicMax: exact and independent of the order of arrival
+__device__ __forceinline__ unsigned int dbits(float d) { return __float_as_uint(d); }
+__device__ __forceinline__ unsigned long long dbits(double d) { return (unsigned long long)__double_as_longlong(d); }
+template <typename real> struct DBits;
+template <> struct DBits<float> { typedef unsigned int type; static __device__ __forceinline__ float val(unsigned int u) { return __uint_as_float(u); } };
+template <> struct DBits<double> { typedef unsigned long long type; static __device__ __forceinline__ double val(unsigned long long u) { return __longlong_as_double((long long)u); } };
 
 template <typename real> struct Pair;
 template <> struct Pair<float> { typedef float2 type; };
@@ -798,7 +813,7 @@ __device__ __forceinline__ void pull_variable(const uint32_t* __restrict__ runs,
 // 32 warps per SM at <= 64 registers: the pass waits on L2 gathers, and occupancy is what hides them -- at
 // 95 registers (2 CTAs per SM) the same code took 1.5x as long on configs[3] (measured: 420 -> 274 us per iteration).
 // LONGT: the instance has LONG-class constraints; their share of the gradient comes summed from k_glong.
-template <typename real, bool EVAL, int RPL, bool LONGT>
+template <typename real, bool EVAL, int RPL, bool LONGT, bool CONV>
 __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const VarArgs<real> a)
 {
     __shared__ __align__(16) uint2 s_stage[VAR_WARPS][PULL_SBUF];
@@ -815,6 +830,19 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
     if (tile_idle(a.rs, tile0)) return;
     const int vbeg = (blockIdx.x * VAR_WARPS + warp) * VAR_VPW;
     const int vend = min(vbeg + VAR_VPW, a.n);
+    // ---- convergence detection: a restart whose last step stayed below tol is frozen from now on
+    typedef typename DBits<real>::type dbits_t;
+    bool frozen[RPL];
+    real dmax[RPL];
+#pragma unroll
+    for (int c = 0; c < RPL; ++c) {
+        frozen[c] = false; dmax[c] = real(0);
+        if (CONV) {
+            frozen[c] = a.conv_in[b + 32 * c] >= 0;
+            if (!frozen[c] && a.delta_prev)
+                frozen[c] = DBits<real>::val(static_cast<const dbits_t*>(a.delta_prev)[b + 32 * c]) < a.tol;
+        }
+    }
     // ---- S10: did the previous iterate improve on the best so far?
     bool imp[RPL];
     unsigned impmask[RPL];
@@ -844,6 +872,11 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
 #pragma unroll
                 for (int c = 0; c < RPL; ++c) {
                     if (a.sat_zero) a.sat_zero[b + 32 * c] = 0;
+                    if (CONV) {   // the step count at which the restart stopped: the previous step was number t
+                        const int ci = a.conv_in[b + 32 * c];
+                        a.conv_out[b + 32 * c] = ci >= 0 ? ci : (frozen[c] ? a.t : -1);
+                        static_cast<dbits_t*>(a.delta_zero)[b + 32 * c] = 0;
+                    }
                     int bs = a.best_sat_in[b + 32 * c], stp = a.best_step_in[b + 32 * c];
                     a.best_sat_out[b + 32 * c] = imp[c] ? sprev[c] : bs;
                     a.best_step_out[b + 32 * c] = imp[c] ? a.t - 1 : stp;
@@ -892,9 +925,10 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
                 real xn = x[c] - a.lr * g[c];
                 xn = xn > one ? one : xn;
                 xn = xn < -one ? -one : xn;
-                if (mk != 0) xn = x[c];
+                if (mk != 0 || (CONV && frozen[c])) xn = x[c];
                 a.Xout[(size_t)v * Bp + b + 32 * c] = xn;
                 if (a.moved && xn != x[c]) a.moved[b + 32 * c] = 1;
+                if (CONV) dmax[c] = fmax(dmax[c], fabs(xn - x[c]));
                 const unsigned sb = __ballot_sync(FULL, xn < real(0)), sa = __ballot_sync(FULL, xn == one || xn == -one);
                 if (lane == 0) {
                     a.S_next[(size_t)v * ntile + tile0 + c] = sb;
@@ -902,6 +936,11 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
                 }
             }
         }
+    }
+    if (CONV) {
+#pragma unroll
+        for (int c = 0; c < RPL; ++c)
+            if (dmax[c] > real(0)) atomicMax(static_cast<dbits_t*>(a.delta_cur) + b + 32 * c, dbits(dmax[c]));
     }
 }
 
@@ -1094,6 +1133,10 @@ struct FinArgs {
     int8_t* best_assign;
     int32_t* best_sat;
     int32_t* best_step;
+    real tol;                     // > 0: convergence detection (afs_pgd_run_conv)
+    const int32_t* conv_in;       // [Bp] steps after which the column stopped (-1: running), before the last step is folded
+    const void* delta_last;       // [Bp] DBits: max |dX| of the last step, NULL = nothing to fold
+    int32_t* conv_step;           // caller's array [B] or NULL
     const RunState* rs;           // only the tiles of active restarts are written (the others were written at retirement)
     const int32_t* orig;          // caller's restart index of every column, -1 = none (pads)
 };
@@ -1146,6 +1189,15 @@ __global__ void __launch_bounds__(256) k_finalize(const FinArgs<real> a)
     if (blockIdx.x == 0 && ty == 0 && ob >= 0) {
         if (a.best_sat) a.best_sat[ob] = best;
         if (a.best_step) a.best_step[ob] = bstep;
+        if (a.conv_step) {
+            int cs = -1;
+            if (a.tol > real(0)) {
+                typedef typename DBits<real>::type dbits_t;
+                cs = a.conv_in[b];
+                if (cs < 0 && a.delta_last && DBits<real>::val(static_cast<const dbits_t*>(a.delta_last)[b]) < a.tol) cs = a.steps;
+            }
+            a.conv_step[ob] = cs;
+        }
     }
 }
 

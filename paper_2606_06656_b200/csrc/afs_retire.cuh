@@ -45,7 +45,12 @@ static __global__ void __launch_bounds__(1024) k_retire_plan(RunState* rs, int t
                                                       int32_t* __restrict__ best_sat_out, int32_t* __restrict__ best_step_out,
                                                       int32_t* __restrict__ orig_out, int32_t* __restrict__ src,
                                                       uint8_t* __restrict__ imp, int32_t* __restrict__ ret,
-                                                      int32_t* __restrict__ ret_sat, int32_t* __restrict__ ret_step)
+                                                      int32_t* __restrict__ ret_sat, int32_t* __restrict__ ret_step,
+                                                      // convergence detection (tol > 0): the step just taken is folded
+                                                      // into the stop count of every column
+                                                      double tol, int is64, const void* __restrict__ delta_t,
+                                                      const int32_t* __restrict__ conv_in, int32_t* __restrict__ conv_out,
+                                                      int32_t* __restrict__ ret_conv)
 {
     __shared__ int s_warp[2][32];
     __shared__ int s_base[2];
@@ -66,6 +71,15 @@ static __global__ void __launch_bounds__(1024) k_retire_plan(RunState* rs, int t
             frozen = moved[p] == 0;
             imp[p] = improved ? 1 : 0;
         }
+        int cs = -1;
+        if (in && tol > 0.0) {
+            cs = conv_in[p];
+            if (cs < 0) {
+                const double d = is64 ? __longlong_as_double(static_cast<const long long*>(delta_t)[p])
+                                      : (double)__uint_as_float(static_cast<const unsigned int*>(delta_t)[p]);
+                if (d < tol) cs = t + 1;
+            }
+        }
         const unsigned mA = __ballot_sync(FULL, in && !frozen), mR = __ballot_sync(FULL, in && frozen);
         if (lane == 0) { s_warp[0][warp] = __popc(mA); s_warp[1][warp] = __popc(mR); }
         __syncthreads();
@@ -75,10 +89,11 @@ static __global__ void __launch_bounds__(1024) k_retire_plan(RunState* rs, int t
         if (in && !frozen) {
             const int q = offA + __popc(mA & lt);
             src[q] = p; orig_out[q] = orig_in[p]; best_sat_out[q] = bs; best_step_out[q] = bt;
+            if (tol > 0.0) conv_out[q] = cs;
         }
         if (in && frozen) {
             const int q = offR + __popc(mR & lt);
-            ret[q] = p; ret_sat[q] = bs; ret_step[q] = bt;
+            ret[q] = p; ret_sat[q] = bs; ret_step[q] = bt; ret_conv[q] = cs;
         }
         __syncthreads();
         if (tid == 0) {
@@ -94,6 +109,7 @@ static __global__ void __launch_bounds__(1024) k_retire_plan(RunState* rs, int t
     const int na32 = (na + 31) & ~31;
     for (int q = na + tid; q < na32; q += 1024) {
         src[q] = src[0]; orig_out[q] = -1; best_sat_out[q] = best_sat_out[0]; best_step_out[q] = best_step_out[0];
+        if (tol > 0.0) conv_out[q] = conv_out[0];
     }
     for (int q = tid; q < na32; q += 1024) moved[q] = 0;
     if (tid == 0) { rs->n_act = na; rs->n_ret = nr; }
@@ -107,7 +123,8 @@ __global__ void __launch_bounds__(256) k_retire_out(const RunState* __restrict__
                                                     const int32_t* __restrict__ ret, const int32_t* __restrict__ ret_sat,
                                                     const int32_t* __restrict__ ret_step, const int32_t* __restrict__ orig,
                                                     real* __restrict__ X, int8_t* __restrict__ best_assign,
-                                                    int32_t* __restrict__ best_sat, int32_t* __restrict__ best_step)
+                                                    int32_t* __restrict__ best_sat, int32_t* __restrict__ best_step,
+                                                    const int32_t* __restrict__ ret_conv, int32_t* __restrict__ conv_step)
 {
     const int n_ret = rs->n_ret;
     if ((int)blockIdx.y * 32 >= n_ret) return;
@@ -127,6 +144,7 @@ __global__ void __launch_bounds__(256) k_retire_out(const RunState* __restrict__
         if (blockIdx.x == 0 && lane == 0) {
             if (best_sat) best_sat[o] = ret_sat[i];
             if (best_step) best_step[o] = ret_step[i];
+            if (conv_step) conv_step[o] = ret_conv[i];
         }
     }
 }

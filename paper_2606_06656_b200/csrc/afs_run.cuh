@@ -16,12 +16,18 @@ namespace afs {
 static int var_grid_x(int n) { return (n + VAR_WARPS * VAR_VPW - 1) / (VAR_WARPS * VAR_VPW); }
 
 // variable pass: as many 32-restart sub-tiles per lane as the batch allows (4, 2 or 1)
-template <typename real, bool EVAL, bool LONGT>
+template <typename real, bool EVAL, bool LONGT, bool CONV>
 static void launch_var_l(const VarArgs<real>& a, int gx, int tiles, cudaStream_t st)
 {
-    if (sizeof(real) == 4 && tiles % 4 == 0) k_var<real, EVAL, 4, LONGT><<<dim3(gx, tiles / 4), VAR_WARPS * 32, 0, st>>>(a);
-    else if (tiles % 2 == 0) k_var<real, EVAL, 2, LONGT><<<dim3(gx, tiles / 2), VAR_WARPS * 32, 0, st>>>(a);
-    else k_var<real, EVAL, 1, LONGT><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
+    if (sizeof(real) == 4 && tiles % 4 == 0) k_var<real, EVAL, 4, LONGT, CONV><<<dim3(gx, tiles / 4), VAR_WARPS * 32, 0, st>>>(a);
+    else if (tiles % 2 == 0) k_var<real, EVAL, 2, LONGT, CONV><<<dim3(gx, tiles / 2), VAR_WARPS * 32, 0, st>>>(a);
+    else k_var<real, EVAL, 1, LONGT, CONV><<<dim3(gx, tiles), VAR_WARPS * 32, 0, st>>>(a);
+}
+template <typename real, bool EVAL, bool LONGT>
+static void launch_var_c(const VarArgs<real>& a, int gx, int tiles, cudaStream_t st)
+{
+    if (!EVAL && a.tol > real(0)) launch_var_l<real, EVAL, LONGT, !EVAL>(a, gx, tiles, st);
+    else launch_var_l<real, EVAL, LONGT, false>(a, gx, tiles, st);
 }
 template <typename real, bool EVAL>
 static void launch_var(afs_problem* P, VarArgs<real>& a, int gx, int tiles, const RunState* rs, cudaStream_t st)
@@ -36,9 +42,9 @@ static void launch_var(afs_problem* P, VarArgs<real>& a, int gx, int tiles, cons
                                                                      (const real*)P->ws.bnd, EVAL ? nullptr : a.mask, GL, rs);
         }
         a.GL = GL;
-        launch_var_l<real, EVAL, true>(a, gx, tiles, st);
+        launch_var_c<real, EVAL, true>(a, gx, tiles, st);
     } else {
-        launch_var_l<real, EVAL, false>(a, gx, tiles, st);
+        launch_var_c<real, EVAL, false>(a, gx, tiles, st);
     }
 }
 
@@ -269,14 +275,16 @@ static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, i
 
 template <typename real>
 static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps, real lr, const int8_t* mask,
-                               int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
+                               int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream,
+                               real tol = real(0), int32_t* conv_step = nullptr)
 {
     afs_status s = enter(P, B);
     if (s != AFS_OK) return s;
     if (!X || steps < 0 || !std::isfinite((double)lr)) return AFS_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const int Bp = ((B + 31) / 32) * 32;
-    const int plan = P->opt_mode == 1 ? -1 : resident_plan<real>(P, Bp / 32);
+    // convergence detection (tol > 0) lives in the streaming path, where stopped restarts are retired
+    const int plan = (P->opt_mode == 1 || tol > real(0)) ? -1 : resident_plan<real>(P, Bp / 32);
     if (P->opt_mode == 2 && plan < 0) return AFS_ERR_UNSUPPORTED;
     // count rows: the resident kernel keeps one per iterate, the streaming path a ring of three
     if ((s = ensure_workspace(P, Bp, sizeof(real), plan >= 0 ? (int64_t)steps + 1 : 3)) != AFS_OK) return s;
@@ -295,6 +303,14 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     int oc = 0;              // orig[oc]
     bool pending = false;    // iterate t-1 is counted but not merged yet (the variable pass of iteration t merges it)
     RunState* rs = w.rs;
+    const bool conv = tol > real(0);
+    typedef typename DBits<real>::type dbits_t;
+    dbits_t* delta = static_cast<dbits_t*>(w.delta);     // [3][Bp], row t % 3 = max |dX| of step t
+    bool dpending = false;                               // the last step's row is not folded into conv yet
+    if (conv) {
+        launch_fill_i32(w.conv[0], (size_t)Bp, -1, st);
+        CU(cudaMemsetAsync(w.delta, 0, (size_t)3 * Bp * sizeof(dbits_t), st));
+    }
     k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT[0], B, P->n, Bp, mask, w.S[0], w.SAT[0]);
     k_run_init<<<(Bp + 255) / 256, 256, 0, st>>>(rs, B, Bp, w.orig[0], w.moved);
     P->last_launches += 2;
@@ -325,6 +341,12 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
         a.best_step_in = w.best_step[bc]; a.best_step_out = w.best_step[bc ^ 1];
         a.S_prev = w.S[sp_]; a.S_next = w.S[sp_]; a.SAT_next = w.SAT[sp_]; a.best_bits = w.best_bits[bb];
         a.rs = rs; a.moved = retire ? w.moved : nullptr;
+        a.tol = tol;
+        if (conv) {
+            a.conv_in = w.conv[bc]; a.conv_out = w.conv[bc ^ 1];
+            a.delta_prev = dpending ? delta + (size_t)((t + 2) % 3) * Bp : nullptr;
+            a.delta_cur = delta + (size_t)(t % 3) * Bp; a.delta_zero = delta + (size_t)((t + 1) % 3) * Bp;
+        }
         // S9 of the pull clauses needs only the (complete) sign words of X_t: it runs on the library's second stream
         // beside the variable pass and is joined before anything reads the count row of X_t
         const bool side = P->n_pull > 0;
@@ -344,16 +366,18 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
         xc = xn;
         { const int tmp = sc_; sc_ = sp_; sp_ = tmp; }   // S[sc_] = words of X_{t+1}, S[sp_] = words of X_t
         pending = true;
+        dpending = conv;
         if (retire) {
             // iterate t is merged by the plan; frozen restarts leave with their results; the rest moves to the front
             ProfSpan span(P, 18, st);
             const int xf = (xc + 1) % 3, sf = 3 - sc_ - sp_;
             k_retire_plan<<<1, 1024, 0, st>>>(rs, t, sat_cur, w.best_sat[bc], w.best_step[bc], w.orig[oc], w.moved,
                                               w.best_sat[bc ^ 1], w.best_step[bc ^ 1], w.orig[oc ^ 1], w.rt_src, w.rt_imp,
-                                              w.rt_ret, w.rt_ret_sat, w.rt_ret_step);
+                                              w.rt_ret, w.rt_ret_sat, w.rt_ret_step, (double)tol, sizeof(real) == 8 ? 1 : 0,
+                                              delta + (size_t)(t % 3) * Bp, w.conv[bc], w.conv[bc ^ 1], w.rt_ret_conv);
             k_retire_out<real><<<tg, 256, 0, st>>>(rs, P->n, Bp, XT[xc], w.S[sp_], w.best_bits[bb], w.rt_imp, w.rt_ret,
                                                    w.rt_ret_sat, w.rt_ret_step, w.orig[oc], X, best_assign, best_sat,
-                                                   best_step);
+                                                   best_step, w.rt_ret_conv, conv_step);
             k_compact<real><<<dim3((P->n + 7) / 8, tiles), 256, 0, st>>>(rs, P->n, Bp, w.rt_src, w.rt_imp, XT[xc], w.S[sp_],
                                                                          w.best_bits[bb], XT[xf], w.S[sf], w.SAT[sf],
                                                                          w.best_bits[bb ^ 1]);
@@ -361,6 +385,7 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
             bc ^= 1; oc ^= 1; bb ^= 1; xc = xf;
             sp_ = sc_; sc_ = sf;      // the words of X_t are not needed any more: the next pass has nothing to merge
             pending = false;
+            dpending = false;
         }
     }
     P->prof.on = false;
@@ -377,6 +402,8 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     f.S_prev = w.S[sp_]; f.best_bits = w.best_bits[bb];
     f.X = X; f.best_assign = best_assign; f.best_sat = best_sat; f.best_step = best_step;
     f.rs = rs; f.orig = w.orig[oc];
+    f.tol = tol; f.conv_in = w.conv[bc]; f.conv_step = conv_step;
+    f.delta_last = dpending ? delta + (size_t)((steps + 2) % 3) * Bp : nullptr;
     k_finalize<real><<<tg, 256, 0, st>>>(f);
     P->last_launches++;
     CU(cudaGetLastError());
