@@ -153,6 +153,19 @@ AFS_API afs_status afs_pgd_run_conv_f64(afs_problem* p, double* X, int32_t B, in
                                         void* cuda_stream);
 
 /*
+ * afs_pgd_run_masks -- afs_pgd_run with one partial assignment PER RESTART (P:L140 partial-assignment completion;
+ * P:L146, L188 (ii): the batch as an enumerator of completions / sub-solver): masks is device int8[B,n], row b fixes
+ * the variables of restart b (0 free, -1 fixed True, +1 fixed False).  Everything else as afs_pgd_run.  Restart b's
+ * result equals afs_pgd_run on that restart alone with mask = masks[b].  Always takes the streaming path; the fixed
+ * variables sit on +-1 and are handled as boundary literals (no per-call folding of the long constraints).
+ */
+AFS_API afs_status afs_pgd_run_masks(afs_problem* p, float* X, int32_t B, int32_t steps, float lr, const int8_t* masks,
+                                     int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* cuda_stream);
+AFS_API afs_status afs_pgd_run_masks_f64(afs_problem* p, double* X, int32_t B, int32_t steps, double lr,
+                                         const int8_t* masks, int8_t* best_assign, int32_t* best_sat, int32_t* best_step,
+                                         void* cuda_stream);
+
+/*
  * afs_pgd_run_host -- the same call with HOST buffers (all pointers host; pinned memory recommended): copies X
  * and mask to the device, runs afs_pgd_run, copies X, best_assign, best_sat, best_step back, synchronises.
  * This is the end-to-end entry point bench.py times ("e2e").  Output pointers may be NULL.

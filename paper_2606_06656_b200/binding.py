@@ -21,7 +21,7 @@ EXPORTS = (
     "afs_problem_create", "afs_problem_destroy", "afs_coeffs", "afs_eval_grad", "afs_eval_grad_f64",
     "afs_round_count", "afs_round_count_f64", "afs_pgd_run", "afs_pgd_run_f64", "afs_pgd_run_host",
     "afs_problem_info", "afs_set_option", "afs_status_string", "afs_abi_version", "afs_last_error_message",
-    "afs_profile_read", "afs_profile_flops", "afs_fp32_fma_peak", "afs_pgd_run_conv", "afs_pgd_run_conv_f64",
+    "afs_profile_read", "afs_profile_flops", "afs_fp32_fma_peak", "afs_pgd_run_conv", "afs_pgd_run_conv_f64", "afs_pgd_run_masks", "afs_pgd_run_masks_f64",
 )
 
 _lib = None
@@ -64,6 +64,10 @@ def lib():
     L.afs_pgd_run_conv.restype = C.c_int
     L.afs_pgd_run_conv_f64.argtypes = [vp, vp, i32, i32, C.c_double, vp, C.c_double, vp, vp, vp, vp, vp, vp, vp]
     L.afs_pgd_run_conv_f64.restype = C.c_int
+    L.afs_pgd_run_masks.argtypes = [vp, vp, i32, i32, C.c_float, vp, vp, vp, vp, vp]
+    L.afs_pgd_run_masks.restype = C.c_int
+    L.afs_pgd_run_masks_f64.argtypes = [vp, vp, i32, i32, C.c_double, vp, vp, vp, vp, vp]
+    L.afs_pgd_run_masks_f64.restype = C.c_int
     L.afs_pgd_run_host.argtypes = [vp, vp, i32, i32, C.c_float, vp, vp, vp, vp, vp]
     L.afs_pgd_run_host.restype = C.c_int
     L.afs_problem_info.argtypes = [vp, i32]
@@ -254,6 +258,22 @@ class Problem:
                 float(tol), ba.data_ptr(), bs.data_ptr(), bt.data_ptr(), cs.data_ptr(), fs.data_ptr(), fF.data_ptr(),
                 _stream_ptr(X.device)), "afs_pgd_run_conv")
         return dict(X=X, best_assign=ba, best_sat=bs, best_step=bt, conv_step=cs, final_sat=fs, final_F=fF)
+
+    def pgd_run_masks(self, X, steps: int, lr: float, masks):
+        """afs_pgd_run_masks / _f64: masks is a CUDA int8 tensor [B, n], one partial assignment per restart."""
+        torch = _torch()
+        f64 = X.dtype == torch.float64
+        self._check_X(X, torch.float64 if f64 else torch.float32)
+        B = X.shape[0]
+        if not (masks.is_cuda and masks.dtype == torch.int8 and tuple(masks.shape) == (B, self.n) and masks.is_contiguous()):
+            raise ValueError("masks must be a contiguous CUDA int8 tensor [B, n]")
+        ba = torch.empty((B, self.n), dtype=torch.int8, device=X.device)
+        bs = torch.empty(B, dtype=torch.int32, device=X.device)
+        bt = torch.empty(B, dtype=torch.int32, device=X.device)
+        fn = lib().afs_pgd_run_masks_f64 if f64 else lib().afs_pgd_run_masks
+        _chk(fn(self._h, X.data_ptr(), B, int(steps), float(lr), masks.data_ptr(), ba.data_ptr(), bs.data_ptr(),
+                bt.data_ptr(), _stream_ptr(X.device)), "afs_pgd_run_masks")
+        return dict(X=X, best_assign=ba, best_sat=bs, best_step=bt)
 
     def pgd_run_host(self, X, steps: int, lr: float, mask=None, out=None):
         """afs_pgd_run_host: X float32 [B,n] HOST tensor/array (pinned recommended), updated in place; H2D and D2H

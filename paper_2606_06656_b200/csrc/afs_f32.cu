@@ -22,3 +22,7 @@ extern "C" afs_status afs_pgd_run_conv(afs_problem* p, float* X, int32_t B, int3
     if (s == AFS_OK && final_F) s = eval_grad_impl<float>(p, X, B, final_F, nullptr, stream);
     return s;
 }
+
+extern "C" afs_status afs_pgd_run_masks(afs_problem* p, float* X, int32_t B, int32_t steps, float lr, const int8_t* masks,
+                                        int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
+{ return pgd_run_impl<float>(p, X, B, steps, lr, masks, best_assign, best_sat, best_step, stream, float(0), nullptr, true); }

@@ -22,3 +22,7 @@ extern "C" afs_status afs_pgd_run_conv_f64(afs_problem* p, double* X, int32_t B,
     if (s == AFS_OK && final_F) s = eval_grad_impl<double>(p, X, B, final_F, nullptr, stream);
     return s;
 }
+
+extern "C" afs_status afs_pgd_run_masks_f64(afs_problem* p, double* X, int32_t B, int32_t steps, double lr, const int8_t* masks,
+                                        int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
+{ return pgd_run_impl<double>(p, X, B, steps, lr, masks, best_assign, best_sat, best_step, stream, double(0), nullptr, true); }

@@ -137,6 +137,8 @@ struct Workspace {
     int32_t* rt_ret_step = nullptr;
     int32_t* rt_ret_conv = nullptr;
     // convergence detection (afs_pgd_run_conv)
+    int8_t* maskT = nullptr;               // [n][Bp] per-restart masks, transposed (afs_pgd_run_masks); allocated on first use
+    int64_t maskT_elems = 0;
     int32_t* conv[2] = {nullptr, nullptr}; // [Bp] steps after which the column stopped, -1 = running
     void* delta = nullptr;                 // [3][Bp] 8-byte cells: max |dX| of a step as order-preserving integer bits
     void* fe_med = nullptr;                // real [n_med][Bp]      (eval_grad only)

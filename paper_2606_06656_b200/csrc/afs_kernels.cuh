@@ -40,8 +40,10 @@ __device__ __forceinline__ real ldx(const real* __restrict__ XT, uint32_t w, int
 template <typename real>
 __global__ void __launch_bounds__(256) k_transpose_in(const real* __restrict__ X, real* __restrict__ XT, int B, int n,
                                                       int Bp, const int8_t* __restrict__ mask,
-                                                      uint32_t* __restrict__ Sw, uint32_t* __restrict__ SATw)
-{
+                                                      uint32_t* __restrict__ Sw, uint32_t* __restrict__ SATw,
+                                                      int mask_stride = 0, int8_t* __restrict__ maskT = nullptr)
+{   // mask_stride = 0: one mask[n] for all restarts; = n: masks[B][n], one per restart (then also written transposed
+    // to maskT[n][Bp] for the variable pass)
     __shared__ real tile[32][33];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int v0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
@@ -58,13 +60,17 @@ __global__ void __launch_bounds__(256) k_transpose_in(const real* __restrict__ X
         int v = v0 + r, b = b0 + tx;
         if (v < n) {
             real x = tile[tx][r];
-            if (mask) { int mk = mask[v]; if (mk != 0) x = (real)mk; }   // fixed at entry
+            if (mask) {   // fixed at entry
+                const int mk = mask[(size_t)min(b, B - 1) * mask_stride + v];
+                if (mk != 0) x = (real)mk;
+                if (maskT) maskT[(size_t)v * Bp + b] = (int8_t)mk;
+            }
             XT[(size_t)v * Bp + b] = x;
         }
         if (Sw) {   // the 32 lanes of a warp hold one variable's tile (v is warp-uniform)
             const real xx = v < n ? tile[tx][r] : real(0);
             real xm = xx;
-            if (mask && v < n) { int mk = mask[v]; if (mk != 0) xm = (real)mk; }
+            if (mask && v < n) { int mk = mask[(size_t)min(b, B - 1) * mask_stride + v]; if (mk != 0) xm = (real)mk; }
             const unsigned sb = __ballot_sync(FULL, xm < real(0)), sa = __ballot_sync(FULL, xm == real(1) || xm == real(-1));
             if (tx == 0 && v < n) { Sw[(size_t)v * (Bp >> 5) + blockIdx.y] = sb; SATw[(size_t)v * (Bp >> 5) + blockIdx.y] = sa; }
         }
@@ -626,6 +632,7 @@ struct VarArgs {
     uint32_t* SAT_next;          // thread reads a word of S_prev before it writes that word of S_next)
     uint32_t* best_bits;
     const real* GL;              // LONGT: [n][Bp] the LONG class's share of the gradient (k_glong)
+    const int8_t* maskT;         // CONV variant only: per-restart masks [n][Bp] (afs_pgd_run_masks), or NULL
     // CONV (afs_pgd_run_conv): a restart stops after the first step with max_v |dX| < tol (G24)
     real tol;
     const int32_t* conv_in;      // [Bp] number of steps after which the restart stopped, -1 = still running
@@ -888,6 +895,10 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
 #pragma unroll
         for (int c = 0; c < RPL; ++c) x[c] = xcol[(size_t)v * Bp + 32 * c];
         if (!EVAL) mk = a.mask ? a.mask[v] : 0;
+        int mkl[RPL];   // per restart (CONV variant with per-restart masks), else the shared value
+#pragma unroll
+        for (int c = 0; c < RPL; ++c) mkl[c] = (CONV && a.maskT) ? (int)a.maskT[(size_t)v * Bp + b + 32 * c] : mk;
+        if (CONV && a.maskT) mk = 0;   // some restart may be free: the gradient is needed
 #pragma unroll
         for (int c = 0; c < RPL; ++c) g[c] = real(0);
         if (mk == 0) {   // a fixed variable never moves: its gradient is not needed
@@ -925,7 +936,7 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
                 real xn = x[c] - a.lr * g[c];
                 xn = xn > one ? one : xn;
                 xn = xn < -one ? -one : xn;
-                if (mk != 0 || (CONV && frozen[c])) xn = x[c];
+                if (mkl[c] != 0 || (CONV && frozen[c])) xn = x[c];
                 a.Xout[(size_t)v * Bp + b + 32 * c] = xn;
                 if (a.moved && xn != x[c]) a.moved[b + 32 * c] = 1;
                 if (CONV) dmax[c] = fmax(dmax[c], fabs(xn - x[c]));
@@ -954,7 +965,7 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
 template <typename real>
 __global__ void __launch_bounds__(256) k_glong(int n, int ntile, int Bp, const int32_t* __restrict__ lslot_ptr,
                                                const int32_t* __restrict__ lslot_info, const real* __restrict__ Xin,
-                                               const real* __restrict__ lrows /* scratch + nslots_a * Bp */,
+                                               const real* __restrict__ lrows /* scratch + nslots_a * Bp: [tile][nl][32] */, int nl,
                                                const real* __restrict__ bnd, const int8_t* __restrict__ mask,
                                                real* __restrict__ GL, const RunState* __restrict__ rs)
 {
@@ -968,7 +979,7 @@ __global__ void __launch_bounds__(256) k_glong(int n, int ntile, int Bp, const i
     const real x = Xin[(size_t)v * Bp + b];
     const bool onb = x == real(1) || x == real(-1);
     const int neg0 = x < real(0) ? 1 : 0;
-    const real* __restrict__ rows = lrows + b;
+    const real* __restrict__ rows = lrows + (size_t)tile * nl * 32 + lane;   // tile-major rows of the class
     const real* __restrict__ bb = bnd + (size_t)b * 2;
     const int s0 = lslot_ptr[v], s1 = lslot_ptr[v + 1];
     real g = real(0);
@@ -984,7 +995,7 @@ __global__ void __launch_bounds__(256) k_glong(int n, int ntile, int Bp, const i
                 const int info = __shfl_sync(FULL, myinfo, kk);
                 ln[h] = info & 1;
                 // literal true (y = -1) iff (x < 0) != negated: the second element of the pair
-                const real* p = onb ? bb + (size_t)(info >> 1) * Bp * 2 + (neg0 ^ ln[h]) : rows + (size_t)(sb0 + kk) * Bp;
+                const real* p = onb ? bb + (size_t)(info >> 1) * Bp * 2 + (neg0 ^ ln[h]) : rows + (size_t)(sb0 + kk) * 32;
                 t[h] = *p;
             }
 #pragma unroll

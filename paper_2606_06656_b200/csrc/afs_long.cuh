@@ -410,7 +410,7 @@ __global__ void __launch_bounds__(WPC * 32) k_long_items(const LongCon* __restri
                                                          const uint32_t* __restrict__ lits, const int32_t* __restrict__ slots,
                                                          const real* __restrict__ XT, const uint32_t* __restrict__ Sw,
                                                          const uint32_t* __restrict__ SATw, int ntile, int Bp,
-                                                         real* __restrict__ scratch, real* __restrict__ bnd,
+                                                         real* __restrict__ lrows, int row0, int nl, real* __restrict__ bnd,
                                                          real* __restrict__ fe_out, const uint4* __restrict__ items,
                                                          const int* __restrict__ count, int LS, int QS,
                                                          unsigned long long* __restrict__ work,
@@ -542,7 +542,9 @@ __global__ void __launch_bounds__(WPC * 32) k_long_items(const LongCon* __restri
             const int j = J[e];
             if (j != 0xffff) {
                 const real g = Rc[e];
-                scratch[(size_t)sw[j] * Bp + b] = (lw[j] >> 31) ? -g : g;
+                // rows of the LONG class are tile-major, [tile][row][32]: the rows of one variable are consecutive, so the
+                // variable-side pass (k_glong) streams them instead of touching one 128-byte piece per 8 KB
+                lrows[((size_t)(b >> 5) * nl + (size_t)(sw[j] - row0)) * 32 + (b & 31)] = (lw[j] >> 31) ? -g : g;
             }
         }
         __syncwarp();

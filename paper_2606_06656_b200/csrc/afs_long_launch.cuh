@@ -35,7 +35,8 @@ static afs_status launch_long_items(afs_problem* P, const LongLists& wl, int set
     unsigned long long* work = nullptr;
     { afs_status ws = prof_work_slot(P, 8 + NR, st, &work); if (ws != AFS_OK) return ws; }
     kern<<<grid, WPC * 32, smem, st>>>(fo ? P->d_long_f : P->d_long, fo ? P->d_long_lits_f : P->d_long_lits,
-                                        fo ? P->d_long_slots_f : P->d_long_slots, XT, Sw, SATw, Bp / 32, Bp, scratch,
+                                        fo ? P->d_long_slots_f : P->d_long_slots, XT, Sw, SATw, Bp / 32, Bp,
+                                        scratch + (size_t)P->nslots_a * Bp, (int)P->nslots_a, (int)(P->nslots - P->nslots_a),
                                         (real*)P->ws.bnd, fe, wl.items[CLS], wl.count + set * LONG_CLASSES + CLS, LS, QS,
                                         work, P->d_long_goff, P->ws.long_MI, P->ws.long_MT);
     P->last_launches++;

@@ -26,7 +26,7 @@ static void launch_var_l(const VarArgs<real>& a, int gx, int tiles, cudaStream_t
 template <typename real, bool EVAL, bool LONGT>
 static void launch_var_c(const VarArgs<real>& a, int gx, int tiles, cudaStream_t st)
 {
-    if (!EVAL && a.tol > real(0)) launch_var_l<real, EVAL, LONGT, !EVAL>(a, gx, tiles, st);
+    if (!EVAL && (a.tol > real(0) || a.maskT)) launch_var_l<real, EVAL, LONGT, !EVAL>(a, gx, tiles, st);
     else launch_var_l<real, EVAL, LONGT, false>(a, gx, tiles, st);
 }
 template <typename real, bool EVAL>
@@ -38,7 +38,7 @@ static void launch_var(afs_problem* P, VarArgs<real>& a, int gx, int tiles, cons
         {
             ProfSpan span(P, 6, st);
             k_glong<real><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P->n, tiles, a.Bp, P->d_lslot_ptr, P->d_lslot_info, a.Xin,
-                                                                     a.scratch + (size_t)P->nslots_a * a.Bp,
+                                                                     a.scratch + (size_t)P->nslots_a * a.Bp, (int)(P->nslots - P->nslots_a),
                                                                      (const real*)P->ws.bnd, EVAL ? nullptr : a.mask, GL, rs);
         }
         a.GL = GL;
@@ -276,7 +276,7 @@ static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, i
 template <typename real>
 static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps, real lr, const int8_t* mask,
                                int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream,
-                               real tol = real(0), int32_t* conv_step = nullptr)
+                               real tol = real(0), int32_t* conv_step = nullptr, bool per_restart_masks = false)
 {
     afs_status s = enter(P, B);
     if (s != AFS_OK) return s;
@@ -284,11 +284,20 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     cudaStream_t st = (cudaStream_t)stream;
     const int Bp = ((B + 31) / 32) * 32;
     // convergence detection (tol > 0) lives in the streaming path, where stopped restarts are retired
-    const int plan = (P->opt_mode == 1 || tol > real(0)) ? -1 : resident_plan<real>(P, Bp / 32);
+    const int plan = (P->opt_mode == 1 || tol > real(0) || per_restart_masks) ? -1 : resident_plan<real>(P, Bp / 32);
+    if (per_restart_masks && !mask) return AFS_ERR_INVALID_ARG;
     if (P->opt_mode == 2 && plan < 0) return AFS_ERR_UNSUPPORTED;
     // count rows: the resident kernel keeps one per iterate, the streaming path a ring of three
     if ((s = ensure_workspace(P, Bp, sizeof(real), plan >= 0 ? (int64_t)steps + 1 : 3)) != AFS_OK) return s;
     Workspace& w = P->ws;
+    if (per_restart_masks && w.maskT_elems < (int64_t)P->n * w.Bp) {
+        CU(cudaDeviceSynchronize());
+        if (w.maskT) cudaFree(w.maskT);
+        w.maskT = nullptr; w.maskT_elems = 0;
+        if (cudaMalloc((void**)&w.maskT, (size_t)P->n * w.Bp) != cudaSuccess) { (void)cudaGetLastError(); return AFS_ERR_ALLOC; }
+        w.maskT_elems = (int64_t)P->n * w.Bp;
+        w.bytes += (size_t)P->n * w.Bp;
+    }
     P->last_resident = 0;
     if (plan >= 0) return pgd_run_resident<real>(P, plan, X, B, steps, lr, mask, best_assign, best_sat, best_step, st);
     real* XT[3] = {(real*)w.XT[0], (real*)w.XT[1], (real*)w.XT[2]};
@@ -303,7 +312,8 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     int oc = 0;              // orig[oc]
     bool pending = false;    // iterate t-1 is counted but not merged yet (the variable pass of iteration t merges it)
     RunState* rs = w.rs;
-    const bool conv = tol > real(0);
+    const bool conv = tol > real(0) || per_restart_masks;   // the extended variable pass (its state must be initialised)
+    const int8_t* mask1 = per_restart_masks ? nullptr : mask;   // the one mask shared by all restarts, if that is the mode
     typedef typename DBits<real>::type dbits_t;
     dbits_t* delta = static_cast<dbits_t*>(w.delta);     // [3][Bp], row t % 3 = max |dX| of step t
     bool dpending = false;                               // the last step's row is not folded into conv yet
@@ -311,7 +321,8 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
         launch_fill_i32(w.conv[0], (size_t)Bp, -1, st);
         CU(cudaMemsetAsync(w.delta, 0, (size_t)3 * Bp * sizeof(dbits_t), st));
     }
-    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT[0], B, P->n, Bp, mask, w.S[0], w.SAT[0]);
+    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT[0], B, P->n, Bp, mask, w.S[0], w.SAT[0], per_restart_masks ? P->n : 0,
+                                             per_restart_masks ? w.maskT : nullptr);
     k_run_init<<<(Bp + 255) / 256, 256, 0, st>>>(rs, B, Bp, w.orig[0], w.moved);
     P->last_launches += 2;
     CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)3 * Bp * sizeof(int32_t), st));
@@ -319,8 +330,8 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     CU(cudaMemsetAsync(w.best_step[0], 0, (size_t)Bp * sizeof(int32_t), st));
     P->last_launches++;
     const int gx = var_grid_x(P->n);
-    if (mask && P->n_long > 0 && steps > 0) {   // the fixed variables' literals leave the long constraints for this run
-        if ((s = launch_long_fold(P, mask, st)) != AFS_OK) return s;
+    if (mask1 && P->n_long > 0 && steps > 0) {   // the fixed variables' literals leave the long constraints for this run
+        if ((s = launch_long_fold(P, mask1, st)) != AFS_OK) return s;
     }
     const int K = P->retire_every;   // 0: never
     for (int t = 0; t < steps; ++t) {
@@ -334,7 +345,8 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
         a.n = P->n; a.Bp = Bp; a.t = t;
         a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
         a.gconst = P->d_pull_gconst; a.slot_ptr = P->d_slot_ptr;
-        a.scratch = scratch; a.Xin = Xin; a.Xout = XT[xn]; a.lr = lr; a.mask = mask;
+        a.scratch = scratch; a.Xin = Xin; a.Xout = XT[xn]; a.lr = lr; a.mask = mask1;
+        a.maskT = per_restart_masks ? w.maskT : nullptr;
         a.sat_prev = pending ? w.sat_hist + (size_t)((t + 2) % 3) * Bp : nullptr;
         a.sat_zero = w.sat_hist + (size_t)((t + 1) % 3) * Bp;
         a.best_sat_in = w.best_sat[bc]; a.best_sat_out = w.best_sat[bc ^ 1];
