@@ -979,28 +979,35 @@ __global__ void __launch_bounds__(256) k_glong(int n, int ntile, int Bp, const i
     const real x = Xin[(size_t)v * Bp + b];
     const bool onb = x == real(1) || x == real(-1);
     const int neg0 = x < real(0) ? 1 : 0;
-    const real* __restrict__ rows = lrows + (size_t)tile * nl * 32 + lane;   // tile-major rows of the class
-    const real* __restrict__ bb = bnd + (size_t)b * 2;
+    // One base pointer and 32-bit element offsets per lane: a restart on the boundary reads the pair table (second
+    // element where the literal is true, i.e. (x < 0) != negated), one inside the cube reads the class's rows.
+    const real* __restrict__ base = onb ? bnd + (size_t)b * 2
+                                        : lrows + ((size_t)tile * nl + (size_t)lslot_ptr[v]) * 32 + lane;
+    const uint32_t sgn = onb ? 0x80000000u : 0u;      // chain rule sign (S5) for pair entries; the rows carry it already
+    const uint32_t pair_stride = (uint32_t)Bp * 2u;
     const int s0 = lslot_ptr[v], s1 = lslot_ptr[v + 1];
     real g = real(0);
     for (int sb0 = s0; sb0 < s1; sb0 += 32) {
         const int myinfo = sb0 + lane < s1 ? lslot_info[sb0 + lane] : 0;   // 32 descriptors with one coalesced load
         const int cnt = min(32, s1 - sb0);
-        for (int k = 0; k < cnt; k += 8) {
+        int k = 0;
+        for (; k + 8 <= cnt; k += 8) {   // eight literals per round, their loads issued together
             real t[8];
-            int ln[8];
+            uint32_t fl[8];
 #pragma unroll
             for (int h = 0; h < 8; ++h) {
-                const int kk = k + h < cnt ? k + h : k;
-                const int info = __shfl_sync(FULL, myinfo, kk);
-                ln[h] = info & 1;
-                // literal true (y = -1) iff (x < 0) != negated: the second element of the pair
-                const real* p = onb ? bb + (size_t)(info >> 1) * Bp * 2 + (neg0 ^ ln[h]) : rows + (size_t)(sb0 + kk) * 32;
-                t[h] = *p;
+                const uint32_t info = (uint32_t)__shfl_sync(FULL, myinfo, k + h);
+                const uint32_t off = onb ? (info >> 1) * pair_stride + ((info & 1u) ^ (uint32_t)neg0) : (uint32_t)(sb0 - s0 + k + h) * 32u;
+                fl[h] = (info & 1u) ? sgn : 0u;
+                t[h] = base[off];
             }
 #pragma unroll
-            for (int h = 0; h < 8; ++h)
-                if (k + h < cnt) g += (onb && ln[h]) ? -t[h] : t[h];   // chain rule sign (S5); the rows carry it already
+            for (int h = 0; h < 8; ++h) g += flip(t[h], fl[h]);
+        }
+        for (; k < cnt; ++k) {
+            const uint32_t info = (uint32_t)__shfl_sync(FULL, myinfo, k);
+            const uint32_t off = onb ? (info >> 1) * pair_stride + ((info & 1u) ^ (uint32_t)neg0) : (uint32_t)(sb0 - s0 + k) * 32u;
+            g += flip(base[off], (info & 1u) ? sgn : 0u);
         }
     }
     GL[(size_t)v * Bp + b] = g;

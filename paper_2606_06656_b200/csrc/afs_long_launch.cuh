@@ -48,6 +48,9 @@ afs_status launch_long_all(afs_problem* P, const real* XT, const uint32_t* Sw, c
                            int32_t* sat, real* fe, const RunState* rs, cudaStream_t st)
 {
     if (P->n_long == 0) return AFS_OK;
+    // k_glong addresses the pair table and the class's rows with 32-bit element offsets
+    if ((unsigned long long)P->n_long * (unsigned long long)Bp * 2ull >= (1ull << 32) ||
+        (unsigned long long)(P->nslots - P->nslots_a) * 32ull >= (1ull << 32)) return AFS_ERR_UNSUPPORTED;
     LongLists wl;
     for (int k = 0; k < LONG_CLASSES; ++k) wl.items[k] = P->ws.long_items[k];
     wl.count = P->ws.long_count;
