@@ -213,7 +213,7 @@ __device__ __forceinline__ bool long_pred(int type, int L, int k, int t)
 template <typename real, int NRR>
 __device__ __forceinline__ real long_forward(const LongCon& lc, const int L, real* __restrict__ Rc, real* __restrict__ Aw,
                                              const int nBr, const int nBr4, const int send, const int Leff, const int nB0,
-                                             const int off, const int lane, const int QS)
+                                             const int off, const int lane, const int QS, const bool want_fe)
 {
     constexpr unsigned FULLM = 0xffffffffu;
     real q[NRR][4];
@@ -258,7 +258,7 @@ __device__ __forceinline__ real long_forward(const LongCon& lc, const int L, rea
             if (t <= Leff) {
                 const real v = q[rr][i] * sc;
                 Aw[off + t] = v;
-                fe += long_pred(lc.type, L, lc.k, t + nB0) ? -v : v;
+                if (want_fe) fe += long_pred(lc.type, L, lc.k, t + nB0) ? -v : v;
             }
         }
     (void)FULLM;
@@ -270,7 +270,8 @@ __device__ __forceinline__ real long_forward(const LongCon& lc, const int L, rea
 template <typename real>
 __device__ __forceinline__ real long_forward_tiny(const LongCon& lc, const int L, const real* __restrict__ Rc,
                                                   real* __restrict__ Aw, const int nBr, const int nBr4, const int nAr,
-                                                  const int Leff, const int nB0, const int off, const int lane)
+                                                  const int Leff, const int nB0, const int off, const int lane,
+                                                  const bool want_fe)
 {
     constexpr unsigned FULLM = 0xffffffffu;
     real q = lane == 0 ? real(1) : real(0), P = real(1);
@@ -298,7 +299,7 @@ __device__ __forceinline__ real long_forward_tiny(const LongCon& lc, const int L
     real fe = real(0);
     if (lane <= Leff) {
         Aw[off + lane] = v;
-        fe = long_pred(lc.type, L, lc.k, lane + nB0) ? -v : v;
+        if (want_fe) fe = long_pred(lc.type, L, lc.k, lane + nB0) ? -v : v;
     }
     return fe;
 }
@@ -480,7 +481,8 @@ __global__ void __launch_bounds__(WPC * 32) k_long_items(const LongCon* __restri
                 const real u = real(0.5) + real(0.5) * y, p = real(0.5) - real(0.5) * y;
                 // the list decides the direction (type B: literal true by sign, p >= 1/2): min / max, divisor >= 1/2.
                 // Correctly rounded reciprocal times the numerator (<= 1 ulp off the IEEE quotient)
-                R = e < nBr4 ? u * recip(p) : p * recip(u);
+                const bool tb = e < nBr4;
+                R = (tb ? u : p) * recip(tb ? p : u);
             }
             Rc[e] = R;
         }
@@ -488,8 +490,8 @@ __global__ void __launch_bounds__(WPC * 32) k_long_items(const LongCon* __restri
         const int off = (3 - Leff) & 3;
         {
             real fe;
-            if (NR == 1 && Leff <= 31) fe = long_forward_tiny<real>(lc, L, Rc, Aw, nBr, nBr4, nAr, Leff, nB0, off, lane);
-            else fe = long_forward<real, NR>(lc, L, Rc, Aw, nBr, nBr4, send, Leff, nB0, off, lane, QS);
+            if (NR == 1 && Leff <= 31) fe = long_forward_tiny<real>(lc, L, Rc, Aw, nBr, nBr4, nAr, Leff, nB0, off, lane, fe_out != nullptr);
+            else fe = long_forward<real, NR>(lc, L, Rc, Aw, nBr, nBr4, send, Leff, nB0, off, lane, QS, fe_out != nullptr);
             if (fe_out) {
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) fe += __shfl_xor_sync(FULLM, fe, o);
