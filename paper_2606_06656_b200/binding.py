@@ -162,7 +162,7 @@ class Problem:
         _chk(lib().afs_set_option(self._h, what, value), "afs_set_option")
 
     KERNEL_CLASSES = (["resident", "var", "sat_pull", "cmed", "med0", "long_scan", "glong", "med3", "med4"] +
-                      ["long%d" % (i + 1) for i in range(9)] + ["boundary"])
+                      ["long1", "long_lane8", "long3", "long_lane32", "long5", "long_lane16", "long7", "long8", "long9", "boundary"])
 
     def profile_read(self):
         """afs_profile_read: {class name: (milliseconds, launches)} of the last pgd_run, non-empty classes only."""

@@ -73,7 +73,7 @@ void free_workspace(afs_problem* P)
     free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.S[2]); free_ptr(w.SAT[0]); free_ptr(w.SAT[1]); free_ptr(w.SAT[2]);
     free_ptr(w.bnd); free_ptr(w.GL); free_ptr(w.best_bits[1]); free_ptr(w.orig[0]); free_ptr(w.orig[1]); free_ptr(w.moved);
     free_ptr(w.rs); free_ptr(w.rt_src); free_ptr(w.rt_imp); free_ptr(w.rt_ret); free_ptr(w.rt_ret_sat); free_ptr(w.rt_ret_step); free_ptr(w.rt_ret_conv); free_ptr(w.maskT); free_ptr(w.conv[0]); free_ptr(w.conv[1]); free_ptr(w.delta);
-    for (int k = 0; k < 4; ++k) free_ptr(w.long_items[k]);
+    for (int k = 0; k < 7; ++k) free_ptr(w.long_items[k]);
     free_ptr(w.long_count); free_ptr(w.long_MI); free_ptr(w.long_MT); free_ptr(w.best_bits[0]);
     free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.fe_cm); free_ptr(w.f_part);
     free_ptr(w.mask_dev); free_ptr(w.host_stage_X); free_ptr(w.host_stage_assign);
@@ -138,11 +138,11 @@ afs_status ensure_workspace(afs_problem* P, int Bp, size_t elem, int64_t sat_row
     A(&w.conv[0], (size_t)nBp); A(&w.conv[1], (size_t)nBp); A((unsigned long long**)&w.delta, (size_t)3 * nBp);
     A((unsigned char**)&w.bnd, (size_t)P->n_long * nBp * 2 * nelem);
     A((unsigned char**)&w.GL, (P->n_long > 0 ? n : 0) * nBp * nelem);
-    for (int k = 0; k < 4; ++k) A(&w.long_items[k], (size_t)P->n_long * nBp);
-    A(&w.long_count, (size_t)8);
+    for (int k = 0; k < 7; ++k) A(&w.long_items[k], (size_t)P->n_long * nBp);
+    A(&w.long_count, (size_t)16);
     A(&w.long_MI, (size_t)P->long_grows * nBp); A(&w.long_MT, (size_t)P->long_grows * nBp);
     if (st != AFS_OK) { afs::free_workspace(P); return st; }
-    CU(cudaMemset(w.long_count, 0, 8 * sizeof(int)));
+    CU(cudaMemset(w.long_count, 0, 16 * sizeof(int)));
     w.Bp = nBp; w.elem = nelem; w.sat_rows = nrows; w.bytes = tot;
     return AFS_OK;
 }

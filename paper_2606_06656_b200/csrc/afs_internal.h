@@ -121,10 +121,10 @@ struct Workspace {
     uint32_t* SAT[3] = {nullptr, nullptr, nullptr}; // saturation bits, same layout: |x_v| = 1 (on the boundary of the cube)
     void* GL = nullptr;                    // real [n][Bp]: the LONG class's share of the gradient (k_glong -> k_var)
     void* bnd = nullptr;                   // real [n_long][Bp][2]: dFE/dy of a boundary literal at y = +1 / y = -1
-    uint4* long_items[4] = {nullptr, nullptr, nullptr, nullptr};   // work lists of the long-constraint kernels, by size class
+    uint4* long_items[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // work lists of the long-constraint kernels, by size class
     uint32_t* long_MI = nullptr;           // [long_grows][Bp] per group of 32 literals and restart: interior-literal mask,
     uint32_t* long_MT = nullptr;           //                  literal-true mask (k_long_scan -> k_long_items)
-    int* long_count = nullptr;             // [2][4] their lengths, two sets used alternately
+    int* long_count = nullptr;             // [2][7] their lengths, two sets used alternately
     uint32_t* best_bits[2] = {nullptr, nullptr};   // [n][Bp/32]
     // retirement of restarts at a fixed point (afs_retire.cuh)
     afs::RunState* rs = nullptr;

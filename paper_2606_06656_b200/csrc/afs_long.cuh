@@ -322,7 +322,8 @@ __device__ __forceinline__ real long_forward_tiny(const LongCon& lc, const int L
 // Output of both: boundary literals get ONE pair (dFE/dy at y = +1, at y = -1) per (constraint, restart) in
 // bnd[c][b][2]; the variable pass picks by its own x (a variable on +-1 is a boundary literal in every constraint it
 // occurs in).  Interior literals get their own scratch rows, as in the other materialising classes.
-constexpr int LONG_CLASSES = 4;
+constexpr int LONG_CLASSES = 7;        // 0..3: one warp per entry, rows 1 / 3 / 5 / 9; 4..6: one LANE per entry (k_long_lane)
+__host__ __device__ constexpr int long_lane_cap(int cls) { return cls == 4 ? 8 : cls == 5 ? 16 : 32; }   // interior literals
 __host__ __device__ constexpr int long_class_rows(int cls) { return cls == 0 ? 1 : cls == 1 ? 3 : cls == 2 ? 5 : 9; }
 // largest Leff of a class: its rows hold cells 0 .. 128 rows - 1, the padded list may run 6 entries beyond Leff
 __host__ __device__ constexpr int long_class_maxleff(int cls) { return 128 * long_class_rows(cls) - 8; }
@@ -390,7 +391,8 @@ __global__ void __launch_bounds__(128) k_long_scan(const LongCon* __restrict__ c
         o[1] = (tA == -1 ? wA : real(0)) + (tB == -1 ? wB : real(0));
         if (fe_out) fe_out[(size_t)c * Bp + b] = long_pred(lc.type, L, lc.k, nB0) ? real(-1) : real(1);
     }
-    const int cls = Leff == 0 ? -1 : Leff <= long_class_maxleff(0) ? 0 : Leff <= long_class_maxleff(1) ? 1
+    const int cls = Leff == 0 ? -1 : Leff <= long_lane_cap(4) ? 4 : Leff <= long_lane_cap(5) ? 5 : Leff <= long_lane_cap(6) ? 6
+                  : Leff <= long_class_maxleff(0) ? 0 : Leff <= long_class_maxleff(1) ? 1
                   : Leff <= long_class_maxleff(2) ? 2 : 3;
     const unsigned lt = (1u << lane) - 1u;
 #pragma unroll
@@ -546,6 +548,145 @@ __global__ void __launch_bounds__(WPC * 32) k_long_items(const LongCon* __restri
                 const real g = Rc[e];
                 // rows of the LONG class are tile-major, [tile][row][32]: the rows of one variable are consecutive, so the
                 // variable-side pass (k_glong) streams them instead of touching one 128-byte piece per 8 KB
+                lrows[((size_t)(b >> 5) * nl + (size_t)(sw[j] - row0)) * 32 + (b & 31)] = (lw[j] >> 31) ? -g : g;
+            }
+        }
+        __syncwarp();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// k_long_lane: work-list entries with few interior literals (classes 4, 5), one LANE per entry -- any 32 entries of the
+// list share a warp, each lane with its own constraint, restart and lists (lane-private columns of shared memory).  The
+// loops run to the warp's maximum with per-lane predicates; which entries share a warp enters no result.
+//   pmf     q_t <- q_t u + q_{t-1} p over the entry's interior literals in literal order (u = (1+y)/2, p = (1-y)/2),
+//   chains  leave-one-out in the stable direction, divisor max(u, p) >= 1/2 (as cm_body_small),
+// boundary literals are exact shifts: one pair per (constraint, restart).  Columns: [0, cap] pmf | cap y | cap g | cap j.
+// ---------------------------------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void __launch_bounds__(256) k_long_lane(const LongCon* __restrict__ cons, const uint32_t* __restrict__ lits,
+                                                   const int32_t* __restrict__ slots, const real* __restrict__ XT, int Bp,
+                                                   real* __restrict__ lrows, int row0, int nl, real* __restrict__ bnd,
+                                                   real* __restrict__ fe_out, const uint4* __restrict__ items,
+                                                   const int* __restrict__ count, int cap,
+                                                   const int32_t* __restrict__ goff, const uint32_t* __restrict__ MI,
+                                                   const uint32_t* __restrict__ MT)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
+    const real half = real(0.5), one = real(1), zero = real(0);
+    const size_t per_warp = (size_t)(3 * cap + 1) * 32 * sizeof(real) + (size_t)cap * 32 * sizeof(uint16_t);
+    real* q = reinterpret_cast<real*>(smem_raw + warp * per_warp) + lane;    // q[t * 32]
+    real* yl = q + (cap + 1) * 32;
+    real* gl = yl + cap * 32;
+    uint16_t* jl = reinterpret_cast<uint16_t*>(gl - lane + cap * 32) + lane;
+    const int n_items = *count;
+#pragma unroll 1
+    for (int it0 = (blockIdx.x * wpc + warp) * 32; it0 < n_items; it0 += gridDim.x * wpc * 32) {
+        const bool have = it0 + lane < n_items;
+        const uint4 ent = have ? items[it0 + lane] : make_uint4(0u, 0u, 0u, 0u);
+        const int c = (int)ent.x, b = (int)ent.y;
+        const int nB0 = (int)(ent.z & 0xffffu), nI = have ? (int)(ent.z >> 16) + (int)ent.w : 0;
+        const LongCon lc = cons[c];
+        const int L = have ? lc.L : 0;
+        const uint32_t* lw = lits + lc.off;
+        const int32_t* sw = slots + lc.off;
+        // ---- interior literal indices, in literal order, from the entry's masks
+        {
+            const int ngr = (L + 31) >> 5, ngr_max = __reduce_max_sync(FULL, ngr);
+            const size_t mrow = (size_t)goff[c] * Bp + b;
+            int pos = 0;
+            for (int g = 0; g < ngr_max; ++g) {
+                uint32_t mi = g < ngr ? MI[mrow + (size_t)g * Bp] : 0u;
+                while (__any_sync(FULL, mi != 0u)) {
+                    if (mi) { jl[pos * 32] = (uint16_t)(g * 32 + __ffs(mi) - 1); ++pos; mi &= mi - 1; }
+                }
+            }
+        }
+        const int maxI = __reduce_max_sync(FULL, nI);
+        // ---- their values (two dependent loads each, independent across the loop)
+#pragma unroll 4
+        for (int e = 0; e < maxI; ++e) {
+            if (e < nI) {
+                const uint32_t w = lw[jl[e * 32]];
+                const real x = XT[(size_t)(w & LIT_VAR) * Bp + b];
+                yl[e * 32] = (w >> 31) ? -x : x;
+            }
+        }
+        // ---- forward pmf; lanes with fewer literals append neutral factors (u = 1, p = 0: exact)
+        q[0] = one;
+        for (int t = 1; t <= maxI; ++t) q[t * 32] = zero;
+        for (int e = 0; e < maxI; ++e) {
+            const real y = e < nI ? yl[e * 32] : one;
+            const real u = fma(half, y, half), p = fma(-half, y, half);
+            real hi = zero;
+            for (int t = e + 1; t >= 1; --t) {
+                const real lo = q[(t - 1) * 32];
+                q[t * 32] = fma(lo, p, hi * u);
+                hi = lo;
+            }
+            q[0] = hi * u;
+        }
+        if (fe_out && have) {
+            real f = zero;
+            for (int t = 0; t <= nI; ++t) {
+                const real v = q[t * 32];
+                f += long_pred(lc.type, L, lc.k, t + nB0) ? -v : v;   // sp = -1 where satisfied
+            }
+            fe_out[(size_t)c * Bp + b] = f;
+        }
+        const real wA = (real)lc.wA, wB = (real)lc.wB;   // zero where the target is unused
+        const int cA = lc.tA - nB0, cB = lc.tB - nB0;    // targets inside the reduced pmf
+        if (have) {   // boundary literals: removing a false one leaves q, removing a true one takes one shift away
+            auto qat = [&](int tau) -> real { return (tau >= 0 && tau <= nI) ? q[tau * 32] : zero; };
+            real* o = bnd + ((size_t)c * Bp + b) * 2;
+            o[0] = wA * qat(cA) + wB * qat(cB);
+            o[1] = wA * qat(cA + 1) + wB * qat(cB + 1);
+        }
+        // ---- interior literals: one chain each, in the stable direction; two literals per round (independent chains)
+        {
+            // steps a chain needs: up to the later of the two capture points (top-down chains count from nI - 1)
+            const int hiT = max(wA != zero ? cA : -1, wB != zero ? cB : -1), loT = min(wA != zero ? cA : nI, wB != zero ? cB : nI);
+            for (int e0 = 0; e0 < maxI; e0 += 2) {
+                bool has[2], fwd[2];
+                real rb[2], R[2], acc[2], vA[2], vB[2];
+                int need = 0;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    has[h] = e0 + h < nI;
+                    const real y = has[h] ? yl[(e0 + h) * 32] : one;
+                    const real u = fma(half, y, half), p = fma(-half, y, half);
+                    fwd[h] = !(y < zero);
+                    rb[h] = recip(fwd[h] ? u : p);
+                    R[h] = -((fwd[h] ? p : u) * rb[h]);
+                    acc[h] = zero; vA[h] = zero; vB[h] = zero;
+                    const int nd = has[h] ? (fwd[h] ? min(hiT, nI - 1) + 1 : min(nI - 1 - loT, nI - 1) + 1) : 0;
+                    need = max(need, nd);
+                }
+                const int steps_w = __reduce_max_sync(FULL, need);
+                for (int s = 0; s < steps_w; ++s) {
+                    const bool in = s <= nI - 1;
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const bool on = has[h] && in;
+                        const int row = fwd[h] ? s : nI - s;
+                        const real a = on ? q[row * 32] : zero;
+                        acc[h] = fma(R[h], acc[h], a);
+                        const int idx = fwd[h] ? s : nI - 1 - s;        // index of q^(-j) this step completes
+                        vA[h] = (on && idx == cA) ? acc[h] : vA[h];
+                        vB[h] = (on && idx == cB) ? acc[h] : vB[h];
+                    }
+                }
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+                    if (has[h]) gl[(e0 + h) * 32] = (wA * vA[h] + wB * vB[h]) * rb[h];
+            }
+        }
+        // ---- S5 + write-out of the interior literals' rows (tile-major rows of the class)
+        for (int e = 0; e < maxI; ++e) {
+            if (e < nI) {
+                const int j = jl[e * 32];
+                const real g = gl[e * 32];
                 lrows[((size_t)(b >> 5) * nl + (size_t)(sw[j] - row0)) * 32 + (b & 31)] = (lw[j] >> 31) ? -g : g;
             }
         }

@@ -43,6 +43,29 @@ static afs_status launch_long_items(afs_problem* P, const LongLists& wl, int set
     return AFS_OK;
 }
 
+// classes 4 / 5: one lane per entry (k_long_lane), at most `cap` interior literals
+template <typename real>
+static afs_status launch_long_lane(afs_problem* P, const LongLists& wl, int set, int cls, int cap, int wpc, int prof_cls,
+                                   const real* XT, int Bp, real* scratch, real* fe, cudaStream_t st)
+{
+    const size_t smem = (size_t)wpc * ((size_t)(3 * cap + 1) * 32 * sizeof(real) + (size_t)cap * 32 * sizeof(uint16_t));
+    auto kern = k_long_lane<real>;
+    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, wpc * 32, smem));
+    if (occ < 1) return AFS_ERR_UNSUPPORTED;
+    long long cap_blocks = ((long long)P->n_long * Bp + wpc * 32 - 1) / (wpc * 32);
+    const int grid = (int)std::min<long long>((long long)P->sm_count * occ, cap_blocks < 1 ? 1 : cap_blocks);
+    ProfSpan span(P, prof_cls, st);
+    const bool fo = P->long_folded;
+    kern<<<grid, wpc * 32, smem, st>>>(fo ? P->d_long_f : P->d_long, fo ? P->d_long_lits_f : P->d_long_lits,
+                                       fo ? P->d_long_slots_f : P->d_long_slots, XT, Bp, scratch + (size_t)P->nslots_a * Bp,
+                                       (int)P->nslots_a, (int)(P->nslots - P->nslots_a), (real*)P->ws.bnd, fe, wl.items[cls],
+                                       wl.count + set * LONG_CLASSES + cls, cap, P->d_long_goff, P->ws.long_MI, P->ws.long_MT);
+    P->last_launches++;
+    return AFS_OK;
+}
+
 template <typename real>
 afs_status launch_long_all(afs_problem* P, const real* XT, const uint32_t* Sw, const uint32_t* SATw, int Bp, real* scratch,
                            int32_t* sat, real* fe, const RunState* rs, cudaStream_t st)
@@ -71,6 +94,9 @@ afs_status launch_long_all(afs_problem* P, const real* XT, const uint32_t* Sw, c
     if (s == AFS_OK) s = launch_long_items<real, 1>(P, wl, set, XT, Sw, SATw, Bp, scratch, fe, st);
     if (s == AFS_OK) s = launch_long_items<real, 2>(P, wl, set, XT, Sw, SATw, Bp, scratch, fe, st);
     if (s == AFS_OK) s = launch_long_items<real, 3>(P, wl, set, XT, Sw, SATw, Bp, scratch, fe, st);
+    if (s == AFS_OK) s = launch_long_lane<real>(P, wl, set, 4, long_lane_cap(4), 8, 10, XT, Bp, scratch, fe, st);
+    if (s == AFS_OK) s = launch_long_lane<real>(P, wl, set, 5, long_lane_cap(5), 8, 14, XT, Bp, scratch, fe, st);
+    if (s == AFS_OK) s = launch_long_lane<real>(P, wl, set, 6, long_lane_cap(6), 4, 12, XT, Bp, scratch, fe, st);
     return s;
 }
 
