@@ -233,6 +233,8 @@ afs_status prof_work_slot(afs_problem* P, int cls, cudaStream_t st, unsigned lon
 
 extern "C" afs_status afs_profile_read(afs_problem* P, double* ms, int64_t* launches, int32_t n)
 {
+    DeviceScope dev_scope(P);
+    if (P && cudaSetDevice(P->device) != cudaSuccess) { (void)cudaGetLastError(); return AFS_ERR_CUDA; }
     if (!P || !ms || !launches || n < 0 || n > PROF_CLASSES) return AFS_ERR_INVALID_ARG;
     Profiler& pr = P->prof;
     if (pr.used > 0) CU(cudaEventSynchronize(pr.pool[pr.used - 1]));
@@ -264,6 +266,7 @@ extern "C" afs_status afs_profile_flops(afs_problem* P, double* flops, int32_t n
 extern "C" afs_status afs_pgd_run_host(afs_problem* P, float* X, int32_t B, int32_t steps, float lr, const int8_t* mask,
                                        int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
 {
+    DeviceScope dev_scope(P);
     afs_status s = enter(P, B);
     if (s != AFS_OK) return s;
     if (!X) return AFS_ERR_INVALID_ARG;
@@ -271,7 +274,7 @@ extern "C" afs_status afs_pgd_run_host(afs_problem* P, float* X, int32_t B, int3
     Workspace& w = P->ws;
     const size_t n = (size_t)P->n;
     // the core workspace first: growing it later would free these staging buffers
-    if ((s = ensure_workspace(P, ((B + 31) / 32) * 32, sizeof(float), (int64_t)steps + 1)) != AFS_OK) return s;
+    if ((s = ensure_workspace(P, ((B + 31) / 32) * 32, sizeof(float), 3)) != AFS_OK) return s;
     if (w.host_stage_B < B) {
         CU(cudaDeviceSynchronize());
         free_ptr(w.mask_dev); free_ptr(w.host_stage_X); free_ptr(w.host_stage_assign);

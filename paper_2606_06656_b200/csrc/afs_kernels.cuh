@@ -61,7 +61,8 @@ __global__ void __launch_bounds__(256) k_transpose_in(const real* __restrict__ X
         if (v < n) {
             real x = tile[tx][r];
             if (mask) {   // fixed at entry
-                const int mk = mask[(size_t)min(b, B - 1) * mask_stride + v];
+                int mk = mask[(size_t)min(b, B - 1) * mask_stride + v];
+                mk = mk > 0 ? 1 : mk < 0 ? -1 : 0;   // any positive value means fixed False (+1), any negative fixed True
                 if (mk != 0) x = (real)mk;
                 if (maskT) maskT[(size_t)v * Bp + b] = (int8_t)mk;
             }
@@ -70,7 +71,11 @@ __global__ void __launch_bounds__(256) k_transpose_in(const real* __restrict__ X
         if (Sw) {   // the 32 lanes of a warp hold one variable's tile (v is warp-uniform)
             const real xx = v < n ? tile[tx][r] : real(0);
             real xm = xx;
-            if (mask && v < n) { int mk = mask[(size_t)min(b, B - 1) * mask_stride + v]; if (mk != 0) xm = (real)mk; }
+            if (mask && v < n) {
+                int mk = mask[(size_t)min(b, B - 1) * mask_stride + v];
+                mk = mk > 0 ? 1 : mk < 0 ? -1 : 0;
+                if (mk != 0) xm = (real)mk;
+            }
             const unsigned sb = __ballot_sync(FULL, xm < real(0)), sa = __ballot_sync(FULL, xm == real(1) || xm == real(-1));
             if (tx == 0 && v < n) { Sw[(size_t)v * (Bp >> 5) + blockIdx.y] = sb; SATw[(size_t)v * (Bp >> 5) + blockIdx.y] = sa; }
         }

@@ -19,6 +19,13 @@
 namespace afs {
 
 struct RunState;
+// the caller's current device is put back when an entry point returns (PyTorch owns device and stream state)
+struct DeviceScope {
+    int prev = -1;
+    explicit DeviceScope(const afs_problem* P) { if (P && cudaGetDevice(&prev) != cudaSuccess) { (void)cudaGetLastError(); prev = -1; } }
+    ~DeviceScope() { if (prev >= 0) { cudaSetDevice(prev); (void)cudaGetLastError(); } }
+};
+
 void free_workspace(afs_problem* P);
 int prof_mark(afs_problem* P, cudaStream_t st);
 struct ProfSpan {   // brackets the launches enqueued during its lifetime

@@ -1,5 +1,5 @@
-// afs_long.cuh -- the LONG class: EK / CARD longer than 64 literals.  warp = (constraint, restart), CTA = one
-// constraint x one tile of 32 restarts.  Count basis (G10):
+// afs_long.cuh -- the LONG class: EK / CARD longer than 64 literals (nothing else is ever sorted into it).
+// Count basis (G10):
 //
 //   Q(z) = prod_j (u_j + p_j z),  u = (1+y)/2, p = (1-y)/2,  q_t = [z^t] Q = Pr[t literals true]
 //

@@ -93,6 +93,9 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
         (void)cudaGetLastError();
         return AFS_ERR_CUDA;
     }
+    int prev_device = -1;
+    if (cudaGetDevice(&prev_device) != cudaSuccess) { (void)cudaGetLastError(); prev_device = -1; }
+    struct Restore { int d; ~Restore() { if (d >= 0) { cudaSetDevice(d); (void)cudaGetLastError(); } } } restore{prev_device};
     CUDA_TRY(cudaSetDevice(device));
 
     afs_problem* P = new (std::nothrow) afs_problem();
@@ -126,6 +129,11 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
                 for (int64_t e = row_ptr[c]; e < row_ptr[c + 1]; ++e) (is_long_cls(c) ? lslot_ptr : slot_ptr)[std::abs(lits[e])]++;
         for (int v = 0; v < n; ++v) { slot_ptr[v + 1] += slot_ptr[v]; lslot_ptr[v + 1] += lslot_ptr[v]; }
         const int64_t nslots_a = slot_ptr[n];
+        {   // slot ids, class offsets and run counts are 32-bit inside the kernels
+            int64_t nonpull = 0;
+            for (int c = 0; c < m; ++c) if (cls[c] != C_PULL) nonpull += row_ptr[c + 1] - row_ptr[c];
+            if (nonpull > 0x7fffff00LL) { delete P; return AFS_ERR_UNSUPPORTED; }
+        }
         P->nslots = nslots_a + lslot_ptr[n];
         P->nslots_a = nslots_a;
         std::vector<int32_t> fill(slot_ptr.begin(), slot_ptr.end() - 1), lfill(lslot_ptr.begin(), lslot_ptr.end() - 1);
@@ -177,6 +185,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
                 size_t e = i;
                 while (e < ov.size() && ov[e].key == ov[i].key) ++e;
                 int kind = ov[i].key / 8, nother = ov[i].key % 8;
+                if (e - i > 0x07ffffffu) { delete P; return AFS_ERR_UNSUPPORTED; }   // 27-bit run count
                 runs.push_back(((uint32_t)kind << 30) | ((uint32_t)nother << 27) | (uint32_t)(e - i));
                 for (; i < e; ++i) {
                     int c = ov[i].c, j = ov[i].j;
@@ -406,6 +415,8 @@ namespace afs { void free_workspace(afs_problem* p); }
 extern "C" void afs_problem_destroy(afs_problem* p)
 {
     if (!p) return;
+    int prev_device = -1;
+    if (cudaGetDevice(&prev_device) != cudaSuccess) { (void)cudaGetLastError(); prev_device = -1; }
     cudaSetDevice(p->device);
     cudaDeviceSynchronize();
     cudaFree(p->d_pull_ptr); cudaFree(p->d_pull_words); cudaFree(p->d_slot_ptr); cudaFree(p->d_lslot_info); cudaFree(p->d_lslot_ptr);
@@ -428,6 +439,7 @@ extern "C" void afs_problem_destroy(afs_problem* p)
     cudaFree(p->prof.d_work);
     (void)cudaGetLastError();
     delete p;
+    if (prev_device >= 0) { cudaSetDevice(prev_device); (void)cudaGetLastError(); }
 }
 
 extern "C" int64_t afs_problem_info(const afs_problem* p, int32_t what)

@@ -13,7 +13,7 @@
 //     and read by others after a
 //     cluster barrier (release / acquire at cluster scope); there is no grid-wide synchronisation and no host
 //     round trip,
-//   * the satisfied counts of iterate t are integer atomics on sat_hist[t][b]; cluster rank 0 keeps the best
+//   * the satisfied counts of iterate t are integer atomics on sat_hist[t mod 3][b]; cluster rank 0 keeps the best
 //     count, its step and its sign bits in shared memory.
 // One iteration:  P1 push gradients + counts | P2 pull gradients of the own variables -> G
 //                 -- cluster barrier --  best-so-far merge of iterate t (rank 0) | P3 S6 + S7 + S8 for the own
@@ -77,7 +77,7 @@ struct ResArgs {
     real* aux0;                  // [ntile][med_nnz][32] prefix states of the MED bodies
     real* aux1;
     int64_t med_nnz;
-    int32_t* sat_hist;           // [steps+1][Bp], zeroed
+    int32_t* sat_hist;           // [3][Bp] ring of count rows (row t mod 3), zeroed at launch
     uint32_t* best_bits;         // [n][ntile]
     int32_t* best_sat;           // [Bp]
     int32_t* best_step;          // [Bp]
@@ -262,13 +262,14 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
                     }
                 }
             }
-            if (satcnt) atomicAdd(a.sat_hist + (size_t)t * a.Bp + b, satcnt);
+            if (satcnt) atomicAdd(a.sat_hist + (size_t)(t % 3) * a.Bp + b, satcnt);
         }
         cluster.sync();
         if (tid == 0) { s_ctr = 0; s_ctr_cm = 0; }
         // ---- S10: iterate t against the best so far (rank 0 holds the record of the tile)
         if (rank == 0) {
-            const int sp = __ldcg(a.sat_hist + (size_t)t * a.Bp + b);
+            const int sp = __ldcg(a.sat_hist + (size_t)(t % 3) * a.Bp + b);
+            if (warp == 1) a.sat_hist[(size_t)((t + 1) % 3) * a.Bp + b] = 0;   // the row of the next iterate (ring of three)
             const bool imp = sp > s_best_sat[lane];
             const unsigned impmask = __ballot_sync(FULL, imp);
             if (impmask)
@@ -334,7 +335,7 @@ __global__ void __launch_bounds__(RES_WARPS * 32, 1) k_resident(const ResArgs<re
         cluster.sync();
         // ---- P4: the record of iterate t, then X_{t+1} and its sign words
         if (rank == 0 && warp == 0) {
-            const int sp = __ldcg(a.sat_hist + (size_t)t * a.Bp + b);
+            const int sp = __ldcg(a.sat_hist + (size_t)(t % 3) * a.Bp + b);
             if (sp > s_best_sat[lane]) { s_best_sat[lane] = sp; s_best_step[lane] = t; }
         }
 #pragma unroll 8
@@ -367,7 +368,7 @@ __global__ void __launch_bounds__(256) k_res_in(const real* __restrict__ X, real
         int v = v0 + r, b = b0 + tx;
         if (v < n) {
             real x = tile[tx][r];
-            if (mask) { int mk = mask[v]; if (mk != 0) x = (real)mk; }
+            if (mask) { int mk = mask[v]; if (mk != 0) x = mk > 0 ? real(1) : real(-1); }
             XT[((size_t)blockIdx.y * n + v) * 32 + tx] = x;
         }
     }

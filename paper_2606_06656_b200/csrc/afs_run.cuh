@@ -105,6 +105,7 @@ static afs_status launch_count(afs_problem* P, const real* XT, int Bp, int32_t* 
 template <typename real>
 static afs_status eval_grad_impl(afs_problem* P, const real* X, int32_t B, real* F, real* G, void* stream)
 {
+    DeviceScope dev_scope(P);
     afs_status s = enter(P, B);
     if (s != AFS_OK) return s;
     if (!X) return AFS_ERR_INVALID_ARG;
@@ -152,6 +153,7 @@ static afs_status eval_grad_impl(afs_problem* P, const real* X, int32_t B, real*
 template <typename real>
 static afs_status round_count_impl(afs_problem* P, const real* X, int32_t B, int8_t* assign, int32_t* sat, void* stream)
 {
+    DeviceScope dev_scope(P);
     afs_status s = enter(P, B);
     if (s != AFS_OK) return s;
     if (!X || !sat) return AFS_ERR_INVALID_ARG;
@@ -229,7 +231,7 @@ static afs_status pgd_run_resident(afs_problem* P, int pi, real* X, int32_t B, i
     real* XT = (real*)w.XT[0];
     dim3 tg((P->n + 31) / 32, ntile);
     k_res_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, mask);
-    CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)(steps + 1) * Bp * sizeof(int32_t), st));
+    CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)3 * Bp * sizeof(int32_t), st));
     ResArgs<real> a{};
     a.n = P->n; a.steps = steps; a.C = rp.C; a.Bp = Bp; a.ntile = ntile; a.nslots = P->nslots;
     const ResLayout lay = resident_layout<real>(P, pi);
@@ -278,6 +280,7 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
                                int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream,
                                real tol = real(0), int32_t* conv_step = nullptr, bool per_restart_masks = false)
 {
+    DeviceScope dev_scope(P);
     afs_status s = enter(P, B);
     if (s != AFS_OK) return s;
     if (!X || steps < 0 || !std::isfinite((double)lr)) return AFS_ERR_INVALID_ARG;
@@ -287,8 +290,8 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     const int plan = (P->opt_mode == 1 || tol > real(0) || per_restart_masks) ? -1 : resident_plan<real>(P, Bp / 32);
     if (per_restart_masks && !mask) return AFS_ERR_INVALID_ARG;
     if (P->opt_mode == 2 && plan < 0) return AFS_ERR_UNSUPPORTED;
-    // count rows: the resident kernel keeps one per iterate, the streaming path a ring of three
-    if ((s = ensure_workspace(P, Bp, sizeof(real), plan >= 0 ? (int64_t)steps + 1 : 3)) != AFS_OK) return s;
+    // count rows: a ring of three on both paths (memory does not grow with the number of steps)
+    if ((s = ensure_workspace(P, Bp, sizeof(real), 3)) != AFS_OK) return s;
     Workspace& w = P->ws;
     if (per_restart_masks && w.maskT_elems < (int64_t)P->n * w.Bp) {
         CU(cudaDeviceSynchronize());
