@@ -527,3 +527,112 @@ int orc_pgd_run_conv(int n, int64_t m, const int64_t *row_ptr, const int32_t *li
     }
     return err;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Per-constraint weights ("adaptive constraint weighting -- informed by per-constraint gradient
+ * magnitudes"; L188 (i); reading G25).  eq. (5) with weights:  F_w(X) = sum_k w_k FE_{C_k}(X), hence
+ * dF_w/dx_v = sum_k w_k sigma dFE_k/dy.  New functions; the unweighted ones above are untouched.
+ *   gm (NULL or [m]) receives the per-constraint gradient magnitude summed over the batch, UNWEIGHTED:
+ *   gm[k] = sum_b sum_j |dFE_k/dy_j (X_b)|  (the l1 norm is this build's reading of "gradient magnitude").
+ * ------------------------------------------------------------------------------------------ */
+static int eval_one_w(int n, int64_t m, const int64_t *row_ptr, const int32_t *lits,
+                      const int32_t *types, const int32_t *k, const double *w, const double *x,
+                      double *F, double *g /* n or NULL */, double *gm /* m or NULL */, int evaluator,
+                      double *ybuf, double *gbuf)
+{
+    double f = 0.0;
+    if (g) for (int v = 0; v < n; ++v) g[v] = 0.0;
+    for (int64_t c = 0; c < m; ++c) {
+        int L = (int)(row_ptr[c + 1] - row_ptr[c]);
+        const int32_t *lc = lits + row_ptr[c];
+        for (int j = 0; j < L; ++j) {
+            int v = abs(lc[j]) - 1;
+            ybuf[j] = lc[j] > 0 ? x[v] : -x[v];
+        }
+        double fe;
+        int need_g = (g != NULL) || (gm != NULL);
+        int rc = evaluator == 0 ? orc_fe_A(types[c], L, k[c], ybuf, &fe, need_g ? gbuf : NULL)
+                                : orc_fe_B(types[c], L, k[c], ybuf, &fe, need_g ? gbuf : NULL, evaluator);
+        if (rc) return rc;
+        const double wc = w ? w[c] : 1.0;
+        f += wc * fe;
+        if (g) for (int j = 0; j < L; ++j) {
+            int v = abs(lc[j]) - 1;
+            g[v] += wc * (lc[j] > 0 ? gbuf[j] : -gbuf[j]);
+        }
+        if (gm) {
+            double s = 0.0;
+            for (int j = 0; j < L; ++j) s += fabs(gbuf[j]);
+            gm[c] = s;
+        }
+    }
+    if (F) *F = f;
+    return 0;
+}
+
+int orc_eval_grad_w(int n, int64_t m, const int64_t *row_ptr, const int32_t *lits,
+                    const int32_t *types, const int32_t *k, const double *w, const double *X, int B,
+                    double *F, double *G, double *GM /* m or NULL, summed over the batch */, int evaluator)
+{
+    if (check_instance(n, m, row_ptr, lits, types, k)) return -1;
+    int Lmax = max_len(m, row_ptr);
+    double *ybuf = (double *)malloc((size_t)Lmax * sizeof(double));
+    double *gbuf = (double *)malloc((size_t)Lmax * sizeof(double));
+    double *gm1 = GM ? (double *)malloc((size_t)(m ? m : 1) * sizeof(double)) : NULL;
+    if (GM) for (int64_t c = 0; c < m; ++c) GM[c] = 0.0;
+    int err = 0;
+    for (int b = 0; b < B && !err; ++b) {          /* plain loop: the batch sum of GM is taken in restart order */
+        err = eval_one_w(n, m, row_ptr, lits, types, k, w, X + (size_t)b * n, F ? F + b : NULL,
+                         G ? G + (size_t)b * n : NULL, gm1, evaluator, ybuf, gbuf);
+        if (GM && !err) for (int64_t c = 0; c < m; ++c) GM[c] += gm1[c];
+    }
+    free(ybuf); free(gbuf); free(gm1);
+    return err;
+}
+
+int orc_pgd_run_w(int n, int64_t m, const int64_t *row_ptr, const int32_t *lits,
+                  const int32_t *types, const int32_t *k, const double *w, double *X, int B, int steps, double lr,
+                  const int8_t *mask, int8_t *best_assign, int32_t *best_sat, int32_t *best_step, int evaluator)
+{
+    if (check_instance(n, m, row_ptr, lits, types, k) || steps < 0) return -1;
+    int Lmax = max_len(m, row_ptr);
+    int err = 0;
+#pragma omp parallel
+    {
+        double *ybuf = (double *)malloc((size_t)Lmax * sizeof(double));
+        double *gbuf = (double *)malloc((size_t)Lmax * sizeof(double));
+        double *g = (double *)malloc((size_t)n * sizeof(double));
+        int8_t *cur = (int8_t *)malloc((size_t)n);
+#pragma omp for schedule(dynamic, 1)
+        for (int b = 0; b < B; ++b) {
+            double *x = X + (size_t)b * n;
+            if (mask) for (int v = 0; v < n; ++v) if (mask[v]) x[v] = (double)mask[v];
+            int32_t best = -1;
+            for (int t = 0; t <= steps; ++t) {
+                int32_t s = count_one(n, m, row_ptr, lits, types, k, x, cur);   /* counts do not see the weights */
+                if (s > best) {
+                    best = s;
+                    if (best_assign) memcpy(best_assign + (size_t)b * n, cur, (size_t)n);
+                    if (best_step) best_step[b] = t;
+                }
+                if (t == steps) break;
+                int rc = eval_one_w(n, m, row_ptr, lits, types, k, w, x, NULL, g, NULL, evaluator, ybuf, gbuf);
+                if (rc) {
+#pragma omp critical
+                    err = rc;
+                    break;
+                }
+                for (int v = 0; v < n; ++v) {
+                    if (mask && mask[v]) continue;
+                    double xn = x[v] - lr * g[v];
+                    if (xn > 1.0) xn = 1.0;
+                    if (xn < -1.0) xn = -1.0;
+                    x[v] = xn;
+                }
+            }
+            if (best_sat) best_sat[b] = best;
+        }
+        free(ybuf); free(gbuf); free(g); free(cur);
+    }
+    return err;
+}

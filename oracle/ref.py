@@ -34,6 +34,8 @@ def lib():
                                          f64p, i32p, C.c_int, C.c_int]
         L.orc_pgd_run_conv.argtypes = inst + [f64p, C.c_int, C.c_int, C.c_double, i8p, C.c_double, i8p, i32p, i32p,
                                               i32p, i32p, f64p, C.c_int, C.c_int]
+        L.orc_eval_grad_w.argtypes = inst + [f64p, f64p, C.c_int, f64p, f64p, f64p, C.c_int]
+        L.orc_pgd_run_w.argtypes = inst + [f64p, f64p, C.c_int, C.c_int, C.c_double, i8p, i8p, i32p, i32p, C.c_int]
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -161,3 +163,37 @@ def pgd_run_conv(inst, X0, max_steps: int, lr: float, tol: float, mask=None, eva
         raise ValueError("oracle error %d" % rc)
     return dict(X=X, best_assign=best_assign, best_sat=best_sat, best_step=best_step, conv_step=conv_step,
                 final_sat=final_sat, final_F=final_F)
+
+
+def eval_grad_w(inst, weights, X, evaluator: int = 2, want_grad: bool = True, want_gm: bool = False):
+    """Weighted objective F_w = sum_k w_k FE_k and its gradient (orc_eval_grad_w); optionally the per-constraint
+    gradient magnitudes gm[k] = sum_b sum_j |dFE_k/dy_j| (unweighted).  Returns (F, G, GM)."""
+    X = np.ascontiguousarray(X, dtype=np.float64)
+    B, n = X.shape
+    w = None if weights is None else np.ascontiguousarray(weights, dtype=np.float64)
+    F = np.zeros(B, dtype=np.float64)
+    G = np.zeros((B, n), dtype=np.float64) if want_grad else None
+    GM = np.zeros(inst.m, dtype=np.float64) if want_gm else None
+    keep, args = _inst_args(inst)
+    rc = lib().orc_eval_grad_w(*args, _p(w, C.c_double), _p(X, C.c_double), B, _p(F, C.c_double), _p(G, C.c_double),
+                               _p(GM, C.c_double), evaluator)
+    if rc:
+        raise ValueError("oracle error %d" % rc)
+    return F, G, GM
+
+
+def pgd_run_w(inst, weights, X0, steps: int, lr: float, mask=None, evaluator: int = 2):
+    """PGD on the weighted objective (orc_pgd_run_w). Returns dict(X, best_assign, best_sat, best_step)."""
+    X = np.array(X0, dtype=np.float64, order="C", copy=True)
+    B, n = X.shape
+    w = None if weights is None else np.ascontiguousarray(weights, dtype=np.float64)
+    m8 = None if mask is None else np.ascontiguousarray(mask, dtype=np.int8)
+    best_assign = np.zeros((B, n), dtype=np.int8)
+    best_sat = np.zeros(B, dtype=np.int32)
+    best_step = np.zeros(B, dtype=np.int32)
+    keep, args = _inst_args(inst)
+    rc = lib().orc_pgd_run_w(*args, _p(w, C.c_double), _p(X, C.c_double), B, int(steps), float(lr), _p(m8, C.c_int8),
+                             _p(best_assign, C.c_int8), _p(best_sat, C.c_int32), _p(best_step, C.c_int32), evaluator)
+    if rc:
+        raise ValueError("oracle error %d" % rc)
+    return dict(X=X, best_assign=best_assign, best_sat=best_sat, best_step=best_step)
