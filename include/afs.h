@@ -83,6 +83,18 @@ typedef enum {
 AFS_API afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const int64_t* row_ptr, const int32_t* lits,
                               const int32_t* types, const int32_t* k, int32_t device, afs_problem** out);
 
+/*
+ * afs_problem_create_w -- afs_problem_create with per-constraint weights w_k of eq. (5):
+ * F_w(X) = sum_k w_k FE_{C_k}(X)  ("adaptive constraint weighting", P:L188 (i); reading G25).  weights: host
+ * float[n_cons], finite (NULL = all 1).  Objective and gradient of afs_eval_grad* / afs_pgd_run* carry the weights;
+ * rounding and satisfied counts do not.  A duplicated constraint equals weight 2.  Re-weighting means
+ * creating a new handle (S0 is host-side and untimed).  Short clauses with w != 1 are evaluated by the
+ * materialising kernels instead of the pull formulation.
+ */
+AFS_API afs_status afs_problem_create_w(int32_t n_vars, int32_t n_cons, const int64_t* row_ptr, const int32_t* lits,
+                                        const int32_t* types, const int32_t* k, const float* weights, int32_t device,
+                                        afs_problem** out);
+
 /* Frees the handle, its device tables and workspace.  NULL is a no-op.  Synchronises the device. */
 AFS_API void afs_problem_destroy(afs_problem* p);
 

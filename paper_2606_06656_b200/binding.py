@@ -21,7 +21,7 @@ EXPORTS = (
     "afs_problem_create", "afs_problem_destroy", "afs_coeffs", "afs_eval_grad", "afs_eval_grad_f64",
     "afs_round_count", "afs_round_count_f64", "afs_pgd_run", "afs_pgd_run_f64", "afs_pgd_run_host",
     "afs_problem_info", "afs_set_option", "afs_status_string", "afs_abi_version", "afs_last_error_message",
-    "afs_profile_read", "afs_profile_flops", "afs_fp32_fma_peak", "afs_pgd_run_conv", "afs_pgd_run_conv_f64", "afs_pgd_run_masks", "afs_pgd_run_masks_f64",
+    "afs_profile_read", "afs_profile_flops", "afs_fp32_fma_peak", "afs_pgd_run_conv", "afs_pgd_run_conv_f64", "afs_pgd_run_masks", "afs_pgd_run_masks_f64", "afs_problem_create_w",
 )
 
 _lib = None
@@ -48,6 +48,8 @@ def lib():
     vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
     L.afs_problem_create.argtypes = [i32, i32, vp, vp, vp, vp, i32, C.POINTER(vp)]
     L.afs_problem_create.restype = C.c_int
+    L.afs_problem_create_w.argtypes = [i32, i32, vp, vp, vp, vp, vp, i32, C.POINTER(vp)]
+    L.afs_problem_create_w.restype = C.c_int
     L.afs_problem_destroy.argtypes = [vp]
     L.afs_problem_destroy.restype = None
     L.afs_coeffs.argtypes = [i32, i32, i32, vp]
@@ -123,7 +125,7 @@ class Problem:
     INFO = {"n_vars": 0, "n_cons": 1, "nnz": 2, "n_pull": 3, "n_med": 4, "n_long": 5, "scratch_slots": 6,
             "launches": 7, "workspace_bytes": 8, "resident": 9}
 
-    def __init__(self, n_vars: int, row_ptr, lits, types, k, device: int = 0):
+    def __init__(self, n_vars: int, row_ptr, lits, types, k, device: int = 0, weights=None):
         self._h = C.c_void_p(None)
         rp = np.ascontiguousarray(row_ptr, dtype=np.int64)
         li = np.ascontiguousarray(lits, dtype=np.int32)
@@ -136,13 +138,20 @@ class Problem:
         self.n, self.m, self.nnz = int(n_vars), int(ty.shape[0]), int(li.shape[0])
         self.device = int(device)
         h = C.c_void_p(None)
-        _chk(lib().afs_problem_create(self.n, self.m, rp.ctypes.data, li.ctypes.data, ty.ctypes.data,
-                                      kk.ctypes.data, self.device, C.byref(h)), "afs_problem_create")
+        if weights is None:
+            _chk(lib().afs_problem_create(self.n, self.m, rp.ctypes.data, li.ctypes.data, ty.ctypes.data,
+                                          kk.ctypes.data, self.device, C.byref(h)), "afs_problem_create")
+        else:
+            ww = np.ascontiguousarray(weights, dtype=np.float32)
+            if ww.shape != ty.shape:
+                raise ValueError("weights must have one entry per constraint")
+            _chk(lib().afs_problem_create_w(self.n, self.m, rp.ctypes.data, li.ctypes.data, ty.ctypes.data,
+                                            kk.ctypes.data, ww.ctypes.data, self.device, C.byref(h)), "afs_problem_create_w")
         self._h = h
 
     @classmethod
-    def from_instance(cls, inst, device: int = 0) -> "Problem":
-        return cls(inst.n, inst.row_ptr, inst.lits, inst.types, inst.k, device)
+    def from_instance(cls, inst, device: int = 0, weights=None) -> "Problem":
+        return cls(inst.n, inst.row_ptr, inst.lits, inst.types, inst.k, device, weights=weights)
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

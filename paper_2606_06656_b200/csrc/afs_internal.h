@@ -41,20 +41,22 @@ constexpr int MAX_VARS = 1 << 24;
 constexpr int CM_BUCKETS = 4;        // EK / CARD with L <= 64, ordered by length class 16, 32, 48, 64
 constexpr int CM_MAX_LEN = 64;
 
-struct MedCon {        // 16 bytes
+struct MedCon {        // 20 bytes
     int32_t off;       // first literal in med_lits / med_slots
     int32_t L;
     int32_t type;
     int32_t k;
+    float w;           // weight w_k of the constraint in eq. (5) (1 unless created with weights)
 };
 
-struct LongCon {       // 32 bytes
+struct LongCon {       // 36 bytes
     int32_t off;       // first literal in long_lits / long_slots
     int32_t L;
     int32_t type;
     int32_t k;
     int32_t tA, tB;    // leave-one-out pmf indices entering the gradient (true-count index, 0..L-1)
     float wA, wB;      // their weights d_t in {-1, 0, +1}
+    float w;           // weight w_k of the constraint in eq. (5)
 };
 
 struct PullClause {    // one PULL-class clause packed for the bit-parallel count: header + its <= 5 literal words, 32 bytes

@@ -233,7 +233,7 @@ __device__ __forceinline__ void cm_body(const LongCon& lc, const uint32_t* __res
             const real v = q[t * 32];
             f += (lc.type == AFS_CARD ? t >= lc.k : t == lc.k) ? -v : v;   // sp_t = -1 where satisfied
         }
-        if (commit) fe = f;
+        if (commit) fe = mul_rn(f, (real)lc.w);
     } else if (commit) {
         fe = zero;
     }
@@ -310,7 +310,7 @@ __device__ __forceinline__ void cm_body(const LongCon& lc, const uint32_t* __res
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             if (j0 + h < L) {
-                const real g = mul_rn(fma(w1[h], v1[h], mul_rn(w2[h], v2[h])), rb[h]);
+                const real g = mul_rn(mul_rn(fma(w1[h], v1[h], mul_rn(w2[h], v2[h])), rb[h]), (real)lc.w);
                 if (commit) sc.put(sw[j0 + h], ng[h] ? -g : g);
             }
         }
@@ -372,7 +372,7 @@ __device__ __forceinline__ unsigned cm_body_small(const LongCon& lc, const uint3
             const real v = q[t * 32];
             f += (lc.type == AFS_CARD ? t + nB0 >= lc.k : t + nB0 == lc.k) ? -v : v;   // sp = -1 where satisfied
         }
-        if (mine) fe = f;
+        if (mine) fe = mul_rn(f, (real)lc.w);
     } else if (mine) {
         fe = zero;
     }
@@ -417,6 +417,7 @@ __device__ __forceinline__ unsigned cm_body_small(const LongCon& lc, const uint3
         if (y == one) g = gA0;
         else if (y == -one) g = gB0;
         else { g = gl[min(e, cap - 1) * 32]; ++e; }
+        g = mul_rn(g, (real)lc.w);
         if (mine) sc.put(sw[j], neg ? -g : g);
     }
     return served;
@@ -444,6 +445,7 @@ __device__ __forceinline__ void med_body(const MedCon& mc, const uint32_t* __res
     const real half = real(0.5), one = real(1), zero = real(0);
     const int L = mc.L, row0 = mc.off;
     const int type = mc.type;
+    const real wk = (real)mc.w;   // eq. (5) weight; 1 unless the problem was created with weights (x * 1 is exact)
     int t = 0;
     if (type == AFS_OR || type == AFS_XOR) {
         const bool is_or = type == AFS_OR;
@@ -468,7 +470,7 @@ __device__ __forceinline__ void med_body(const MedCon& mc, const uint32_t* __res
             const bool neg = (w >> 31) != 0;
             const real y = neg ? -x : x;
             const real g = mul_rn(ax0.get(row0 + j), suf);
-            sw.put(sc[j], neg ? -g : g);
+            sw.put(sc[j], mul_rn(neg ? -g : g, wk));
             suf = mul_rn(suf, is_or ? fma(half, y, half) : y);
         }
     } else if (type == AFS_NAE) {
@@ -494,7 +496,7 @@ __device__ __forceinline__ void med_body(const MedCon& mc, const uint32_t* __res
             const bool neg = (w >> 31) != 0;
             const real y = neg ? -x : x;
             const real g = fma(ax0.get(row0 + j), su, -mul_rn(ax1.get(row0 + j), sp));
-            sw.put(sc[j], neg ? -g : g);
+            sw.put(sc[j], mul_rn(neg ? -g : g, wk));
             su = mul_rn(su, fma(half, y, half));
             sp = mul_rn(sp, fma(-half, y, half));
         }
@@ -527,12 +529,13 @@ __device__ __forceinline__ void med_body(const MedCon& mc, const uint32_t* __res
             const real q0 = mul_rn(P0, s0);
             const real q1 = fma(P1, s0, mul_rn(P0, s1));
             const real g = is_eo ? q0 - q1 : -q1;
-            sw.put(sc[j], neg ? -g : g);
+            sw.put(sc[j], mul_rn(neg ? -g : g, wk));
             s1 = fma(s1, u, mul_rn(s0, p));
             s0 = mul_rn(s0, u);
         }
     }
     satcnt += pred(type, L, mc.k, t) ? 1 : 0;
+    fe = mul_rn(fe, wk);
 }
 
 template <typename real>

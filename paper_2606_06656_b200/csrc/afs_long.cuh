@@ -385,11 +385,11 @@ __global__ void __launch_bounds__(128) k_long_scan(const LongCon* __restrict__ c
     if (Leff == 0) {
         // removing a false literal leaves the point mass at nB0, removing a true one moves it to nB0 - 1
         const int tA = lc.tA - nB0, tB = lc.tB - nB0;
-        const real wA = (real)lc.wA, wB = (real)lc.wB;
+        const real wA = (real)lc.wA * (real)lc.w, wB = (real)lc.wB * (real)lc.w;   // d_t times the constraint's weight
         real* o = bnd + ((size_t)c * Bp + b) * 2;
         o[0] = (tA == 0 ? wA : real(0)) + (tB == 0 ? wB : real(0));
         o[1] = (tA == -1 ? wA : real(0)) + (tB == -1 ? wB : real(0));
-        if (fe_out) fe_out[(size_t)c * Bp + b] = long_pred(lc.type, L, lc.k, nB0) ? real(-1) : real(1);
+        if (fe_out) fe_out[(size_t)c * Bp + b] = long_pred(lc.type, L, lc.k, nB0) ? -(real)lc.w : (real)lc.w;
     }
     const int cls = Leff == 0 ? -1 : Leff <= long_lane_cap(4) ? 4 : Leff <= long_lane_cap(5) ? 5 : Leff <= long_lane_cap(6) ? 6
                   : Leff <= long_class_maxleff(0) ? 0 : Leff <= long_class_maxleff(1) ? 1
@@ -497,7 +497,7 @@ __global__ void __launch_bounds__(WPC * 32) k_long_items(const LongCon* __restri
             if (fe_out) {
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) fe += __shfl_xor_sync(FULLM, fe, o);
-                if (lane == 0) fe_out[(size_t)c * Bp + b] = fe;
+                if (lane == 0) fe_out[(size_t)c * Bp + b] = fe * (real)lc.w;
             }
         }
         __syncwarp();
@@ -505,7 +505,7 @@ __global__ void __launch_bounds__(WPC * 32) k_long_items(const LongCon* __restri
         const bool useA = lc.wA != 0.f, useB = lc.wB != 0.f;
         // capture points in true-count index space, t1 <= t2 (equal if only one is used)
         int t1 = lc.tA, t2 = lc.tB;
-        real w1 = (real)lc.wA, w2 = (real)lc.wB;
+        real w1 = (real)lc.wA * (real)lc.w, w2 = (real)lc.wB * (real)lc.w;   // d_t times the constraint's weight
         if (!useA) { t1 = t2; w1 = real(0); }
         if (!useB) { t2 = t1; w2 = w1; w1 = real(0); }
         if (t1 > t2) { int tt = t1; t1 = t2; t2 = tt; real ww = w1; w1 = w2; w2 = ww; }
@@ -633,9 +633,9 @@ __global__ void __launch_bounds__(256) k_long_lane(const LongCon* __restrict__ c
                 const real v = q[t * 32];
                 f += long_pred(lc.type, L, lc.k, t + nB0) ? -v : v;   // sp = -1 where satisfied
             }
-            fe_out[(size_t)c * Bp + b] = f;
+            fe_out[(size_t)c * Bp + b] = f * (real)lc.w;
         }
-        const real wA = (real)lc.wA, wB = (real)lc.wB;   // zero where the target is unused
+        const real wA = (real)lc.wA * (real)lc.w, wB = (real)lc.wB * (real)lc.w;   // zero where the target is unused
         const int cA = lc.tA - nB0, cB = lc.tB - nB0;    // targets inside the reduced pmf
         if (have) {   // boundary literals: removing a false one leaves q, removing a true one takes one shift away
             auto qat = [&](int tau) -> real { return (tau >= 0 && tau <= nI) ? q[tau * 32] : zero; };

@@ -57,8 +57,27 @@ static void long_targets(int type, int L, int k, LongCon& c)
     }
 }
 
+static afs_status create_impl(int32_t n_vars, int32_t n_cons, const int64_t* row_ptr, const int32_t* lits,
+                              const int32_t* types, const int32_t* k, const float* weights, int32_t device,
+                              afs_problem** out);
+
 extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const int64_t* row_ptr, const int32_t* lits,
                                          const int32_t* types, const int32_t* k, int32_t device, afs_problem** out)
+{ return create_impl(n_vars, n_cons, row_ptr, lits, types, k, nullptr, device, out); }
+
+extern "C" afs_status afs_problem_create_w(int32_t n_vars, int32_t n_cons, const int64_t* row_ptr, const int32_t* lits,
+                                           const int32_t* types, const int32_t* k, const float* weights, int32_t device,
+                                           afs_problem** out)
+{
+    if (weights)
+        for (int c = 0; c < n_cons; ++c)
+            if (!std::isfinite(weights[c])) { if (out) *out = nullptr; return AFS_ERR_INVALID_ARG; }
+    return create_impl(n_vars, n_cons, row_ptr, lits, types, k, weights, device, out);
+}
+
+static afs_status create_impl(int32_t n_vars, int32_t n_cons, const int64_t* row_ptr, const int32_t* lits,
+                              const int32_t* types, const int32_t* k, const float* weights, int32_t device,
+                              afs_problem** out)
 {
     if (!out) return AFS_ERR_INVALID_ARG;
     *out = nullptr;
@@ -112,7 +131,9 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
             int L = (int)(row_ptr[c + 1] - row_ptr[c]);
             int ty = types[c];
             bool prod = (ty == AFS_OR || ty == AFS_XOR);
-            if ((prod || ty == AFS_NAE) && L <= PULL_MAX_LEN) cls[c] = C_PULL;
+            // a weighted short clause is materialised like any other constraint: the pull streams stay weight-free
+            const bool unit_w = !weights || weights[c] == 1.0f;
+            if ((prod || ty == AFS_NAE) && L <= PULL_MAX_LEN && unit_w) cls[c] = C_PULL;
             else if (prod || ty == AFS_NAE || ty == AFS_EO || ty == AFS_AMO) cls[c] = C_MED;   // any length
             else if ((ty == AFS_EK || ty == AFS_CARD) && L <= CM_MAX_LEN) cls[c] = C_CMED;
             else cls[c] = C_LONG;
@@ -224,7 +245,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
                 MedCon mc;
                 int64_t L = row_ptr[c + 1] - row_ptr[c];
                 mc.off = (int32_t)med_lits.size(); mc.L = (int32_t)L;
-                mc.type = types[c]; mc.k = k[c];
+                mc.type = types[c]; mc.k = k[c]; mc.w = weights ? weights[c] : 1.0f;
                 if (types[c] != AFS_OR && types[c] != AFS_XOR) P->med_two = true;
                 for (int64_t e = row_ptr[c]; e < row_ptr[c + 1]; ++e) {
                     med_lits.push_back(lit_word(lits[e]));
@@ -256,7 +277,7 @@ extern "C" afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const i
                 while (cur < bk) begin[++cur] = (int32_t)i;
                 LongCon lc;
                 lc.off = (int32_t)olits.size(); lc.L = (int32_t)(row_ptr[c + 1] - row_ptr[c]);
-                lc.type = types[c]; lc.k = k[c];
+                lc.type = types[c]; lc.k = k[c]; lc.w = weights ? weights[c] : 1.0f;
                 long_targets(lc.type, lc.L, lc.k, lc);
                 if (maxL) maxL[bk] = std::max(maxL[bk], lc.L);
                 for (int64_t e = row_ptr[c]; e < row_ptr[c + 1]; ++e) {
