@@ -117,6 +117,17 @@ AFS_API afs_status afs_eval_grad(afs_problem* p, const float* X, int32_t B, floa
 AFS_API afs_status afs_eval_grad_f64(afs_problem* p, const double* X, int32_t B, double* F, double* G, void* cuda_stream);
 
 /*
+ * afs_constraint_grad_l1 -- per-constraint gradient magnitudes over a batch ("adaptive constraint weighting --
+ * informed by per-constraint gradient magnitudes"; reading G25):  gm[k] = sum_b sum_j |dFE_k/dy_j (X_b)|, UNWEIGHTED
+ * (also on a handle created with weights), in the caller's constraint order.
+ *   X  device float[B,n] (read only)      gm  device float[n_cons]
+ * Fixed summation order (no float atomics).  A host loop "gm -> new weights -> afs_problem_create_w" is the adaptive
+ * weighting the paper names as future work; the library provides the two device-side pieces.
+ */
+AFS_API afs_status afs_constraint_grad_l1(afs_problem* p, const float* X, int32_t B, float* gm, void* cuda_stream);
+AFS_API afs_status afs_constraint_grad_l1_f64(afs_problem* p, const double* X, int32_t B, double* gm, void* cuda_stream);
+
+/*
  * afs_round_count -- S9: round by sign and count satisfied constraints.  x < 0 -> True (-1); x >= 0,
  * +-0.0 and NaN -> False (+1) (G13).  Integer arithmetic, bit-exact.
  *   X  device float[B,n]     assign  device int8[B,n] or NULL (-1 True, +1 False)     sat  device int32[B]

@@ -21,7 +21,7 @@ EXPORTS = (
     "afs_problem_create", "afs_problem_destroy", "afs_coeffs", "afs_eval_grad", "afs_eval_grad_f64",
     "afs_round_count", "afs_round_count_f64", "afs_pgd_run", "afs_pgd_run_f64", "afs_pgd_run_host",
     "afs_problem_info", "afs_set_option", "afs_status_string", "afs_abi_version", "afs_last_error_message",
-    "afs_profile_read", "afs_profile_flops", "afs_fp32_fma_peak", "afs_pgd_run_conv", "afs_pgd_run_conv_f64", "afs_pgd_run_masks", "afs_pgd_run_masks_f64", "afs_problem_create_w",
+    "afs_profile_read", "afs_profile_flops", "afs_fp32_fma_peak", "afs_pgd_run_conv", "afs_pgd_run_conv_f64", "afs_pgd_run_masks", "afs_pgd_run_masks_f64", "afs_problem_create_w", "afs_constraint_grad_l1", "afs_constraint_grad_l1_f64",
 )
 
 _lib = None
@@ -58,6 +58,8 @@ def lib():
         f = getattr(L, name); f.argtypes = [vp, vp, i32, vp, vp, vp]; f.restype = C.c_int
     for name in ("afs_round_count", "afs_round_count_f64"):
         f = getattr(L, name); f.argtypes = [vp, vp, i32, vp, vp, vp]; f.restype = C.c_int
+    for name in ("afs_constraint_grad_l1", "afs_constraint_grad_l1_f64"):
+        f = getattr(L, name); f.argtypes = [vp, vp, i32, vp, vp]; f.restype = C.c_int
     L.afs_pgd_run.argtypes = [vp, vp, i32, i32, C.c_float, vp, vp, vp, vp, vp]
     L.afs_pgd_run.restype = C.c_int
     L.afs_pgd_run_f64.argtypes = [vp, vp, i32, i32, C.c_double, vp, vp, vp, vp, vp]
@@ -209,6 +211,16 @@ class Problem:
         _chk(fn(self._h, X.data_ptr(), B, F.data_ptr() if want_F else None, G.data_ptr() if want_G else None,
                 _stream_ptr(X.device)), "afs_eval_grad")
         return F, G
+
+    def constraint_grad_l1(self, X):
+        """afs_constraint_grad_l1 / _f64: gm[n_cons] = sum_b sum_j |dFE_k/dy_j(X_b)| (unweighted)."""
+        torch = _torch()
+        f64 = X.dtype == torch.float64
+        self._check_X(X, torch.float64 if f64 else torch.float32)
+        gm = torch.empty(self.m, dtype=X.dtype, device=X.device)
+        fn = lib().afs_constraint_grad_l1_f64 if f64 else lib().afs_constraint_grad_l1
+        _chk(fn(self._h, X.data_ptr(), X.shape[0], gm.data_ptr(), _stream_ptr(X.device)), "afs_constraint_grad_l1")
+        return gm
 
     def round_count(self, X, want_assign: bool = True):
         """afs_round_count. Returns (assign int8[B,n] or None, sat int32[B])."""

@@ -72,7 +72,7 @@ void free_workspace(afs_problem* P)
     free_ptr(w.sat_hist); free_ptr(w.best_sat[0]); free_ptr(w.best_sat[1]);
     free_ptr(w.best_step[0]); free_ptr(w.best_step[1]); free_ptr(w.S[0]); free_ptr(w.S[1]); free_ptr(w.S[2]); free_ptr(w.SAT[0]); free_ptr(w.SAT[1]); free_ptr(w.SAT[2]);
     free_ptr(w.bnd); free_ptr(w.GL); free_ptr(w.best_bits[1]); free_ptr(w.orig[0]); free_ptr(w.orig[1]); free_ptr(w.moved);
-    free_ptr(w.rs); free_ptr(w.rt_src); free_ptr(w.rt_imp); free_ptr(w.rt_ret); free_ptr(w.rt_ret_sat); free_ptr(w.rt_ret_step); free_ptr(w.rt_ret_conv); free_ptr(w.maskT); free_ptr(w.conv[0]); free_ptr(w.conv[1]); free_ptr(w.delta);
+    free_ptr(w.rs); free_ptr(w.rt_src); free_ptr(w.rt_imp); free_ptr(w.rt_ret); free_ptr(w.rt_ret_sat); free_ptr(w.rt_ret_step); free_ptr(w.rt_ret_conv); free_ptr(w.maskT); free_ptr(w.gm_part); free_ptr(w.conv[0]); free_ptr(w.conv[1]); free_ptr(w.delta);
     for (int k = 0; k < 7; ++k) free_ptr(w.long_items[k]);
     free_ptr(w.long_count); free_ptr(w.long_MI); free_ptr(w.long_MT); free_ptr(w.best_bits[0]);
     free_ptr(w.fe_med); free_ptr(w.fe_long); free_ptr(w.fe_cm); free_ptr(w.f_part);

@@ -26,3 +26,6 @@ extern "C" afs_status afs_pgd_run_conv(afs_problem* p, float* X, int32_t B, int3
 extern "C" afs_status afs_pgd_run_masks(afs_problem* p, float* X, int32_t B, int32_t steps, float lr, const int8_t* masks,
                                         int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
 { return pgd_run_impl<float>(p, X, B, steps, lr, masks, best_assign, best_sat, best_step, stream, float(0), nullptr, true); }
+
+extern "C" afs_status afs_constraint_grad_l1(afs_problem* p, const float* X, int32_t B, float* gm, void* stream)
+{ return grad_l1_impl<float>(p, X, B, gm, stream); }

@@ -26,3 +26,6 @@ extern "C" afs_status afs_pgd_run_conv_f64(afs_problem* p, double* X, int32_t B,
 extern "C" afs_status afs_pgd_run_masks_f64(afs_problem* p, double* X, int32_t B, int32_t steps, double lr, const int8_t* masks,
                                         int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)
 { return pgd_run_impl<double>(p, X, B, steps, lr, masks, best_assign, best_sat, best_step, stream, double(0), nullptr, true); }
+
+extern "C" afs_status afs_constraint_grad_l1_f64(afs_problem* p, const double* X, int32_t B, double* gm, void* stream)
+{ return grad_l1_impl<double>(p, X, B, gm, stream); }

@@ -147,6 +147,8 @@ struct Workspace {
     void* fe_long = nullptr;               // real [n_long][Bp]
     void* fe_cm = nullptr;                 // real [n_cm][Bp]
     void* f_part = nullptr;                // real [n_parts][Bp]
+    void* gm_part = nullptr;               // real [m][Bp/32] per-constraint gradient magnitude, one partial per restart tile
+    int64_t gm_elems = 0;
     int32_t fe_Bp = 0;
     int8_t* mask_dev = nullptr;            // staging for afs_pgd_run_host
     void* host_stage_X = nullptr;          // device X[B,n] staging for afs_pgd_run_host
@@ -210,6 +212,13 @@ struct afs_problem {
     int32_t* d_cm_slots = nullptr;
     int32_t cm_begin[afs::CM_BUCKETS + 1] = {0};
     int32_t cm_maxL = 0;                // longest CMED constraint (rows of the shared-memory pmf buffer - 1)
+
+    // original constraint index of every class entry, and (problems created with weights only) unit-weight twins of the
+    // class records: the per-constraint gradient magnitudes (afs_constraint_grad_l1) are taken without the weights
+    int32_t *d_pull_id = nullptr, *d_med_id = nullptr, *d_cm_id = nullptr, *d_long_id = nullptr;
+    afs::MedCon* d_med_u = nullptr;
+    afs::LongCon *d_cm_u = nullptr, *d_long_u = nullptr;
+    bool unit_w_mode = false;           // the push launches of the current call read the unit-weight twins
 
     afs::CountCon* d_count = nullptr;   // all m constraints, original order
     uint32_t* d_count_lits = nullptr;

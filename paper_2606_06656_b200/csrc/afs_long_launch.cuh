@@ -34,7 +34,7 @@ static afs_status launch_long_items(afs_problem* P, const LongLists& wl, int set
     const bool fo = P->long_folded;
     unsigned long long* work = nullptr;
     { afs_status ws = prof_work_slot(P, 8 + NR, st, &work); if (ws != AFS_OK) return ws; }
-    kern<<<grid, WPC * 32, smem, st>>>(fo ? P->d_long_f : P->d_long, fo ? P->d_long_lits_f : P->d_long_lits,
+    kern<<<grid, WPC * 32, smem, st>>>(fo ? P->d_long_f : (P->unit_w_mode && P->d_long_u) ? P->d_long_u : P->d_long, fo ? P->d_long_lits_f : P->d_long_lits,
                                         fo ? P->d_long_slots_f : P->d_long_slots, XT, Sw, SATw, Bp / 32, Bp,
                                         scratch + (size_t)P->nslots_a * Bp, (int)P->nslots_a, (int)(P->nslots - P->nslots_a),
                                         (real*)P->ws.bnd, fe, wl.items[CLS], wl.count + set * LONG_CLASSES + CLS, LS, QS,
@@ -58,7 +58,7 @@ static afs_status launch_long_lane(afs_problem* P, const LongLists& wl, int set,
     const int grid = (int)std::min<long long>((long long)P->sm_count * occ, cap_blocks < 1 ? 1 : cap_blocks);
     ProfSpan span(P, prof_cls, st);
     const bool fo = P->long_folded;
-    kern<<<grid, wpc * 32, smem, st>>>(fo ? P->d_long_f : P->d_long, fo ? P->d_long_lits_f : P->d_long_lits,
+    kern<<<grid, wpc * 32, smem, st>>>(fo ? P->d_long_f : (P->unit_w_mode && P->d_long_u) ? P->d_long_u : P->d_long, fo ? P->d_long_lits_f : P->d_long_lits,
                                        fo ? P->d_long_slots_f : P->d_long_slots, XT, Bp, scratch + (size_t)P->nslots_a * Bp,
                                        (int)P->nslots_a, (int)(P->nslots - P->nslots_a), (real*)P->ws.bnd, fe, wl.items[cls],
                                        wl.count + set * LONG_CLASSES + cls, cap, P->d_long_goff, P->ws.long_MI, P->ws.long_MT);
@@ -84,7 +84,7 @@ afs_status launch_long_all(afs_problem* P, const real* XT, const uint32_t* Sw, c
     if ((warps + 3) / 4 > 0x7fffffffLL) return AFS_ERR_UNSUPPORTED;
     {
         ProfSpan span(P, 5, st);
-        k_long_scan<real><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(fo ? P->d_long_f : P->d_long, (int)P->n_long,
+        k_long_scan<real><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(fo ? P->d_long_f : (P->unit_w_mode && P->d_long_u) ? P->d_long_u : P->d_long, (int)P->n_long,
                                                                       fo ? P->d_long_lits_f : P->d_long_lits, Sw, SATw, ntile,
                                                                       Bp, (real*)P->ws.bnd, sat, fe, wl, set, rs, P->d_long_goff, P->ws.long_MI,
                                                                       P->ws.long_MT);

@@ -176,9 +176,11 @@ static afs_status create_impl(int32_t n_vars, int32_t n_cons, const int64_t* row
         std::vector<CountCon> pc;
         std::vector<uint32_t> pc_lits;
         std::vector<PullClause> pcp;
+        std::vector<int32_t> pull_id, med_id, cm_id, long_id;   // original constraint index of every class entry
         for (int c = 0; c < m; ++c) {
             if (cls[c] != C_PULL) continue;
             P->n_pull++;
+            pull_id.push_back(c);
             int L = (int)(row_ptr[c + 1] - row_ptr[c]);
             const int32_t* lc = lits + row_ptr[c];
             CountCon cc; cc.off = (int64_t)pc_lits.size(); cc.L = L; cc.type = (int16_t)types[c]; cc.pad = 0; cc.k = k[c]; cc.pad2 = 0;
@@ -252,6 +254,7 @@ static afs_status create_impl(int32_t n_vars, int32_t n_cons, const int64_t* row
                     med_slots.push_back(slot_of[e]);
                 }
                 med.push_back(mc);
+                med_id.push_back(c);
             }
             P->med_nnz = (int64_t)med_lits.size();
             P->n_med = (int64_t)ids.size();
@@ -261,7 +264,8 @@ static afs_status create_impl(int32_t n_vars, int32_t n_cons, const int64_t* row
         std::vector<uint32_t> long_lits, cm_lits;
         std::vector<int32_t> long_slots, cm_slots;
         auto build_count_class = [&](int want_cls, auto bucket_fn, int nbuckets, int32_t* begin, int32_t* maxL,
-                                     std::vector<LongCon>& out, std::vector<uint32_t>& olits, std::vector<int32_t>& oslots) {
+                                     std::vector<LongCon>& out, std::vector<uint32_t>& olits, std::vector<int32_t>& oslots,
+                                     std::vector<int32_t>& oid) {
             std::vector<int> ids;
             for (int c = 0; c < m; ++c) if (cls[c] == want_cls) ids.push_back(c);
             std::stable_sort(ids.begin(), ids.end(), [&](int a, int b) {
@@ -285,14 +289,15 @@ static afs_status create_impl(int32_t n_vars, int32_t n_cons, const int64_t* row
                     oslots.push_back(slot_of[e]);
                 }
                 out.push_back(lc);
+                oid.push_back(c);
             }
             while (cur < nbuckets) begin[++cur] = (int32_t)ids.size();
             return (int64_t)ids.size();
         };
         P->n_long = build_count_class(C_LONG, [&](int c) { return (int)((row_ptr[c + 1] - row_ptr[c] + 1 + 127) / 128) - 1; },
-                                      LONG_BUCKETS, P->long_begin, P->long_maxL, lng, long_lits, long_slots);
+                                      LONG_BUCKETS, P->long_begin, P->long_maxL, lng, long_lits, long_slots, long_id);
         P->n_cm = build_count_class(C_CMED, [&](int c) { return (int)((row_ptr[c + 1] - row_ptr[c] + 15) / 16) - 1; },
-                                    CM_BUCKETS, P->cm_begin, nullptr, cmv, cm_lits, cm_slots);
+                                    CM_BUCKETS, P->cm_begin, nullptr, cmv, cm_lits, cm_slots, cm_id);
         for (const LongCon& x : cmv) P->cm_maxL = std::max(P->cm_maxL, x.L);
         // ------------------------------------------------------------ generic forward CSR for the count-only kernel
         std::vector<CountCon> cnt(m);
@@ -412,6 +417,14 @@ static afs_status create_impl(int32_t n_vars, int32_t n_cons, const int64_t* row
         up(&P->d_cm, cmv);
         up(&P->d_cm_lits, cm_lits);
         up(&P->d_cm_slots, cm_slots);
+        up(&P->d_pull_id, pull_id); up(&P->d_med_id, med_id); up(&P->d_cm_id, cm_id); up(&P->d_long_id, long_id);
+        if (weights) {   // unit-weight twins of the class records, for the per-constraint gradient magnitudes
+            std::vector<MedCon> med_u(med); for (auto& x : med_u) x.w = 1.0f;
+            std::vector<LongCon> cm_u(cmv), lng_u(lng);
+            for (auto& x : cm_u) x.w = 1.0f;
+            for (auto& x : lng_u) x.w = 1.0f;
+            up(&P->d_med_u, med_u); up(&P->d_cm_u, cm_u); up(&P->d_long_u, lng_u);
+        }
         up(&P->d_count, cnt);
         up(&P->d_count_lits, cnt_lits);
         if (st != AFS_OK) { afs_problem_destroy(P); return st; }
@@ -441,6 +454,8 @@ extern "C" void afs_problem_destroy(afs_problem* p)
     cudaSetDevice(p->device);
     cudaDeviceSynchronize();
     cudaFree(p->d_pull_ptr); cudaFree(p->d_pull_words); cudaFree(p->d_slot_ptr); cudaFree(p->d_lslot_info); cudaFree(p->d_lslot_ptr);
+    cudaFree(p->d_pull_id); cudaFree(p->d_med_id); cudaFree(p->d_cm_id); cudaFree(p->d_long_id);
+    cudaFree(p->d_med_u); cudaFree(p->d_cm_u); cudaFree(p->d_long_u);
     cudaFree(p->d_run_ptr); cudaFree(p->d_runs); cudaFree(p->d_pull_gconst); cudaFree(p->d_pc); cudaFree(p->d_pc_lits); cudaFree(p->d_pcp);
     cudaFree(p->d_med); cudaFree(p->d_med_lits); cudaFree(p->d_med_slots);
     cudaFree(p->d_long); cudaFree(p->d_long_lits); cudaFree(p->d_long_slots);

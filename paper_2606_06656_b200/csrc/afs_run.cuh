@@ -9,6 +9,7 @@
 
 #include "afs_kernels.cuh"
 #include "afs_resident.cuh"
+#include "afs_gm.cuh"
 #include "afs_launch.h"
 
 namespace afs {
@@ -68,7 +69,7 @@ static afs_status launch_push(afs_problem* P, const real* XT, const uint32_t* Sw
         if (smem > 48 * 1024)
             CU(cudaFuncSetAttribute(k_cmed<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ProfSpan span(P, 3, st);
-        k_cmed<real><<<dim3(gx, tiles), 128, smem, st>>>(P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat,
+        k_cmed<real><<<dim3(gx, tiles), 128, smem, st>>>((P->unit_w_mode && P->d_cm_u) ? P->d_cm_u : P->d_cm, c0, c1, P->d_cm_lits, P->d_cm_slots, XT, Bp, scratch, sat,
                                                         fe_cm, qrows, rs);
         P->last_launches++;
     }
@@ -77,7 +78,7 @@ static afs_status launch_push(afs_problem* P, const real* XT, const uint32_t* Sw
         int cap = (P->sm_count * 16 + tiles - 1) / tiles;   // enough CTAs to fill the chip, grid-stride beyond
         if (gx > cap) gx = cap < 1 ? 1 : cap;
         ProfSpan span(P, 4, st);
-        k_med<real><<<dim3(gx, tiles), 128, 0, st>>>(P->d_med, 0, (int)P->n_med, P->d_med_lits, P->d_med_slots, XT, Bp, scratch,
+        k_med<real><<<dim3(gx, tiles), 128, 0, st>>>((P->unit_w_mode && P->d_med_u) ? P->d_med_u : P->d_med, 0, (int)P->n_med, P->d_med_lits, P->d_med_slots, XT, Bp, scratch,
                                                     (real*)P->ws.aux[0], (real*)P->ws.aux[1], sat, fe_med, rs);
         P->last_launches++;
     }
@@ -146,6 +147,57 @@ static afs_status eval_grad_impl(afs_problem* P, const real* X, int32_t B, real*
         k_transpose_out<real><<<tg, 256, 0, st>>>(GT, G, B, P->n, wBp);
         P->last_launches++;
     }
+    CU(cudaGetLastError());
+    return AFS_OK;
+}
+
+// per-constraint gradient magnitudes (afs_gm.cuh): one evaluation with unit weights, then a reduction per class
+template <typename real>
+static afs_status grad_l1_impl(afs_problem* P, const real* X, int32_t B, real* gm, void* stream)
+{
+    DeviceScope dev_scope(P);
+    afs_status s = enter(P, B);
+    if (s != AFS_OK) return s;
+    if (!X || !gm) return AFS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int Bp = ((B + 31) / 32) * 32, ntile = Bp / 32;
+    if ((s = ensure_workspace(P, Bp, sizeof(real), 3)) != AFS_OK) return s;
+    if ((s = ensure_eval_buffers(P, Bp, sizeof(real))) != AFS_OK) return s;
+    Workspace& w = P->ws;
+    const int64_t need = (int64_t)(P->m > 0 ? P->m : 1) * (w.Bp / 32) * 8;
+    if (w.gm_elems < need) {
+        CU(cudaDeviceSynchronize());
+        if (w.gm_part) cudaFree(w.gm_part);
+        w.gm_part = nullptr; w.gm_elems = 0;
+        if (cudaMalloc(&w.gm_part, (size_t)need) != cudaSuccess) { (void)cudaGetLastError(); return AFS_ERR_ALLOC; }
+        w.gm_elems = need; w.bytes += (size_t)need;
+    }
+    real* XT = (real*)w.XT[0];
+    real* scratch = (real*)w.scratch;
+    real* part = (real*)w.gm_part;
+    dim3 tg((P->n + 31) / 32, ntile);
+    k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT, B, P->n, Bp, nullptr, w.S[0], w.SAT[0]);
+    P->unit_w_mode = true;
+    s = launch_push<real>(P, XT, w.S[0], w.SAT[0], Bp, scratch, nullptr, nullptr, nullptr, nullptr, nullptr, st);
+    P->unit_w_mode = false;
+    if (s != AFS_OK) return s;
+    if (P->n_pull > 0)
+        k_gm_pull<real><<<dim3((unsigned)((P->n_pull + 3) / 4), ntile), 128, 0, st>>>(P->d_pcp, (int)P->n_pull, P->d_pull_id, XT, Bp, B, part);
+    if (P->n_med > 0)
+        k_gm_rows<real, MedCon><<<dim3((unsigned)((P->n_med + 3) / 4), ntile), 128, 0, st>>>(P->d_med, (int)P->n_med, P->d_med_slots,
+                                                                                           P->d_med_id, scratch, Bp, B, part);
+    if (P->n_cm > 0)
+        k_gm_rows<real, LongCon><<<dim3((unsigned)((P->n_cm + 3) / 4), ntile), 128, 0, st>>>(P->d_cm, (int)P->n_cm, P->d_cm_slots,
+                                                                                           P->d_cm_id, scratch, Bp, B, part);
+    if (P->n_long > 0) {
+        const long long warps = (long long)P->n_long * ntile;
+        k_gm_long<real><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(P->d_long, (int)P->n_long, P->d_long_lits, P->d_long_slots,
+                                                                   P->d_long_id, w.S[0], w.SAT[0], ntile, Bp, B,
+                                                                   scratch + (size_t)P->nslots_a * Bp, (int)P->nslots_a,
+                                                                   (int)(P->nslots - P->nslots_a), (const real*)w.bnd, part);
+    }
+    if (P->m > 0) k_gm_final<real><<<(P->m + 255) / 256, 256, 0, st>>>(part, P->m, ntile, gm);
+    P->last_launches += 6;
     CU(cudaGetLastError());
     return AFS_OK;
 }

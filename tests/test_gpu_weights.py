@@ -83,3 +83,24 @@ def test_unit_weights_change_nothing(afs):
     with pytest.raises(afs.AfsError):
         afs.Problem.from_instance(inst, weights=np.full(inst.m, np.nan, np.float32))
     Pa.close(); Pb.close()
+
+
+@pytest.mark.parametrize("name", ["mixed", "long", "cnf"])
+def test_per_constraint_gradient_magnitudes(afs, name):
+    """afs_constraint_grad_l1 = the oracle's gm[k] = sum_b sum_j |dFE_k/dy_j|, unweighted also on a weighted handle; at
+    X0 and at a point with 60 % of the coordinates clipped to +-1 (boundary literals of the long constraints)."""
+    import torch
+    inst = cases()[name]
+    rng = np.random.default_rng(6)
+    Xc = inst.X0.copy()
+    face = rng.random(Xc.shape) < 0.6
+    Xc[face] = np.where(Xc[face] < 0, -1.0, 1.0).astype(np.float32)
+    for weights in (None, weights_for(inst, 7)):
+        P = afs.Problem.from_instance(inst, weights=weights)
+        for X in (inst.X0, Xc):
+            _, _, gmo = ref.eval_grad_w(inst, None, X.astype(np.float64), want_grad=False, want_gm=True)
+            g64 = P.constraint_grad_l1(dev(X, torch.float64)).cpu().numpy()
+            assert np.all(np.abs(g64 - gmo) <= 1e-10 * np.maximum(gmo, 1.0)), np.abs(g64 - gmo).max()
+            g32 = P.constraint_grad_l1(dev(X)).cpu().numpy().astype(np.float64)
+            assert np.all(np.abs(g32 - gmo) <= 1e-4 * np.maximum(gmo, 1e-3) + 1e-5), np.abs(g32 - gmo).max()
+        P.close()
