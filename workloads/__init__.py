@@ -18,3 +18,4 @@ from .generate import (  # noqa: F401
     random_kcnf, planted_kcnf, mixed_pb, xor_dup, long_pb, tiny_mixed,
     concat, true_counts, plant_satisfies,
 )
+from .encoders import sudoku, sudoku_assignment, ramsey, ramsey_assignment  # noqa: F401
