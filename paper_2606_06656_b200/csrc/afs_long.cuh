@@ -570,7 +570,7 @@ __global__ void __launch_bounds__(256) k_long_lane(const LongCon* __restrict__ c
                                                    real* __restrict__ fe_out, const uint4* __restrict__ items,
                                                    const int* __restrict__ count, int cap,
                                                    const int32_t* __restrict__ goff, const uint32_t* __restrict__ MI,
-                                                   const uint32_t* __restrict__ MT)
+                                                   const uint32_t* __restrict__ MT, unsigned long long* __restrict__ work)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
@@ -637,6 +637,17 @@ __global__ void __launch_bounds__(256) k_long_lane(const LongCon* __restrict__ c
         }
         const real wA = (real)lc.wA * (real)lc.w, wB = (real)lc.wB * (real)lc.w;   // zero where the target is unused
         const int cA = lc.tA - nB0, cB = lc.tB - nB0;    // targets inside the reduced pmf
+        if (work) {   // timing mode: the counted algorithmic work, 6 Leff Keff per entry (as k_long_items)
+            unsigned long long fl = 0ull;
+            const int keff = lc.k - nB0;
+            if (have && (lc.wA != 0.f || lc.wB != 0.f) && keff >= (lc.type == AFS_EK ? 0 : 1) && keff <= nI) {
+                int K = min(keff, nI - keff + 1) + 1;
+                fl = 6ull * (unsigned long long)nI * (unsigned long long)(K < 1 ? 1 : K);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) fl += __shfl_xor_sync(FULL, fl, o);
+            if (lane == 0 && fl) atomicAdd(work + (blockIdx.x & 31u), fl);
+        }
         if (have) {   // boundary literals: removing a false one leaves q, removing a true one takes one shift away
             auto qat = [&](int tau) -> real { return (tau >= 0 && tau <= nI) ? q[tau * 32] : zero; };
             real* o = bnd + ((size_t)c * Bp + b) * 2;

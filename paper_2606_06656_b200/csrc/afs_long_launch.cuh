@@ -58,10 +58,12 @@ static afs_status launch_long_lane(afs_problem* P, const LongLists& wl, int set,
     const int grid = (int)std::min<long long>((long long)P->sm_count * occ, cap_blocks < 1 ? 1 : cap_blocks);
     ProfSpan span(P, prof_cls, st);
     const bool fo = P->long_folded;
+    unsigned long long* work = nullptr;
+    { afs_status ws = prof_work_slot(P, prof_cls, st, &work); if (ws != AFS_OK) return ws; }
     kern<<<grid, wpc * 32, smem, st>>>(fo ? P->d_long_f : (P->unit_w_mode && P->d_long_u) ? P->d_long_u : P->d_long, fo ? P->d_long_lits_f : P->d_long_lits,
                                        fo ? P->d_long_slots_f : P->d_long_slots, XT, Bp, scratch + (size_t)P->nslots_a * Bp,
                                        (int)P->nslots_a, (int)(P->nslots - P->nslots_a), (real*)P->ws.bnd, fe, wl.items[cls],
-                                       wl.count + set * LONG_CLASSES + cls, cap, P->d_long_goff, P->ws.long_MI, P->ws.long_MT);
+                                       wl.count + set * LONG_CLASSES + cls, cap, P->d_long_goff, P->ws.long_MI, P->ws.long_MT, work);
     P->last_launches++;
     return AFS_OK;
 }
