@@ -265,41 +265,51 @@ __device__ __forceinline__ real long_forward(const LongCon& lc, const int L, rea
     return fe;
 }
 
-// The same for Leff <= 31: one pmf cell per lane (cell t in lane t), two instructions per literal.  No rescaling on
-// the way: the un-normalised coefficients grow by at most 2 per literal (R <= 1), 2^31 in all.
-template <typename real>
-__device__ __forceinline__ real long_forward_tiny(const LongCon& lc, const int L, const real* __restrict__ Rc,
-                                                  real* __restrict__ Aw, const int nBr, const int nBr4, const int nAr,
-                                                  const int Leff, const int nB0, const int off, const int lane,
-                                                  const bool want_fe)
+// The same for Leff < 32 CPL: the whole pmf in CPL cells per lane (cell t = lane * CPL + i), CPL + 5 instructions per
+// literal, no rows to manage.  No rescaling on the way: the un-normalised coefficients grow by at most 2 per literal
+// (R <= 1), 2^120 in all, inside the fp32 range.
+template <typename real, int CPL>
+__device__ __forceinline__ real long_forward_small(const LongCon& lc, const int L, const real* __restrict__ Rc,
+                                                   real* __restrict__ Aw, const int nBr, const int nBr4, const int nAr,
+                                                   const int Leff, const int nB0, const int off, const int lane,
+                                                   const int QS, const bool want_fe)
 {
     constexpr unsigned FULLM = 0xffffffffu;
-    real q = lane == 0 ? real(1) : real(0), P = real(1);
-    for (int e = 0; e < nBr; ++e) {
-        const real R = Rc[e];
-        real lo = __shfl_up_sync(FULLM, q, 1);
+    real q[CPL];
+#pragma unroll
+    for (int i = 0; i < CPL; ++i) q[i] = real(0);
+    if (lane == 0) q[0] = real(1);
+    real P = real(1);
+    auto step = [&](const real R) {
+        real lo = __shfl_up_sync(FULLM, q[CPL - 1], 1);
         if (lane == 0) lo = real(0);
-        q = fma(R, lo, q);
+#pragma unroll
+        for (int i = CPL - 1; i >= 1; --i) q[i] = fma(R, q[i - 1], q[i]);
+        q[0] = fma(R, lo, q[0]);
         P = fma(P, R, P);
+    };
+    for (int e = 0; e < nBr; ++e) step(Rc[e]);
+    if (nBr > 0) {   // prod_B (z + R_j) is the reversal of prod_B (1 + R_j w): c_t -> c_{nBr - t}, through shared memory
+#pragma unroll
+        for (int i = 0; i < CPL; ++i) { const int t = lane * CPL + i; if (t <= nBr) Aw[t] = q[i]; }
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < CPL; ++i) { const int t = lane * CPL + i; q[i] = t <= nBr ? Aw[nBr - t] : real(0); }
+        __syncwarp();
     }
-    if (nBr > 0) {   // prod_B (z + R_j) is the reversal of prod_B (1 + R_j w)
-        const real rv = __shfl_sync(FULLM, q, (nBr - lane) & 31);
-        q = lane <= nBr ? rv : real(0);
-    }
-    for (int e = 0; e < nAr; ++e) {
-        const real R = Rc[nBr4 + e];
-        real lo = __shfl_up_sync(FULLM, q, 1);
-        if (lane == 0) lo = real(0);
-        q = fma(R, lo, q);
-        P = fma(P, R, P);
-    }
-    const real v = q * recip(P);
-    Aw[lane] = real(0); Aw[32 + lane] = real(0);   // cells the pmf (offset <= 3) and the chains' 16-byte blocks touch
+    for (int e = 0; e < nAr; ++e) step(Rc[nBr4 + e]);
+    const real sc = recip(P);
+    for (int t = lane; t < min(QS, Leff + 12); t += 32) Aw[t] = real(0);   // cells the chains' 16-byte blocks touch
     __syncwarp();
     real fe = real(0);
-    if (lane <= Leff) {
-        Aw[off + lane] = v;
-        if (want_fe) fe = long_pred(lc.type, L, lc.k, lane + nB0) ? -v : v;
+#pragma unroll
+    for (int i = 0; i < CPL; ++i) {
+        const int t = lane * CPL + i;
+        if (t <= Leff) {
+            const real v = q[i] * sc;
+            Aw[off + t] = v;
+            if (want_fe) fe += long_pred(lc.type, L, lc.k, t + nB0) ? -v : v;
+        }
     }
     return fe;
 }
@@ -492,7 +502,8 @@ __global__ void __launch_bounds__(WPC * 32) k_long_items(const LongCon* __restri
         const int off = (3 - Leff) & 3;
         {
             real fe;
-            if (NR == 1 && Leff <= 31) fe = long_forward_tiny<real>(lc, L, Rc, Aw, nBr, nBr4, nAr, Leff, nB0, off, lane, fe_out != nullptr);
+            if (NR == 1 && Leff <= 63) fe = long_forward_small<real, 2>(lc, L, Rc, Aw, nBr, nBr4, nAr, Leff, nB0, off, lane, QS, fe_out != nullptr);
+            else if (NR == 1) fe = long_forward_small<real, 4>(lc, L, Rc, Aw, nBr, nBr4, nAr, Leff, nB0, off, lane, QS, fe_out != nullptr);
             else fe = long_forward<real, NR>(lc, L, Rc, Aw, nBr, nBr4, send, Leff, nB0, off, lane, QS, fe_out != nullptr);
             if (fe_out) {
 #pragma unroll
