@@ -970,7 +970,9 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
 // constraint, picked by the literal's truth value (a variable on +-1 is a boundary literal in every constraint it
 // occurs in).  Eight literals per round, their loads issued together: the pass waits on L2 / HBM latency, not on issue.
 // ------------------------------------------------------------------------------------------------------------------
-template <typename real>
+// TPW = restart tiles per warp (the lane works on restarts lane, lane + 32 of a group of TPW tiles): one descriptor
+// shuffle and one offset computation serve TPW loads.
+template <typename real, int TPW>
 __global__ void __launch_bounds__(256) k_glong(int n, int ntile, int Bp, const int32_t* __restrict__ lslot_ptr,
                                                const int32_t* __restrict__ lslot_info, const real* __restrict__ Xin,
                                                const real* __restrict__ lrows /* scratch + nslots_a * Bp: [tile][nl][32] */, int nl,
@@ -978,47 +980,59 @@ __global__ void __launch_bounds__(256) k_glong(int n, int ntile, int Bp, const i
                                                real* __restrict__ GL, const RunState* __restrict__ rs)
 {
     const int lane = threadIdx.x & 31;
+    const int ngrp = ntile / TPW;
     const long long wid = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
-    if (wid >= (long long)n * ntile) return;
-    const int v = (int)(wid / ntile), tile = (int)(wid % ntile);
-    if (tile_idle(rs, tile)) return;
+    if (wid >= (long long)n * ngrp) return;
+    const int v = (int)(wid / ngrp), tile0 = (int)(wid % ngrp) * TPW;
+    if (tile_idle(rs, tile0)) return;
     if (mask && mask[v] != 0) return;   // a fixed variable never moves: its gradient is not needed
-    const int b = tile * 32 + lane;
-    const real x = Xin[(size_t)v * Bp + b];
-    const bool onb = x == real(1) || x == real(-1);
-    const int neg0 = x < real(0) ? 1 : 0;
-    // One base pointer and 32-bit element offsets per lane: a restart on the boundary reads the pair table (second
-    // element where the literal is true, i.e. (x < 0) != negated), one inside the cube reads the class's rows.
-    const real* __restrict__ base = onb ? bnd + (size_t)b * 2
-                                        : lrows + ((size_t)tile * nl + (size_t)lslot_ptr[v]) * 32 + lane;
-    const uint32_t sgn = onb ? 0x80000000u : 0u;      // chain rule sign (S5) for pair entries; the rows carry it already
-    const uint32_t pair_stride = (uint32_t)Bp * 2u;
     const int s0 = lslot_ptr[v], s1 = lslot_ptr[v + 1];
-    real g = real(0);
+    // One base pointer and 32-bit element offsets per lane and tile: a restart on the boundary reads the pair table
+    // (second element where the literal is true, i.e. (x < 0) != negated), one inside the cube reads the class's rows.
+    const real* __restrict__ base[TPW];
+    uint32_t sgn[TPW], neg0[TPW];
+    bool onb[TPW];
+    real g[TPW];
+#pragma unroll
+    for (int c = 0; c < TPW; ++c) {
+        const int b = (tile0 + c) * 32 + lane;
+        const real x = Xin[(size_t)v * Bp + b];
+        onb[c] = x == real(1) || x == real(-1);
+        neg0[c] = x < real(0) ? 1u : 0u;
+        base[c] = onb[c] ? bnd + (size_t)b * 2 : lrows + ((size_t)(tile0 + c) * nl + (size_t)s0) * 32 + lane;
+        sgn[c] = onb[c] ? 0x80000000u : 0u;      // chain rule sign (S5) for pair entries; the rows carry it already
+        g[c] = real(0);
+    }
+    const uint32_t pair_stride = (uint32_t)Bp * 2u;
     for (int sb0 = s0; sb0 < s1; sb0 += 32) {
         const int myinfo = sb0 + lane < s1 ? lslot_info[sb0 + lane] : 0;   // 32 descriptors with one coalesced load
         const int cnt = min(32, s1 - sb0);
         int k = 0;
         for (; k + 8 <= cnt; k += 8) {   // eight literals per round, their loads issued together
-            real t[8];
-            uint32_t fl[8];
+            real t[8][TPW];
+            uint32_t ln[8];
 #pragma unroll
             for (int h = 0; h < 8; ++h) {
                 const uint32_t info = (uint32_t)__shfl_sync(FULL, myinfo, k + h);
-                const uint32_t off = onb ? (info >> 1) * pair_stride + ((info & 1u) ^ (uint32_t)neg0) : (uint32_t)(sb0 - s0 + k + h) * 32u;
-                fl[h] = (info & 1u) ? sgn : 0u;
-                t[h] = base[off];
+                const uint32_t offB = (info >> 1) * pair_stride, offS = (uint32_t)(sb0 - s0 + k + h) * 32u;
+                ln[h] = info & 1u;
+#pragma unroll
+                for (int c = 0; c < TPW; ++c) t[h][c] = base[c][onb[c] ? offB + (ln[h] ^ neg0[c]) : offS];
             }
 #pragma unroll
-            for (int h = 0; h < 8; ++h) g += flip(t[h], fl[h]);
+            for (int h = 0; h < 8; ++h)
+#pragma unroll
+                for (int c = 0; c < TPW; ++c) g[c] += flip(t[h][c], ln[h] ? sgn[c] : 0u);
         }
         for (; k < cnt; ++k) {
             const uint32_t info = (uint32_t)__shfl_sync(FULL, myinfo, k);
-            const uint32_t off = onb ? (info >> 1) * pair_stride + ((info & 1u) ^ (uint32_t)neg0) : (uint32_t)(sb0 - s0 + k) * 32u;
-            g += flip(base[off], (info & 1u) ? sgn : 0u);
+            const uint32_t offB = (info >> 1) * pair_stride, offS = (uint32_t)(sb0 - s0 + k) * 32u, l1 = info & 1u;
+#pragma unroll
+            for (int c = 0; c < TPW; ++c) g[c] += flip(base[c][onb[c] ? offB + (l1 ^ neg0[c]) : offS], l1 ? sgn[c] : 0u);
         }
     }
-    GL[(size_t)v * Bp + b] = g;
+#pragma unroll
+    for (int c = 0; c < TPW; ++c) GL[(size_t)v * Bp + (tile0 + c) * 32 + lane] = g[c];
 }
 
 // ------------------------------------------------------------------------------------------------------------------

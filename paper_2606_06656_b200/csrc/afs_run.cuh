@@ -34,13 +34,21 @@ template <typename real, bool EVAL>
 static void launch_var(afs_problem* P, VarArgs<real>& a, int gx, int tiles, const RunState* rs, cudaStream_t st)
 {
     if (P->n_long > 0) {   // the LONG class's share first (k_glong), from the pairs and rows the long kernels just wrote
-        const long long warps = (long long)P->n * tiles;
         real* GL = (real*)P->ws.GL;
         {
             ProfSpan span(P, 6, st);
-            k_glong<real><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P->n, tiles, a.Bp, P->d_lslot_ptr, P->d_lslot_info, a.Xin,
-                                                                     a.scratch + (size_t)P->nslots_a * a.Bp, (int)(P->nslots - P->nslots_a),
-                                                                     (const real*)P->ws.bnd, EVAL ? nullptr : a.mask, GL, rs);
+            const real* lrows = a.scratch + (size_t)P->nslots_a * a.Bp;
+            const int nl = (int)(P->nslots - P->nslots_a);
+            const int8_t* mk = EVAL ? nullptr : a.mask;
+            if (tiles % 2 == 0) {
+                const long long warps = (long long)P->n * (tiles / 2);
+                k_glong<real, 2><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P->n, tiles, a.Bp, P->d_lslot_ptr, P->d_lslot_info,
+                                                                            a.Xin, lrows, nl, (const real*)P->ws.bnd, mk, GL, rs);
+            } else {
+                const long long warps = (long long)P->n * tiles;
+                k_glong<real, 1><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P->n, tiles, a.Bp, P->d_lslot_ptr, P->d_lslot_info,
+                                                                            a.Xin, lrows, nl, (const real*)P->ws.bnd, mk, GL, rs);
+            }
         }
         a.GL = GL;
         launch_var_c<real, EVAL, true>(a, gx, tiles, st);
