@@ -53,7 +53,8 @@ typedef enum {
     AFS_ERR_DUP_VAR = 5,      /* the same variable twice in one constraint (G8; P:L41 assumes distinct)       */
     AFS_ERR_ALLOC = 6,        /* host or device allocation failed                                             */
     AFS_ERR_CUDA = 7,         /* CUDA runtime error, or no CUDA device                                        */
-    AFS_ERR_UNSUPPORTED = 8   /* valid request outside what this build supports (see each entry point)        */
+    AFS_ERR_UNSUPPORTED = 8,  /* valid request outside what this build supports (see each entry point)        */
+    AFS_ERR_STATIC_LIMIT = 9  /* afs_round_count_static: n and B need more than AFS_STATIC_SCRATCH_BYTES of scratch    */
 } afs_status;
 
 /* Symmetric constraint family of P:L60 (section 2.2) plus clauses (eq. 4). */
@@ -136,6 +137,38 @@ AFS_API afs_status afs_round_count(afs_problem* p, const float* X, int32_t B, in
                            void* cuda_stream);
 AFS_API afs_status afs_round_count_f64(afs_problem* p, const double* X, int32_t B, int8_t* assign, int32_t* sat,
                                void* cuda_stream);
+
+/*
+ * afs_round_count_static -- afs_round_count (fp32) for callers that must not allocate device memory at call time.
+ *
+ * Which callers: a solver loop living inside a host program whose framework already owns all of HBM through its own
+ * pool allocator (a cudaMalloc there fails or makes the pool shrink), a latency-bound thread that cannot afford the
+ * device-wide synchronisation cudaMalloc / cudaFree imply, or a component whose host forbids driver allocations after
+ * set-up.  afs_round_count grows the handle's workspace with cudaMalloc the first time it sees a larger batch; this
+ * entry point never does: it calls no cudaMalloc, no cudaFree and no allocating library routine, and leaves the
+ * handle's workspace alone.  (The handle itself is created earlier, by afs_problem_create, which does allocate.)
+ *
+ * Its working memory -- the transposed copy of X and one counter per restart -- is a fixed array of
+ * AFS_STATIC_SCRATCH_BYTES that is part of the library image: every GPU that loads the library holds that much until
+ * the process exits.  A request needs  256-aligned(4 Bp) + 4 n Bp  bytes of it, Bp = B rounded up to a multiple of 32
+ * (e.g. n = 5000 with B <= 832, or n = 1000 with B <= 4160); anything larger is refused with AFS_ERR_STATIC_LIMIT and
+ * nothing is enqueued.
+ *
+ * Arguments, layouts, rounding rule and results are those of afs_round_count: X device float[B,n] (read only),
+ * assign device int8[B,n] or NULL, sat device int32[B]; the results are bit-identical to afs_round_count's.
+ * Work is enqueued on `cuda_stream`; the call does not synchronise.
+ *
+ * First call on a device: looks up the array's device address (once per device, under a lock) before enqueuing
+ * anything.  Make that first call during set-up, before any stream capture is begun.
+ *
+ * Sharing: there is one array per GPU, shared by every handle, thread and stream in the process, and it keeps the
+ * previous call's contents (the entry point clears what has to start at zero).  Two calls that overlap on the same GPU
+ * -- different streams, or different handles -- race on it and give wrong counts; issue them on one stream, or order
+ * them with events.
+ */
+#define AFS_STATIC_SCRATCH_BYTES (16u << 20)
+AFS_API afs_status afs_round_count_static(afs_problem* p, const float* X, int32_t B, int8_t* assign, int32_t* sat,
+                                          void* cuda_stream);
 
 /*
  * afs_pgd_run -- S1..S10 looped `steps` times with no host round trip (P:L69 PGD; G11, G12, G14, G16):

@@ -22,6 +22,7 @@ EXPORTS = (
     "afs_round_count", "afs_round_count_f64", "afs_pgd_run", "afs_pgd_run_f64", "afs_pgd_run_host",
     "afs_problem_info", "afs_set_option", "afs_status_string", "afs_abi_version", "afs_last_error_message",
     "afs_profile_read", "afs_profile_flops", "afs_fp32_fma_peak", "afs_pgd_run_conv", "afs_pgd_run_conv_f64", "afs_pgd_run_masks", "afs_pgd_run_masks_f64", "afs_problem_create_w", "afs_constraint_grad_l1", "afs_constraint_grad_l1_f64",
+    "afs_round_count_static",
 )
 
 _lib = None
@@ -56,7 +57,7 @@ def lib():
     L.afs_coeffs.restype = C.c_int
     for name in ("afs_eval_grad", "afs_eval_grad_f64"):
         f = getattr(L, name); f.argtypes = [vp, vp, i32, vp, vp, vp]; f.restype = C.c_int
-    for name in ("afs_round_count", "afs_round_count_f64"):
+    for name in ("afs_round_count", "afs_round_count_f64", "afs_round_count_static"):
         f = getattr(L, name); f.argtypes = [vp, vp, i32, vp, vp, vp]; f.restype = C.c_int
     for name in ("afs_constraint_grad_l1", "afs_constraint_grad_l1_f64"):
         f = getattr(L, name); f.argtypes = [vp, vp, i32, vp, vp]; f.restype = C.c_int
@@ -233,6 +234,29 @@ class Problem:
         fn = lib().afs_round_count_f64 if f64 else lib().afs_round_count
         _chk(fn(self._h, X.data_ptr(), B, assign.data_ptr() if want_assign else None, sat.data_ptr(),
                 _stream_ptr(X.device)), "afs_round_count")
+        return assign, sat
+
+    def round_count_static(self, X, assign=None, sat=None):
+        """afs_round_count_static: round and count without any device allocation inside the library call.
+
+        For callers that cannot allocate on the device when they call (all of HBM already owned by a pool, a thread that
+        cannot take cudaMalloc's device-wide synchronisation, a host that forbids allocations after set-up): the
+        library's working memory is a fixed 16 MiB array inside the library image, so (n, B) must satisfy
+        256-aligned(4 Bp) + 4 n Bp <= 16 MiB or AfsError(status 9) is raised.  Pass preallocated ``assign`` int8[B,n]
+        and ``sat`` int32[B] to keep this wrapper allocation-free too (they are created here only when left out;
+        ``assign=False`` skips the assignment).  One array per GPU is shared by all calls: calls that overlap on the
+        GPU race.  Returns (assign or None, sat), bit-identical to ``round_count``."""
+        torch = _torch()
+        self._check_X(X, torch.float32)
+        B = X.shape[0]
+        if sat is None:
+            sat = torch.empty(B, dtype=torch.int32, device=X.device)
+        if assign is None:
+            assign = torch.empty((B, self.n), dtype=torch.int8, device=X.device)
+        elif assign is False:
+            assign = None
+        _chk(lib().afs_round_count_static(self._h, X.data_ptr(), B, assign.data_ptr() if assign is not None else None,
+                                          sat.data_ptr(), _stream_ptr(X.device)), "afs_round_count_static")
         return assign, sat
 
     def pgd_run(self, X, steps: int, lr: float, mask=None, out=None):

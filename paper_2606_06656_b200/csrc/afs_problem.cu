@@ -517,6 +517,7 @@ extern "C" const char* afs_status_string(afs_status s)
     case AFS_ERR_ALLOC: return "allocation failed";
     case AFS_ERR_CUDA: return "CUDA error or no CUDA device";
     case AFS_ERR_UNSUPPORTED: return "unsupported by this build";
+    case AFS_ERR_STATIC_LIMIT: return "n and B exceed the static scratch array (AFS_STATIC_SCRATCH_BYTES) of afs_round_count_static";
     default: return "unknown status";
     }
 }
