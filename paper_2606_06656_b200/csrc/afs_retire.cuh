@@ -176,4 +176,19 @@ __global__ void __launch_bounds__(256) k_compact(const RunState* __restrict__ rs
     }
 }
 
+// Per-restart masks (afs_pgd_run_masks) follow their restarts: the rows of maskT[n][Bp] gathered like the iterate.
+// warp = (variable, new tile), lane <-> new column; pads take the mask of the column they copy.
+static __global__ void __launch_bounds__(256) k_compact_mask(const RunState* __restrict__ rs, int n, int Bp,
+                                                             const int32_t* __restrict__ src,
+                                                             const int8_t* __restrict__ mask_old,
+                                                             int8_t* __restrict__ mask_new)
+{
+    const int tile = blockIdx.y;
+    if (tile * 32 >= rs->n_act) return;
+    const int lane = threadIdx.x & 31;
+    const int v = blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (v >= n) return;
+    mask_new[(size_t)v * Bp + tile * 32 + lane] = mask_old[(size_t)v * Bp + src[tile * 32 + lane]];
+}
+
 }  // namespace afs

@@ -357,9 +357,10 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
         CU(cudaDeviceSynchronize());
         if (w.maskT) cudaFree(w.maskT);
         w.maskT = nullptr; w.maskT_elems = 0;
-        if (cudaMalloc((void**)&w.maskT, (size_t)P->n * w.Bp) != cudaSuccess) { (void)cudaGetLastError(); return AFS_ERR_ALLOC; }
+        // two copies: a compaction gathers the masks of the active restarts from one into the other
+        if (cudaMalloc((void**)&w.maskT, (size_t)2 * P->n * w.Bp) != cudaSuccess) { (void)cudaGetLastError(); return AFS_ERR_ALLOC; }
         w.maskT_elems = (int64_t)P->n * w.Bp;
-        w.bytes += (size_t)P->n * w.Bp;
+        w.bytes += (size_t)2 * P->n * w.Bp;
     }
     P->last_resident = 0;
     if (plan >= 0) return pgd_run_resident<real>(P, plan, X, B, steps, lr, mask, best_assign, best_sat, best_step, st);
@@ -380,12 +381,14 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     typedef typename DBits<real>::type dbits_t;
     dbits_t* delta = static_cast<dbits_t*>(w.delta);     // [3][Bp], row t % 3 = max |dX| of step t
     bool dpending = false;                               // the last step's row is not folded into conv yet
+    int8_t* maskT[2] = {w.maskT, w.maskT ? w.maskT + (size_t)P->n * w.Bp : nullptr};
+    int mc = 0;              // maskT[mc] = the per-restart masks in the current column order
     if (conv) {
         launch_fill_i32(w.conv[0], (size_t)Bp, -1, st);
         CU(cudaMemsetAsync(w.delta, 0, (size_t)3 * Bp * sizeof(dbits_t), st));
     }
     k_transpose_in<real><<<tg, 256, 0, st>>>(X, XT[0], B, P->n, Bp, mask, w.S[0], w.SAT[0], per_restart_masks ? P->n : 0,
-                                             per_restart_masks ? w.maskT : nullptr);
+                                             per_restart_masks ? maskT[0] : nullptr);
     k_run_init<<<(Bp + 255) / 256, 256, 0, st>>>(rs, B, Bp, w.orig[0], w.moved);
     P->last_launches += 2;
     CU(cudaMemsetAsync(w.sat_hist, 0, (size_t)3 * Bp * sizeof(int32_t), st));
@@ -409,7 +412,7 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
         a.pull_ptr = P->d_pull_ptr; a.pull_words = P->d_pull_words; a.run_ptr = P->d_run_ptr; a.runs = P->d_runs;
         a.gconst = P->d_pull_gconst; a.slot_ptr = P->d_slot_ptr;
         a.scratch = scratch; a.Xin = Xin; a.Xout = XT[xn]; a.lr = lr; a.mask = mask1;
-        a.maskT = per_restart_masks ? w.maskT : nullptr;
+        a.maskT = per_restart_masks ? maskT[mc] : nullptr;
         a.sat_prev = pending ? w.sat_hist + (size_t)((t + 2) % 3) * Bp : nullptr;
         a.sat_zero = w.sat_hist + (size_t)((t + 1) % 3) * Bp;
         a.best_sat_in = w.best_sat[bc]; a.best_sat_out = w.best_sat[bc ^ 1];
@@ -457,6 +460,11 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
                                                                          w.best_bits[bb], XT[xf], w.S[sf], w.SAT[sf],
                                                                          w.best_bits[bb ^ 1]);
             P->last_launches += 3;
+            if (per_restart_masks) {   // the masks move with their restarts
+                k_compact_mask<<<dim3((P->n + 7) / 8, tiles), 256, 0, st>>>(rs, P->n, Bp, w.rt_src, maskT[mc], maskT[mc ^ 1]);
+                P->last_launches++;
+                mc ^= 1;
+            }
             bc ^= 1; oc ^= 1; bb ^= 1; xc = xf;
             sp_ = sc_; sc_ = sf;      // the words of X_t are not needed any more: the next pass has nothing to merge
             pending = false;

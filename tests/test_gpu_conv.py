@@ -136,3 +136,44 @@ def test_per_restart_masks_equal_one_run_per_restart(afs, name):
     else:
         assert (Xa - Xb).abs().max().item() < 1e-4
     P.close()
+
+
+@pytest.mark.parametrize("name", ["mixed", "long"])
+def test_per_restart_masks_follow_their_restarts_through_retirement(afs, name):
+    """A compaction moves restarts to other columns; their masks must move with them.  70 steps with retirement every
+    step / every 32 steps / never, rows that are fixed points from the start (everything fixed) in the middle of the
+    batch so that the columns behind them shift: fp64 build against one oracle run per restart with its own mask, and
+    the fp32 entry bit-identical across the three retirement settings."""
+    import torch
+    inst = cases()[name]
+    B, steps = 70, 70
+    rng = np.random.default_rng(21)
+    masks = np.zeros((B, inst.n), np.int8)
+    for b in range(B):
+        frac = 1.0 if b in (0, 3, 40, 41) else rng.uniform(0.0, 0.95)
+        fix = rng.choice(inst.n, size=int(frac * inst.n), replace=False)
+        masks[b, fix] = 1 - 2 * rng.integers(0, 2, size=fix.size)
+    X0 = np.random.default_rng(22).uniform(-1, 1, size=(B, inst.n))
+    orc = [ref.pgd_run(inst, X0[b:b + 1], steps, LR, mask=masks[b]) for b in range(B)]
+    P = afs.Problem.from_instance(inst)
+    md = dev(masks)
+    f32 = []
+    for every in (0, 1, 32):
+        P.set_option(2, every)
+        X = dev(X0, torch.float64)
+        g = P.pgd_run_masks(X, steps, LR, md)
+        torch.cuda.synchronize()
+        Xg = X.cpu().numpy()
+        for b in range(B):
+            o = orc[b]
+            assert np.abs(Xg[b] - o["X"][0]).max() <= 1e-9, (every, b)
+            assert g["best_sat"][b].item() == o["best_sat"][0] and g["best_step"][b].item() == o["best_step"][0], (every, b)
+            assert np.array_equal(g["best_assign"][b].cpu().numpy(), o["best_assign"][0]), (every, b)
+        Xf = dev(X0.astype(np.float32))
+        gf = P.pgd_run_masks(Xf, steps, LR, md)
+        f32.append((Xf.clone(), gf["best_sat"].clone(), gf["best_step"].clone(), gf["best_assign"].clone()))
+        fixed = masks != 0
+        assert np.array_equal(Xf.cpu().numpy()[fixed], masks[fixed].astype(np.float32)), every
+    for r in f32[1:]:
+        assert all(torch.equal(x, y) for x, y in zip(f32[0], r))
+    P.close()
