@@ -78,7 +78,7 @@ typedef enum {
  *   k        host    int32[n_cons]; EK: exactly k; CARD: at least k; XOR: required parity (1 = odd); otherwise ignored
  *   device           CUDA device ordinal
  *   out              receives the handle (NULL on error)
- * Limits of this build: EK / CARD up to L = 1151 literals, otherwise AFS_ERR_UNSUPPORTED; the other types have no
+ * Limits of this build: EK / CARD up to L = 1144 literals, otherwise AFS_ERR_UNSUPPORTED; the other types have no
  * length limit.
  */
 AFS_API afs_status afs_problem_create(int32_t n_vars, int32_t n_cons, const int64_t* row_ptr, const int32_t* lits,

@@ -25,7 +25,7 @@ constexpr uint32_t LIT_VAR = 0x7fffffffu;
 //  LONG : warp per (constraint, restart), count-basis DP + stable-direction leave-one-out recurrences:
 //         EK/CARD longer than 64.
 constexpr int PULL_MAX_LEN = 5;
-constexpr int LONG_MAX_LEN = 1151;   // 9 rows x 128 cells hold q_0..q_L
+constexpr int LONG_MAX_LEN = 1144;   // = long_class_maxleff(3): the item kernel's lists of 9 x 128 entries hold Leff + 6 <= 1150 padded entries
 constexpr int LONG_BUCKETS = 9;      // NR = 1..9 rows of 128 pmf cells
 
 // pull streams (S0 output for the PULL class).  Per variable its occurrences are grouped into RUNS of equal

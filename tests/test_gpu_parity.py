@@ -123,6 +123,34 @@ def test_eval_grad_at_clipped_points(afs, name):
     check_eval(afs, inst, X)
 
 
+def test_eval_grad_at_the_longest_supported_count_constraints(afs):
+    """EK / CARD at the longest length the build accepts (1144) and just below it, every literal strictly inside the
+    cube (the largest interior list the item kernel can meet) and with 1, 2, 3 literals on the boundary (every padding of
+    its two lists); fp64 build against the oracle.  One literal more is refused at create."""
+    rng = np.random.default_rng(31)
+    n = 1300
+    rows, types, ks = [], [], []
+    for L in (1141, 1142, 1143, 1144):
+        for ty in (W.AFS_EK, W.AFS_CARD):
+            v = rng.choice(n, size=L, replace=False)
+            sg = 1 - 2 * rng.integers(0, 2, size=L)
+            rows.append((sg * (v + 1)).astype(np.int32)); types.append(ty); ks.append(L // 2 + int(rng.integers(-3, 4)))
+    inst = W.generate._pack("longest", n, rows, types, ks, None, 31)
+    B = 6
+    X = rng.uniform(-0.3, 0.3, size=(B, n))
+    for b in range(1, 4):                      # restart b: b literals of every constraint on the boundary
+        for r in rows:
+            X[b, np.abs(r[:b]) - 1] = rng.choice([-1.0, 1.0], size=b)
+    X[4] = np.where(rng.random(n) < 0.5, np.sign(X[4]), X[4])     # about half of everything saturated
+    X = X.astype(np.float32)                   # the same representable point for both builds and the oracle
+    check_eval(afs, inst, X, f64=True)
+    check_eval(afs, inst, X)
+    too_long = W.generate._pack("too_long", n, [np.arange(1, 1146, dtype=np.int32)], [W.AFS_CARD], [500], None, 0)
+    with pytest.raises(afs.AfsError) as e:
+        afs.Problem.from_instance(too_long)
+    assert e.value.status == 8
+
+
 def sub_instance(inst, keep):
     rows = [inst.lits[inst.row_ptr[c]:inst.row_ptr[c + 1]] for c in np.nonzero(keep)[0]]
     return W.generate._pack("sub", inst.n, rows, inst.types[keep], inst.k[keep], None, 0)

@@ -85,7 +85,7 @@ def test_create_rejects_invalid_input_before_touching_the_device(afs):
     assert _create(afs, 3, [1, 3], [1, 2, 3], [afs.AFS_OR], [0]) == 4           # row_ptr[0] != 0
     assert _create(afs, 0, *ok3) == 1                                           # n < 1
     big = list(range(1, 1301))
-    assert _create(afs, 1300, [0, 1300], big, [afs.AFS_CARD], [600]) == 8       # count type longer than 1151
+    assert _create(afs, 1300, [0, 1300], big, [afs.AFS_CARD], [600]) == 8       # count type longer than 1144
     # valid input: succeeds on a GPU box, AFS_ERR_CUDA (7) without a device -- never a silent CPU fallback
     import torch
     st = _create(afs, 3, *ok3)
