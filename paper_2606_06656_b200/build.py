@@ -38,8 +38,16 @@ def _obj(src: str) -> str:
 
 
 def _compile(src: str, verbose: bool):
-    cmd = [NVCC] + CFLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", _obj(src)]
-    return src, subprocess.run(cmd, capture_output=True, text=True)
+    # to a private name first, then an atomic rename: two processes building at once (pytest-xdist, ranks started
+    # together) must never link an object the other one is still writing
+    tmp = _obj(src) + ".tmp.%d" % os.getpid()
+    cmd = [NVCC] + CFLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", tmp]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode == 0:
+        os.replace(tmp, _obj(src))
+    elif os.path.exists(tmp):
+        os.remove(tmp)
+    return src, r
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

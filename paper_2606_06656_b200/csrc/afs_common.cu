@@ -238,6 +238,9 @@ extern "C" afs_status afs_profile_read(afs_problem* P, double* ms, int64_t* laun
     if (!P || !ms || !launches || n < 0 || n > PROF_CLASSES) return AFS_ERR_INVALID_ARG;
     Profiler& pr = P->prof;
     if (pr.used > 0) CU(cudaEventSynchronize(pr.pool[pr.used - 1]));
+    // spans of the pull-clause counts are recorded on the library's second stream, which the caller's stream joins
+    // only AFTER its own last event: wait for that stream too before reading their events
+    if (pr.used > 0 && P->aux_stream) CU(cudaStreamSynchronize(P->aux_stream));
     for (const Profiler::Span& sp : pr.spans) {
         float t = 0.f;
         CU(cudaEventElapsedTime(&t, pr.pool[sp.e0], pr.pool[sp.e1]));

@@ -14,14 +14,7 @@ extern "C" afs_status afs_pgd_run(afs_problem* p, float* X, int32_t B, int32_t s
 extern "C" afs_status afs_pgd_run_conv(afs_problem* p, float* X, int32_t B, int32_t max_steps, float lr, const int8_t* mask,
                                        float tol, int8_t* best_assign, int32_t* best_sat, int32_t* best_step,
                                        int32_t* conv_step, int32_t* final_sat, float* final_F, void* stream)
-{
-    if (!(tol >= float(0)) || !std::isfinite((double)tol)) return AFS_ERR_INVALID_ARG;
-    if (p && conv_step && B >= 1) launch_fill_i32(conv_step, (size_t)B, -1, (cudaStream_t)stream);
-    afs_status s = pgd_run_impl<float>(p, X, B, max_steps, lr, mask, best_assign, best_sat, best_step, stream, tol, conv_step);
-    if (s == AFS_OK && final_sat) s = round_count_impl<float>(p, X, B, nullptr, final_sat, stream);
-    if (s == AFS_OK && final_F) s = eval_grad_impl<float>(p, X, B, final_F, nullptr, stream);
-    return s;
-}
+{ return pgd_run_conv_impl<float>(p, X, B, max_steps, lr, mask, tol, best_assign, best_sat, best_step, conv_step, final_sat, final_F, stream); }
 
 extern "C" afs_status afs_pgd_run_masks(afs_problem* p, float* X, int32_t B, int32_t steps, float lr, const int8_t* masks,
                                         int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)

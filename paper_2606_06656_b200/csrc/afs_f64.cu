@@ -14,14 +14,7 @@ extern "C" afs_status afs_pgd_run_f64(afs_problem* p, double* X, int32_t B, int3
 extern "C" afs_status afs_pgd_run_conv_f64(afs_problem* p, double* X, int32_t B, int32_t max_steps, double lr, const int8_t* mask,
                                        double tol, int8_t* best_assign, int32_t* best_sat, int32_t* best_step,
                                        int32_t* conv_step, int32_t* final_sat, double* final_F, void* stream)
-{
-    if (!(tol >= double(0)) || !std::isfinite((double)tol)) return AFS_ERR_INVALID_ARG;
-    if (p && conv_step && B >= 1) launch_fill_i32(conv_step, (size_t)B, -1, (cudaStream_t)stream);
-    afs_status s = pgd_run_impl<double>(p, X, B, max_steps, lr, mask, best_assign, best_sat, best_step, stream, tol, conv_step);
-    if (s == AFS_OK && final_sat) s = round_count_impl<double>(p, X, B, nullptr, final_sat, stream);
-    if (s == AFS_OK && final_F) s = eval_grad_impl<double>(p, X, B, final_F, nullptr, stream);
-    return s;
-}
+{ return pgd_run_conv_impl<double>(p, X, B, max_steps, lr, mask, tol, best_assign, best_sat, best_step, conv_step, final_sat, final_F, stream); }
 
 extern "C" afs_status afs_pgd_run_masks_f64(afs_problem* p, double* X, int32_t B, int32_t steps, double lr, const int8_t* masks,
                                         int8_t* best_assign, int32_t* best_sat, int32_t* best_step, void* stream)

@@ -493,4 +493,30 @@ static afs_status pgd_run_impl(afs_problem* P, real* X, int32_t B, int32_t steps
     return AFS_OK;
 }
 
+// afs_pgd_run_conv: the run, then the Fig. 4-5 outputs of the returned iterate.  The trailing evaluations belong to the
+// same call: the launch count and the timing spans of the run survive them.
+template <typename real>
+static afs_status pgd_run_conv_impl(afs_problem* P, real* X, int32_t B, int32_t max_steps, real lr, const int8_t* mask,
+                                    real tol, int8_t* best_assign, int32_t* best_sat, int32_t* best_step,
+                                    int32_t* conv_step, int32_t* final_sat, real* final_F, void* stream)
+{
+    if (!(tol >= real(0)) || !std::isfinite((double)tol)) return AFS_ERR_INVALID_ARG;
+    if (P && conv_step && B >= 1) {   // -1 unless the run says otherwise (tol = 0 may take the resident path); on the handle's device
+        DeviceScope dev_scope(P);
+        if (cudaSetDevice(P->device) != cudaSuccess) { (void)cudaGetLastError(); return AFS_ERR_CUDA; }
+        launch_fill_i32(conv_step, (size_t)B, -1, (cudaStream_t)stream);
+    }
+    afs_status s = pgd_run_impl<real>(P, X, B, max_steps, lr, mask, best_assign, best_sat, best_step, stream, tol, conv_step);
+    if (s != AFS_OK) return s;
+    int64_t launches = P->last_launches + (conv_step ? 1 : 0);
+    const int32_t resident = P->last_resident;
+    const std::vector<Profiler::Span> spans = P->prof.spans;
+    const size_t used = P->prof.used;
+    if (final_sat) { s = round_count_impl<real>(P, X, B, nullptr, final_sat, stream); launches += P->last_launches; }
+    if (s == AFS_OK && final_F) { s = eval_grad_impl<real>(P, X, B, final_F, nullptr, stream); launches += P->last_launches; }
+    P->last_launches = launches; P->last_resident = resident;
+    P->prof.spans = spans; P->prof.used = used;   // the evaluations record no events: the run's spans are intact
+    return s;
+}
+
 }  // namespace afs

@@ -354,7 +354,7 @@ def test_resident_kernel_equals_streaming_path(afs, name, B):
             else:
                 assert dX.max() <= 2e-6, dX.max()
                 same = dX.max(axis=1) == 0
-                assert same.mean() >= 0.5
+                assert same.mean() >= 0.9     # measured on B200: 1.0 in every case of this test
                 for a, b in zip(res[1][1:], res[2][1:]):
                     assert np.array_equal(a[same], b[same])
     P.set_option(0, 0)
@@ -544,7 +544,7 @@ def test_full_size_instances_fp64_trajectory_20_steps_on_sampled_restarts(afs, c
 
 # ------------------------------------------------------------------------------------------------ full BASELINE.json sizes
 FULL = {0: dict(sample=64, steps=200), 1: dict(sample=48, steps=500), 2: dict(sample=48, steps=1000),
-        3: dict(sample=24, steps=300), 4: dict(sample=4, steps=20)}
+        3: dict(sample=24, steps=300), 4: dict(sample=4, steps=500)}
 
 
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])

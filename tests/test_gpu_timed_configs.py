@@ -109,7 +109,7 @@ def test_configs1_fp32_resident_full_batch_against_the_oracle(afs):
     _, recount = ref.round_count(inst, ba.astype(np.float64), want_assign=False)
     assert np.array_equal(recount, out["best_sat"].cpu().numpy()[idx])
     # where fp32 and fp64 round every iterate alike the counts agree; allow the restarts that cross zero differently
-    assert np.mean(out["best_sat"].cpu().numpy()[idx] == o["best_sat"]) >= 0.5
+    assert np.mean(out["best_sat"].cpu().numpy()[idx] == o["best_sat"]) >= 7 / 8     # measured on B200: 8 of 8
     P.close()
 
 
@@ -119,6 +119,48 @@ def test_configs4_fp64_build_100_step_trajectory_boundary_steady_state(afs):
     inst = W.config(4)
     idx = sample_of(inst.B, 4, 44)
     run_full_batch_fp64(afs, inst, inst.X0, 100, idx)
+
+
+def test_configs4_the_timed_call_500_iterations_full_batch(afs):
+    """configs[4] exactly as bench.py times it: fp32, B = 2048, 500 iterations, mask, retirement every 32 iterations.
+    About 400 of the 500 iterations run with > 90 % of the restarts retired and compacted, a regime the 20- and 100-step
+    tests do not reach.  (1) Every output is bit-identical to the same call without retirement (afs_set_option(2, 0)),
+    which works on the full batch for all 500 iterations.  (2) The oracle recounts every best_assign: it satisfies
+    exactly best_sat constraints, honours the mask, and beats or equals the start.  (3) The fp64 build over the first 250
+    iterations (by 200, 96 % of the restarts are retired) equals the oracle's run on the first and the last restart:
+    iterates to 1e-8, integer outputs exactly."""
+    import torch
+    inst = W.config(4)
+    steps = 500
+    P = afs.Problem.from_instance(inst)
+    mask = dev(inst.mask)
+    got = {}
+    for every in (32, 0):
+        P.set_option(2, every)
+        X = dev(inst.X0)
+        out = P.pgd_run(X, steps, LR, mask=mask)
+        torch.cuda.synchronize()
+        assert P.info("resident") == 0
+        got[every] = [X] + [out[k] for k in ("best_sat", "best_step", "best_assign")]
+    for a, b in zip(got[32], got[0]):
+        assert torch.equal(a, b)
+    P.set_option(2, 32)
+    Xf, bs, bt, ba = (t.cpu().numpy() for t in got[32])
+    fixed = inst.mask != 0
+    assert np.all(Xf[:, fixed] == inst.mask[fixed].astype(np.float32)) and np.all(np.abs(Xf) <= 1.0)
+    assert np.all(ba[:, fixed] == inst.mask[fixed])
+    _, recount = ref.round_count(inst, ba.astype(np.float64), want_assign=False)
+    assert np.array_equal(recount, bs)
+    X0m = inst.X0.astype(np.float64)
+    X0m[:, fixed] = inst.mask[fixed]
+    assert np.all(bs >= ref.round_count(inst, X0m, want_assign=False)[1]) and np.all((bt >= 0) & (bt <= steps))
+    # the retired regime is really reached: nearly every restart is at a fixed point of the PGD map at the end
+    X1 = got[32][0].clone()
+    P.pgd_run(X1, 1, LR, mask=mask)
+    frozen = (X1 == got[32][0]).all(dim=1).float().mean().item()
+    assert frozen >= 0.9, frozen
+    P.close()
+    run_full_batch_fp64(afs, inst, inst.X0, 250, np.array([0, inst.B - 1]))
 
 
 # ------------------------------------------------------------------------------------------------ LONG class alone, fp32
