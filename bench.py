@@ -86,15 +86,18 @@ def algorithmic_flops_per_constraint(inst) -> np.ndarray:
     return f
 
 
-def algorithmic_work(inst):
-    """Per kernel class and per PGD iteration over the whole batch: (flops, compulsory HBM bytes)."""
+def algorithmic_work(inst, B=None):
+    """Per kernel class and per PGD iteration over B restarts (default: the whole batch): (flops, compulsory HBM bytes).
+    The rule of the bench line: a restart's work counts in the iterations in which the method has to move it -- retired
+    restarts (fixed points of the PGD map) need none -- so B is the MEAN NUMBER OF ACTIVE restarts per
+    iteration for the timed call, and the full batch for the pass timed with retirement switched off."""
     cls = kernel_class_of_constraints(inst)
     f = algorithmic_flops_per_constraint(inst)
     L = inst.lengths().astype(np.float64)
     if inst.mask is not None:      # literals of fixed variables are constants of the run: neither gathered nor written
         fixed = (inst.mask[np.abs(inst.lits) - 1] != 0).astype(np.float64)
         L = L - np.add.reduceat(fixed, inst.row_ptr[:-1]) if inst.m else L
-    B = float(inst.B)
+    B = float(inst.B if B is None else B)
     work = {}
     for name in set(cls):
         sel = cls == name
@@ -114,6 +117,33 @@ def algorithmic_work(inst):
     total_f = float(f.sum() + inst.nnz + 5 * inst.n) * B
     work["step"] = (total_f, float(2 * B * inst.n * 4 + inst.nnz * 4))
     return work
+
+
+def active_trace(P, X0, pgd_steps, lr, mask, every):
+    """Active restarts in each PGD iteration of the timed call, re-derived through the public API (untimed): the call
+    retires, after every `every`-th iteration, the restarts whose last step left the iterate unchanged.  The same
+    iterates are produced here in chunks without retirement (the PGD map is deterministic, so resuming from X is exact)
+    and compared step against step."""
+    import torch
+    B = X0.shape[0]
+    if every <= 0:
+        return np.full(pgd_steps, B, dtype=np.int64)
+    P.set_option(2, 0)
+    X = X0.clone()
+    active = torch.ones(B, dtype=torch.bool, device=X.device)
+    n_act, t = [], 0
+    while t < pgd_steps:
+        nxt = min((t // every + 1) * every, pgd_steps)
+        n_act += [int(active.sum().item())] * (nxt - t)
+        if nxt >= pgd_steps:
+            break
+        P.pgd_run(X, nxt - t - 1, lr, mask=mask)
+        Xp = X.clone()
+        P.pgd_run(X, 1, lr, mask=mask)
+        active &= (X != Xp).any(dim=1)
+        t = nxt
+    P.set_option(2, every)
+    return np.asarray(n_act, dtype=np.int64)
 
 
 def load_traffic(workload, kernel):
@@ -341,20 +371,35 @@ def measure_config(cfg, args, afs, shard, rank, world, local, peaks):
         P.close()
         return None
 
-    # ---- roofline of the dominant kernel: its launches timed live with CUDA events on the launching stream
-    # (afs_set_option(1, stride) + afs_profile_read), in a second pass so that the events do not sit in `value`
-    work = algorithmic_work(inst)
+    # ---- roofline.  ONE rule for every class: the work of a PGD iteration is the work of the
+    # restarts that are active in it.  `step.frac` divides that by the time of the timed call (retirement on);
+    # `step.no_retire` is a second timed pass with retirement off (afs_set_option(2, 0)): full-batch work over
+    # full-batch time; `step.static_formula` is SURVEY.md 8(d)'s state-independent count over the time of the timed call.
+    RETIRE = 32                                                             # the library's default, which `value` ran with
+    every = 0 if resident else RETIRE
+    n_act = active_trace(P, X0, pgd_steps, lr, mask, every)
+    act_mean = float(n_act.mean()) if len(n_act) else float(inst.B)
+    work = algorithmic_work(inst, act_mean)                                 # active restarts only
+    work_act_static = dict(work)                                            # ... before the counted flops replace 6 L K
+    work_full = algorithmic_work(inst)                                      # every restart in every iteration
     fp32_meas, fp32_derived = fp32_peak(local, peaks)
     stride = max(1, pgd_steps // 64)
-    P.set_option(1, stride)
-    prof, counted = {}, {}
-    for _ in range(max(1, min(args.steps, 3))):
-        one_call(False)
-        for k, (ms, cnt) in P.profile_read().items():
-            a = prof.setdefault(k, [0.0, 0]); a[0] += ms; a[1] += cnt
-        for k, fl in P.profile_flops().items():          # state-dependent flops counted by the long-constraint kernels
-            counted[k] = counted.get(k, 0.0) + fl
-    P.set_option(1, 0)
+
+    def profile_pass(ncalls):
+        """per-launch spans (CUDA events on the launching stream, every stride-th iteration) in a pass of its own, so
+        that the events do not sit in `value`; returns ({class: [ms, launches]}, {class: counted flops})"""
+        P.set_option(1, stride)
+        prof, counted = {}, {}
+        for _ in range(ncalls):
+            one_call(False)
+            for k, (ms, cnt) in P.profile_read().items():
+                a = prof.setdefault(k, [0.0, 0]); a[0] += ms; a[1] += cnt
+            for k, fl in P.profile_flops().items():      # state-dependent flops counted by the long-constraint kernels
+                counted[k] = counted.get(k, 0.0) + fl
+        P.set_option(1, 0)
+        return prof, counted
+
+    prof, counted = profile_pass(max(1, min(args.steps, 3)))
     # the launches that serve the LONG class in one iteration count as one kernel group
     grp = [k for k in prof if k.startswith("long") or k == "glong"]
     if grp:
@@ -371,22 +416,37 @@ def measure_config(cfg, args, afs, shard, rank, world, local, peaks):
         long_parts = None
     # Long EK/CARD kernels: literals on the boundary of the cube (clipped iterates, fixed variables) are exact shifts
     # and cost no arithmetic, so their algorithmic flops are the 6 Leff Keff the kernels count at the iterates they
-    # actually see; the state-independent 6 L K stays beside it as `static_formula`.
-    static_work = dict(work)
+    # actually see (active restarts only, by construction); the state-independent 6 L K stays beside it as
+    # `static_formula`.
     for k, fl in counted.items():
         if k in prof and prof[k][1] > 0 and k in work:
             work[k] = (fl / prof[k][1], work[k][1])
     if counted:
-        step_f = work["step"][0] - sum(static_work[k][0] for k in counted if k in static_work) + \
+        step_f = work["step"][0] - sum(work_act_static[k][0] for k in counted if k in work_act_static) + \
             sum(work[k][0] for k in counted if k in work)
         work["step"] = (step_f, work["step"][1])
-    dom = max(prof, key=lambda k: prof[k][0]) if prof else None
-    roof = dict(bound=None, achieved=None, peak=None, unit=None, frac=None, traffic=None)
+    # k_sat_pull runs on the library's second stream BESIDE the variable pass: its span overlaps the others and is
+    # reported on its own, not added to the time of the iteration
+    overlapped = {k: prof.pop(k) for k in ("sat_pull",) if k in prof}
     per_iter_s = dev_ms * 1e-3 / (args.steps * max(pgd_steps, 1))           # whole PGD iteration, this rank
+    # Event records between the launches of one iteration keep them from running back to back, so the spans of the
+    # profile pass add up to more than the iteration takes in the timed call.  Each group's launch duration is its span
+    # scaled by (time of the iteration in the timed call) / (sum of the spans per sampled iteration) when that is < 1:
+    # launch_ms x launches per call <= ms_per_step then holds by construction; the raw span stays beside it.
+    sampled_iters = max((v[1] for k, v in prof.items() if k != "boundary"), default=0)
+    span_sum_s = sum(v[0] for k, v in prof.items() if k != "boundary") * 1e-3 / max(sampled_iters, 1)
+    scale = 1.0
+    if not resident and span_sum_s > per_iter_s > 0:
+        scale = per_iter_s / span_sum_s
+    dom = max((k for k in prof if k != "boundary"), key=lambda k: prof[k][0], default=None)
+    roof = dict(bound=None, achieved=None, peak=None, unit=None, frac=None, traffic=None)
     alu_src = ("afs_fp32_fma_peak: FFMA micro-benchmark measured on this GPU in this run (derived bound "
                "148 SMs x 128 lanes x 2 flop x %.0f MHz = %.2f)" % (peaks["sm_max_mhz"], fp32_derived))
     if dom is not None:
-        dur_s = prof[dom][0] * 1e-3 / prof[dom][1]                          # average launch duration
+        raw_s = prof[dom][0] * 1e-3 / prof[dom][1]                          # mean event-timed span of one launch (group)
+        if resident:                                                        # one launch: never longer than the call it is in
+            scale = min(1.0, dev_ms * 1e-3 / args.steps / raw_s)
+        dur_s = raw_s * scale
         if dom == "resident":                                               # one launch = every iteration of the call
             flops, hbm = work["step"][0] * pgd_steps, 2 * inst.B * inst.n * 4 + inst.nnz * 4
         else:
@@ -403,25 +463,55 @@ def measure_config(cfg, args, afs, shard, rank, world, local, peaks):
         if dom == "long":
             roof["kernel_group_us_per_launch"] = long_parts
         roof["launch_ms"] = dur_s * 1e3
+        roof["launch_ms_event_span"] = raw_s * 1e3
+        roof["span_scale"] = scale
         roof["launches_timed"] = prof[dom][1]
-        roof["algorithmic_per_launch"] = dict(flops=flops, hbm_bytes=hbm)
-        if dom in counted and dom in static_work:
-            sf0 = static_work[dom][0]
+        launches_per_call = 1 if dom == "resident" else pgd_steps
+        assert roof["launch_ms"] * launches_per_call <= dev_ms / args.steps * 1.0001, "launch_ms x launches exceeds ms_per_step"
+        roof["algorithmic_per_launch"] = dict(flops=flops, hbm_bytes=hbm, restarts="active (mean %.1f of %d)" % (act_mean, inst.B))
+        if dom in counted and dom in work_full:
+            sf0 = work_full[dom][0]
             roof["static_formula"] = dict(flops_per_launch=sf0, frac_alu=sf0 / dur_s / 1e12 / fp32_meas,
-                                          note="6 L K on the unfixed literals, whatever the iterate; the kernel skips boundary literals")
-        tot_ms = sum(v[0] for v in prof.values())
+                                          note="6 L K on the unfixed literals of the whole batch, whatever the iterate; the kernel skips boundary literals and retired restarts")
+        tot_ms = sum(v[0] for k, v in prof.items())
         roof["share_of_timed_launches"] = {k: round(v[0] / tot_ms, 4) for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}
+        if overlapped:
+            roof["overlapped_side_stream_us_per_launch"] = {k: round(v[0] / max(v[1], 1) * 1e3, 2) for k, v in overlapped.items()}
         roof["traffic"] = load_traffic(inst.name, dom)
     # the whole PGD iteration against the same two ceilings (every kernel of the step, launch gaps included): the
     # figure BASELINE.json's ">= 50 % of its roofline" target is judged on
-    sf, sb = work["step"]
-    t_alu, t_hbm = sf / (fp32_meas * 1e12), sb / (peaks["hbm_gbs"] * 1e9)
-    roof["step"] = dict(bound="alu" if t_alu >= t_hbm else "hbm", roofline_us=max(t_alu, t_hbm) * 1e6,
-                        measured_us=per_iter_s * 1e6, frac=max(t_alu, t_hbm) / per_iter_s,
-                        algorithmic_per_iteration=dict(flops=sf, hbm_bytes=sb))
-    if counted:
-        s0 = static_work["step"][0]
-        roof["step"]["static_formula"] = dict(flops=s0, frac_alu=s0 / (fp32_meas * 1e12) / per_iter_s)
+    def step_roof(sf, sb, t_iter):
+        t_alu, t_hbm = sf / (fp32_meas * 1e12), sb / (peaks["hbm_gbs"] * 1e9)
+        return dict(bound="alu" if t_alu >= t_hbm else "hbm", roofline_us=max(t_alu, t_hbm) * 1e6,
+                    measured_us=t_iter * 1e6, frac=max(t_alu, t_hbm) / t_iter,
+                    algorithmic_per_iteration=dict(flops=sf, hbm_bytes=sb))
+    roof["step"] = step_roof(work["step"][0], work["step"][1], per_iter_s)
+    roof["step"]["active_restarts"] = dict(mean=act_mean, of=int(inst.B), retire_every=every,
+                                           at_iteration={str(t): int(n_act[t]) for t in sorted({0, pgd_steps // 10, pgd_steps // 4, pgd_steps // 2, pgd_steps - 1}) if 0 <= t < len(n_act)})
+    s0 = work_full["step"][0]
+    roof["step"]["static_formula"] = dict(flops=s0, hbm_bytes=work_full["step"][1],
+                                          frac=max(s0 / (fp32_meas * 1e12), work_full["step"][1] / (peaks["hbm_gbs"] * 1e9)) / per_iter_s,
+                                          note="SURVEY.md 8(d): every restart in every iteration, 6 L K for EK / CARD, over the time of the timed call")
+    if not resident:
+        # retirement off: the same call on the full batch for every iteration, timed the same way (CUDA events around
+        # the call, L2 flushed before it); work = the full batch, the LONG class by its counted flops of THIS pass
+        P.set_option(2, 0)
+        one_call(False)
+        torch.cuda.synchronize()
+        nr = [one_call(True) for _ in range(max(1, min(args.steps, 2)))]
+        torch.cuda.synchronize()
+        nr_iter_s = sum(a.elapsed_time(b) for a, b in nr) * 1e-3 / (len(nr) * max(pgd_steps, 1))
+        prof_nr, counted_nr = profile_pass(1)
+        fl_nr = sum(v for k, v in counted_nr.items() if k.startswith("long"))
+        it_nr = max((prof_nr[k][1] for k in prof_nr if k.startswith("long") or k == "glong"), default=0)
+        sf_nr = work_full["step"][0]
+        if fl_nr and it_nr and "long" in work_full:
+            sf_nr = sf_nr - work_full["long"][0] + fl_nr / it_nr
+        P.set_option(2, RETIRE)
+        roof["step"]["no_retire"] = step_roof(sf_nr, work_full["step"][1], nr_iter_s)
+    else:
+        roof["step"]["no_retire"] = dict(note="the tile-resident kernel never retires: same figure as step.frac",
+                                         frac=roof["step"]["frac"], measured_us=per_iter_s * 1e6)
 
     # ---- the oracle beside it (bounded sample, rank 0, N = 1 only)
     cpu = None
