@@ -299,6 +299,8 @@ def measure_config(cfg, args, afs, shard, rank, world, local, peaks):
     P = afs.Problem.from_instance(inst, device=local)
     if args.mode is not None:
         P.set_option(0, args.mode)
+    if args.retire_every is not None:
+        P.set_option(2, args.retire_every)
     X0 = torch.from_numpy(inst.X0).cuda()
     X = torch.empty_like(X0)
     mask = None if inst.mask is None else torch.from_numpy(inst.mask).cuda()
@@ -375,7 +377,7 @@ def measure_config(cfg, args, afs, shard, rank, world, local, peaks):
     # restarts that are active in it.  `step.frac` divides that by the time of the timed call (retirement on);
     # `step.no_retire` is a second timed pass with retirement off (afs_set_option(2, 0)): full-batch work over
     # full-batch time; `step.static_formula` is SURVEY.md 8(d)'s state-independent count over the time of the timed call.
-    RETIRE = 32                                                             # the library's default, which `value` ran with
+    RETIRE = 32 if args.retire_every is None else args.retire_every         # the period `value` ran with (library default 32)
     every = 0 if resident else RETIRE
     n_act = active_trace(P, X0, pgd_steps, lr, mask, every)
     act_mean = float(n_act.mean()) if len(n_act) else float(inst.B)
@@ -492,6 +494,27 @@ def measure_config(cfg, args, afs, shard, rank, world, local, peaks):
     roof["step"]["static_formula"] = dict(flops=s0, hbm_bytes=work_full["step"][1],
                                           frac=max(s0 / (fp32_meas * 1e12), work_full["step"][1] / (peaks["hbm_gbs"] * 1e9)) / per_iter_s,
                                           note="SURVEY.md 8(d): every restart in every iteration, 6 L K for EK / CARD, over the time of the timed call")
+    if not resident and pgd_steps >= 20:
+        # where the time of the call goes: the same call cut short at a few lengths (the PGD map is deterministic, so
+        # the first k iterations of every call are the same work); differences of the call times = cost of the
+        # iterations in between, entry / exit layout changes included in the first range
+        cuts = sorted({max(pgd_steps // 50, 1), pgd_steps // 5, pgd_steps // 2, pgd_steps})
+        t_cut = []
+        for k in cuts:
+            ts = []
+            for _ in range(2):
+                X.copy_(X0); flush.fill_(1)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream); P.pgd_run(X, k, lr, mask=mask, out=out); e1.record(stream)
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            t_cut.append(min(ts))
+        lo, phases = 0, {}
+        for k, t_ms, t_prev in zip(cuts, t_cut, [0.0] + t_cut[:-1]):
+            phases["%d-%d" % (lo, k)] = dict(us_per_iteration=round((t_ms - t_prev) * 1e3 / (k - lo), 2),
+                                             mean_active_restarts=round(float(n_act[lo:k].mean()), 1))
+            lo = k
+        roof["step"]["phases"] = phases
     if not resident:
         # retirement off: the same call on the full batch for every iteration, timed the same way (CUDA events around
         # the call, L2 flushed before it); work = the full batch, the LONG class by its counted flops of THIS pass
@@ -599,6 +622,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--pgd-steps", type=int, default=None, help="override the configuration's PGD iteration count")
     ap.add_argument("--mode", type=int, default=None, help="afs_set_option(0, mode): 1 streaming, 2 resident")
+    ap.add_argument("--retire-every", type=int, default=None,
+                    help="afs_set_option(2, K): retire restarts at a fixed point every K iterations (0 never; default: the library's 32)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.gpus > 1 and "RANK" not in os.environ:

@@ -839,10 +839,10 @@ __global__ void __launch_bounds__(VAR_WARPS * 32, 32 / VAR_WARPS) k_var(const Va
     const real one = real(1);
     const real* __restrict__ xcol = a.Xin + b;
     const ColGlobal<real> xg{reinterpret_cast<const char*>(xcol)};
+    if (tile_idle(a.rs, tile0)) return;       // first thing: late in a run most CTAs of the grid are of this kind
     uint2* sbuf = s_stage[warp];
     for (int i = lane; i < PULL_SBUF; i += 32) sbuf[i] = make_uint2(0u, 0u);   // slack slots must stay valid offsets
     __syncwarp();
-    if (tile_idle(a.rs, tile0)) return;
     const int vbeg = (blockIdx.x * VAR_WARPS + warp) * VAR_VPW;
     const int vend = min(vbeg + VAR_VPW, a.n);
     // ---- convergence detection: a restart whose last step stayed below tol is frozen from now on
@@ -980,12 +980,14 @@ __global__ void __launch_bounds__(256) k_glong(int n, int ntile, int Bp, const i
                                                real* __restrict__ GL, const RunState* __restrict__ rs)
 {
     const int lane = threadIdx.x & 31;
-    const int ngrp = ntile / TPW;
-    const long long wid = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
-    if (wid >= (long long)n * ngrp) return;
+    // Grid-stride over (variable, group of TPW tiles) for the groups that hold active restarts; the active count lives
+    // on the device, so the grid is sized for the SMs, not for the batch (idle tiles cost nothing).
+    const int ngrp = rs != nullptr ? min(ntile / TPW, (rs->n_act + 32 * TPW - 1) / (32 * TPW)) : ntile / TPW;
+    const long long total = (long long)n * ngrp;
+#pragma unroll 1
+    for (long long wid = (long long)blockIdx.x * 8 + (threadIdx.x >> 5); wid < total; wid += (long long)gridDim.x * 8) {
     const int v = (int)(wid / ngrp), tile0 = (int)(wid % ngrp) * TPW;
-    if (tile_idle(rs, tile0)) return;
-    if (mask && mask[v] != 0) return;   // a fixed variable never moves: its gradient is not needed
+    if (mask && mask[v] != 0) continue;   // a fixed variable never moves: its gradient is not needed
     const int s0 = lslot_ptr[v], s1 = lslot_ptr[v + 1];
     // One base pointer and 32-bit element offsets per lane and tile: a restart on the boundary reads the pair table
     // (second element where the literal is true, i.e. (x < 0) != negated), one inside the cube reads the class's rows.
@@ -1033,6 +1035,7 @@ __global__ void __launch_bounds__(256) k_glong(int n, int ntile, int Bp, const i
     }
 #pragma unroll
     for (int c = 0; c < TPW; ++c) GL[(size_t)v * Bp + (tile0 + c) * 32 + lane] = g[c];
+    }   // grid-stride loop
 }
 
 // ------------------------------------------------------------------------------------------------------------------

@@ -353,11 +353,15 @@ __global__ void __launch_bounds__(128) k_long_scan(const LongCon* __restrict__ c
                                                    uint32_t* __restrict__ MI, uint32_t* __restrict__ MT)
 {
     const int lane = threadIdx.x & 31;
-    const long long wid = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
     if (blockIdx.x == 0 && threadIdx.x < LONG_CLASSES) wl.count[(set ^ 1) * LONG_CLASSES + threadIdx.x] = 0;
-    if (wid >= (long long)n_long * ntile) return;
-    const int c = (int)(wid / ntile), tile = (int)(wid % ntile);
-    if (tile_idle(rs, tile)) return;
+    // Grid-stride over the (constraint, tile) pairs of the tiles that hold active restarts: the count lives on the device
+    // (the host cannot size the grid by it), and a grid sized for the whole batch spends a late iteration starting and
+    // ending CTAs for idle tiles.
+    const int atile = rs != nullptr ? min(ntile, (rs->n_act + 31) >> 5) : ntile;
+    const long long total = (long long)n_long * atile;
+#pragma unroll 1
+    for (long long wid = (long long)blockIdx.x * 4 + (threadIdx.x >> 5); wid < total; wid += (long long)gridDim.x * 4) {
+    const int c = (int)(wid / atile), tile = (int)(wid % atile);
     const LongCon lc = cons[c];
     const int L = lc.L;
     const uint32_t* lw = lits + lc.off;
@@ -415,6 +419,7 @@ __global__ void __launch_bounds__(128) k_long_scan(const LongCon* __restrict__ c
             if (cls == k) wl.items[k][base + __popc(m & lt)] = make_uint4((unsigned)c, (unsigned)b, (unsigned)nB0 | ((unsigned)nBr << 16), (unsigned)nAr);
         }
     }
+    }   // grid-stride loop
 }
 
 // WPC warps per CTA, each with its own list / pmf buffers of LS / QS entries; persistent over the class's work list.

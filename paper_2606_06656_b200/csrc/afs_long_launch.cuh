@@ -86,7 +86,8 @@ afs_status launch_long_all(afs_problem* P, const real* XT, const uint32_t* Sw, c
     if ((warps + 3) / 4 > 0x7fffffffLL) return AFS_ERR_UNSUPPORTED;
     {
         ProfSpan span(P, 5, st);
-        k_long_scan<real><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(fo ? P->d_long_f : (P->unit_w_mode && P->d_long_u) ? P->d_long_u : P->d_long, (int)P->n_long,
+        // persistent over the (constraint, active tile) pairs: one resident wave of CTAs
+        k_long_scan<real><<<(unsigned)std::min<long long>((warps + 3) / 4, (long long)P->sm_count * 16), 128, 0, st>>>(fo ? P->d_long_f : (P->unit_w_mode && P->d_long_u) ? P->d_long_u : P->d_long, (int)P->n_long,
                                                                       fo ? P->d_long_lits_f : P->d_long_lits, Sw, SATw, ntile,
                                                                       Bp, (real*)P->ws.bnd, sat, fe, wl, set, rs, P->d_long_goff, P->ws.long_MI,
                                                                       P->ws.long_MT);

@@ -42,11 +42,11 @@ static void launch_var(afs_problem* P, VarArgs<real>& a, int gx, int tiles, cons
             const int8_t* mk = EVAL ? nullptr : a.mask;
             if (tiles % 2 == 0) {
                 const long long warps = (long long)P->n * (tiles / 2);
-                k_glong<real, 2><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P->n, tiles, a.Bp, P->d_lslot_ptr, P->d_lslot_info,
+                k_glong<real, 2><<<(unsigned)std::min<long long>((warps + 7) / 8, (long long)P->sm_count * 16), 256, 0, st>>>(P->n, tiles, a.Bp, P->d_lslot_ptr, P->d_lslot_info,
                                                                             a.Xin, lrows, nl, (const real*)P->ws.bnd, mk, GL, rs);
             } else {
                 const long long warps = (long long)P->n * tiles;
-                k_glong<real, 1><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(P->n, tiles, a.Bp, P->d_lslot_ptr, P->d_lslot_info,
+                k_glong<real, 1><<<(unsigned)std::min<long long>((warps + 7) / 8, (long long)P->sm_count * 16), 256, 0, st>>>(P->n, tiles, a.Bp, P->d_lslot_ptr, P->d_lslot_info,
                                                                             a.Xin, lrows, nl, (const real*)P->ws.bnd, mk, GL, rs);
             }
         }
