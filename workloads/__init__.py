@@ -18,4 +18,5 @@ from .generate import (  # noqa: F401
     random_kcnf, planted_kcnf, mixed_pb, xor_dup, long_pb, tiny_mixed,
     concat, true_counts, plant_satisfies,
 )
-from .encoders import sudoku, sudoku_assignment, ramsey, ramsey_assignment  # noqa: F401
+from .encoders import (sudoku, sudoku_assignment, sudoku_unit_clues, ramsey, ramsey_assignment, ramsey3c,  # noqa: F401
+                       ramsey3c_assignment, costas, costas_assignment)
