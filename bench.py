@@ -297,6 +297,13 @@ def measure_config(cfg, args, afs, shard, rank, world, local, peaks):
     pgd_steps = inst.steps if args.pgd_steps is None else args.pgd_steps
     lr = float(np.float32(inst.lr))
     P = afs.Problem.from_instance(inst, device=local)
+    # bench.py restates the library's class rules to attribute work to kernels: fail loudly if the two ever drift apart
+    cls_here = kernel_class_of_constraints(inst)
+    counts_here = {"var": int((cls_here == "var").sum()), "med0": int((cls_here == "med0").sum()),
+                   "cmed+long": int(((cls_here == "cmed") | (cls_here == "long")).sum())}
+    counts_lib = {"var": P.info("n_pull"), "med0": P.info("n_med"), "cmed+long": P.info("n_long")}   # info 5 counts both EK / CARD classes
+    if getattr(inst, "weights", None) is None:      # weighted short clauses leave the pull path
+        assert counts_here == counts_lib, ("bench.py's class rules differ from the library's", counts_here, counts_lib)
     if args.mode is not None:
         P.set_option(0, args.mode)
     if args.retire_every is not None:

@@ -38,6 +38,10 @@
 #define AFS_API
 #endif
 
+/* AFS_DIAG marks exported MEASUREMENT AIDS (per-launch timing, counted flops, the FMA micro-benchmark): bench.py and the
+ * tests use them; nothing on the product path calls them, and a product build may leave them out. */
+#define AFS_DIAG AFS_API
+
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -264,7 +268,7 @@ AFS_API afs_status afs_set_option(afs_problem* p, int32_t what, int64_t value);
  *   final count, fills)
  */
 #define AFS_KERNEL_CLASSES 19
-AFS_API afs_status afs_profile_read(afs_problem* p, double* ms, int64_t* launches, int32_t n);
+AFS_DIAG afs_status afs_profile_read(afs_problem* p, double* ms, int64_t* launches, int32_t n);
 
 /*
  * afs_profile_flops -- after afs_profile_read: adds to flops[0..n) (host, caller-zeroed) the STATE-DEPENDENT
@@ -275,7 +279,7 @@ AFS_API afs_status afs_profile_read(afs_problem* p, double* ms, int64_t* launche
  * boundary (clipped iterates, fixed variables) are exact shifts of the pmf and cost no arithmetic, so
  * the state-independent 6 L K over-counts what these kernels have to do.  Other classes add nothing.
  */
-AFS_API afs_status afs_profile_flops(afs_problem* p, double* flops, int32_t n);
+AFS_DIAG afs_status afs_profile_flops(afs_problem* p, double* flops, int32_t n);
 
 /*
  * afs_fp32_fma_peak -- measures the plain-FP32 FMA throughput of `device` (TFLOP/s, FMA = 2 flops) with a hand-written
@@ -283,7 +287,7 @@ AFS_API afs_status afs_profile_flops(afs_problem* p, double* flops, int32_t n);
  * path: bench.py uses it as the denominator of its "alu" roofline.  Synchronous; restores the caller's
  * current device.
  */
-AFS_API afs_status afs_fp32_fma_peak(int32_t device, double* tflops);
+AFS_DIAG afs_status afs_fp32_fma_peak(int32_t device, double* tflops);
 
 /* Static, never NULL. */
 AFS_API const char* afs_status_string(afs_status s);

@@ -23,7 +23,7 @@ def afs():
 
 def declared_symbols():
     text = open(os.path.join(ROOT, "include", "afs.h")).read()
-    return sorted(set(re.findall(r"AFS_API[^;(]*?\b(afs_[a-z0-9_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"AFS_(?:API|DIAG)[^;(]*?\b(afs_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_header_declares_the_boundary():
